@@ -1,0 +1,176 @@
+"""Pins for the oracle's LL right-hand side and integrators (oracle/mo.c: mo_llg_rhs, mo_step)."""
+from fractions import Fraction as F
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2406_16064_b200 import workloads as wl
+
+MU0 = 4e-7 * np.pi
+
+
+def macrospin(alpha=0.5, gamma=2.21e5, Hz=1e5, integrator=oracle.DOPRI5, demag=False):
+    o = oracle.Oracle(1, 1, 1, 1e-9, 1e-9, 1e-9)
+    o.set_Ms(8e5)
+    o.set_alpha(alpha)
+    o.set_gamma(gamma)
+    o.set_H_ext(0, 0, Hz)
+    o.set_integrator(integrator)
+    o.set_demag(1 if demag else 0)
+    if demag:
+        o.init_demag()
+    return o
+
+
+def eq53(t, alpha, gamma, Hz):
+    """PAPER.md:409-417, Eq. 53."""
+    g = gamma / (1 + alpha**2)
+    return np.array([np.cos(g * Hz * t) / np.cosh(alpha * g * Hz * t),
+                     np.sin(g * Hz * t) / np.cosh(alpha * g * Hz * t), np.tanh(alpha * g * Hz * t)])
+
+
+def run(o, T, n, tol=0.0):
+    m = np.array([1.0, 0.0, 0.0]).reshape(3, 1, 1, 1).copy()
+    dt = T / n
+    for _ in range(n):
+        o.step(m, dt, tol)
+    return m.reshape(3)
+
+
+def test_rhs_orthogonal_to_m_and_masked():
+    w = wl.cfg4(8, 8, 4)
+    Ms = 8.6e5 * wl.random_mask(1, 8, 8, 4)
+    o = oracle.Oracle(8, 8, 4, w.dx, w.dy, w.dz)
+    w.Ms = Ms
+    wl.apply(o, w)
+    m = w.m0 * (Ms > 0)
+    k = o.llg_rhs(m)
+    assert np.abs((k * m).sum(axis=0)).max() < 1e-4 * np.abs(k).max()
+    assert np.all(k[:, Ms == 0] == 0)
+    assert np.abs(k).max() > 1e9
+
+
+def test_rhs_matches_hand_value():
+    """m = x^, H = Hz z^: m x H = -Hz y^; m x (m x H) = -Hz z^  =>  dm/dt = g'Hz y^ + a g'Hz z^."""
+    o = macrospin(alpha=0.5, gamma=2.21e5, Hz=1e5)
+    k = o.llg_rhs(np.array([1.0, 0, 0]).reshape(3, 1, 1, 1)).reshape(3)
+    gp = 2.21e5 / 1.25
+    assert np.allclose(k, [0.0, gp * 1e5, 0.5 * gp * 1e5], rtol=1e-15)
+
+
+@pytest.mark.parametrize("integ", [oracle.RK4, oracle.DOPRI5])
+@pytest.mark.parametrize("demag", [False, True])
+def test_macrospin_eq53(integ, demag):
+    """Fig. 3 parameters. With demag on, a single cube cell has H_d = -Ms m/3 || m: no torque."""
+    T = 0.2e-9
+    o = macrospin(integrator=integ, demag=demag)
+    m = run(o, T, 400)
+    assert np.allclose(m, eq53(T, 0.5, 2.21e5, 1e5), atol=1e-9)
+    assert abs(np.linalg.norm(m) - 1) < 1e-15
+    assert np.isclose(o.time(), T, rtol=1e-12)
+
+
+def test_convergence_orders():
+    T = 0.1e-9
+    ref = eq53(T, 0.5, 2.21e5, 1e6)
+    errs = {}
+    for integ, ns in [(oracle.RK4, (80, 160, 320)), (oracle.DOPRI5, (40, 80, 160))]:
+        e = []
+        for n in ns:
+            o = macrospin(alpha=0.5, Hz=1e6, integrator=integ)
+            e.append(np.linalg.norm(run(o, T, n) - ref))
+        errs[integ] = e
+    r4 = np.log2(errs[oracle.RK4][0] / errs[oracle.RK4][1]), np.log2(errs[oracle.RK4][1] / errs[oracle.RK4][2])
+    r5 = np.log2(errs[oracle.DOPRI5][0] / errs[oracle.DOPRI5][1]), np.log2(errs[oracle.DOPRI5][1] / errs[oracle.DOPRI5][2])
+    assert all(3.8 < r < 4.2 for r in r4), r4
+    assert all(4.8 < r < 5.3 for r in r5), r5
+
+
+def test_dopri5_tableau_identities():
+    """Exact-rational order conditions on the coefficients the oracle actually uses."""
+    a, e = oracle.dopri5_tableau()
+    c = [F(0), F(1, 5), F(3, 10), F(4, 5), F(8, 9), F(1), F(1)]
+    A = [[F(x).limit_denominator(10**7) for x in row] for row in a]
+    E = [F(x).limit_denominator(10**7) for x in e]
+    for i in range(7):
+        assert np.allclose([float(x) for x in A[i]], a[i], rtol=1e-15, atol=0)
+        assert sum(A[i]) == c[i]
+    b5 = A[6] + [F(0)]
+    b4 = [b5[j] - E[j] for j in range(7)]
+    assert sum(b5) == 1 and sum(b4) == 1
+    for b, order in ((b5, 5), (b4, 4)):
+        for p in range(1, order):
+            assert sum(b[j] * c[j] ** p for j in range(7)) == F(1, p + 1)       # quadrature conditions
+        assert sum(b[i] * sum(A[i][j] * c[j] for j in range(6)) for i in range(7)) == F(1, 6)
+        assert sum(b[i] * c[i] * sum(A[i][j] * c[j] for j in range(6)) for i in range(7)) == F(1, 8)
+        assert sum(b[i] * sum(A[i][j] * c[j] ** 2 for j in range(6)) for i in range(7)) == F(1, 12)
+    # a genuinely fifth-order condition that b4 must fail and b5 must meet
+    assert sum(b5[j] * c[j] ** 4 for j in range(7)) == F(1, 5)
+    assert sum(b4[j] * c[j] ** 4 for j in range(7)) != F(1, 5)
+
+
+def test_adaptive_step_controller_rules():
+    o = macrospin(alpha=0.05, Hz=1e6)
+    m = np.array([1.0, 0.0, 0.0]).reshape(3, 1, 1, 1).copy()
+    m0 = m.copy()
+    ok, err, dn, md = o.step(m, 2e-11, 1e-9)                 # far too large a step
+    assert not ok and err > 1e-9 and np.array_equal(m, m0) and o.time() == 0.0
+    assert np.isclose(dn, 2e-11 * max(0.2, 0.9 * (1e-9 / err) ** 0.2))
+    ok, err2, dn2, _ = o.step(m, 1e-13, 1e-9)
+    assert ok and err2 <= 1e-9 and np.isclose(dn2, 1e-13 * min(5.0, 0.9 * (1e-9 / err2) ** 0.2))
+    assert np.isclose(md, 2.21e5 / (1 + 0.05**2) * 1e6 * np.sqrt(1 + 0.05**2), rtol=1e-12)   # |k1| at m=x^
+    # embedded error estimate scales like dt^5
+    e = []
+    for dt in (4e-13, 2e-13):
+        mm = m0.copy()
+        e.append(o.step(mm, dt, 1.0)[1])
+    assert 4.5 < np.log2(e[0] / e[1]) < 5.5
+
+
+def test_energy_decay_and_dissipation_rate():
+    """alpha>0, constant H_ext: E non-increasing along RK4 steps; dE/dt = -mu0 a g' sum V Ms |m x H|^2."""
+    nx, ny, nz = 8, 8, 2
+    w = wl.cfg4(nx, ny, nz)
+    w.Ms = 8.6e5 * wl.random_mask(7, nx, ny, nz, 0.85)
+    for kind in (wl.DMI_BULK, wl.DMI_INTERFACIAL):
+        w.dmi_kind = kind
+        w.integrator = wl.RK4
+        o = oracle.Oracle(nx, ny, nz, w.dx, w.dy, w.dz)
+        wl.apply(o, w)
+        m = np.ascontiguousarray(w.m0 * (w.Ms > 0))
+        dt = 1e-14
+        E0, _ = o.energy(m)
+        H = o.effective_field(m)
+        mxH = np.cross(m.reshape(3, -1).T, H.reshape(3, -1).T)
+        gp = w.gamma / (1 + w.alpha**2)
+        rate = -MU0 * w.alpha * gp * (w.dx * w.dy * w.dz) * (w.Ms.reshape(-1) * (mxH**2).sum(axis=1)).sum()
+        Es = [E0]
+        for _ in range(20):
+            o.step(m, dt)
+            Es.append(o.energy(m)[0])
+            n = np.sqrt((m * m).sum(axis=0))
+            assert np.abs(n[w.Ms > 0] - 1).max() < 1e-14
+        assert all(Es[i + 1] < Es[i] for i in range(20))
+        assert np.isclose((Es[1] - Es[0]) / dt, rate, rtol=2e-2)
+
+
+def test_stoner_wohlfarth_switching_field():
+    """Listing 2: 4x4x4 cube, Ku=5e4 along (1,1,0), field swept along x.  For a 45 deg
+    easy axis the coherent-rotation switching field is H_K/2 = Ku/(mu0 Ms).  A cube of cubes has an
+    isotropic mean demag factor 1/3, so shape adds no anisotropy to the macrospin."""
+    Ms, Ku = 8e5, 5e4
+    Hsw = Ku / (MU0 * Ms)
+
+    def relaxed_mx(Hx):
+        o = oracle.Oracle(1, 1, 1, 4e-9, 4e-9, 4e-9)
+        o.set_Ms(Ms); o.set_Ku(Ku); o.set_axis(1, 1, 0); o.set_alpha(0.5); o.set_demag(0)
+        o.set_H_ext(Hx, 0, 0)
+        m = (np.array([1.0, 1.0, 1e-3]) / np.linalg.norm([1.0, 1.0, 1e-3])).reshape(3, 1, 1, 1).copy()
+        o.relax(m, 1e-7, 1e5, 20000, 1e-12)
+        return m.reshape(3)
+
+    m_lo = relaxed_mx(-0.90 * Hsw)
+    m_hi = relaxed_mx(-1.10 * Hsw)
+    assert m_lo[0] > 0 or m_lo[1] > 0.5          # still in the original well
+    assert m_hi[0] < -0.5 and m_hi[1] < 0.0      # switched
