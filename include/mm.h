@@ -1,0 +1,143 @@
+/*
+ * mm.h — C ABI of the B200-native LLG hot path (arxiv 2406.16064, "MicroMagnetic.jl").
+ *
+ * One handle = one finite-difference micromagnetic problem on a regular nx*ny*nz mesh
+ * ("FDMesh", "cell-based" Ms).  The calls below are the hot path of
+ * one Landau-Lifshitz-Gilbert time step: effective field (Eq. 1; demag Eq. 8
+ * PAPER.md:138-140 as a zero-padded FFT convolution; exchange Eq. 5; DMI Eq. 15
+ * PAPER.md:173-175; uniaxial anisotropy Eq. 32 PAPER.md:269 in its continuum reading; Zeeman
+ * Eq. 35), the LL torque (Eq. 37) and a Dormand-Prince / RK4 step with
+ * projection onto |m| = 1.  Every step of the path runs in the library's
+ * CUDA kernels (sm_100a); there is no CPU fallback.
+ *
+ * Conventions
+ *  - Every function returns an mm_status (0 = MM_OK) unless stated; no exception crosses the ABI.
+ *  - Pointers named dev_* are DEVICE pointers on the handle's device, in the handle's precision
+ *    (float for MM_F32, double for MM_F64), owned by the caller.  Pointers named host_* are HOST
+ *    pointers.  Out-parameters (int*, double*, long*) are HOST pointers and may be NULL.
+ *  - Layout: x fastest, cell index idx = i + nx*(j + ny*k); vector fields are SoA: component c of
+ *    cell idx is at [c*N + idx], N = nx*ny*nz, c in {x, y, z}.  Ms is N reals; Ms = 0 marks vacuum.
+ *  - Units: SI.  m dimensionless unit vectors; H in A/m; Ms in A/m; A in J/m; D in J/m^2; Ku in
+ *    J/m^3; gamma in m/(A s); time in s; cell edges in m.  mu0 = 4 pi 1e-7.
+ *  - A neighbour outside the mesh or with Ms = 0 is absent (free boundary).  Cells with Ms = 0 get
+ *    H = 0 and dm/dt = 0, and are never touched by the integrators.
+ *  - All work is enqueued on the CUDA stream given to mm_create and is asynchronous with respect
+ *    to the host unless a non-NULL host out-parameter (or a host_* buffer) forces a
+ *    synchronisation of that stream.
+ *  - Supported meshes: nx, ny, nz powers of two (nz = 1 allowed: thin film); with demag enabled
+ *    additionally nx >= 4, ny >= 2 and the per-CTA shared-memory tiles must fit (see
+ *    DESIGN.md "Limits"); otherwise mm_init_demag returns MM_ERR_UNSUPPORTED.
+ */
+#ifndef MM_H
+#define MM_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mm_sim mm_sim;  /* opaque; created/destroyed only by the library */
+
+typedef enum { MM_F32 = 0, MM_F64 = 1 } mm_prec;
+typedef enum {
+    MM_OK = 0,
+    MM_ERR_ARG = -1,          /* bad argument (NULL, non-positive size, zero axis, ...)        */
+    MM_ERR_UNSUPPORTED = -2,  /* mesh shape outside the supported set                           */
+    MM_ERR_STATE = -3,        /* call order: e.g. demag enabled but mm_init_demag not called,   */
+                              /* or workspace not set                                           */
+    MM_ERR_CUDA = -4,         /* a CUDA runtime call or kernel launch failed                    */
+    MM_ERR_NOMEM = -5,        /* workspace too small / allocation failed                        */
+    MM_ERR_NAN = -6           /* non-finite error norm met in mm_step / mm_relax                */
+} mm_status;
+typedef enum { MM_DMI_NONE = 0, MM_DMI_BULK = 1, MM_DMI_INTERFACIAL = 2 } mm_dmi_kind;
+typedef enum { MM_RK4 = 0, MM_DOPRI5 = 1 } mm_integrator;
+
+/* Create a problem on `device`, all later work on `cuda_stream` (a cudaStream_t; NULL = default
+ * stream).  dx, dy, dz: cell edges in metres.  Defaults: Ms = 0 everywhere, A = D = Ku = 0, axis =
+ * z, H_ext = 0, alpha = 0.5, gamma = 2.211e5, integrator = MM_DOPRI5, demag enabled. */
+int mm_create(mm_sim** out, int nx, int ny, int nz, double dx, double dy, double dz,
+              mm_prec prec, int device, void* cuda_stream);
+int mm_destroy(mm_sim* sim);
+
+/* Persistent device memory the library needs (cached tensor spectrum K^, FFT spectra, RK stage
+ * vectors, Ms).  The CALLER allocates it (e.g. torch.empty) and keeps it alive until mm_destroy;
+ * the library only carves it up.  Must be called before mm_set_Ms / mm_init_demag / any compute.
+ * mm_init_demag additionally uses transient cudaMalloc'ed scratch that it frees before returning. */
+size_t mm_workspace_bytes(const mm_sim* sim);
+int mm_set_workspace(mm_sim* sim, void* dev_ptr, size_t bytes);   /* dev_ptr 256-byte aligned */
+
+/* Material / run parameters (Listing 2 names). */
+int mm_set_Ms_uniform(mm_sim* sim, double Ms);
+int mm_set_Ms(mm_sim* sim, const void* dev_Ms);                   /* N reals, copied            */
+int mm_set_A(mm_sim* sim, double A);
+int mm_set_D(mm_sim* sim, double D, mm_dmi_kind kind);
+int mm_set_Ku(mm_sim* sim, double Ku);
+int mm_set_axis(mm_sim* sim, double ux, double uy, double uz);    /* normalised inside; 0 => ARG */
+int mm_set_H_ext(mm_sim* sim, double hx, double hy, double hz);
+int mm_set_alpha(mm_sim* sim, double alpha);
+int mm_set_gamma(mm_sim* sim, double gamma);
+int mm_set_integrator(mm_sim* sim, mm_integrator integ);
+int mm_set_demag(mm_sim* sim, int on);                            /* 0/1; default 1             */
+
+/* Build and cache the spectrum of the demag tensor (depends on mesh and cell size
+ * only).  Tensor in fp64 (near field: closed forms of ref [20] in __float128 on the host; far
+ * field: Gauss-Legendre quadrature of the defining dipole integral in fp64 on the device), its
+ * FFT in fp64, rounded once to the handle's precision.  Synchronous. */
+int mm_init_demag(mm_sim* sim);
+
+/* H_eff(m) — Eq. 1 with all enabled terms.  dev_m, dev_H: 3N reals each. */
+int mm_effective_field(mm_sim* sim, const void* dev_m, void* dev_H);
+/* dm/dt — Eq. 37.  dev_dmdt: 3N reals, 1/s. */
+int mm_llg_rhs(mm_sim* sim, const void* dev_m, void* dev_dmdt);
+
+/* One step of the selected integrator, m updated in place on acceptance, time advanced.
+ * tol <= 0: fixed step, always accepted.  DOPRI5 (R8): err = max_i |dt sum_j e_j k_j|,
+ * accept iff err <= tol, dt_next = dt * clamp(0.9 (tol/err)^(1/5), 0.2, 5).  7 RHS evaluations per
+ * step (no FSAL).  RK4: 4 RHS evaluations, err = 0.  max_dmdt = max_i |k_1,i|.
+ * If all four out-pointers are NULL the call does not synchronise. */
+int mm_step(mm_sim* sim, void* dev_m, double dt, double tol,
+            int* accepted, double* err, double* dt_next, double* max_dmdt);
+
+/* Adaptive steps (DOPRI5) from dt0 until max|dm/dt| < stop_dmdt (rad/s) or max_steps steps
+ * (accepted + rejected).  The step controller runs on the device; the host polls every
+ * `poll` steps (<=0: library default). */
+int mm_relax(mm_sim* sim, void* dev_m, double tol, double stop_dmdt, long max_steps, double dt0,
+             long* steps_done, double* max_dmdt);
+
+/* Advance by adaptive DOPRI5 steps until exactly t_end (last step clipped). */
+int mm_run_until(mm_sim* sim, void* dev_m, double t_end, double tol, double dt0, long max_steps,
+                 long* steps_done);
+
+/* End-to-end convenience with HOST buffers: copies host_m (3N reals) to the device, takes
+ * nsteps fixed-dt steps (tol <= 0) or adaptive attempts (tol > 0), copies m back.  Synchronous. */
+int mm_run_host(mm_sim* sim, void* host_m, int nsteps, double dt, double tol);
+/* Same for one RHS evaluation: host_m in, host_dmdt out. */
+int mm_llg_rhs_host(mm_sim* sim, const void* host_m, void* host_dmdt);
+
+double mm_time(const mm_sim* sim);
+int mm_set_time(mm_sim* sim, double t);
+
+/* Diagnostics, off the hot path (synchronous). */
+int mm_average_m(mm_sim* sim, const void* dev_m, double out3[3]);   /* mean over cells with Ms>0 */
+/* E = -mu0 V sum_i Ms_i m_i.(H_d/2 + H_ex/2 + H_dmi/2 + H_an/2 + H_ext); terms in that order. */
+int mm_energy(mm_sim* sim, const void* dev_m, double* E_total, double E_terms[5]);
+/* Real-space tensor component (0..5 = xx,yy,zz,xy,xz,yz) at offsets i,j,k >= 0: N doubles (fp64
+ * regardless of precision) to dev_out.  Valid after mm_init_demag. */
+int mm_get_demag_kernel(mm_sim* sim, int comp, void* dev_out);
+/* Per-kernel timing for roofline accounting (bench.py).  While on, the library brackets each hot-path
+ * kernel with CUDA events on the handle's stream; mm_get_profile synchronises the stream, sums the
+ * elapsed milliseconds and launch counts per kernel class since the last call — [0] pass A
+ * fwd_xz, [1] pass B y_conv, [2] pass C inv_zx, [3] fused local-field/torque/RK-stage kernel —
+ * and clears the record.  Off by default (no events are recorded). */
+int mm_set_profiling(mm_sim* sim, int on);
+int mm_get_profile(mm_sim* sim, double ms_out[4], long count_out[4]);
+/* Number of kernel launches issued by this handle so far (for bench accounting). */
+long mm_launch_count(const mm_sim* sim);
+const char* mm_last_error(const mm_sim* sim);
+const char* mm_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MM_H */

@@ -1,0 +1,220 @@
+// mm_fft.cuh — shared-memory FFT core of the demag convolution ("three forward
+// Fourier transforms and three inverse Fourier transforms").
+//
+// Tile model.  A CTA holds a tile of `nlines` independent lines of `n` complex points in shared
+// memory, element (point q, line l) at s[q*pitch + l] — the LINE index is the fastest one, so the
+// threads of a warp work on the same butterfly of neighbouring lines: every shared-memory access
+// of a stage is unit-stride across the warp (bank-conflict free for any radix and any stage) and
+// the twiddle factor is warp-uniform.
+//
+// Transform.  Forward = in-place decimation-in-frequency (Gentleman-Sande), radix 8/4/2, natural
+// order in, BIT-REVERSED order out.  Inverse = the exact adjoint, decimation-in-time, bit-reversed
+// in, natural out, unnormalised.  Nothing is ever re-ordered: the spectrum lives in bit-reversed
+// positions everywhere (HBM included) and the cached tensor spectrum K^ is permuted once at setup.
+//
+// Zero padding / cropping (R3) are pruned stages: a line of n = 2m points
+// whose upper half is zero enters as  s[i] = a_i, s[i+m] = a_i w_n^i  (the first radix-2 DIF stage
+// with the zeros folded in) followed by the stages of two independent length-m blocks; the
+// cropped inverse ends with  out_i = s[i] + conj(w_n^i) s[i+m], i < m.
+//
+// Everything here is __host__ __device__ so the index arithmetic can be exercised on the CPU
+// (thread loops run with tid = 0, nthr = 1; MM_SYNC is a no-op there).
+#pragma once
+
+#if defined(__CUDACC__)
+#define MM_HD __host__ __device__ __forceinline__
+#else
+#define MM_HD inline
+#endif
+
+#if defined(__CUDA_ARCH__)
+#define MM_SYNC() __syncthreads()
+#else
+#define MM_SYNC() ((void)0)
+#endif
+
+namespace mm {
+
+template <typename T> struct alignas(2 * sizeof(T)) cx {
+    T x, y;
+};
+
+template <typename T> MM_HD cx<T> mk(T a, T b) { cx<T> r; r.x = a; r.y = b; return r; }
+template <typename T> MM_HD cx<T> operator+(cx<T> a, cx<T> b) { return mk<T>(a.x + b.x, a.y + b.y); }
+template <typename T> MM_HD cx<T> operator-(cx<T> a, cx<T> b) { return mk<T>(a.x - b.x, a.y - b.y); }
+template <typename T> MM_HD cx<T> cmul(cx<T> a, cx<T> b) { return mk<T>(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+// a * conj(b)
+template <typename T> MM_HD cx<T> cmulc(cx<T> a, cx<T> b) { return mk<T>(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y); }
+template <typename T> MM_HD cx<T> conj(cx<T> a) { return mk<T>(a.x, -a.y); }
+template <typename T> MM_HD cx<T> mul_mi(cx<T> a) { return mk<T>(a.y, -a.x); }   // * (-i)
+template <typename T> MM_HD cx<T> mul_pi(cx<T> a) { return mk<T>(-a.y, a.x); }   // * (+i)
+template <typename T> MM_HD cx<T> scale(cx<T> a, T s) { return mk<T>(a.x * s, a.y * s); }
+template <typename T> MM_HD void bf2(cx<T>& a, cx<T>& b) { cx<T> t = a; a = t + b; b = t - b; }
+
+MM_HD int ilog2(int n) { int l = 0; while ((1 << l) < n) l++; return l; }
+// bit reversal of v within `bits` bits
+MM_HD unsigned brev(unsigned v, int bits)
+{
+#if defined(__CUDA_ARCH__)
+    return bits ? (__brev(v) >> (32 - bits)) : 0u;
+#else
+    unsigned r = 0;
+    for (int b = 0; b < bits; b++) r |= ((v >> b) & 1u) << (bits - 1 - b);
+    return r;
+#endif
+}
+
+// ---- radix kernels: forward = natural in, bit-reversed out; inverse = the adjoint -------------
+template <typename T, int R> struct radix;
+
+template <typename T> struct radix<T, 2> {
+    static MM_HD void fwd(cx<T>* v) { bf2(v[0], v[1]); }
+    static MM_HD void inv(cx<T>* v) { bf2(v[0], v[1]); }
+};
+template <typename T> struct radix<T, 4> {
+    static MM_HD void fwd(cx<T>* v)
+    {
+        bf2(v[0], v[2]); bf2(v[1], v[3]); v[3] = mul_mi(v[3]);
+        bf2(v[0], v[1]); bf2(v[2], v[3]);
+    }
+    static MM_HD void inv(cx<T>* v)
+    {
+        bf2(v[0], v[1]); bf2(v[2], v[3]);
+        v[3] = mul_pi(v[3]); bf2(v[0], v[2]); bf2(v[1], v[3]);
+    }
+};
+template <typename T> struct radix<T, 8> {
+    static MM_HD void fwd(cx<T>* v)
+    {
+        const T c = (T)0.70710678118654752440;
+#pragma unroll
+        for (int r = 0; r < 4; r++) bf2(v[r], v[r + 4]);
+        v[5] = mk<T>(c * (v[5].x + v[5].y), c * (v[5].y - v[5].x));      // * (1-i)/sqrt2
+        v[6] = mul_mi(v[6]);
+        v[7] = mk<T>(c * (v[7].y - v[7].x), -c * (v[7].x + v[7].y));     // * (-1-i)/sqrt2
+        radix<T, 4>::fwd(v);
+        radix<T, 4>::fwd(v + 4);
+    }
+    static MM_HD void inv(cx<T>* v)
+    {
+        const T c = (T)0.70710678118654752440;
+        radix<T, 4>::inv(v);
+        radix<T, 4>::inv(v + 4);
+        v[5] = mk<T>(c * (v[5].x - v[5].y), c * (v[5].x + v[5].y));      // * (1+i)/sqrt2
+        v[6] = mul_pi(v[6]);
+        v[7] = mk<T>(-c * (v[7].x + v[7].y), c * (v[7].x - v[7].y));     // * (-1+i)/sqrt2
+#pragma unroll
+        for (int r = 0; r < 4; r++) bf2(v[r], v[r + 4]);
+    }
+};
+
+// Twiddle table: tw[k] = exp(-2 pi i k / twN), k in [0, twN/2]; generated in fp64, rounded once.
+template <typename T> struct twiddles {
+    const cx<T>* tw;
+    int twN;
+    // w_L^i for i < L/2 (L divides twN)
+    MM_HD cx<T> get(int i, int L) const { return tw[i * (twN / L)]; }
+};
+
+// powers w^0..w^(R-1) stored in bit-reversed slot order: pw[r] = w^{brev(r)}
+template <typename T, int R> MM_HD void twiddle_powers(cx<T> w1, cx<T>* pw)
+{
+    if (R == 2) { pw[1] = w1; }
+    else if (R == 4) {
+        cx<T> w2 = cmul(w1, w1);
+        pw[1] = w2; pw[2] = w1; pw[3] = cmul(w2, w1);
+    } else {
+        cx<T> w2 = cmul(w1, w1), w3 = cmul(w2, w1), w4 = cmul(w2, w2);
+        pw[1] = w4; pw[2] = w2; pw[3] = cmul(w3, w3); pw[4] = w1; pw[5] = cmul(w4, w1); pw[6] = w3; pw[7] = cmul(w4, w3);
+    }
+}
+
+// One forward radix-R DIF stage on blocks of current length Lc, all lines of the tile.
+template <typename T, int R>
+MM_HD void dif_stage(cx<T>* s, int pitch, int nlines, int n, int Lc, twiddles<T> tw, int tid, int nthr)
+{
+    const int sub = Lc / R;
+    const int total = (n / R) * nlines;
+    for (int f = tid; f < total; f += nthr) {
+        const int l = f % nlines, b = f / nlines;
+        const int blk = b / sub, i = b - blk * sub;
+        cx<T>* p = s + (size_t)(blk * Lc + i) * pitch + l;
+        cx<T> v[R];
+#pragma unroll
+        for (int r = 0; r < R; r++) v[r] = p[(size_t)r * sub * pitch];
+        radix<T, R>::fwd(v);
+        if (i != 0) {
+            cx<T> pw[R];
+            twiddle_powers<T, R>(tw.get(i, Lc), pw);
+#pragma unroll
+            for (int r = 1; r < R; r++) v[r] = cmul(v[r], pw[r]);
+        }
+#pragma unroll
+        for (int r = 0; r < R; r++) p[(size_t)r * sub * pitch] = v[r];
+    }
+}
+
+// The adjoint stage (inverse DIT), unnormalised.
+template <typename T, int R>
+MM_HD void dit_stage(cx<T>* s, int pitch, int nlines, int n, int Lc, twiddles<T> tw, int tid, int nthr)
+{
+    const int sub = Lc / R;
+    const int total = (n / R) * nlines;
+    for (int f = tid; f < total; f += nthr) {
+        const int l = f % nlines, b = f / nlines;
+        const int blk = b / sub, i = b - blk * sub;
+        cx<T>* p = s + (size_t)(blk * Lc + i) * pitch + l;
+        cx<T> v[R];
+#pragma unroll
+        for (int r = 0; r < R; r++) v[r] = p[(size_t)r * sub * pitch];
+        if (i != 0) {
+            cx<T> pw[R];
+            twiddle_powers<T, R>(tw.get(i, Lc), pw);
+#pragma unroll
+            for (int r = 1; r < R; r++) v[r] = cmulc(v[r], pw[r]);
+        }
+        radix<T, R>::inv(v);
+#pragma unroll
+        for (int r = 0; r < R; r++) p[(size_t)r * sub * pitch] = v[r];
+    }
+}
+
+// Radix schedule for a block length m: 8 while >= 8, then the remainder (4 or 2).
+MM_HD int next_radix(int Lc) { return Lc >= 8 ? 8 : Lc; }
+
+// Forward transform of every length-m block of the n-point lines (n a multiple of m).
+template <typename T>
+MM_HD void fft_fwd_blocks(cx<T>* s, int pitch, int nlines, int n, int m, twiddles<T> tw, int tid, int nthr)
+{
+    int Lc = m;
+    while (Lc > 1) {
+        const int R = next_radix(Lc);
+        if (R == 8) dif_stage<T, 8>(s, pitch, nlines, n, Lc, tw, tid, nthr);
+        else if (R == 4) dif_stage<T, 4>(s, pitch, nlines, n, Lc, tw, tid, nthr);
+        else dif_stage<T, 2>(s, pitch, nlines, n, Lc, tw, tid, nthr);
+        MM_SYNC();
+        Lc /= R;
+    }
+}
+
+// Inverse (adjoint) of fft_fwd_blocks: stages in reverse order.
+template <typename T>
+MM_HD void fft_inv_blocks(cx<T>* s, int pitch, int nlines, int n, int m, twiddles<T> tw, int tid, int nthr)
+{
+    // the forward schedule is 8,8,...,8,rem ; walk it backwards
+    int rem = m;
+    while (rem >= 8) rem /= 8;           // rem in {1,2,4}
+    int Lc = rem;
+    if (rem > 1) {
+        if (rem == 4) dit_stage<T, 4>(s, pitch, nlines, n, 4, tw, tid, nthr);
+        else dit_stage<T, 2>(s, pitch, nlines, n, 2, tw, tid, nthr);
+        MM_SYNC();
+    }
+    while (Lc < m) {
+        Lc *= 8;
+        dit_stage<T, 8>(s, pitch, nlines, n, Lc, tw, tid, nthr);
+        MM_SYNC();
+    }
+}
+
+}  // namespace mm

@@ -1,0 +1,1045 @@
+// mm_lib.cu — libmm.so: the C ABI of include/mm.h, its host runtime and the __global__ kernels.
+// Hand-written CUDA for sm_100a; no cuFFT, no cuBLAS, no CPU fallback.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+#include <string>
+#include <vector>
+
+#include "../../include/mm.h"
+#include "mm_fft.cuh"
+#include "mm_kernels.cuh"
+#include "mm_llg.cuh"
+
+extern "C" void mm_newell_near_box(int bx, int by, int bz, double dx, double dy, double dz, double* out);
+
+namespace mm {
+
+static const double MU0 = 4.0e-7 * 3.14159265358979323846264338327950288;
+
+// Device-resident step controller state.
+struct DevState {
+    double dt, t, tol, err, maxk, t_end, stop_dmdt;
+    unsigned long long err_bits, maxk_bits;
+    int accepted, done, nan, mode;     // mode: 0 single step, 1 relax, 2 run_until
+    long long nacc, nrej, nsteps;
+};
+
+// ------------------------------------------------------------------------------------------------
+// __global__ wrappers of the convolution passes
+// ------------------------------------------------------------------------------------------------
+extern __shared__ __align__(16) unsigned char mm_smem[];
+
+template <typename T>
+__global__ void __launch_bounds__(256) fwd_xz_kernel(Geom g, const T* m, const T* Ms, cx<T>* S, twiddles<T> tw, const DevState* st)
+{
+    if (st->done) return;
+    fwd_xz_body<T>(g, m, Ms, S, tw, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x);
+}
+template <typename T>
+__global__ void __launch_bounds__(512) y_conv_kernel(Geom g, cx<T>* S, const T* Kh, twiddles<T> tw, const DevState* st)
+{
+    if (st->done) return;
+    y_conv_body<T>(g, S, Kh, tw, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x);
+}
+template <typename T>
+__global__ void __launch_bounds__(256) inv_zx_kernel(Geom g, const cx<T>* S, T* Hd, twiddles<T> tw, T inv_scale, const DevState* st)
+{
+    if (st->done) return;
+    inv_zx_body<T>(g, S, Hd, tw, inv_scale, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Fused local field + LL torque + RK stage + reductions
+// ------------------------------------------------------------------------------------------------
+template <typename T> struct StageArgs {
+    const T* m0;          // step start magnetisation
+    const T* kprev[6];    // earlier stage derivatives k_0..k_{s-1}
+    T* ynext;             // next stage input (or the RK4 solution); may be NULL
+    double coef[7];       // ynext = m0 + dt * sum_{j<=s} coef[j] k_j
+    double ecoef[7];      // E = dt * sum_{j<=s} ecoef[j] k_j   (do_err)
+    int s;                // index of this stage
+    int do_err, do_maxk;
+};
+
+__device__ __forceinline__ unsigned long long norm_bits(float v) { return (unsigned long long)__float_as_uint(v); }
+__device__ __forceinline__ unsigned long long norm_bits(double v) { return (unsigned long long)__double_as_longlong(v); }
+
+__device__ __forceinline__ void block_max_bits(unsigned long long v, unsigned long long* dst)
+{
+    // non-negative IEEE values order like their bit patterns; a NaN pattern beats everything
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        unsigned long long w = __shfl_xor_sync(0xffffffffu, v, o);
+        v = w > v ? w : v;
+    }
+    __shared__ unsigned long long red[32];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    if (lane == 0) red[wid] = v;
+    __syncthreads();
+    if (wid == 0) {
+        const int nw = (blockDim.x + 31) >> 5;
+        v = lane < nw ? red[lane] : 0ull;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            unsigned long long w = __shfl_xor_sync(0xffffffffu, v, o);
+            v = w > v ? w : v;
+        }
+        if (lane == 0 && v != 0ull) atomicMax(dst, v);
+    }
+    __syncthreads();
+}
+
+// mode 0: out = H_eff ; mode 1: out = k = LL torque (+ optional RK stage algebra)
+template <typename T, int MODE>
+__global__ void __launch_bounds__(256) llg_stage_kernel(Geom g, LocalP<T> lp, const T* __restrict__ y, const T* __restrict__ Ms,
+                                                        const T* __restrict__ Hd, T* __restrict__ out, StageArgs<T> sa, DevState* st)
+{
+    if (st->done) return;
+    const long N = g.N;
+    const long q = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    T errn = 0, kn = 0;
+    if (q < N) {
+        const T Msi = Ms[q];
+        v3<T> res = { 0, 0, 0 };
+        const bool live = Msi != (T)0;
+        if (live) {
+            const int i = (int)(q % g.nx), j = (int)((q / g.nx) % g.ny), k = (int)(q / ((long)g.nx * g.ny));
+            const v3<T> mi = ld3(y, N, q);
+            v3<T> H = { 0, 0, 0 };
+            if (Hd != nullptr) H = ld3(Hd, N, q);
+            H = local_field<T>(g, lp, y, Ms, i, j, k, q, Msi, mi, H);
+            res = MODE == 0 ? H : ll_torque<T>(lp, mi, H);
+        }
+        out[q] = res.x; out[N + q] = res.y; out[2 * N + q] = res.z;
+        if (MODE == 1 && (sa.ynext != nullptr || sa.do_err)) {
+            const T dt = (T)st->dt;
+            v3<T> acc = { (T)sa.coef[sa.s] * res.x, (T)sa.coef[sa.s] * res.y, (T)sa.coef[sa.s] * res.z };
+            v3<T> ea = { (T)sa.ecoef[sa.s] * res.x, (T)sa.ecoef[sa.s] * res.y, (T)sa.ecoef[sa.s] * res.z };
+            for (int jj = 0; jj < sa.s; jj++) {
+                const T cj = (T)sa.coef[jj], ej = (T)sa.ecoef[jj];
+                if (cj == (T)0 && ej == (T)0) continue;
+                const v3<T> kj = ld3(sa.kprev[jj], N, q);
+                acc.x += cj * kj.x; acc.y += cj * kj.y; acc.z += cj * kj.z;
+                ea.x += ej * kj.x; ea.y += ej * kj.y; ea.z += ej * kj.z;
+            }
+            if (sa.ynext != nullptr) {
+                const v3<T> m0 = ld3(sa.m0, N, q);
+                sa.ynext[q] = m0.x + dt * acc.x; sa.ynext[N + q] = m0.y + dt * acc.y; sa.ynext[2 * N + q] = m0.z + dt * acc.z;
+            }
+            if (sa.do_err && live) errn = sqrt((dt * ea.x) * (dt * ea.x) + (dt * ea.y) * (dt * ea.y) + (dt * ea.z) * (dt * ea.z));
+        }
+        if (MODE == 1 && sa.do_maxk && live) kn = sqrt(res.x * res.x + res.y * res.y + res.z * res.z);
+    }
+    if (MODE == 1 && sa.do_err) block_max_bits(norm_bits(errn), &st->err_bits);
+    if (MODE == 1 && sa.do_maxk) block_max_bits(norm_bits(kn), &st->maxk_bits);
+}
+
+// Step controller: one thread.  DESIGN.md R8.
+__global__ void ctrl_kernel(DevState* st, int is_f64, int adaptive_mode)
+{
+    if (st->done) return;
+    double err, maxk;
+    if (is_f64) { err = __longlong_as_double((long long)st->err_bits); maxk = __longlong_as_double((long long)st->maxk_bits); }
+    else { err = (double)__uint_as_float((unsigned)st->err_bits); maxk = (double)__uint_as_float((unsigned)st->maxk_bits); }
+    st->err_bits = 0ull; st->maxk_bits = 0ull;
+    st->err = err; st->maxk = maxk;
+    const double tol = st->tol, dt = st->dt;
+    const bool bad = !(err == err) || !(maxk == maxk);
+    const int ok = !bad && (tol <= 0.0 || err <= tol);
+    st->accepted = ok;
+    st->nsteps++;
+    if (bad) st->nan = 1;
+    if (ok) { st->t += dt; st->nacc++; } else st->nrej++;
+    double dn = dt;
+    if (tol > 0.0) {
+        double fac = bad ? 0.2 : (err == 0.0 ? 5.0 : 0.9 * pow(tol / err, 0.2));
+        fac = fac < 0.2 ? 0.2 : (fac > 5.0 ? 5.0 : fac);
+        dn = dt * fac;
+    }
+    if (adaptive_mode == 0) { st->dt = dn; return; }          // single step: dt_next reported through st->dt
+    if (adaptive_mode == 1) {                                   // relax
+        if (maxk < st->stop_dmdt || bad) st->done = 1;
+        st->dt = dn;
+    } else {                                                    // run until t_end
+        const double left = st->t_end - st->t;
+        if (left <= 1e-12 * fabs(st->t_end) || bad) { st->done = 1; st->dt = dn; }
+        else st->dt = dn < left ? dn : left;
+    }
+}
+
+// On acceptance: m <- y / |y| on cells with Ms > 0 (projection)
+template <typename T>
+__global__ void __launch_bounds__(256) accept_kernel(long N, const DevState* st, const T* __restrict__ ysol, const T* __restrict__ Ms, T* __restrict__ m, int check_done_before)
+{
+    if (!st->accepted) return;
+    const long q = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= N || Ms[q] == (T)0) return;
+    const T x = ysol[q], y = ysol[N + q], z = ysol[2 * N + q];
+    const T n = sqrt(x * x + y * y + z * z);
+    m[q] = x / n; m[N + q] = y / n; m[2 * N + q] = z / n;
+}
+
+__global__ void set_state_kernel(DevState* st, double dt, double tol, double t_end, double stop, int mode, int reset_done)
+{
+    st->dt = dt; st->tol = tol; st->t_end = t_end; st->stop_dmdt = stop; st->mode = mode;
+    st->err_bits = 0ull; st->maxk_bits = 0ull;
+    if (reset_done) { st->done = 0; st->nan = 0; st->nsteps = 0; st->nacc = 0; st->nrej = 0; }
+}
+
+// per-block partial sums: out[block*4 + {0,1,2,3}] = sum w*a.b (w = Ms or 1), components / count
+template <typename T>
+__global__ void __launch_bounds__(256) dot_kernel(long N, const T* __restrict__ a, const T* __restrict__ b, const T* __restrict__ Ms, int mode, double* out)
+{
+    // mode 0: sum Ms * a.b  -> out[4*blk]; mode 1: sums of a.x, a.y, a.z over Ms>0 and the count
+    __shared__ double red[4][256];
+    double v[4] = { 0, 0, 0, 0 };
+    for (long q = (long)blockIdx.x * blockDim.x + threadIdx.x; q < N; q += (long)gridDim.x * blockDim.x) {
+        const double w = (double)Ms[q];
+        if (w == 0.0) continue;
+        if (mode == 0) v[0] += w * ((double)a[q] * (double)b[q] + (double)a[N + q] * (double)b[N + q] + (double)a[2 * N + q] * (double)b[2 * N + q]);
+        else { v[0] += (double)a[q]; v[1] += (double)a[N + q]; v[2] += (double)a[2 * N + q]; v[3] += 1.0; }
+    }
+    for (int c = 0; c < 4; c++) red[c][threadIdx.x] = v[c];
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) for (int c = 0; c < 4; c++) red[c][threadIdx.x] += red[c][threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) for (int c = 0; c < 4; c++) out[4 * blockIdx.x + c] = red[c][0];
+}
+
+template <typename T> __global__ void fill_kernel(long n, T* p, T v)
+{
+    const long q = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q < n) p[q] = v;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Setup (S0): demag tensor in real space, its spectrum, packing.  fp64 throughout.  PAPER.md:136.
+// ------------------------------------------------------------------------------------------------
+struct QuadRule { int n[3]; double s[3][32]; double w[3][32]; };
+
+// Far field: N_ab(r) = -(1/(4 pi V)) int_cell int_cell' d_a d_b (1/|r + u - u'|) du du'  — the definition
+// of the cell-averaged tensor — by a 5-point Gauss-Legendre rule in each of the six variables,
+// collapsed to a rule in the differences s = u - u' (rule.s / rule.w, weights sum to 1 per axis).
+// Near box (|offset| < b in every axis): values from the host quad-precision closed forms.
+__global__ void __launch_bounds__(128) tensor_real_kernel(int nx, int ny, int nz, double dx, double dy, double dz, QuadRule rule,
+                                                          int bx, int by, int bz, const double* __restrict__ near, double* __restrict__ Nr)
+{
+    const long N = (long)nx * ny * nz;
+    const long q = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= N) return;
+    const int i = (int)(q % nx), j = (int)((q / nx) % ny), k = (int)(q / ((long)nx * ny));
+    if (i < bx && j < by && k < bz) {
+        const long Bn = (long)bx * by * bz, o = i + (long)bx * (j + (long)by * k);
+        for (int c = 0; c < 6; c++) Nr[c * N + q] = near[c * Bn + o];
+        return;
+    }
+    const double X = i * dx, Y = j * dy, Z = k * dz;
+    double a[6] = { 0, 0, 0, 0, 0, 0 };
+    for (int c3 = 0; c3 < rule.n[2]; c3++) {
+        const double rz = Z + rule.s[2][c3], wz = rule.w[2][c3];
+        for (int b = 0; b < rule.n[1]; b++) {
+            const double ry = Y + rule.s[1][b], wyz = wz * rule.w[1][b];
+            for (int aa = 0; aa < rule.n[0]; aa++) {
+                const double rx = X + rule.s[0][aa], w = wyz * rule.w[0][aa];
+                const double r2 = rx * rx + ry * ry + rz * rz;
+                const double ir = rsqrt(r2), ir2 = ir * ir, ir5 = ir2 * ir2 * ir * w;
+                a[0] += (3.0 * rx * rx - r2) * ir5; a[1] += (3.0 * ry * ry - r2) * ir5; a[2] += (3.0 * rz * rz - r2) * ir5;
+                a[3] += 3.0 * rx * ry * ir5; a[4] += 3.0 * rx * rz * ir5; a[5] += 3.0 * ry * rz * ir5;
+            }
+        }
+    }
+    const double pref = -(dx * dy * dz) / (4.0 * 3.14159265358979323846264338327950288);
+    for (int c = 0; c < 6; c++) Nr[c * N + q] = pref * a[c];
+}
+
+// Kernel array on the padded grid with wrap indexing (R3): padded index p is offset p for
+// p < n, p - 2n for p > n, slot p = n is 0.  Off-diagonal components are odd in their two axes.
+__global__ void __launch_bounds__(256) wrap_kernel(Geom g, int comp, const double* __restrict__ Nr, cx<double>* __restrict__ A)
+{
+    const long P = (long)g.px * g.py * g.pz;
+    const long q = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= P) return;
+    const int a = (int)(q % g.px), b = (int)((q / g.px) % g.py), c = (int)(q / ((long)g.px * g.py));
+    double v = 0.0;
+    const bool hole = (g.nx > 1 && a == g.nx) || (g.ny > 1 && b == g.ny) || (g.nz > 1 && c == g.nz);
+    if (!hole) {
+        const int di = a < g.nx ? a : a - g.px, dj = b < g.ny ? b : b - g.py, dk = c < g.nz ? c : c - g.pz;
+        const int sx = di < 0 ? -1 : 1, sy = dj < 0 ? -1 : 1, sz = dk < 0 ? -1 : 1;
+        const long o = abs(di) + (long)g.nx * (abs(dj) + (long)g.ny * abs(dk));
+        v = Nr[comp * g.N + o];
+        if (comp == 3) v *= sx * sy;
+        if (comp == 4) v *= sx * sz;
+        if (comp == 5) v *= sy * sz;
+    }
+    A[q] = mk<double>(v, 0.0);
+}
+
+// Generic batched line FFT (forward DIF, output in bit-reversed positions) used only at setup.
+// Line l = (outer, inner): base = outer*so + inner*si ; points stride sp.  One CTA: LT lines.
+__global__ void __launch_bounds__(256) setup_fft_kernel(cx<double>* A, int n, long sp, int ninner, long si, long so, int LT, int point_fastest,
+                                                        twiddles<double> tw)
+{
+    cx<double>* s = reinterpret_cast<cx<double>*>(mm_smem);
+    const int pitch = odd_pitch(LT);
+    const long line0 = (long)blockIdx.x * LT;
+    for (int f = threadIdx.x; f < n * LT; f += blockDim.x) {
+        const int p = point_fastest ? f % n : f / LT, l = point_fastest ? f / n : f % LT;
+        const long line = line0 + l;
+        s[(size_t)p * pitch + l] = A[(line / ninner) * so + (line % ninner) * si + (long)p * sp];
+    }
+    __syncthreads();
+    fft_fwd_blocks<double>(s, pitch, LT, n, n, tw, threadIdx.x, blockDim.x);
+    for (int f = threadIdx.x; f < n * LT; f += blockDim.x) {
+        const int p = point_fastest ? f % n : f / LT, l = point_fastest ? f / n : f % LT;
+        const long line = line0 + l;
+        A[(line / ninner) * so + (line % ninner) * si + (long)p * sp] = s[(size_t)p * pitch + l];
+    }
+}
+
+// Symmetric-packed real spectrum in the positions pass B reads: Kh[comp][kz'][ky'][xpos].
+// Also accumulates max |Im| and max |Re| (bit patterns) for the "K^ is real" check.
+template <typename T>
+__global__ void __launch_bounds__(256) pack_khat_kernel(Geom g, int comp, const cx<double>* __restrict__ A, T* __restrict__ Kh, unsigned long long* maxbits)
+{
+    const int nkz = g.nz > 1 ? g.nz + 1 : 1;
+    const long total = (long)nkz * (g.ny + 1) * g.Lx;
+    const long q = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    double re = 0.0, im = 0.0;
+    if (q < total) {
+        const int xp = (int)(q % g.Lx), kyp = (int)((q / g.Lx) % (g.ny + 1)), kzp = (int)(q / ((long)g.Lx * (g.ny + 1)));
+        if (xp <= g.nx) {
+            const int kx = xp < g.nx ? (int)brev((unsigned)xp, g.lognx) : g.nx;
+            const long a = brev((unsigned)kx, g.lognx + 1), b = brev((unsigned)kyp, g.logpy), c = g.nz > 1 ? brev((unsigned)kzp, g.logpz) : 0;
+            const cx<double> v = A[a + (long)g.px * (b + (long)g.py * c)];
+            re = v.x; im = v.y;
+        }
+        Kh[(long)comp * g.kcomp + q] = (T)re;
+    }
+    block_max_bits(norm_bits(fabs(re)), maxbits);
+    block_max_bits(norm_bits(fabs(im)), maxbits + 1);
+}
+
+}  // namespace mm
+
+// ================================================================================================
+// Host runtime
+// ================================================================================================
+using namespace mm;
+
+struct mm_sim {
+    Geom g;
+    mm_prec prec;
+    int device;
+    cudaStream_t stream;
+    double dx, dy, dz;
+    double A, D, Ku, u[3], hext[3], alpha, gamma;
+    int dmi_kind, integ, demag_on, demag_ready, Ms_set;
+    // workspace
+    void* ws;
+    size_t ws_bytes, ws_need;
+    size_t off_Ms, off_S, off_Kh, off_Hd, off_k[7], off_y[2], off_tw, off_Nr, off_st, off_part;
+    int twN;
+    size_t smemA, smemB;
+    int thrA, thrB;
+    double khat_imag_ratio;
+    double t_host;
+    long launches;
+    std::string err;
+    // optional per-pass profiling (mm_set_profiling): event pairs around each kernel class
+    int prof_on;
+    std::vector<cudaEvent_t> prof_ev;      // pairs
+    std::vector<int> prof_cls;             // class of pair i: 0 pass A, 1 pass B, 2 pass C, 3 stage kernel
+    size_t prof_used;
+};
+
+static void prof_begin(mm_sim* s, int cls)
+{
+    if (!s->prof_on) return;
+    if (s->prof_used + 1 > s->prof_cls.size()) {
+        cudaEvent_t a, b;
+        cudaEventCreate(&a); cudaEventCreate(&b);
+        s->prof_ev.push_back(a); s->prof_ev.push_back(b); s->prof_cls.push_back(cls);
+    }
+    s->prof_cls[s->prof_used] = cls;
+    cudaEventRecord(s->prof_ev[2 * s->prof_used], s->stream);
+}
+static void prof_end(mm_sim* s)
+{
+    if (!s->prof_on) return;
+    cudaEventRecord(s->prof_ev[2 * s->prof_used + 1], s->stream);
+    s->prof_used++;
+}
+
+#define MM_TRY(sim, call)                                                                          \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess) {                                                                   \
+            (sim)->err = std::string(#call) + ": " + cudaGetErrorString(e_);                       \
+            return MM_ERR_CUDA;                                                                    \
+        }                                                                                          \
+    } while (0)
+
+static int fail(mm_sim* s, int code, const char* msg) { if (s) s->err = msg; return code; }
+static size_t esize(const mm_sim* s) { return s->prec == MM_F64 ? sizeof(double) : sizeof(float); }
+static size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
+static bool is_pow2(int v) { return v >= 1 && (v & (v - 1)) == 0; }
+template <typename T> static T* wsp(const mm_sim* s, size_t off) { return reinterpret_cast<T*>(static_cast<char*>(s->ws) + off); }
+static const size_t SMEM_CAP = 200 * 1024;
+
+// Tile configuration.
+static void configure(mm_sim* s)
+{
+    Geom& g = s->g;
+    const size_t cs = 2 * esize(s);
+    const int target = 2 * 148;
+    // passes A/C: G rows per CTA
+    int G = 1;
+    if (g.nz < 8) {
+        G = 16;
+        while (G > 1 && (G > g.ny || 3 * (g.ny / G) < target)) G /= 2;
+    }
+    g.G = G;
+    g.CH = 64;
+    if (g.nz > 1) while (g.CH > 8 && (size_t)g.pz * g.G * g.CH * cs > 32 * 1024) g.CH /= 2;
+    while (g.G > 1 && (size_t)smemA_elems(g) * cs > 100 * 1024) g.G /= 2;
+    // pass B: TC columns per CTA
+    int TC = s->prec == MM_F64 ? 4 : 8;
+    g.TC = TC;
+    while (g.TC > 1 && (size_t)smemB_elems(g) * cs > SMEM_CAP) g.TC /= 2;
+    while (g.TC > 2 && ((g.nx + g.TC) / g.TC) * g.pz < target) g.TC /= 2;
+    g.Lx = ((g.nx + 1 + g.TC - 1) / g.TC) * g.TC;
+    g.plane = (long)g.ny * g.Lx;
+    g.comp = (long)g.pz * g.plane;
+    g.kplane = (long)(g.ny + 1) * g.Lx;
+    g.kcomp = (long)(g.nz > 1 ? g.nz + 1 : 1) * g.kplane;
+    s->smemA = (size_t)smemA_elems(g) * cs;
+    s->smemB = (size_t)smemB_elems(g) * cs;
+    s->thrA = 256;
+    s->thrB = s->smemB > 64 * 1024 ? 512 : 256;
+}
+
+static void layout(mm_sim* s)
+{
+    const Geom& g = s->g;
+    const size_t es = esize(s), N = (size_t)g.N;
+    size_t o = 0;
+    auto take = [&](size_t bytes) { size_t r = o; o = align256(o + bytes); return r; };
+    s->off_st = take(sizeof(DevState));
+    s->off_Ms = take(N * es);
+    s->off_S = take((size_t)3 * g.comp * 2 * es);
+    s->off_Kh = take((size_t)6 * g.kcomp * es);
+    s->off_Hd = take(3 * N * es);
+    for (int i = 0; i < 7; i++) s->off_k[i] = take(3 * N * es);
+    for (int i = 0; i < 2; i++) s->off_y[i] = take(3 * N * es);
+    s->off_tw = take((size_t)(s->twN / 2 + 1) * 2 * es);
+    s->off_Nr = take(6 * N * sizeof(double));
+    s->off_part = take(4 * 1024 * sizeof(double));
+    s->ws_need = o;
+}
+
+extern "C" const char* mm_version(void) { return "mm-b200 0.1 (sm_100a)"; }
+
+extern "C" int mm_create(mm_sim** out, int nx, int ny, int nz, double dx, double dy, double dz, mm_prec prec, int device, void* cuda_stream)
+{
+    if (!out) return MM_ERR_ARG;
+    *out = nullptr;
+    if (nx < 1 || ny < 1 || nz < 1 || !(dx > 0) || !(dy > 0) || !(dz > 0) || (prec != MM_F32 && prec != MM_F64)) return MM_ERR_ARG;
+    if (!is_pow2(nx) || !is_pow2(ny) || !is_pow2(nz)) return MM_ERR_UNSUPPORTED;
+    if ((long)nx * ny * nz > (1L << 30)) return MM_ERR_UNSUPPORTED;
+    mm_sim* s = new mm_sim();
+    s->prec = prec; s->device = device; s->stream = static_cast<cudaStream_t>(cuda_stream);
+    s->dx = dx; s->dy = dy; s->dz = dz;
+    s->A = s->D = s->Ku = 0; s->u[0] = s->u[1] = 0; s->u[2] = 1; s->hext[0] = s->hext[1] = s->hext[2] = 0;
+    s->alpha = 0.5; s->gamma = 2.211e5; s->dmi_kind = 0; s->integ = MM_DOPRI5; s->demag_on = 1; s->demag_ready = 0; s->Ms_set = 0;
+    s->ws = nullptr; s->ws_bytes = 0; s->khat_imag_ratio = -1; s->t_host = 0; s->launches = 0; s->prof_on = 0; s->prof_used = 0;
+    Geom& g = s->g;
+    memset(&g, 0, sizeof(g));
+    g.nx = nx; g.ny = ny; g.nz = nz;
+    g.px = nx > 1 ? 2 * nx : 1; g.py = ny > 1 ? 2 * ny : 1; g.pz = nz > 1 ? 2 * nz : 1;
+    g.lognx = ilog2(nx); g.logpy = ilog2(g.py); g.logpz = ilog2(g.pz);
+    g.N = (long)nx * ny * nz;
+    s->twN = g.px > g.py ? g.px : g.py;
+    if (g.pz > s->twN) s->twN = g.pz;
+    if (s->twN < 4) s->twN = 4;
+    configure(s);
+    layout(s);
+    *out = s;
+    return MM_OK;
+}
+
+extern "C" int mm_destroy(mm_sim* s)
+{
+    if (s) for (cudaEvent_t e : s->prof_ev) cudaEventDestroy(e);
+    delete s;
+    return MM_OK;
+}
+
+extern "C" int mm_set_profiling(mm_sim* s, int on)
+{
+    if (!s) return MM_ERR_ARG;
+    s->prof_on = on ? 1 : 0;
+    s->prof_used = 0;
+    return MM_OK;
+}
+
+extern "C" int mm_get_profile(mm_sim* s, double ms_out[4], long count_out[4])
+{
+    if (!s || !ms_out || !count_out) return MM_ERR_ARG;
+    MM_TRY(s, cudaStreamSynchronize(s->stream));
+    for (int c = 0; c < 4; c++) { ms_out[c] = 0; count_out[c] = 0; }
+    for (size_t i = 0; i < s->prof_used; i++) {
+        float ms = 0;
+        MM_TRY(s, cudaEventElapsedTime(&ms, s->prof_ev[2 * i], s->prof_ev[2 * i + 1]));
+        ms_out[s->prof_cls[i]] += ms;
+        count_out[s->prof_cls[i]]++;
+    }
+    s->prof_used = 0;
+    return MM_OK;
+}
+extern "C" size_t mm_workspace_bytes(const mm_sim* s) { return s ? s->ws_need : 0; }
+extern "C" const char* mm_last_error(const mm_sim* s) { return s ? s->err.c_str() : "null handle"; }
+extern "C" long mm_launch_count(const mm_sim* s) { return s ? s->launches : 0; }
+
+template <typename T> static int upload_twiddles(mm_sim* s)
+{
+    const int n = s->twN / 2 + 1;
+    std::vector<cx<T>> h(n);
+    for (int k = 0; k < n; k++) {
+        const long double a = -2.0L * 3.14159265358979323846264338327950288L * (long double)k / (long double)s->twN;
+        h[k].x = (T)cosl(a); h[k].y = (T)sinl(a);
+    }
+    // exact values at the octants
+    h[0].x = 1; h[0].y = 0;
+    if (s->twN % 4 == 0) { h[s->twN / 4].x = 0; h[s->twN / 4].y = -1; }
+    h[s->twN / 2].x = -1; h[s->twN / 2].y = 0;
+    MM_TRY(s, cudaMemcpyAsync(wsp<char>(s, s->off_tw), h.data(), n * sizeof(cx<T>), cudaMemcpyHostToDevice, s->stream));
+    MM_TRY(s, cudaStreamSynchronize(s->stream));
+    return MM_OK;
+}
+
+extern "C" int mm_set_workspace(mm_sim* s, void* dev_ptr, size_t bytes)
+{
+    if (!s || !dev_ptr) return MM_ERR_ARG;
+    if (bytes < s->ws_need) return fail(s, MM_ERR_NOMEM, "workspace smaller than mm_workspace_bytes()");
+    if ((uintptr_t)dev_ptr & 255) return fail(s, MM_ERR_ARG, "workspace must be 256-byte aligned");
+    MM_TRY(s, cudaSetDevice(s->device));
+    s->ws = dev_ptr; s->ws_bytes = bytes;
+    // zero state, Ms and the spectrum (pad columns of S are never written by pass A)
+    MM_TRY(s, cudaMemsetAsync(dev_ptr, 0, s->off_Kh, s->stream));
+    s->demag_ready = 0; s->Ms_set = 0;
+    return s->prec == MM_F64 ? upload_twiddles<double>(s) : upload_twiddles<float>(s);
+}
+
+#define NEED_WS(s) do { if (!(s)) return MM_ERR_ARG; if (!(s)->ws) return fail((s), MM_ERR_STATE, "mm_set_workspace not called"); } while (0)
+
+extern "C" int mm_set_Ms_uniform(mm_sim* s, double Ms)
+{
+    NEED_WS(s);
+    if (!(Ms >= 0)) return fail(s, MM_ERR_ARG, "Ms must be >= 0");
+    const long N = s->g.N;
+    const int blocks = (int)((N + 255) / 256);
+    if (s->prec == MM_F64) fill_kernel<double><<<blocks, 256, 0, s->stream>>>(N, wsp<double>(s, s->off_Ms), Ms);
+    else fill_kernel<float><<<blocks, 256, 0, s->stream>>>(N, wsp<float>(s, s->off_Ms), (float)Ms);
+    s->launches++;
+    MM_TRY(s, cudaGetLastError());
+    s->Ms_set = 1;
+    return MM_OK;
+}
+extern "C" int mm_set_Ms(mm_sim* s, const void* dev_Ms)
+{
+    NEED_WS(s);
+    if (!dev_Ms) return MM_ERR_ARG;
+    MM_TRY(s, cudaMemcpyAsync(wsp<char>(s, s->off_Ms), dev_Ms, s->g.N * esize(s), cudaMemcpyDeviceToDevice, s->stream));
+    s->Ms_set = 1;
+    return MM_OK;
+}
+extern "C" int mm_set_A(mm_sim* s, double A) { if (!s) return MM_ERR_ARG; s->A = A; return MM_OK; }
+extern "C" int mm_set_D(mm_sim* s, double D, mm_dmi_kind kind)
+{
+    if (!s || kind < 0 || kind > 2) return MM_ERR_ARG;
+    s->D = D; s->dmi_kind = kind; return MM_OK;
+}
+extern "C" int mm_set_Ku(mm_sim* s, double Ku) { if (!s) return MM_ERR_ARG; s->Ku = Ku; return MM_OK; }
+extern "C" int mm_set_axis(mm_sim* s, double ux, double uy, double uz)
+{
+    if (!s) return MM_ERR_ARG;
+    const double n = sqrt(ux * ux + uy * uy + uz * uz);
+    if (!(n > 0)) return fail(s, MM_ERR_ARG, "zero anisotropy axis");
+    s->u[0] = ux / n; s->u[1] = uy / n; s->u[2] = uz / n; return MM_OK;
+}
+extern "C" int mm_set_H_ext(mm_sim* s, double hx, double hy, double hz) { if (!s) return MM_ERR_ARG; s->hext[0] = hx; s->hext[1] = hy; s->hext[2] = hz; return MM_OK; }
+extern "C" int mm_set_alpha(mm_sim* s, double a) { if (!s || !(a >= 0)) return MM_ERR_ARG; s->alpha = a; return MM_OK; }
+extern "C" int mm_set_gamma(mm_sim* s, double g) { if (!s) return MM_ERR_ARG; s->gamma = g; return MM_OK; }
+extern "C" int mm_set_integrator(mm_sim* s, mm_integrator i) { if (!s || (i != MM_RK4 && i != MM_DOPRI5)) return MM_ERR_ARG; s->integ = i; return MM_OK; }
+extern "C" int mm_set_demag(mm_sim* s, int on) { if (!s) return MM_ERR_ARG; s->demag_on = on ? 1 : 0; return MM_OK; }
+
+// ------------------------------------------------------------------------------------------------
+// mm_init_demag
+// ------------------------------------------------------------------------------------------------
+static void make_rule(double d, int* n_out, double* s_out, double* w_out)
+{
+    // 5-point Gauss-Legendre on [-d/2, d/2] for u and u'; rule for s = u - u' with merged nodes
+    static const double x5[5] = { -0.9061798459386640, -0.5384693101056831, 0.0, 0.5384693101056831, 0.9061798459386640 };
+    static const double w5[5] = { 0.2369268850561891, 0.4786286704993665, 0.5688888888888889, 0.4786286704993665, 0.2369268850561891 };
+    int n = 0;
+    for (int a = 0; a < 5; a++)
+        for (int b = 0; b < 5; b++) {
+            const double sv = (x5[a] - x5[b]) * d / 2, wv = w5[a] * w5[b] / 4;
+            int hit = -1;
+            for (int k = 0; k < n; k++) if (fabs(s_out[k] - sv) < 1e-13 * d) hit = k;
+            if (hit >= 0) w_out[hit] += wv; else { s_out[n] = sv; w_out[n] = wv; n++; }
+        }
+    *n_out = n;
+}
+
+template <typename T> static int init_demag_t(mm_sim* s)
+{
+    const Geom& g = s->g;
+    const long N = g.N, P = (long)g.px * g.py * g.pz;
+    cudaStream_t st = s->stream;
+    // near box: 8 largest-cell-edges in every direction (quadrature error there < 1e-16)
+    const double dmax = fmax(s->dx, fmax(s->dy, s->dz));
+    const int bx = (int)fmin((double)g.nx, ceil(8.0 * dmax / s->dx)), by = (int)fmin((double)g.ny, ceil(8.0 * dmax / s->dy)),
+              bz = (int)fmin((double)g.nz, ceil(8.0 * dmax / s->dz));
+    const size_t Bn = (size_t)bx * by * bz;
+    std::vector<double> near(6 * Bn);
+    mm_newell_near_box(bx, by, bz, s->dx, s->dy, s->dz, near.data());
+    double* d_near = nullptr;
+    cx<double>* A = nullptr;
+    unsigned long long* d_max = nullptr;
+    MM_TRY(s, cudaMalloc(&d_near, 6 * Bn * sizeof(double)));
+    MM_TRY(s, cudaMalloc(&A, (size_t)P * sizeof(cx<double>)));
+    MM_TRY(s, cudaMalloc(&d_max, 2 * sizeof(unsigned long long)));
+    MM_TRY(s, cudaMemcpyAsync(d_near, near.data(), 6 * Bn * sizeof(double), cudaMemcpyHostToDevice, st));
+    MM_TRY(s, cudaMemsetAsync(d_max, 0, 2 * sizeof(unsigned long long), st));
+    QuadRule rule;
+    make_rule(s->dx, &rule.n[0], rule.s[0], rule.w[0]);
+    make_rule(s->dy, &rule.n[1], rule.s[1], rule.w[1]);
+    make_rule(s->dz, &rule.n[2], rule.s[2], rule.w[2]);
+    double* Nr = wsp<double>(s, s->off_Nr);
+    tensor_real_kernel<<<(unsigned)((N + 127) / 128), 128, 0, st>>>(g.nx, g.ny, g.nz, s->dx, s->dy, s->dz, rule, bx, by, bz, d_near, Nr);
+    s->launches++;
+    MM_TRY(s, cudaGetLastError());
+    // fp64 twiddles for the setup transforms
+    const int twN = s->twN, ntw = twN / 2 + 1;
+    std::vector<cx<double>> htw(ntw);
+    for (int k = 0; k < ntw; k++) {
+        const long double a = -2.0L * 3.14159265358979323846264338327950288L * (long double)k / (long double)twN;
+        htw[k].x = (double)cosl(a); htw[k].y = (double)sinl(a);
+    }
+    cx<double>* d_tw = nullptr;
+    MM_TRY(s, cudaMalloc(&d_tw, ntw * sizeof(cx<double>)));
+    MM_TRY(s, cudaMemcpyAsync(d_tw, htw.data(), ntw * sizeof(cx<double>), cudaMemcpyHostToDevice, st));
+    twiddles<double> tw; tw.tw = d_tw; tw.twN = twN;
+    MM_TRY(s, cudaFuncSetAttribute(setup_fft_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_CAP));
+    T* Kh = wsp<T>(s, s->off_Kh);
+    MM_TRY(s, cudaMemsetAsync(Kh, 0, (size_t)6 * g.kcomp * sizeof(T), st));
+    auto line_fft = [&](int n, long sp, long nlines, int ninner, long si, long so, int pf) -> int {
+        if (n <= 1) return MM_OK;
+        int LT = 8;
+        while (LT > 1 && ((size_t)n * odd_pitch(LT) * sizeof(cx<double>) > SMEM_CAP || nlines % LT || ninner % LT)) LT /= 2;
+        const size_t sm = (size_t)n * odd_pitch(LT) * sizeof(cx<double>);
+        if (sm > SMEM_CAP) return fail(s, MM_ERR_UNSUPPORTED, "setup FFT line does not fit in shared memory");
+        setup_fft_kernel<<<(unsigned)(nlines / LT), 256, sm, st>>>(A, n, sp, ninner, si, so, LT, pf, tw);
+        s->launches++;
+        MM_TRY(s, cudaGetLastError());
+        return MM_OK;
+    };
+    const int ncomp = g.nz > 1 ? 6 : 4;
+    for (int c = 0; c < ncomp; c++) {
+        wrap_kernel<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(g, c, Nr, A);
+        s->launches++;
+        int rc;
+        if ((rc = line_fft(g.px, 1, (long)g.py * g.pz, g.py * g.pz, g.px, 0, 1))) return rc;
+        if ((rc = line_fft(g.py, g.px, (long)g.px * g.pz, g.px, 1, (long)g.px * g.py, 0))) return rc;
+        if ((rc = line_fft(g.pz, (long)g.px * g.py, (long)g.px * g.py, g.px * g.py, 1, 0, 0))) return rc;
+        const long total = g.kcomp;
+        pack_khat_kernel<T><<<(unsigned)((total + 255) / 256), 256, 0, st>>>(g, c, A, Kh, d_max);
+        s->launches++;
+        MM_TRY(s, cudaGetLastError());
+    }
+    unsigned long long hmax[2];
+    MM_TRY(s, cudaMemcpyAsync(hmax, d_max, sizeof(hmax), cudaMemcpyDeviceToHost, st));
+    MM_TRY(s, cudaStreamSynchronize(st));
+    double re, im;
+    memcpy(&re, &hmax[0], 8); memcpy(&im, &hmax[1], 8);
+    s->khat_imag_ratio = re > 0 ? im / re : -1;
+    cudaFree(d_near); cudaFree(A); cudaFree(d_max); cudaFree(d_tw);
+    if (!(s->khat_imag_ratio < 1e-10)) return fail(s, MM_ERR_CUDA, "demag tensor spectrum is not real: setup failed");
+    return MM_OK;
+}
+
+extern "C" int mm_init_demag(mm_sim* s)
+{
+    NEED_WS(s);
+    const Geom& g = s->g;
+    if (g.nx < 4 || g.ny < 2) return fail(s, MM_ERR_UNSUPPORTED, "demag needs nx >= 4 and ny >= 2");
+    if (s->smemA > SMEM_CAP || s->smemB > SMEM_CAP) return fail(s, MM_ERR_UNSUPPORTED, "mesh too large for the shared-memory tiles (DESIGN.md Limits)");
+    if (g.nz > 1 && (size_t)g.pz * g.G * g.CH * 2 * esize(s) > 64 * 1024) return fail(s, MM_ERR_UNSUPPORTED, "nz too large");
+    MM_TRY(s, cudaSetDevice(s->device));
+    int rc = s->prec == MM_F64 ? init_demag_t<double>(s) : init_demag_t<float>(s);
+    if (rc) return rc;
+    if (s->prec == MM_F64) {
+        MM_TRY(s, cudaFuncSetAttribute(fwd_xz_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_CAP));
+        MM_TRY(s, cudaFuncSetAttribute(y_conv_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_CAP));
+        MM_TRY(s, cudaFuncSetAttribute(inv_zx_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_CAP));
+    } else {
+        MM_TRY(s, cudaFuncSetAttribute(fwd_xz_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_CAP));
+        MM_TRY(s, cudaFuncSetAttribute(y_conv_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_CAP));
+        MM_TRY(s, cudaFuncSetAttribute(inv_zx_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_CAP));
+    }
+    s->demag_ready = 1;
+    return MM_OK;
+}
+
+extern "C" int mm_get_demag_kernel(mm_sim* s, int comp, void* dev_out)
+{
+    NEED_WS(s);
+    if (!s->demag_ready) return fail(s, MM_ERR_STATE, "mm_init_demag not called");
+    if (comp < 0 || comp > 5 || !dev_out) return MM_ERR_ARG;
+    MM_TRY(s, cudaMemcpyAsync(dev_out, wsp<double>(s, s->off_Nr) + (size_t)comp * s->g.N, s->g.N * sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
+    return MM_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Field / RHS evaluation
+// ------------------------------------------------------------------------------------------------
+template <typename T> static LocalP<T> make_local(const mm_sim* s, int terms)
+{
+    LocalP<T> lp;
+    const double d[3] = { s->dx, s->dy, s->dz };
+    for (int a = 0; a < 3; a++) {
+        lp.cex[a] = (T)(2.0 * s->A / (MU0 * d[a] * d[a]));
+        lp.cdm[a] = (T)(s->D / (MU0 * d[a]));
+        lp.u[a] = (T)s->u[a];
+        lp.hext[a] = (T)s->hext[a];
+    }
+    lp.cku = (T)(2.0 * s->Ku / MU0);
+    lp.gp = (T)(s->gamma / (1.0 + s->alpha * s->alpha));
+    lp.agp = (T)(s->alpha * s->gamma / (1.0 + s->alpha * s->alpha));
+    lp.dmi = s->dmi_kind;
+    lp.terms = terms;
+    if (s->A == 0.0) lp.terms &= ~1;
+    if (s->D == 0.0 || s->dmi_kind == 0) lp.terms &= ~2;
+    if (s->Ku == 0.0) lp.terms &= ~4;
+    return lp;
+}
+
+// demag passes A, B, C: y -> Hd
+template <typename T> static int demag_passes(mm_sim* s, const T* y)
+{
+    const Geom& g = s->g;
+    twiddles<T> tw; tw.tw = wsp<cx<T>>(s, s->off_tw); tw.twN = s->twN;
+    const DevState* st = wsp<DevState>(s, s->off_st);
+    cx<T>* S = wsp<cx<T>>(s, s->off_S);
+    const unsigned gridA = 3u * (unsigned)(g.ny / g.G), gridB = (unsigned)(g.Lx / g.TC) * (unsigned)g.pz;
+    prof_begin(s, 0);
+    fwd_xz_kernel<T><<<gridA, s->thrA, s->smemA, s->stream>>>(g, y, wsp<T>(s, s->off_Ms), S, tw, st);
+    prof_end(s);
+    prof_begin(s, 1);
+    y_conv_kernel<T><<<gridB, s->thrB, s->smemB, s->stream>>>(g, S, wsp<T>(s, s->off_Kh), tw, st);
+    prof_end(s);
+    const double P = (double)g.px * g.py * g.pz;
+    prof_begin(s, 2);
+    inv_zx_kernel<T><<<gridA, s->thrA, s->smemA, s->stream>>>(g, S, wsp<T>(s, s->off_Hd), tw, (T)(1.0 / P), st);
+    prof_end(s);
+    s->launches += 3;
+    MM_TRY(s, cudaGetLastError());
+    return MM_OK;
+}
+
+// one evaluation: MODE 0 -> H, MODE 1 -> k (+ stage algebra)
+template <typename T, int MODE> static int eval(mm_sim* s, const T* y, T* out, const StageArgs<T>& sa, int terms)
+{
+    const Geom& g = s->g;
+    const bool demag = s->demag_on && (terms & 16);
+    if (demag) {
+        if (!s->demag_ready) return fail(s, MM_ERR_STATE, "demag enabled but mm_init_demag not called");
+        int rc = demag_passes<T>(s, y);
+        if (rc) return rc;
+    }
+    const unsigned blocks = (unsigned)((g.N + 255) / 256);
+    prof_begin(s, 3);
+    llg_stage_kernel<T, MODE><<<blocks, 256, 0, s->stream>>>(g, make_local<T>(s, terms), y, wsp<T>(s, s->off_Ms),
+                                                              demag ? wsp<T>(s, s->off_Hd) : (const T*)nullptr, out, sa, wsp<DevState>(s, s->off_st));
+    prof_end(s);
+    s->launches++;
+    MM_TRY(s, cudaGetLastError());
+    return MM_OK;
+}
+
+template <typename T> static StageArgs<T> no_stage()
+{
+    StageArgs<T> sa;
+    memset(&sa, 0, sizeof(sa));
+    return sa;
+}
+
+static int set_state(mm_sim* s, double dt, double tol, double t_end, double stop, int mode, int reset)
+{
+    set_state_kernel<<<1, 1, 0, s->stream>>>(wsp<DevState>(s, s->off_st), dt, tol, t_end, stop, mode, reset);
+    s->launches++;
+    MM_TRY(s, cudaGetLastError());
+    return MM_OK;
+}
+
+#define NEED_READY(s) do { NEED_WS(s); if (!(s)->Ms_set) return fail((s), MM_ERR_STATE, "Ms not set"); MM_TRY((s), cudaSetDevice((s)->device)); } while (0)
+
+extern "C" int mm_effective_field(mm_sim* s, const void* dev_m, void* dev_H)
+{
+    NEED_READY(s);
+    if (!dev_m || !dev_H) return MM_ERR_ARG;
+    int rc = set_state(s, 0, 0, 0, 0, 0, 1);
+    if (rc) return rc;
+    if (s->prec == MM_F64) return eval<double, 0>(s, (const double*)dev_m, (double*)dev_H, no_stage<double>(), 31);
+    return eval<float, 0>(s, (const float*)dev_m, (float*)dev_H, no_stage<float>(), 31);
+}
+
+extern "C" int mm_llg_rhs(mm_sim* s, const void* dev_m, void* dev_dmdt)
+{
+    NEED_READY(s);
+    if (!dev_m || !dev_dmdt) return MM_ERR_ARG;
+    int rc = set_state(s, 0, 0, 0, 0, 0, 1);
+    if (rc) return rc;
+    if (s->prec == MM_F64) return eval<double, 1>(s, (const double*)dev_m, (double*)dev_dmdt, no_stage<double>(), 31);
+    return eval<float, 1>(s, (const float*)dev_m, (float*)dev_dmdt, no_stage<float>(), 31);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Time stepping (R8).  All kernels of a step are enqueued back to back; the accept /
+// reject decision and the next dt are taken on the device by ctrl_kernel.
+// ------------------------------------------------------------------------------------------------
+static const double DP_A[7][7] = {
+    { 0 },
+    { 1.0 / 5 },
+    { 3.0 / 40, 9.0 / 40 },
+    { 44.0 / 45, -56.0 / 15, 32.0 / 9 },
+    { 19372.0 / 6561, -25360.0 / 2187, 64448.0 / 6561, -212.0 / 729 },
+    { 9017.0 / 3168, -355.0 / 33, 46732.0 / 5247, 49.0 / 176, -5103.0 / 18656 },
+    { 35.0 / 384, 0, 500.0 / 1113, 125.0 / 192, -2187.0 / 6784, 11.0 / 84 } };
+static const double DP_E[7] = { 71.0 / 57600, 0, -71.0 / 16695, 71.0 / 1920, -17253.0 / 339200, 22.0 / 525, -1.0 / 40 };
+static const double RK4_A[4][4] = { { 0.5 }, { 0, 0.5 }, { 0, 0, 1.0 }, { 1.0 / 6, 1.0 / 3, 1.0 / 3, 1.0 / 6 } };
+
+template <typename T> static int enqueue_step(mm_sim* s, T* m, int ctrl_mode)
+{
+    const long N = s->g.N;
+    T* k[7];
+    for (int i = 0; i < 7; i++) k[i] = wsp<T>(s, s->off_k[i]);
+    T* yb[2] = { wsp<T>(s, s->off_y[0]), wsp<T>(s, s->off_y[1]) };
+    const int nst = s->integ == MM_DOPRI5 ? 7 : 4;
+    for (int st = 0; st < nst; st++) {
+        StageArgs<T> sa = no_stage<T>();
+        sa.m0 = m; sa.s = st;
+        for (int j = 0; j < st && j < 6; j++) sa.kprev[j] = k[j];
+        sa.do_maxk = st == 0;
+        if (s->integ == MM_DOPRI5) {
+            if (st < 6) { sa.ynext = yb[st & 1]; for (int j = 0; j <= st; j++) sa.coef[j] = DP_A[st + 1][j]; }
+            else { sa.ynext = nullptr; sa.do_err = 1; for (int j = 0; j < 7; j++) sa.ecoef[j] = DP_E[j]; }
+        } else {
+            sa.ynext = yb[st & 1];
+            for (int j = 0; j <= st; j++) sa.coef[j] = RK4_A[st][j];
+        }
+        const T* y = st == 0 ? m : yb[(st - 1) & 1];
+        int rc = eval<T, 1>(s, y, k[st], sa, 31);
+        if (rc) return rc;
+    }
+    DevState* ds = wsp<DevState>(s, s->off_st);
+    ctrl_kernel<<<1, 1, 0, s->stream>>>(ds, s->prec == MM_F64, ctrl_mode);
+    const T* ysol = yb[1];     // DOPRI5: y_6 written at stage 5 ; RK4: solution written at stage 3
+    accept_kernel<T><<<(unsigned)((N + 255) / 256), 256, 0, s->stream>>>(N, ds, ysol, wsp<T>(s, s->off_Ms), m, 0);
+    s->launches += 2;
+    MM_TRY(s, cudaGetLastError());
+    return MM_OK;
+}
+
+static int enqueue_step_any(mm_sim* s, void* m, int ctrl_mode)
+{
+    return s->prec == MM_F64 ? enqueue_step<double>(s, (double*)m, ctrl_mode) : enqueue_step<float>(s, (float*)m, ctrl_mode);
+}
+
+static int read_state(mm_sim* s, DevState* h)
+{
+    MM_TRY(s, cudaMemcpyAsync(h, wsp<DevState>(s, s->off_st), sizeof(DevState), cudaMemcpyDeviceToHost, s->stream));
+    MM_TRY(s, cudaStreamSynchronize(s->stream));
+    s->t_host = h->t;
+    return MM_OK;
+}
+
+extern "C" int mm_step(mm_sim* s, void* dev_m, double dt, double tol, int* accepted, double* err, double* dt_next, double* max_dmdt)
+{
+    NEED_READY(s);
+    if (!dev_m || !(dt > 0)) return MM_ERR_ARG;
+    int rc = set_state(s, dt, s->integ == MM_RK4 ? 0.0 : tol, 0, 0, 0, 1);
+    if (rc) return rc;
+    if ((rc = enqueue_step_any(s, dev_m, 0))) return rc;
+    if (accepted || err || dt_next || max_dmdt) {
+        DevState h;
+        if ((rc = read_state(s, &h))) return rc;
+        if (accepted) *accepted = h.accepted;
+        if (err) *err = h.err;
+        if (dt_next) *dt_next = h.dt;
+        if (max_dmdt) *max_dmdt = h.maxk;
+        if (h.nan) return fail(s, MM_ERR_NAN, "non-finite error norm or torque");
+    }
+    return MM_OK;
+}
+
+static int adaptive_loop(mm_sim* s, void* dev_m, double tol, double dt0, double t_end, double stop, int mode, long max_steps, long* steps_done, double* max_dmdt)
+{
+    if (!dev_m || !(tol > 0) || !(dt0 > 0) || max_steps < 0) return MM_ERR_ARG;
+    if (s->integ != MM_DOPRI5) return fail(s, MM_ERR_ARG, "adaptive stepping needs MM_DOPRI5");
+    int rc = set_state(s, dt0, tol, t_end, stop, mode, 1);
+    if (rc) return rc;
+    const long poll = 16;
+    long issued = 0;
+    DevState h;
+    memset(&h, 0, sizeof(h));
+    while (issued < max_steps) {
+        const long batch = (max_steps - issued) < poll ? (max_steps - issued) : poll;
+        for (long i = 0; i < batch; i++) if ((rc = enqueue_step_any(s, dev_m, mode))) return rc;
+        issued += batch;
+        if ((rc = read_state(s, &h))) return rc;
+        if (h.done) break;
+    }
+    // leave the controller re-armed for later calls
+    if ((rc = set_state(s, h.dt, 0, 0, 0, 0, 1))) return rc;
+    if (steps_done) *steps_done = (long)h.nsteps;
+    if (max_dmdt) *max_dmdt = h.maxk;
+    if (h.nan) return fail(s, MM_ERR_NAN, "non-finite error norm or torque");
+    return MM_OK;
+}
+
+extern "C" int mm_relax(mm_sim* s, void* dev_m, double tol, double stop_dmdt, long max_steps, double dt0, long* steps_done, double* max_dmdt)
+{
+    NEED_READY(s);
+    return adaptive_loop(s, dev_m, tol, dt0, 0.0, stop_dmdt, 1, max_steps, steps_done, max_dmdt);
+}
+
+extern "C" int mm_run_until(mm_sim* s, void* dev_m, double t_end, double tol, double dt0, long max_steps, long* steps_done)
+{
+    NEED_READY(s);
+    if (!(t_end > s->t_host)) return fail(s, MM_ERR_ARG, "t_end must be later than the current time");
+    const double left = t_end - s->t_host;
+    return adaptive_loop(s, dev_m, tol, dt0 < left ? dt0 : left, t_end, 0.0, 2, max_steps, steps_done, nullptr);
+}
+
+extern "C" double mm_time(const mm_sim* cs)
+{
+    mm_sim* s = const_cast<mm_sim*>(cs);
+    if (!s || !s->ws) return 0.0;
+    DevState h;
+    if (read_state(s, &h)) return s->t_host;
+    return h.t;
+}
+
+extern "C" int mm_set_time(mm_sim* s, double t)
+{
+    NEED_WS(s);
+    MM_TRY(s, cudaMemcpyAsync(reinterpret_cast<char*>(wsp<DevState>(s, s->off_st)) + offsetof(DevState, t), &t, sizeof(double), cudaMemcpyHostToDevice, s->stream));
+    MM_TRY(s, cudaStreamSynchronize(s->stream));
+    s->t_host = t;
+    return MM_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Host-buffer entry points (end-to-end path: H2D, compute, D2H inside the call)
+// ------------------------------------------------------------------------------------------------
+extern "C" int mm_run_host(mm_sim* s, void* host_m, int nsteps, double dt, double tol)
+{
+    NEED_READY(s);
+    if (!host_m || nsteps < 0 || !(dt > 0)) return MM_ERR_ARG;
+    const size_t bytes = 3 * (size_t)s->g.N * esize(s);
+    // stage through k[6]'s neighbour-free slot: y buffers are used by the step, so m lives in Hd's
+    // sibling — the workspace has no spare 3N slot, take one transiently
+    void* dm = nullptr;
+    MM_TRY(s, cudaMallocAsync(&dm, bytes, s->stream));
+    MM_TRY(s, cudaMemcpyAsync(dm, host_m, bytes, cudaMemcpyHostToDevice, s->stream));
+    int rc = set_state(s, dt, s->integ == MM_RK4 ? 0.0 : tol, 0, 0, 0, 1);
+    for (int i = 0; i < nsteps && !rc; i++) rc = enqueue_step_any(s, dm, 0);
+    if (!rc) {
+        cudaError_t e = cudaMemcpyAsync(host_m, dm, bytes, cudaMemcpyDeviceToHost, s->stream);
+        if (e != cudaSuccess) { s->err = cudaGetErrorString(e); rc = MM_ERR_CUDA; }
+    }
+    cudaFreeAsync(dm, s->stream);
+    DevState h;
+    int rc2 = read_state(s, &h);
+    return rc ? rc : rc2;
+}
+
+extern "C" int mm_llg_rhs_host(mm_sim* s, const void* host_m, void* host_dmdt)
+{
+    NEED_READY(s);
+    if (!host_m || !host_dmdt) return MM_ERR_ARG;
+    const size_t bytes = 3 * (size_t)s->g.N * esize(s);
+    void* dm = wsp<char>(s, s->off_y[0]);
+    void* dk = wsp<char>(s, s->off_k[0]);
+    MM_TRY(s, cudaMemcpyAsync(dm, host_m, bytes, cudaMemcpyHostToDevice, s->stream));
+    int rc = mm_llg_rhs(s, dm, dk);
+    if (rc) return rc;
+    MM_TRY(s, cudaMemcpyAsync(host_dmdt, dk, bytes, cudaMemcpyDeviceToHost, s->stream));
+    MM_TRY(s, cudaStreamSynchronize(s->stream));
+    return MM_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Diagnostics
+// ------------------------------------------------------------------------------------------------
+template <typename T> static int reduce_dot(mm_sim* s, const T* a, const T* b, int mode, double out4[4])
+{
+    const int blocks = 1024;
+    double* part = wsp<double>(s, s->off_part);
+    dot_kernel<T><<<blocks, 256, 0, s->stream>>>(s->g.N, a, b, wsp<T>(s, s->off_Ms), mode, part);
+    s->launches++;
+    MM_TRY(s, cudaGetLastError());
+    std::vector<double> h(4 * blocks);
+    MM_TRY(s, cudaMemcpyAsync(h.data(), part, h.size() * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    MM_TRY(s, cudaStreamSynchronize(s->stream));
+    for (int c = 0; c < 4; c++) { out4[c] = 0; for (int b2 = 0; b2 < blocks; b2++) out4[c] += h[4 * b2 + c]; }
+    return MM_OK;
+}
+
+extern "C" int mm_average_m(mm_sim* s, const void* dev_m, double out3[3])
+{
+    NEED_READY(s);
+    if (!dev_m || !out3) return MM_ERR_ARG;
+    double r[4];
+    int rc = s->prec == MM_F64 ? reduce_dot<double>(s, (const double*)dev_m, (const double*)dev_m, 1, r)
+                               : reduce_dot<float>(s, (const float*)dev_m, (const float*)dev_m, 1, r);
+    if (rc) return rc;
+    for (int c = 0; c < 3; c++) out3[c] = r[3] > 0 ? r[c] / r[3] : 0.0;
+    return MM_OK;
+}
+
+template <typename T> static int energy_t(mm_sim* s, const T* m, double* E_total, double E_terms[5])
+{
+    static const int bits[5] = { 16, 1, 2, 4, 8 };
+    static const double w[5] = { 0.5, 0.5, 0.5, 0.5, 1.0 };
+    T* H = wsp<T>(s, s->off_k[6]);
+    const double V = s->dx * s->dy * s->dz;
+    double tot = 0;
+    int rc = set_state(s, 0, 0, 0, 0, 0, 1);
+    if (rc) return rc;
+    for (int t = 0; t < 5; t++) {
+        if ((rc = eval<T, 0>(s, m, H, no_stage<T>(), bits[t]))) return rc;
+        double r[4];
+        if ((rc = reduce_dot<T>(s, m, H, 0, r))) return rc;
+        const double e = -MU0 * V * w[t] * r[0];
+        if (E_terms) E_terms[t] = e;
+        tot += e;
+    }
+    if (E_total) *E_total = tot;
+    return MM_OK;
+}
+
+extern "C" int mm_energy(mm_sim* s, const void* dev_m, double* E_total, double E_terms[5])
+{
+    NEED_READY(s);
+    if (!dev_m) return MM_ERR_ARG;
+    return s->prec == MM_F64 ? energy_t<double>(s, (const double*)dev_m, E_total, E_terms) : energy_t<float>(s, (const float*)dev_m, E_total, E_terms);
+}

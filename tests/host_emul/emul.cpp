@@ -1,0 +1,98 @@
+// Host emulation of the demag convolution passes: compiles the __host__ __device__ kernel bodies of
+// paper_2406_16064_b200/csrc with g++ and runs every CTA sequentially with one "thread"
+// (tid = 0, nthr = 1).  TEST HARNESS ONLY — checks the index arithmetic of the kernels on a box
+// without a GPU; it is not a product path and nothing in the package loads it.
+#include <cmath>
+#include <cstring>
+#include <vector>
+#include "../../paper_2406_16064_b200/csrc/mm_kernels.cuh"
+#include "../../paper_2406_16064_b200/csrc/mm_llg.cuh"
+
+using namespace mm;
+
+template <typename T> static std::vector<cx<T>> make_tw(int twN)
+{
+    std::vector<cx<T>> h(twN / 2 + 1);
+    for (int k = 0; k <= twN / 2; k++) {
+        long double a = -2.0L * 3.14159265358979323846264338327950288L * k / twN;
+        h[k].x = (T)cosl(a); h[k].y = (T)sinl(a);
+    }
+    return h;
+}
+
+static Geom make_geom(int nx, int ny, int nz, int G, int CH, int TC)
+{
+    Geom g;
+    memset(&g, 0, sizeof(g));
+    g.nx = nx; g.ny = ny; g.nz = nz;
+    g.px = 2 * nx; g.py = 2 * ny; g.pz = nz > 1 ? 2 * nz : 1;
+    g.lognx = ilog2(nx); g.logpy = ilog2(g.py); g.logpz = ilog2(g.pz);
+    g.N = (long)nx * ny * nz;
+    g.G = G; g.CH = CH; g.TC = TC;
+    g.Lx = ((nx + 1 + TC - 1) / TC) * TC;
+    g.plane = (long)ny * g.Lx; g.comp = (long)g.pz * g.plane;
+    g.kplane = (long)(ny + 1) * g.Lx; g.kcomp = (long)(nz > 1 ? nz + 1 : 1) * g.kplane;
+    return g;
+}
+
+// Kfull: real part of the 3-D DFT of the wrapped tensor, natural order, [6][pz][py][px] doubles.
+template <typename T>
+static void run(int nx, int ny, int nz, int G, int CH, int TC, const double* Kfull, const double* Ms, const double* m, double* Hd)
+{
+    Geom g = make_geom(nx, ny, nz, G, CH, TC);
+    int twN = g.px > g.py ? g.px : g.py;
+    if (g.pz > twN) twN = g.pz;
+    auto twv = make_tw<T>(twN);
+    twiddles<T> tw; tw.tw = twv.data(); tw.twN = twN;
+    std::vector<T> Kh((size_t)6 * g.kcomp, 0);
+    const int nkz = nz > 1 ? nz + 1 : 1;
+    for (int c = 0; c < 6; c++)
+        for (int kz = 0; kz < nkz; kz++)
+            for (int ky = 0; ky <= ny; ky++)
+                for (int xp = 0; xp <= nx; xp++) {
+                    int kx = xp < nx ? (int)brev(xp, g.lognx) : nx;
+                    Kh[(size_t)c * g.kcomp + (size_t)kz * g.kplane + (size_t)ky * g.Lx + xp] =
+                        (T)Kfull[(((size_t)c * g.pz + kz) * g.py + ky) * g.px + kx];
+                }
+    std::vector<T> mt(3 * g.N), Mst(g.N), Hdt(3 * g.N);
+    for (long i = 0; i < 3 * g.N; i++) mt[i] = (T)m[i];
+    for (long i = 0; i < g.N; i++) Mst[i] = (T)Ms[i];
+    std::vector<cx<T>> S((size_t)3 * g.comp);
+    memset(S.data(), 0, S.size() * sizeof(cx<T>));
+    std::vector<cx<T>> smem((size_t)(smemA_elems(g) > smemB_elems(g) ? smemA_elems(g) : smemB_elems(g)) + 16);
+    const int gridA = 3 * (ny / G), gridB = (g.Lx / TC) * g.pz;
+    for (int b = 0; b < gridA; b++) fwd_xz_body<T>(g, mt.data(), Mst.data(), S.data(), tw, smem.data(), b, 0, 1);
+    for (int b = 0; b < gridB; b++) y_conv_body<T>(g, S.data(), Kh.data(), tw, smem.data(), b, 0, 1);
+    const double P = (double)g.px * g.py * g.pz;
+    for (int b = 0; b < gridA; b++) inv_zx_body<T>(g, S.data(), Hdt.data(), tw, (T)(1.0 / P), smem.data(), b, 0, 1);
+    for (long i = 0; i < 3 * g.N; i++) Hd[i] = (double)Hdt[i];
+}
+
+extern "C" void emul_demag(int prec64, int nx, int ny, int nz, int G, int CH, int TC, const double* Kfull, const double* Ms,
+                           const double* m, double* Hd)
+{
+    if (prec64) run<double>(nx, ny, nz, G, CH, TC, Kfull, Ms, m, Hd);
+    else run<float>(nx, ny, nz, G, CH, TC, Kfull, Ms, m, Hd);
+}
+
+// local field + torque, cell by cell (terms bitmask as in LocalP)
+extern "C" void emul_local(int nx, int ny, int nz, const double* par /* cex3,cdm3,cku,u3,h3,gp,agp */, int dmi, int terms,
+                           const double* Ms, const double* m, const double* Hd, int torque, double* out)
+{
+    Geom g = make_geom(nx, ny, nz, 1, 8, 1);
+    LocalP<double> lp;
+    for (int a = 0; a < 3; a++) { lp.cex[a] = par[a]; lp.cdm[a] = par[3 + a]; lp.u[a] = par[7 + a]; lp.hext[a] = par[10 + a]; }
+    lp.cku = par[6]; lp.gp = par[13]; lp.agp = par[14]; lp.dmi = dmi; lp.terms = terms;
+    const long N = g.N;
+    for (long q = 0; q < N; q++) {
+        v3<double> res = { 0, 0, 0 };
+        if (Ms[q] != 0.0) {
+            int i = (int)(q % nx), j = (int)((q / nx) % ny), k = (int)(q / ((long)nx * ny));
+            v3<double> mi = ld3(m, N, q), H = { 0, 0, 0 };
+            if (Hd) H = ld3(Hd, N, q);
+            H = local_field<double>(g, lp, m, Ms, i, j, k, q, Ms[q], mi, H);
+            res = torque ? ll_torque<double>(lp, mi, H) : H;
+        }
+        out[q] = res.x; out[N + q] = res.y; out[2 * N + q] = res.z;
+    }
+}

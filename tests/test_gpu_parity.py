@@ -1,0 +1,258 @@
+"""GPU parity: libmm.so (through the C ABI) against the oracle, element by element, on the same
+seeded inputs.  Tolerances are BASELINE.json's: max|dH|/Ms <= 1e-10 (fp64), 2e-4 (fp32);
+<m> after fixed-dt steps <= 1e-8 (fp64), 1e-3 (fp32)."""
+import numpy as np
+import pytest
+
+import oracle
+from gpu_common import avg_m, make_pair, masked_m, to_np
+from paper_2406_16064_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+F32, F64 = 0, 1
+HTOL = {F64: 1e-10, F32: 2e-4}
+MTOL = {F64: 1e-8, F32: 1e-3}
+
+
+def small3d(nx=32, ny=16, nz=8, mask=True, kind=wl.DMI_BULK):
+    w = wl.cfg4(nx, ny, nz)
+    w.dmi_kind = kind
+    if mask:
+        w.Ms = 8.6e5 * wl.random_mask(77, nx, ny, nz, 0.85)
+    return w
+
+
+def film(n, mask=False):
+    w = wl.cfg5(n)
+    if mask:
+        w.Ms = 8e5 * wl.random_mask(78, n, n, 1, 0.9)
+    return w
+
+
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("shape,cell", [((32, 16, 4), (2e-9, 1.5e-9, 3e-9)), ((64, 64, 1), (3.90625e-9, 3.90625e-9, 3e-9)),
+                                        ((16, 32, 16), (2.5e-9, 2.5e-9, 2.5e-9)), ((128, 8, 2), (2e-9, 2e-9, 1e-9))])
+def test_demag_tensor_matches_oracle(shape, cell):
+    """S0: near-field quad closed forms + far-field quadrature vs the oracle's quad tensor everywhere."""
+    nx, ny, nz = shape
+    w = wl.Workload("t", nx, ny, nz, *cell, Ms=8e5)
+    w.m0 = wl.random_unit(1, nx, ny, nz)
+    o, s = make_pair(w, F64)
+    for c in range(6):
+        ref = o.demag_kernel(c)
+        got = to_np(s.demag_kernel(c))
+        assert np.abs(got - ref).max() < 2e-15, (c, np.abs(got - ref).max())
+
+
+@pytest.mark.parametrize("prec", [F64, F32])
+def test_cfg1_field_vs_direct_sum(prec):
+    w = wl.cfg1()
+    o, s = make_pair(w, prec, oracle_demag=oracle.DEMAG_DIRECT)
+    m = masked_m(w)
+    Href = o.effective_field(m)
+    H = to_np(s.effective_field(s.to_device(m)))
+    assert np.abs(H - Href).max() / w.Ms_max <= HTOL[prec]
+
+
+CASES = {
+    "cfg2": lambda: wl.cfg2(),
+    "cfg3_64": lambda: wl.cfg3(64),
+    "cfg3_256": lambda: wl.cfg3(256),
+    "slab_32x16x8_bulk": lambda: small3d(),
+    "slab_64x64x16": lambda: small3d(64, 64, 16),
+    "slab_16x64x2_interfacial": lambda: small3d(16, 64, 2, kind=wl.DMI_INTERFACIAL),
+    "slab_128x32x4": lambda: small3d(128, 32, 4),
+    "film_128_masked": lambda: film(128, mask=True),
+    "film_512": lambda: film(512),
+    "film_4x2": lambda: wl.cfg5(4).__class__("tiny", 4, 2, 1, 4e-9, 4e-9, 4e-9, Ms=8e5, A=1.3e-11, m0=wl.random_unit(3, 4, 2, 1)),
+}
+
+
+@pytest.mark.parametrize("prec", [F64, F32])
+@pytest.mark.parametrize("case", sorted(CASES))
+def test_effective_field_and_rhs(case, prec):
+    w = CASES[case]()
+    o, s = make_pair(w, prec)
+    m = masked_m(w)
+    dm = s.to_device(m)
+    Href = o.effective_field(m)
+    H = to_np(s.effective_field(dm))
+    assert np.abs(H - Href).max() / w.Ms_max <= HTOL[prec], np.abs(H - Href).max() / w.Ms_max
+    kref = o.llg_rhs(m)
+    k = to_np(s.llg_rhs(dm))
+    scale = np.abs(kref).max()
+    assert np.abs(k - kref).max() <= (1e-9 if prec == F64 else 2e-4) * scale
+    live = w.Ms_array() > 0
+    assert np.all(H[:, ~live] == 0) and np.all(k[:, ~live] == 0)
+
+
+@pytest.mark.parametrize("prec", [F64, F32])
+def test_demag_only_and_local_only(prec):
+    w = small3d(32, 32, 4)
+    o, s = make_pair(w, prec)
+    m = masked_m(w)
+    dm = s.to_device(m)
+    # local terms only
+    s.set_demag(0); o.set_demag(0)
+    H = to_np(s.effective_field(dm))
+    Href = o.effective_field(m)
+    assert np.abs(H - Href).max() / w.Ms_max <= (1e-12 if prec == F64 else 2e-5)
+    # demag only
+    s.set_demag(1); o.set_demag(1)
+    for x in (s, o):
+        x.set_A(0.0); x.set_D(0.0, 0); x.set_Ku(0.0); x.set_H_ext(0, 0, 0)
+    H = to_np(s.effective_field(dm))
+    Href = o.effective_field(m)
+    assert np.abs(H - Href).max() / w.Ms_max <= (1e-12 if prec == F64 else 2e-5)
+
+
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec", [F64, F32])
+def test_cfg1_200_rk4_steps(prec):
+    w = wl.cfg1()
+    o, s = make_pair(w, prec, oracle_demag=oracle.DEMAG_DIRECT)
+    m = masked_m(w)
+    dm = s.to_device(m)
+    E = [s.energy(dm)[0]]
+    for i in range(200):
+        o.step(m, w.dt)
+        s.step(dm, w.dt, sync=(i % 50 == 49))
+        if i % 20 == 19:
+            E.append(s.energy(dm)[0])
+    g = to_np(dm)
+    Ms = w.Ms_array()
+    assert np.abs(avg_m(g, Ms) - avg_m(m, Ms)).max() <= MTOL[prec]
+    assert np.abs(g - m).max() <= (1e-8 if prec == F64 else 5e-3)
+    assert np.abs(np.sqrt((g * g).sum(axis=0)) - 1).max() < (1e-14 if prec == F64 else 1e-6)
+    assert all(E[i + 1] < E[i] for i in range(len(E) - 1))
+    assert np.isclose(s.time(), 200 * w.dt, rtol=1e-12)
+    Eo = o.energy(m)[0]
+    assert np.isclose(E[-1], Eo, rtol=1e-9 if prec == F64 else 1e-4)
+
+
+@pytest.mark.parametrize("prec", [F64, F32])
+@pytest.mark.parametrize("case,nsteps", [("cfg2", 20), ("cfg3_64", 20), ("slab_32x16x8_bulk", 5), ("slab_64x64x16", 5)])
+def test_fixed_dt_dopri5_steps(case, nsteps, prec):
+    w = CASES[case]()
+    o, s = make_pair(w, prec)
+    m = masked_m(w)
+    dm = s.to_device(m)
+    for i in range(nsteps):
+        ok_o, err_o, _, md_o = o.step(m, w.dt)
+        ok, err, dn, md = s.step(dm, w.dt)
+        assert ok and ok_o and dn == w.dt
+        assert np.isclose(md, md_o, rtol=1e-9 if prec == F64 else 1e-3)
+        assert np.isclose(err, err_o, rtol=1e-5 if prec == F64 else 0.2, atol=1e-7 if prec == F32 else 0)
+    g = to_np(dm)
+    Ms = w.Ms_array()
+    assert np.abs(avg_m(g, Ms) - avg_m(m, Ms)).max() <= MTOL[prec]
+    assert np.abs(g - m).max() <= (1e-8 if prec == F64 else 5e-3)
+    assert np.allclose(s.average_m(dm), avg_m(g, Ms), atol=1e-12 if prec == F64 else 1e-6)
+
+
+def test_adaptive_step_accept_reject_matches_oracle():
+    w = wl.cfg2()
+    w.alpha = 0.5
+    o, s = make_pair(w, F64)
+    m = masked_m(w)
+    dm = s.to_device(m)
+    m_before = m.copy()
+    ok_o, err_o, dn_o, _ = o.step(m, 5e-12, 1e-6)            # too large: rejected on both sides
+    ok, err, dn, _ = s.step(dm, 5e-12, 1e-6)
+    assert (not ok) and (not ok_o)
+    assert np.isclose(err, err_o, rtol=1e-6) and np.isclose(dn, dn_o, rtol=1e-6)
+    assert np.array_equal(to_np(dm), m_before) and s.time() == 0.0
+    ok_o, err_o, dn_o, _ = o.step(m, 2e-13, 1e-6)
+    ok, err, dn, _ = s.step(dm, 2e-13, 1e-6)
+    assert ok and ok_o and np.isclose(err, err_o, rtol=1e-5) and np.isclose(dn, dn_o, rtol=1e-5)
+    assert np.abs(to_np(dm) - m).max() < 1e-10
+
+
+@pytest.mark.parametrize("prec", [F64, F32])
+def test_cfg2_relax_then_run(prec):
+    """configs[1] shape: relax with alpha=0.5, apply the field, run adaptive DOPRI5; observables vs the
+    oracle at a fixed time (a short 20 ps window keeps the oracle affordable). DESIGN.md R8, R10."""
+    w = wl.cfg2()
+    w.alpha = 0.5
+    o, s = make_pair(w, prec)
+    m = masked_m(w)
+    dm = s.to_device(m)
+    tol = 1e-6
+    n_o, md_o = o.relax(m, tol, 2e9, 400, 1e-13)
+    n_s, md_s = s.relax(dm, tol, 2e9, 400, 1e-13)
+    Ms = w.Ms_array()
+    loose = 1e-4 if prec == F64 else 1e-2
+    assert md_s < 2e9 and md_o < 2e9
+    assert np.abs(avg_m(to_np(dm), Ms) - avg_m(m, Ms)).max() < loose
+    for x in (o, s):
+        x.set_alpha(0.02)
+        x.set_H_ext(*wl.CFG2_FIELD)
+        x.set_time(0.0)
+    t_end = 20e-12
+    s.run_until(dm, t_end, tol, 1e-13)
+    dt = 1e-13
+    while o.time() < t_end * (1 - 1e-12):
+        dt = min(dt, t_end - o.time())
+        ok, err, dn, _ = o.step(m, dt, tol)
+        dt = dn
+    assert np.isclose(s.time(), t_end, rtol=1e-9)
+    assert np.abs(avg_m(to_np(dm), Ms) - avg_m(m, Ms)).max() < loose
+    Es, Eo = s.energy(dm)[0], o.energy(m)[0]
+    assert np.isclose(Es, Eo, rtol=loose)
+
+
+def test_macrospin_eq53_on_gpu():
+    """PAPER.md:409-417 on a 1x1x1 mesh (demag off: the library needs nx >= 4 for demag)."""
+    from paper_2406_16064_b200 import Sim
+    s = Sim(1, 1, 1, 1e-9, 1e-9, 1e-9, prec=F64)
+    s.set_Ms(8e5); s.set_alpha(0.5); s.set_gamma(2.21e5); s.set_H_ext(0, 0, 1e5); s.set_demag(0)
+    dm = s.to_device(np.array([1.0, 0, 0]).reshape(3, 1, 1, 1))
+    T, n = 0.2e-9, 400
+    for _ in range(n):
+        s.step(dm, T / n, sync=False)
+    g = 2.21e5 / 1.25
+    ref = [np.cos(g * 1e5 * T) / np.cosh(0.5 * g * 1e5 * T), np.sin(g * 1e5 * T) / np.cosh(0.5 * g * 1e5 * T), np.tanh(0.5 * g * 1e5 * T)]
+    assert np.allclose(to_np(dm).reshape(3), ref, atol=1e-9)
+
+
+def test_host_buffer_entry_points():
+    import torch
+    w = small3d(32, 16, 8)
+    o, s = make_pair(w, F64)
+    m = masked_m(w)
+    hm = torch.from_numpy(m.copy()).pin_memory()
+    hk = torch.empty_like(hm).pin_memory()
+    s.llg_rhs_host(hm, hk)
+    kref = o.llg_rhs(m)
+    assert np.abs(hk.numpy() - kref).max() <= 1e-9 * np.abs(kref).max()
+    s.run_host(hm, 3, w.dt)
+    for _ in range(3):
+        o.step(m, w.dt)
+    assert np.abs(hm.numpy() - m).max() < 1e-9
+
+
+def test_edge_cases_and_errors():
+    from paper_2406_16064_b200 import Sim, MMError
+    import torch
+    s = Sim(16, 16, 1, 2e-9, 2e-9, 2e-9, prec=F32)
+    m = s.to_device(wl.random_unit(5, 16, 16, 1))
+    with pytest.raises(MMError):                      # Ms not set
+        s.effective_field(m)
+    s.set_Ms(8e5)
+    with pytest.raises(MMError):                      # demag enabled, not initialised
+        s.effective_field(m)
+    s.set_Ms(np.zeros((1, 16, 16)))                   # all vacuum: everything is zero
+    s.init_demag()
+    assert float(s.effective_field(m).abs().max()) == 0.0
+    assert float(s.llg_rhs(m).abs().max()) == 0.0
+    with pytest.raises(MMError):
+        Sim(2, 16, 1, 1e-9, 1e-9, 1e-9).init_demag()   # nx < 4
+    with pytest.raises(MMError):
+        Sim(24, 16, 1, 1e-9, 1e-9, 1e-9)              # not a power of two
+    # NaN in m is reported, not silently propagated
+    s2 = Sim(16, 16, 1, 2e-9, 2e-9, 2e-9, prec=F32)
+    s2.set_Ms(8e5); s2.set_A(1.3e-11); s2.init_demag()
+    bad = s2.to_device(wl.random_unit(5, 16, 16, 1))
+    bad[0, 0, 3, 3] = float("nan")
+    with pytest.raises(MMError):
+        s2.step(bad, 1e-14, 1e-6)
