@@ -218,3 +218,171 @@ MM_HD void fft_inv_blocks(cx<T>* s, int pitch, int nlines, int n, int m, twiddle
 }
 
 }  // namespace mm
+
+// ================================================================================================
+// v2 building blocks: V-wide column vectors (16-byte shared/global accesses for fp32), radix
+// kernels on any element type, shift/mask index arithmetic.
+// ================================================================================================
+namespace mm {
+
+template <typename T, int V> struct alignas(V * 2 * sizeof(T)) cvec {
+    cx<T> e[V];
+};
+template <typename T, int V> MM_HD cvec<T, V> operator+(cvec<T, V> a, cvec<T, V> b)
+{
+    cvec<T, V> r;
+#pragma unroll
+    for (int k = 0; k < V; k++) r.e[k] = a.e[k] + b.e[k];
+    return r;
+}
+template <typename T, int V> MM_HD cvec<T, V> operator-(cvec<T, V> a, cvec<T, V> b)
+{
+    cvec<T, V> r;
+#pragma unroll
+    for (int k = 0; k < V; k++) r.e[k] = a.e[k] - b.e[k];
+    return r;
+}
+template <typename T, int V> MM_HD cvec<T, V> cmul(cvec<T, V> a, cx<T> w)
+{
+    cvec<T, V> r;
+#pragma unroll
+    for (int k = 0; k < V; k++) r.e[k] = cmul(a.e[k], w);
+    return r;
+}
+template <typename T, int V> MM_HD cvec<T, V> cmulc(cvec<T, V> a, cx<T> w)
+{
+    cvec<T, V> r;
+#pragma unroll
+    for (int k = 0; k < V; k++) r.e[k] = cmulc(a.e[k], w);
+    return r;
+}
+template <typename T, int V> MM_HD cvec<T, V> mul_mi(cvec<T, V> a)
+{
+    cvec<T, V> r;
+#pragma unroll
+    for (int k = 0; k < V; k++) r.e[k] = mul_mi(a.e[k]);
+    return r;
+}
+template <typename T, int V> MM_HD cvec<T, V> mul_pi(cvec<T, V> a)
+{
+    cvec<T, V> r;
+#pragma unroll
+    for (int k = 0; k < V; k++) r.e[k] = mul_pi(a.e[k]);
+    return r;
+}
+// multiplication by a compile-time-known constant (c + i s)
+template <typename T> MM_HD cx<T> crot(cx<T> a, T c, T s) { return mk<T>(c * a.x - s * a.y, c * a.y + s * a.x); }
+template <typename T, int V> MM_HD cvec<T, V> crot(cvec<T, V> a, T c, T s)
+{
+    cvec<T, V> r;
+#pragma unroll
+    for (int k = 0; k < V; k++) r.e[k] = crot(a.e[k], c, s);
+    return r;
+}
+template <typename T> struct scalar_of;
+template <typename T> struct scalar_of<cx<T>> { typedef T type; };
+template <typename T, int V> struct scalar_of<cvec<T, V>> { typedef T type; };
+
+template <typename E> MM_HD void bfe(E& a, E& b) { E t = a; a = t + b; b = t - b; }
+
+// Radix kernels on element type E (cx<T> or cvec<T,V>): fwd = natural in, bit-reversed out; inv = adjoint.
+template <typename E, int R> struct rad;
+template <typename E> struct rad<E, 1> {
+    static MM_HD void fwd(E*) {}
+    static MM_HD void inv(E*) {}
+};
+template <typename E> struct rad<E, 2> {
+    static MM_HD void fwd(E* v) { bfe(v[0], v[1]); }
+    static MM_HD void inv(E* v) { bfe(v[0], v[1]); }
+};
+template <typename E> struct rad<E, 4> {
+    static MM_HD void fwd(E* v)
+    {
+        bfe(v[0], v[2]); bfe(v[1], v[3]); v[3] = mul_mi(v[3]);
+        bfe(v[0], v[1]); bfe(v[2], v[3]);
+    }
+    static MM_HD void inv(E* v)
+    {
+        bfe(v[0], v[1]); bfe(v[2], v[3]);
+        v[3] = mul_pi(v[3]); bfe(v[0], v[2]); bfe(v[1], v[3]);
+    }
+};
+template <typename E> struct rad<E, 8> {
+    typedef typename scalar_of<E>::type T;
+    static MM_HD void fwd(E* v)
+    {
+        const T c = (T)0.70710678118654752440;
+#pragma unroll
+        for (int r = 0; r < 4; r++) bfe(v[r], v[r + 4]);
+        v[5] = crot(v[5], c, -c); v[6] = mul_mi(v[6]); v[7] = crot(v[7], -c, -c);
+        rad<E, 4>::fwd(v); rad<E, 4>::fwd(v + 4);
+    }
+    static MM_HD void inv(E* v)
+    {
+        const T c = (T)0.70710678118654752440;
+        rad<E, 4>::inv(v); rad<E, 4>::inv(v + 4);
+        v[5] = crot(v[5], c, c); v[6] = mul_pi(v[6]); v[7] = crot(v[7], -c, c);
+#pragma unroll
+        for (int r = 0; r < 4; r++) bfe(v[r], v[r + 4]);
+    }
+};
+template <typename E> struct rad<E, 16> {
+    typedef typename scalar_of<E>::type T;
+    static MM_HD void fwd(E* v)
+    {
+        const T c1 = (T)0.92387953251128675613, s1 = (T)0.38268343236508977173, c = (T)0.70710678118654752440;
+#pragma unroll
+        for (int r = 0; r < 8; r++) bfe(v[r], v[r + 8]);
+        // * w16^r = exp(-i pi r / 8)
+        v[9] = crot(v[9], c1, -s1); v[10] = crot(v[10], c, -c); v[11] = crot(v[11], s1, -c1); v[12] = mul_mi(v[12]);
+        v[13] = crot(v[13], -s1, -c1); v[14] = crot(v[14], -c, -c); v[15] = crot(v[15], -c1, -s1);
+        rad<E, 8>::fwd(v); rad<E, 8>::fwd(v + 8);
+    }
+    static MM_HD void inv(E* v)
+    {
+        const T c1 = (T)0.92387953251128675613, s1 = (T)0.38268343236508977173, c = (T)0.70710678118654752440;
+        rad<E, 8>::inv(v); rad<E, 8>::inv(v + 8);
+        v[9] = crot(v[9], c1, s1); v[10] = crot(v[10], c, c); v[11] = crot(v[11], s1, c1); v[12] = mul_pi(v[12]);
+        v[13] = crot(v[13], -s1, c1); v[14] = crot(v[14], -c, c); v[15] = crot(v[15], -c1, s1);
+#pragma unroll
+        for (int r = 0; r < 8; r++) bfe(v[r], v[r + 8]);
+    }
+};
+template <typename E> struct rad<E, 32> {
+    typedef typename scalar_of<E>::type T;
+    static MM_HD void tw32(int r, T& c, T& s)   // exp(-i pi r / 16), r = 1..15
+    {
+        const T C[16] = { (T)1.0, (T)0.98078528040323044913, (T)0.92387953251128675613, (T)0.83146961230254523708,
+                          (T)0.70710678118654752440, (T)0.55557023301960222474, (T)0.38268343236508977173, (T)0.19509032201612826785,
+                          (T)0.0, (T)-0.19509032201612826785, (T)-0.38268343236508977173, (T)-0.55557023301960222474,
+                          (T)-0.70710678118654752440, (T)-0.83146961230254523708, (T)-0.92387953251128675613, (T)-0.98078528040323044913 };
+        c = C[r]; s = -C[(r + 8) & 15] * (r < 8 ? (T)-1 : (T)1);
+    }
+    static MM_HD void fwd(E* v)
+    {
+#pragma unroll
+        for (int r = 0; r < 16; r++) bfe(v[r], v[r + 16]);
+#pragma unroll
+        for (int r = 1; r < 16; r++) {
+            T c, s; tw32(r, c, s);
+            v[16 + r] = crot(v[16 + r], c, s);
+        }
+        rad<E, 16>::fwd(v); rad<E, 16>::fwd(v + 16);
+    }
+    static MM_HD void inv(E* v)
+    {
+        rad<E, 16>::inv(v); rad<E, 16>::inv(v + 16);
+#pragma unroll
+        for (int r = 1; r < 16; r++) {
+            T c, s; tw32(r, c, s);
+            v[16 + r] = crot(v[16 + r], c, -s);
+        }
+#pragma unroll
+        for (int r = 0; r < 16; r++) bfe(v[r], v[r + 16]);
+    }
+};
+
+// first radix of the v2 schedule for block length m >= 16: remainder first, then 8s
+MM_HD int first_radix(int m) { int r = m; while (r > 8) r >>= 3; return r; }
+
+}  // namespace mm

@@ -1,0 +1,440 @@
+// mm_kernels2.cuh — v2 bodies of the convolution passes: same math and memory layout as
+// mm_kernels.cuh (which stays as the fallback for tiny meshes), restructured for instruction
+// count and shared-memory traffic:
+//   * global loads / stores are fused into the first / last radix stage of each transform
+//     (zero-padding and cropping included), so the tile makes 8 shared-memory round trips in
+//     pass B instead of 16;
+//   * in pass B the last forward stage, the spectral 3x3 multiply (Eq. 8 in k-space,
+//     PAPER.md:138) and the first inverse stage run in registers on the three components of one
+//     column;
+//   * the z transform of passes A / C (nz <= 32) runs in registers, one thread per x position;
+//   * all index arithmetic is shifts and masks; twiddle powers are shared by the three components
+//     (pass B) or by a group of lines (passes A / C); pass B moves 16 bytes per shared-memory access.
+#pragma once
+#include "mm_fft.cuh"
+#include "mm_kernels.cuh"
+
+namespace mm {
+
+template <typename E, typename T> MM_HD E ldv(const cx<T>* p) { return *reinterpret_cast<const E*>(p); }
+template <typename E, typename T> MM_HD void stv(cx<T>* p, const E& v) { *reinterpret_cast<E*>(p) = v; }
+
+// ------------------------------------------------------------------------------------------------
+// Pass B v2
+// ------------------------------------------------------------------------------------------------
+// first stage: global load + zero-pad twiddle + radix R on both blocks
+template <typename T, int V, int R>
+MM_HD void yB_first(const Geom& g, const cx<T>* Sz, cx<T>* s, twiddles<T> tw, int tid, int nthr)
+{
+    typedef cvec<T, V> E;
+    const int TC = g.TC, LC = TC / V, logLC = ilog2(LC), pitch = 3 * TC;
+    const int m = g.ny, n = g.py, sub = m / R;
+    for (int f = tid; f < sub * LC; f += nthr) {
+        const int lc = f & (LC - 1), i = f >> logLC;
+        cx<T> pw[R], wp[R];
+        if (R > 1 && i != 0) twiddle_powers<T, R>(tw.get(i, m), pw);
+#pragma unroll
+        for (int r = 0; r < R; r++) wp[r] = tw.get(i + r * sub, n);
+#pragma unroll
+        for (int c = 0; c < 3; c++) {
+            const cx<T>* src = Sz + (long)c * g.comp + (long)i * g.Lx + lc * V;
+            cx<T>* dst = s + i * pitch + c * TC + lc * V;
+            E a[R], u[R];
+#pragma unroll
+            for (int r = 0; r < R; r++) a[r] = ldv<E, T>(src + (long)r * sub * g.Lx);
+#pragma unroll
+            for (int r = 0; r < R; r++) u[r] = cmul(a[r], wp[r]);
+            rad<E, R>::fwd(a);
+            rad<E, R>::fwd(u);
+            if (i != 0) {
+#pragma unroll
+                for (int r = 1; r < R; r++) { a[r] = cmul(a[r], pw[r]); u[r] = cmul(u[r], pw[r]); }
+            }
+#pragma unroll
+            for (int r = 0; r < R; r++) { stv<E, T>(dst + r * sub * pitch, a[r]); stv<E, T>(dst + (m + r * sub) * pitch, u[r]); }
+        }
+    }
+}
+
+// last stage: inverse radix R on both blocks + crop combine + global store
+template <typename T, int V, int R>
+MM_HD void yB_last(const Geom& g, cx<T>* Sz, const cx<T>* s, twiddles<T> tw, int tid, int nthr)
+{
+    typedef cvec<T, V> E;
+    const int TC = g.TC, LC = TC / V, logLC = ilog2(LC), pitch = 3 * TC;
+    const int m = g.ny, n = g.py, sub = m / R;
+    for (int f = tid; f < sub * LC; f += nthr) {
+        const int lc = f & (LC - 1), i = f >> logLC;
+        cx<T> pw[R], wp[R];
+        if (R > 1 && i != 0) twiddle_powers<T, R>(tw.get(i, m), pw);
+#pragma unroll
+        for (int r = 0; r < R; r++) wp[r] = tw.get(i + r * sub, n);
+#pragma unroll
+        for (int c = 0; c < 3; c++) {
+            cx<T>* dstg = Sz + (long)c * g.comp + (long)i * g.Lx + lc * V;
+            const cx<T>* src = s + i * pitch + c * TC + lc * V;
+            E a[R], u[R];
+#pragma unroll
+            for (int r = 0; r < R; r++) { a[r] = ldv<E, T>(src + r * sub * pitch); u[r] = ldv<E, T>(src + (m + r * sub) * pitch); }
+            if (i != 0) {
+#pragma unroll
+                for (int r = 1; r < R; r++) { a[r] = cmulc(a[r], pw[r]); u[r] = cmulc(u[r], pw[r]); }
+            }
+            rad<E, R>::inv(a);
+            rad<E, R>::inv(u);
+#pragma unroll
+            for (int r = 0; r < R; r++) stv<E, T>(dstg + (long)r * sub * g.Lx, a[r] + cmulc(u[r], wp[r]));
+        }
+    }
+}
+
+// middle radix-8 stage (DIR = 0 forward DIF, 1 inverse DIT) on blocks of length Lc over all n points
+template <typename T, int V, int DIR>
+MM_HD void yB_mid8(const Geom& g, cx<T>* s, int Lc, twiddles<T> tw, int tid, int nthr)
+{
+    typedef cvec<T, V> E;
+    const int TC = g.TC, LC = TC / V, logLC = ilog2(LC), pitch = 3 * TC;
+    const int n = g.py, sub = Lc >> 3, logsub = ilog2(sub);
+    for (int f = tid; f < (n >> 3) * LC; f += nthr) {
+        const int lc = f & (LC - 1), b = f >> logLC;
+        const int blk = b >> logsub, i = b & (sub - 1);
+        cx<T> pw[8];
+        if (i != 0) twiddle_powers<T, 8>(tw.get(i, Lc), pw);
+        cx<T>* base = s + (blk * Lc + i) * pitch + lc * V;
+#pragma unroll
+        for (int c = 0; c < 3; c++) {
+            cx<T>* p = base + c * TC;
+            E v[8];
+#pragma unroll
+            for (int r = 0; r < 8; r++) v[r] = ldv<E, T>(p + r * sub * pitch);
+            if (DIR == 0) {
+                rad<E, 8>::fwd(v);
+                if (i != 0) {
+#pragma unroll
+                    for (int r = 1; r < 8; r++) v[r] = cmul(v[r], pw[r]);
+                }
+            } else {
+                if (i != 0) {
+#pragma unroll
+                    for (int r = 1; r < 8; r++) v[r] = cmulc(v[r], pw[r]);
+                }
+                rad<E, 8>::inv(v);
+            }
+#pragma unroll
+            for (int r = 0; r < 8; r++) stv<E, T>(p + r * sub * pitch, v[r]);
+        }
+    }
+}
+
+// last forward radix-8 stage (Lc = 8) + multiply by K^ + first inverse stage, three components in registers
+template <typename T, bool IS3D>
+MM_HD void yB_mul8(const Geom& g, cx<T>* s, const T* Kz, T sz, twiddles<T> tw, int tid, int nthr)
+{
+    const int TC = g.TC, logTC = ilog2(TC), pitch = 3 * TC;
+    const int n = g.py, ny = g.ny;
+    for (int f = tid; f < (n >> 3) * TC; f += nthr) {
+        const int col = f & (TC - 1), b8 = f >> logTC;
+        cx<T>* p = s + (b8 * 8) * pitch + col;
+        cx<T> M[3][8];
+#pragma unroll
+        for (int c = 0; c < 3; c++) {
+#pragma unroll
+            for (int r = 0; r < 8; r++) M[c][r] = p[r * pitch + c * TC];
+            rad<cx<T>, 8>::fwd(M[c]);
+        }
+#pragma unroll
+        for (int r = 0; r < 8; r++) {
+            const int ky = (int)brev((unsigned)(b8 * 8 + r), g.logpy);
+            const int kyp = ky <= ny ? ky : n - ky;
+            const T sy = ky > ny ? (T)-1 : (T)1;
+            const T* Kp = Kz + (long)kyp * g.Lx + col;
+            const T kxx = Kp[0], kyy = Kp[g.kcomp], kzz = Kp[2 * g.kcomp], kxy = sy * Kp[3 * g.kcomp];
+            const cx<T> Mx = M[0][r], My = M[1][r], Mz = M[2][r];
+            if (IS3D) {
+                const T kxz = sz * Kp[4 * g.kcomp], kyz = sy * sz * Kp[5 * g.kcomp];
+                M[0][r] = mk<T>(-(kxx * Mx.x + kxy * My.x + kxz * Mz.x), -(kxx * Mx.y + kxy * My.y + kxz * Mz.y));
+                M[1][r] = mk<T>(-(kxy * Mx.x + kyy * My.x + kyz * Mz.x), -(kxy * Mx.y + kyy * My.y + kyz * Mz.y));
+                M[2][r] = mk<T>(-(kxz * Mx.x + kyz * My.x + kzz * Mz.x), -(kxz * Mx.y + kyz * My.y + kzz * Mz.y));
+            } else {
+                M[0][r] = mk<T>(-(kxx * Mx.x + kxy * My.x), -(kxx * Mx.y + kxy * My.y));
+                M[1][r] = mk<T>(-(kxy * Mx.x + kyy * My.x), -(kxy * Mx.y + kyy * My.y));
+                M[2][r] = mk<T>(-(kzz * Mz.x), -(kzz * Mz.y));
+            }
+        }
+#pragma unroll
+        for (int c = 0; c < 3; c++) {
+            rad<cx<T>, 8>::inv(M[c]);
+#pragma unroll
+            for (int r = 0; r < 8; r++) p[r * pitch + c * TC] = M[c][r];
+        }
+    }
+}
+
+// requires ny >= 16 (so the schedule has >= 2 stages and ends with radix 8) and TC % V == 0
+template <typename T, int V>
+MM_HD void y_conv_body2(const Geom g, cx<T>* __restrict__ S, const T* __restrict__ Kh, twiddles<T> tw, cx<T>* s,
+                        int bid, int tid, int nthr)
+{
+    const int ntile = g.Lx / g.TC;
+    const int x0 = (bid % ntile) * g.TC, zq = bid / ntile;
+    const int m = g.ny;
+    cx<T>* Sz = S + (long)zq * g.plane + x0;
+    const int R1 = first_radix(m);
+    if (R1 == 8) yB_first<T, V, 8>(g, Sz, s, tw, tid, nthr);
+    else if (R1 == 4) yB_first<T, V, 4>(g, Sz, s, tw, tid, nthr);
+    else yB_first<T, V, 2>(g, Sz, s, tw, tid, nthr);
+    MM_SYNC();
+    int Lc = m / R1;
+    for (; Lc > 8; Lc >>= 3) { yB_mid8<T, V, 0>(g, s, Lc, tw, tid, nthr); MM_SYNC(); }
+    const int kz = (int)brev((unsigned)zq, g.logpz);
+    const bool is3d = g.nz > 1;
+    const int kzp = is3d ? (kz <= g.nz ? kz : g.pz - kz) : 0;
+    const T sz = (is3d && kz > g.nz) ? (T)-1 : (T)1;
+    const T* Kz = Kh + (long)kzp * g.kplane + x0;
+    if (is3d) yB_mul8<T, true>(g, s, Kz, sz, tw, tid, nthr);
+    else yB_mul8<T, false>(g, s, Kz, sz, tw, tid, nthr);
+    MM_SYNC();
+    for (Lc = 64; Lc <= m / R1; Lc <<= 3) { yB_mid8<T, V, 1>(g, s, Lc, tw, tid, nthr); MM_SYNC(); }
+    if (R1 == 8) yB_last<T, V, 8>(g, Sz, s, tw, tid, nthr);
+    else if (R1 == 4) yB_last<T, V, 4>(g, Sz, s, tw, tid, nthr);
+    else yB_last<T, V, 2>(g, Sz, s, tw, tid, nthr);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Passes A / C v2 (x transform of packed pairs with m = nx/2, n = nx; z transform in registers)
+// ------------------------------------------------------------------------------------------------
+// generic radix-8 middle stage for the x tile: lines fastest in groups of LG lines sharing twiddles
+template <typename T, int DIR>
+MM_HD void xs_mid8(cx<T>* s, int pitch, int L, int n, int Lc, twiddles<T> tw, int tid, int nthr)
+{
+    const int LG = L < 4 ? L : 4, NG = L / LG, logNG = ilog2(NG);
+    const int sub = Lc >> 3, logsub = ilog2(sub);
+    for (int f = tid; f < (n >> 3) * NG; f += nthr) {
+        const int lg = f & (NG - 1), b = f >> logNG;
+        const int blk = b >> logsub, i = b & (sub - 1);
+        cx<T> pw[8];
+        if (i != 0) twiddle_powers<T, 8>(tw.get(i, Lc), pw);
+        cx<T>* base = s + (blk * Lc + i) * pitch + lg * LG;
+        for (int t = 0; t < LG; t++) {
+            cx<T>* p = base + t;
+            cx<T> v[8];
+#pragma unroll
+            for (int r = 0; r < 8; r++) v[r] = p[r * sub * pitch];
+            if (DIR == 0) {
+                rad<cx<T>, 8>::fwd(v);
+                if (i != 0) {
+#pragma unroll
+                    for (int r = 1; r < 8; r++) v[r] = cmul(v[r], pw[r]);
+                }
+            } else {
+                if (i != 0) {
+#pragma unroll
+                    for (int r = 1; r < 8; r++) v[r] = cmulc(v[r], pw[r]);
+                }
+                rad<cx<T>, 8>::inv(v);
+            }
+#pragma unroll
+            for (int r = 0; r < 8; r++) p[r * sub * pitch] = v[r];
+        }
+    }
+}
+
+// first x stage: load Ms*m pairs from global (i fastest: coalesced), pad twiddle, radix R, both blocks
+template <typename T, int R>
+MM_HD void xA_first(const Geom& g, const T* mc, const T* Ms, cx<T>* s, int pitch, int j0, twiddles<T> tw, int tid, int nthr)
+{
+    const int n = g.nx, m = n / 2, sub = m / R, logsub = ilog2(sub), L = g.G * g.nz, lognz = ilog2(g.nz);
+    for (int f = tid; f < sub * L; f += nthr) {
+        const int i = f & (sub - 1), l = f >> logsub;
+        const int gg = l >> lognz, z = l & (g.nz - 1);
+        const long row = ((long)z * g.ny + (j0 + gg)) * g.nx;
+        cx<T> a[R], u[R];
+#pragma unroll
+        for (int r = 0; r < R; r++) {
+            const long cell = row + 2 * (i + r * sub);
+            const cx<T> mm2 = *reinterpret_cast<const cx<T>*>(mc + cell);
+            const cx<T> ms2 = *reinterpret_cast<const cx<T>*>(Ms + cell);
+            a[r] = mk<T>(ms2.x == (T)0 ? (T)0 : ms2.x * mm2.x, ms2.y == (T)0 ? (T)0 : ms2.y * mm2.y);
+            u[r] = cmul(a[r], tw.get(i + r * sub, n));
+        }
+        rad<cx<T>, R>::fwd(a);
+        rad<cx<T>, R>::fwd(u);
+        if (R > 1 && i != 0) {
+            cx<T> pw[R];
+            twiddle_powers<T, R>(tw.get(i, m), pw);
+#pragma unroll
+            for (int r = 1; r < R; r++) { a[r] = cmul(a[r], pw[r]); u[r] = cmul(u[r], pw[r]); }
+        }
+        cx<T>* dst = s + i * pitch + l;
+#pragma unroll
+        for (int r = 0; r < R; r++) { dst[r * sub * pitch] = a[r]; dst[(m + r * sub) * pitch] = u[r]; }
+    }
+}
+
+// last x stage of pass C: inverse radix R on both blocks, crop combine, scale, store H_d pairs
+template <typename T, int R>
+MM_HD void xC_last(const Geom& g, T* Hc, const cx<T>* s, int pitch, int j0, T inv_scale, twiddles<T> tw, int tid, int nthr)
+{
+    const int n = g.nx, m = n / 2, sub = m / R, logsub = ilog2(sub), L = g.G * g.nz, lognz = ilog2(g.nz);
+    for (int f = tid; f < sub * L; f += nthr) {
+        const int i = f & (sub - 1), l = f >> logsub;
+        const int gg = l >> lognz, z = l & (g.nz - 1);
+        const long row = ((long)z * g.ny + (j0 + gg)) * g.nx;
+        const cx<T>* src = s + i * pitch + l;
+        cx<T> a[R], u[R];
+#pragma unroll
+        for (int r = 0; r < R; r++) { a[r] = src[r * sub * pitch]; u[r] = src[(m + r * sub) * pitch]; }
+        if (R > 1 && i != 0) {
+            cx<T> pw[R];
+            twiddle_powers<T, R>(tw.get(i, m), pw);
+#pragma unroll
+            for (int r = 1; r < R; r++) { a[r] = cmulc(a[r], pw[r]); u[r] = cmulc(u[r], pw[r]); }
+        }
+        rad<cx<T>, R>::inv(a);
+        rad<cx<T>, R>::inv(u);
+#pragma unroll
+        for (int r = 0; r < R; r++) {
+            const cx<T> o = a[r] + cmulc(u[r], tw.get(i + r * sub, n));
+            *reinterpret_cast<cx<T>*>(Hc + row + 2 * (i + r * sub)) = scale(o, inv_scale);
+        }
+    }
+}
+
+// split (DIR 0: Z -> X half spectrum) / merge (DIR 1: X -> 2Z) of the packed real transform
+template <typename T, int DIR>
+MM_HD void x_split_merge(const Geom& g, cx<T>* s, int pitch, twiddles<T> tw, int tid, int nthr)
+{
+    const int n = g.nx, h = n / 2, L = g.G * g.nz, logL = ilog2(L);
+    for (int f = tid; f < L * (h + 1); f += nthr) {
+        const int l = f & (L - 1), k = f >> logL;
+        if (k == 0) {
+            if (DIR == 0) {
+                const cx<T> z0 = s[l];
+                s[l] = mk<T>(z0.x + z0.y, (T)0);
+                s[n * pitch + l] = mk<T>(z0.x - z0.y, (T)0);
+            } else {
+                const cx<T> A = s[l], B = conj(s[n * pitch + l]);
+                s[l] = (A + B) + mul_pi(A - B);
+            }
+        } else if (k == h) {
+            const int p = (int)brev(k, g.lognx) * pitch + l;
+            s[p] = DIR == 0 ? conj(s[p]) : scale(conj(s[p]), (T)2);
+        } else {
+            const int pa = (int)brev(k, g.lognx) * pitch + l, pb = (int)brev(n - k, g.lognx) * pitch + l;
+            const cx<T> A = s[pa], B = conj(s[pb]);
+            if (DIR == 0) {
+                const cx<T> E = scale(A + B, (T)0.5), D = scale(A - B, (T)0.5);
+                const cx<T> t = cmul(tw.get(k, 2 * n), D);
+                s[pa] = E + mul_mi(t);
+                s[pb] = conj(E) + mul_mi(conj(t));
+            } else {
+                const cx<T> E = A + B, O = cmulc(A - B, tw.get(k, 2 * n));
+                s[pa] = E + mul_pi(O);
+                s[pb] = conj(E) + mul_pi(conj(O));
+            }
+        }
+    }
+}
+
+// z transform in registers, forward: tile -> S.  One item per (x position, row gg).
+template <typename T, int NZ>
+MM_HD void zA_regs(const Geom& g, cx<T>* Sc, const cx<T>* s, int pitch, int j0, twiddles<T> tw, int tid, int nthr)
+{
+    const int np = g.nx + 1;
+    for (int f = tid; f < np * g.G; f += nthr) {
+        const int xp = f % np, gg = f / np;
+        const cx<T>* src = s + xp * pitch + gg * NZ;
+        cx<T>* dst = Sc + (long)(j0 + gg) * g.Lx + xp;
+        cx<T> a[NZ];
+#pragma unroll
+        for (int z = 0; z < NZ; z++) a[z] = src[z];
+        {
+            cx<T> v[NZ];
+#pragma unroll
+            for (int z = 0; z < NZ; z++) v[z] = a[z];
+            rad<cx<T>, NZ>::fwd(v);
+#pragma unroll
+            for (int z = 0; z < NZ; z++) dst[(long)z * g.plane] = v[z];
+        }
+#pragma unroll
+        for (int z = 1; z < NZ; z++) a[z] = cmul(a[z], tw.get(z, 2 * NZ));
+        rad<cx<T>, NZ>::fwd(a);
+#pragma unroll
+        for (int z = 0; z < NZ; z++) dst[(long)(NZ + z) * g.plane] = a[z];
+    }
+}
+
+// z transform in registers, inverse + crop: S -> tile
+template <typename T, int NZ>
+MM_HD void zC_regs(const Geom& g, const cx<T>* Sc, cx<T>* s, int pitch, int j0, twiddles<T> tw, int tid, int nthr)
+{
+    const int np = g.nx + 1;
+    for (int f = tid; f < np * g.G; f += nthr) {
+        const int xp = f % np, gg = f / np;
+        cx<T>* dst = s + xp * pitch + gg * NZ;
+        const cx<T>* src = Sc + (long)(j0 + gg) * g.Lx + xp;
+        cx<T> a[NZ], u[NZ];
+#pragma unroll
+        for (int z = 0; z < NZ; z++) { a[z] = src[(long)z * g.plane]; u[z] = src[(long)(NZ + z) * g.plane]; }
+        rad<cx<T>, NZ>::inv(a);
+        rad<cx<T>, NZ>::inv(u);
+        dst[0] = a[0] + u[0];
+#pragma unroll
+        for (int z = 1; z < NZ; z++) dst[z] = a[z] + cmulc(u[z], tw.get(z, 2 * NZ));
+    }
+}
+
+// NZ = 0: nz > 32 (not supported by v2; host falls back to v1).  Requires nx >= 32.
+template <typename T, int NZ>
+MM_HD void fwd_xz_body2(const Geom g, const T* __restrict__ mvec, const T* __restrict__ Ms, cx<T>* __restrict__ S,
+                        twiddles<T> tw, cx<T>* s, int bid, int tid, int nthr)
+{
+    const int c = bid % 3, j0 = (bid / 3) * g.G;
+    const int n = g.nx, m = n / 2, L = g.G * g.nz, pitch = odd_pitch(L);
+    const T* mc = mvec + (long)c * g.N;
+    const int R1 = first_radix(m);
+    if (R1 == 8) xA_first<T, 8>(g, mc, Ms, s, pitch, j0, tw, tid, nthr);
+    else if (R1 == 4) xA_first<T, 4>(g, mc, Ms, s, pitch, j0, tw, tid, nthr);
+    else xA_first<T, 2>(g, mc, Ms, s, pitch, j0, tw, tid, nthr);
+    MM_SYNC();
+    for (int Lc = m / R1; Lc > 1; Lc >>= 3) { xs_mid8<T, 0>(s, pitch, L, n, Lc, tw, tid, nthr); MM_SYNC(); }
+    x_split_merge<T, 0>(g, s, pitch, tw, tid, nthr);
+    MM_SYNC();
+    cx<T>* Sc = S + (long)c * g.comp;
+    if (NZ == 1) {
+        for (int f = tid; f < L * (n + 1); f += nthr) {
+            const int xp = f % (n + 1), l = f / (n + 1);
+            Sc[(long)(j0 + l) * g.Lx + xp] = s[xp * pitch + l];
+        }
+    } else {
+        zA_regs<T, NZ>(g, Sc, s, pitch, j0, tw, tid, nthr);
+    }
+}
+
+template <typename T, int NZ>
+MM_HD void inv_zx_body2(const Geom g, const cx<T>* __restrict__ S, T* __restrict__ Hd, twiddles<T> tw, T inv_scale,
+                        cx<T>* s, int bid, int tid, int nthr)
+{
+    const int c = bid % 3, j0 = (bid / 3) * g.G;
+    const int n = g.nx, m = n / 2, L = g.G * g.nz, pitch = odd_pitch(L);
+    const cx<T>* Sc = S + (long)c * g.comp;
+    if (NZ == 1) {
+        for (int f = tid; f < L * (n + 1); f += nthr) {
+            const int xp = f % (n + 1), l = f / (n + 1);
+            s[xp * pitch + l] = Sc[(long)(j0 + l) * g.Lx + xp];
+        }
+    } else {
+        zC_regs<T, NZ>(g, Sc, s, pitch, j0, tw, tid, nthr);
+    }
+    MM_SYNC();
+    x_split_merge<T, 1>(g, s, pitch, tw, tid, nthr);
+    MM_SYNC();
+    const int R1 = first_radix(m);
+    for (int Lc = 8; Lc <= m / R1; Lc <<= 3) { xs_mid8<T, 1>(s, pitch, L, n, Lc, tw, tid, nthr); MM_SYNC(); }
+    T* Hc = Hd + (long)c * g.N;
+    if (R1 == 8) xC_last<T, 8>(g, Hc, s, pitch, j0, inv_scale, tw, tid, nthr);
+    else if (R1 == 4) xC_last<T, 4>(g, Hc, s, pitch, j0, inv_scale, tw, tid, nthr);
+    else xC_last<T, 2>(g, Hc, s, pitch, j0, inv_scale, tw, tid, nthr);
+}
+
+}  // namespace mm

@@ -12,6 +12,7 @@
 #include "../../include/mm.h"
 #include "mm_fft.cuh"
 #include "mm_kernels.cuh"
+#include "mm_kernels2.cuh"
 #include "mm_llg.cuh"
 
 extern "C" void mm_newell_near_box(int bx, int by, int bz, double dx, double dy, double dz, double* out);
@@ -50,6 +51,26 @@ __global__ void __launch_bounds__(256) inv_zx_kernel(Geom g, const cx<T>* S, T* 
 {
     if (st->done) return;
     inv_zx_body<T>(g, S, Hd, tw, inv_scale, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x);
+}
+
+// v2 wrappers (mm_kernels2.cuh)
+template <typename T, int NZ>
+__global__ void __launch_bounds__(256) fwd_xz2_kernel(Geom g, const T* m, const T* Ms, cx<T>* S, twiddles<T> tw, const DevState* st)
+{
+    if (st->done) return;
+    fwd_xz_body2<T, NZ>(g, m, Ms, S, tw, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x);
+}
+template <typename T, int V>
+__global__ void __launch_bounds__(sizeof(T) == 8 ? 256 : 512) y_conv2_kernel(Geom g, cx<T>* S, const T* Kh, twiddles<T> tw, const DevState* st)
+{
+    if (st->done) return;
+    y_conv_body2<T, V>(g, S, Kh, tw, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x);
+}
+template <typename T, int NZ>
+__global__ void __launch_bounds__(256) inv_zx2_kernel(Geom g, const cx<T>* S, T* Hd, twiddles<T> tw, T inv_scale, const DevState* st)
+{
+    if (st->done) return;
+    inv_zx_body2<T, NZ>(g, S, Hd, tw, inv_scale, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -352,6 +373,7 @@ struct mm_sim {
     long launches;
     std::string err;
     // optional per-pass profiling (mm_set_profiling): event pairs around each kernel class
+    int use_v2;
     int prof_on;
     std::vector<cudaEvent_t> prof_ev;      // pairs
     std::vector<int> prof_cls;             // class of pair i: 0 pass A, 1 pass B, 2 pass C, 3 stage kernel
@@ -421,7 +443,7 @@ static void configure(mm_sim* s)
     s->smemA = (size_t)smemA_elems(g) * cs;
     s->smemB = (size_t)smemB_elems(g) * cs;
     s->thrA = 256;
-    s->thrB = s->smemB > 64 * 1024 ? 512 : 256;
+    s->thrB = (s->prec == MM_F32 && s->smemB > 64 * 1024) ? 512 : 256;
 }
 
 static void layout(mm_sim* s)
@@ -457,7 +479,7 @@ extern "C" int mm_create(mm_sim** out, int nx, int ny, int nz, double dx, double
     s->dx = dx; s->dy = dy; s->dz = dz;
     s->A = s->D = s->Ku = 0; s->u[0] = s->u[1] = 0; s->u[2] = 1; s->hext[0] = s->hext[1] = s->hext[2] = 0;
     s->alpha = 0.5; s->gamma = 2.211e5; s->dmi_kind = 0; s->integ = MM_DOPRI5; s->demag_on = 1; s->demag_ready = 0; s->Ms_set = 0;
-    s->ws = nullptr; s->ws_bytes = 0; s->khat_imag_ratio = -1; s->t_host = 0; s->launches = 0; s->prof_on = 0; s->prof_used = 0;
+    s->ws = nullptr; s->ws_bytes = 0; s->khat_imag_ratio = -1; s->t_host = 0; s->launches = 0; s->prof_on = 0; s->prof_used = 0; s->use_v2 = getenv("MM_FORCE_V1") ? 0 : 1;
     Geom& g = s->g;
     memset(&g, 0, sizeof(g));
     g.nx = nx; g.ny = ny; g.nz = nz;
@@ -731,7 +753,26 @@ template <typename T> static LocalP<T> make_local(const mm_sim* s, int terms)
     return lp;
 }
 
-// demag passes A, B, C: y -> Hd
+// demag passes A, B, C: y -> Hd.  v2 kernels where the mesh allows, v1 otherwise (tiny meshes).
+template <typename T, int NZ> static void launch_A2(mm_sim* s, unsigned grid, const T* y, cx<T>* S, twiddles<T> tw, const DevState* st)
+{
+    static bool attr = false;
+    if (!attr) { cudaFuncSetAttribute(fwd_xz2_kernel<T, NZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_CAP); attr = true; }
+    fwd_xz2_kernel<T, NZ><<<grid, s->thrA, s->smemA, s->stream>>>(s->g, y, wsp<T>(s, s->off_Ms), S, tw, st);
+}
+template <typename T, int NZ> static void launch_C2(mm_sim* s, unsigned grid, cx<T>* S, twiddles<T> tw, T sc, const DevState* st)
+{
+    static bool attr = false;
+    if (!attr) { cudaFuncSetAttribute(inv_zx2_kernel<T, NZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_CAP); attr = true; }
+    inv_zx2_kernel<T, NZ><<<grid, s->thrA, s->smemA, s->stream>>>(s->g, S, wsp<T>(s, s->off_Hd), tw, sc, st);
+}
+template <typename T, int V> static void launch_B2(mm_sim* s, unsigned grid, cx<T>* S, twiddles<T> tw, const DevState* st)
+{
+    static bool attr = false;
+    if (!attr) { cudaFuncSetAttribute(y_conv2_kernel<T, V>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_CAP); attr = true; }
+    y_conv2_kernel<T, V><<<grid, s->thrB, s->smemB, s->stream>>>(s->g, S, wsp<T>(s, s->off_Kh), tw, st);
+}
+
 template <typename T> static int demag_passes(mm_sim* s, const T* y)
 {
     const Geom& g = s->g;
@@ -739,15 +780,35 @@ template <typename T> static int demag_passes(mm_sim* s, const T* y)
     const DevState* st = wsp<DevState>(s, s->off_st);
     cx<T>* S = wsp<cx<T>>(s, s->off_S);
     const unsigned gridA = 3u * (unsigned)(g.ny / g.G), gridB = (unsigned)(g.Lx / g.TC) * (unsigned)g.pz;
+    const double P = (double)g.px * g.py * g.pz;
+    const bool a2 = s->use_v2 && g.nx >= 32 && g.nz <= (sizeof(T) == 8 ? 16 : 32);
+    const bool b2 = s->use_v2 && g.ny >= 16;
     prof_begin(s, 0);
-    fwd_xz_kernel<T><<<gridA, s->thrA, s->smemA, s->stream>>>(g, y, wsp<T>(s, s->off_Ms), S, tw, st);
+    if (!a2) fwd_xz_kernel<T><<<gridA, s->thrA, s->smemA, s->stream>>>(g, y, wsp<T>(s, s->off_Ms), S, tw, st);
+    else switch (g.nz) {
+        case 1: launch_A2<T, 1>(s, gridA, y, S, tw, st); break;
+        case 2: launch_A2<T, 2>(s, gridA, y, S, tw, st); break;
+        case 4: launch_A2<T, 4>(s, gridA, y, S, tw, st); break;
+        case 8: launch_A2<T, 8>(s, gridA, y, S, tw, st); break;
+        case 16: launch_A2<T, 16>(s, gridA, y, S, tw, st); break;
+        default: launch_A2<T, 32>(s, gridA, y, S, tw, st); break;
+    }
     prof_end(s);
     prof_begin(s, 1);
-    y_conv_kernel<T><<<gridB, s->thrB, s->smemB, s->stream>>>(g, S, wsp<T>(s, s->off_Kh), tw, st);
+    if (!b2) y_conv_kernel<T><<<gridB, s->thrB, s->smemB, s->stream>>>(g, S, wsp<T>(s, s->off_Kh), tw, st);
+    else if (sizeof(T) == 4 && g.TC % 2 == 0) launch_B2<T, (sizeof(T) == 4 ? 2 : 1)>(s, gridB, S, tw, st);
+    else launch_B2<T, 1>(s, gridB, S, tw, st);
     prof_end(s);
-    const double P = (double)g.px * g.py * g.pz;
     prof_begin(s, 2);
-    inv_zx_kernel<T><<<gridA, s->thrA, s->smemA, s->stream>>>(g, S, wsp<T>(s, s->off_Hd), tw, (T)(1.0 / P), st);
+    if (!a2) inv_zx_kernel<T><<<gridA, s->thrA, s->smemA, s->stream>>>(g, S, wsp<T>(s, s->off_Hd), tw, (T)(1.0 / P), st);
+    else switch (g.nz) {
+        case 1: launch_C2<T, 1>(s, gridA, S, tw, (T)(1.0 / P), st); break;
+        case 2: launch_C2<T, 2>(s, gridA, S, tw, (T)(1.0 / P), st); break;
+        case 4: launch_C2<T, 4>(s, gridA, S, tw, (T)(1.0 / P), st); break;
+        case 8: launch_C2<T, 8>(s, gridA, S, tw, (T)(1.0 / P), st); break;
+        case 16: launch_C2<T, 16>(s, gridA, S, tw, (T)(1.0 / P), st); break;
+        default: launch_C2<T, 32>(s, gridA, S, tw, (T)(1.0 / P), st); break;
+    }
     prof_end(s);
     s->launches += 3;
     MM_TRY(s, cudaGetLastError());

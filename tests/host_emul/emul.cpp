@@ -6,6 +6,7 @@
 #include <cstring>
 #include <vector>
 #include "../../paper_2406_16064_b200/csrc/mm_kernels.cuh"
+#include "../../paper_2406_16064_b200/csrc/mm_kernels2.cuh"
 #include "../../paper_2406_16064_b200/csrc/mm_llg.cuh"
 
 using namespace mm;
@@ -37,7 +38,7 @@ static Geom make_geom(int nx, int ny, int nz, int G, int CH, int TC)
 
 // Kfull: real part of the 3-D DFT of the wrapped tensor, natural order, [6][pz][py][px] doubles.
 template <typename T>
-static void run(int nx, int ny, int nz, int G, int CH, int TC, const double* Kfull, const double* Ms, const double* m, double* Hd)
+static void run(int ver, int nx, int ny, int nz, int G, int CH, int TC, const double* Kfull, const double* Ms, const double* m, double* Hd)
 {
     Geom g = make_geom(nx, ny, nz, G, CH, TC);
     int twN = g.px > g.py ? g.px : g.py;
@@ -61,18 +62,35 @@ static void run(int nx, int ny, int nz, int G, int CH, int TC, const double* Kfu
     memset(S.data(), 0, S.size() * sizeof(cx<T>));
     std::vector<cx<T>> smem((size_t)(smemA_elems(g) > smemB_elems(g) ? smemA_elems(g) : smemB_elems(g)) + 16);
     const int gridA = 3 * (ny / G), gridB = (g.Lx / TC) * g.pz;
-    for (int b = 0; b < gridA; b++) fwd_xz_body<T>(g, mt.data(), Mst.data(), S.data(), tw, smem.data(), b, 0, 1);
-    for (int b = 0; b < gridB; b++) y_conv_body<T>(g, S.data(), Kh.data(), tw, smem.data(), b, 0, 1);
     const double P = (double)g.px * g.py * g.pz;
-    for (int b = 0; b < gridA; b++) inv_zx_body<T>(g, S.data(), Hdt.data(), tw, (T)(1.0 / P), smem.data(), b, 0, 1);
+    const bool a2 = ver == 2 && nx >= 32 && nz <= 32, b2 = ver == 2 && ny >= 16;
+    for (int b = 0; b < gridA; b++) {
+        if (!a2) fwd_xz_body<T>(g, mt.data(), Mst.data(), S.data(), tw, smem.data(), b, 0, 1);
+        else switch (nz) {
+#define CASE_A(NZ) case NZ: fwd_xz_body2<T, NZ>(g, mt.data(), Mst.data(), S.data(), tw, smem.data(), b, 0, 1); break;
+            CASE_A(1) CASE_A(2) CASE_A(4) CASE_A(8) CASE_A(16) CASE_A(32)
+        }
+    }
+    for (int b = 0; b < gridB; b++) {
+        if (!b2) y_conv_body<T>(g, S.data(), Kh.data(), tw, smem.data(), b, 0, 1);
+        else if (sizeof(T) == 4 && TC % 2 == 0) y_conv_body2<T, (sizeof(T) == 4 ? 2 : 1)>(g, S.data(), Kh.data(), tw, smem.data(), b, 0, 1);
+        else y_conv_body2<T, 1>(g, S.data(), Kh.data(), tw, smem.data(), b, 0, 1);
+    }
+    for (int b = 0; b < gridA; b++) {
+        if (!a2) inv_zx_body<T>(g, S.data(), Hdt.data(), tw, (T)(1.0 / P), smem.data(), b, 0, 1);
+        else switch (nz) {
+#define CASE_C(NZ) case NZ: inv_zx_body2<T, NZ>(g, S.data(), Hdt.data(), tw, (T)(1.0 / P), smem.data(), b, 0, 1); break;
+            CASE_C(1) CASE_C(2) CASE_C(4) CASE_C(8) CASE_C(16) CASE_C(32)
+        }
+    }
     for (long i = 0; i < 3 * g.N; i++) Hd[i] = (double)Hdt[i];
 }
 
-extern "C" void emul_demag(int prec64, int nx, int ny, int nz, int G, int CH, int TC, const double* Kfull, const double* Ms,
+extern "C" void emul_demag(int ver, int prec64, int nx, int ny, int nz, int G, int CH, int TC, const double* Kfull, const double* Ms,
                            const double* m, double* Hd)
 {
-    if (prec64) run<double>(nx, ny, nz, G, CH, TC, Kfull, Ms, m, Hd);
-    else run<float>(nx, ny, nz, G, CH, TC, Kfull, Ms, m, Hd);
+    if (prec64) run<double>(ver, nx, ny, nz, G, CH, TC, Kfull, Ms, m, Hd);
+    else run<float>(ver, nx, ny, nz, G, CH, TC, Kfull, Ms, m, Hd);
 }
 
 // local field + torque, cell by cell (terms bitmask as in LocalP)

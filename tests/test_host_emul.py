@@ -20,11 +20,11 @@ _dp = C.POINTER(C.c_double)
 
 @pytest.fixture(scope="module")
 def emul():
-    deps = [SRC] + [os.path.join(ROOT, "paper_2406_16064_b200", "csrc", f) for f in ("mm_fft.cuh", "mm_kernels.cuh", "mm_llg.cuh")]
+    deps = [SRC] + [os.path.join(ROOT, "paper_2406_16064_b200", "csrc", f) for f in ("mm_fft.cuh", "mm_kernels.cuh", "mm_kernels2.cuh", "mm_llg.cuh")]
     if not os.path.exists(LIB) or os.path.getmtime(LIB) < max(os.path.getmtime(d) for d in deps):
         subprocess.run(["g++", "-O1", "-std=c++17", "-fPIC", "-shared", "-o", LIB, SRC], check=True)
     L = C.CDLL(LIB)
-    L.emul_demag.argtypes = [C.c_int] * 7 + [_dp] * 4
+    L.emul_demag.argtypes = [C.c_int] * 8 + [_dp] * 4
     L.emul_local.argtypes = [C.c_int] * 3 + [_dp, C.c_int, C.c_int, _dp, _dp, _dp, C.c_int, _dp]
     return L
 
@@ -52,9 +52,12 @@ def khat_full(o, nx, ny, nz):
 
 
 @pytest.mark.parametrize("shape,cfg", [((16, 16, 1), (2, 8, 4)), ((32, 8, 1), (1, 8, 2)), ((8, 16, 4), (1, 4, 2)),
-                                       ((16, 8, 2), (2, 8, 8)), ((64, 4, 8), (1, 16, 1)), ((4, 2, 1), (1, 8, 1))])
+                                       ((16, 8, 2), (2, 8, 8)), ((64, 4, 8), (1, 16, 1)), ((4, 2, 1), (1, 8, 1)),
+                                       ((32, 16, 1), (4, 8, 8)), ((64, 32, 2), (2, 8, 4)), ((32, 64, 16), (1, 8, 8)),
+                                       ((128, 128, 1), (2, 8, 2)), ((256, 16, 4), (1, 8, 1)), ((32, 32, 32), (1, 8, 4))])
 @pytest.mark.parametrize("prec64", [1, 0])
-def test_demag_passes_match_oracle(emul, shape, cfg, prec64):
+@pytest.mark.parametrize("ver", [1, 2])
+def test_demag_passes_match_oracle(emul, shape, cfg, prec64, ver):
     nx, ny, nz = shape
     G, CH, TC = cfg
     cell = (2e-9, 1.5e-9, 3e-9)
@@ -67,7 +70,7 @@ def test_demag_passes_match_oracle(emul, shape, cfg, prec64):
     K = khat_full(o, nx, ny, nz)
     Hd = np.zeros(3 * nx * ny * nz)
     Msf = np.ascontiguousarray(Ms.reshape(-1))
-    emul.emul_demag(prec64, nx, ny, nz, G, CH, TC, K.ctypes.data_as(_dp), Msf.ctypes.data_as(_dp),
+    emul.emul_demag(ver, prec64, nx, ny, nz, G, CH, TC, K.ctypes.data_as(_dp), Msf.ctypes.data_as(_dp),
                     m.ctypes.data_as(_dp), Hd.ctypes.data_as(_dp))
     Hd = Hd.reshape(3, nz, ny, nx) * (Ms > 0)
     tol = 1e-12 if prec64 else 2e-5
