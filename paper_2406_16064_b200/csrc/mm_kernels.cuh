@@ -21,7 +21,7 @@ namespace mm {
 struct Geom {
     int nx, ny, nz;        // cells
     int px, py, pz;        // padded sizes (2n, or 1 when n == 1)
-    int lognx, logpy, logpz;
+    int lognx, logny, logpy, logpz;
     int Lx;                // spectrum row pitch in complex elements
     int G;                 // rows (j) per CTA in passes A and C
     int CH;                // x positions per z-chunk in passes A and C (3-D only)

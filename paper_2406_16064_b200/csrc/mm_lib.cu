@@ -80,8 +80,8 @@ template <typename T> struct StageArgs {
     const T* m0;          // step start magnetisation
     const T* kprev[6];    // earlier stage derivatives k_0..k_{s-1}
     T* ynext;             // next stage input (or the RK4 solution); may be NULL
-    double coef[7];       // ynext = m0 + dt * sum_{j<=s} coef[j] k_j
-    double ecoef[7];      // E = dt * sum_{j<=s} ecoef[j] k_j   (do_err)
+    T coef[7];            // ynext = m0 + dt * sum_{j<=s} coef[j] k_j
+    T ecoef[7];           // E = dt * sum_{j<=s} ecoef[j] k_j   (do_err)
     int s;                // index of this stage
     int do_err, do_maxk;
 };
@@ -114,49 +114,52 @@ __device__ __forceinline__ void block_max_bits(unsigned long long v, unsigned lo
     __syncthreads();
 }
 
-// mode 0: out = H_eff ; mode 1: out = k = LL torque (+ optional RK stage algebra)
-template <typename T, int MODE>
+// MODE 0: out = H_eff ; MODE 1: out = k = LL torque, then the RK stage algebra selected at compile
+// time: S earlier stages, NEXT (write the next stage input), ERR (embedded error norm), MAXK (max |k|).
+// One thread per cell; indices by shifts (all mesh sizes are powers of two).
+template <typename T, int MODE, int S, bool NEXT, bool ERR, bool MAXK>
 __global__ void __launch_bounds__(256) llg_stage_kernel(Geom g, LocalP<T> lp, const T* __restrict__ y, const T* __restrict__ Ms,
                                                         const T* __restrict__ Hd, T* __restrict__ out, StageArgs<T> sa, DevState* st)
 {
     if (st->done) return;
     const long N = g.N;
-    const long q = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;
     T errn = 0, kn = 0;
     if (q < N) {
         const T Msi = Ms[q];
-        v3<T> res = { 0, 0, 0 };
         const bool live = Msi != (T)0;
-        if (live) {
-            const int i = (int)(q % g.nx), j = (int)((q / g.nx) % g.ny), k = (int)(q / ((long)g.nx * g.ny));
-            const v3<T> mi = ld3(y, N, q);
-            v3<T> H = { 0, 0, 0 };
-            if (Hd != nullptr) H = ld3(Hd, N, q);
-            H = local_field<T>(g, lp, y, Ms, i, j, k, q, Msi, mi, H);
-            res = MODE == 0 ? H : ll_torque<T>(lp, mi, H);
-        }
+        const int i = q & (g.nx - 1), j = (q >> g.lognx) & (g.ny - 1), k = q >> (g.lognx + g.logny);
+        const v3<T> mi = ld3(y, N, q);
+        v3<T> H = { 0, 0, 0 };
+        if (Hd != nullptr) H = ld3(Hd, N, q);
+        v3<T> kj[S > 0 ? S : 1];
+#pragma unroll
+        for (int jj = 0; jj < S; jj++) kj[jj] = ld3(sa.kprev[jj], N, q);
+        v3<T> m0 = { 0, 0, 0 };
+        if (NEXT) m0 = ld3(sa.m0, N, q);
+        H = local_field<T>(g, lp, y, Ms, i, j, k, q, live ? Msi : (T)1, mi, H);
+        v3<T> res = MODE == 0 ? H : ll_torque<T>(lp, mi, H);
+        if (!live) { res.x = 0; res.y = 0; res.z = 0; }
         out[q] = res.x; out[N + q] = res.y; out[2 * N + q] = res.z;
-        if (MODE == 1 && (sa.ynext != nullptr || sa.do_err)) {
+        if (MODE == 1 && (NEXT || ERR)) {
             const T dt = (T)st->dt;
-            v3<T> acc = { (T)sa.coef[sa.s] * res.x, (T)sa.coef[sa.s] * res.y, (T)sa.coef[sa.s] * res.z };
-            v3<T> ea = { (T)sa.ecoef[sa.s] * res.x, (T)sa.ecoef[sa.s] * res.y, (T)sa.ecoef[sa.s] * res.z };
-            for (int jj = 0; jj < sa.s; jj++) {
-                const T cj = (T)sa.coef[jj], ej = (T)sa.ecoef[jj];
-                if (cj == (T)0 && ej == (T)0) continue;
-                const v3<T> kj = ld3(sa.kprev[jj], N, q);
-                acc.x += cj * kj.x; acc.y += cj * kj.y; acc.z += cj * kj.z;
-                ea.x += ej * kj.x; ea.y += ej * kj.y; ea.z += ej * kj.z;
-            }
-            if (sa.ynext != nullptr) {
-                const v3<T> m0 = ld3(sa.m0, N, q);
+            if (NEXT) {
+                v3<T> acc = { sa.coef[S] * res.x, sa.coef[S] * res.y, sa.coef[S] * res.z };
+#pragma unroll
+                for (int jj = 0; jj < S; jj++) { acc.x += sa.coef[jj] * kj[jj].x; acc.y += sa.coef[jj] * kj[jj].y; acc.z += sa.coef[jj] * kj[jj].z; }
                 sa.ynext[q] = m0.x + dt * acc.x; sa.ynext[N + q] = m0.y + dt * acc.y; sa.ynext[2 * N + q] = m0.z + dt * acc.z;
             }
-            if (sa.do_err && live) errn = sqrt((dt * ea.x) * (dt * ea.x) + (dt * ea.y) * (dt * ea.y) + (dt * ea.z) * (dt * ea.z));
+            if (ERR) {
+                v3<T> ea = { sa.ecoef[S] * res.x, sa.ecoef[S] * res.y, sa.ecoef[S] * res.z };
+#pragma unroll
+                for (int jj = 0; jj < S; jj++) { ea.x += sa.ecoef[jj] * kj[jj].x; ea.y += sa.ecoef[jj] * kj[jj].y; ea.z += sa.ecoef[jj] * kj[jj].z; }
+                if (live) errn = sqrt((dt * ea.x) * (dt * ea.x) + (dt * ea.y) * (dt * ea.y) + (dt * ea.z) * (dt * ea.z));
+            }
         }
-        if (MODE == 1 && sa.do_maxk && live) kn = sqrt(res.x * res.x + res.y * res.y + res.z * res.z);
+        if (MODE == 1 && MAXK && live) kn = sqrt(res.x * res.x + res.y * res.y + res.z * res.z);
     }
-    if (MODE == 1 && sa.do_err) block_max_bits(norm_bits(errn), &st->err_bits);
-    if (MODE == 1 && sa.do_maxk) block_max_bits(norm_bits(kn), &st->maxk_bits);
+    if (MODE == 1 && ERR) block_max_bits(norm_bits(errn), &st->err_bits);
+    if (MODE == 1 && MAXK) block_max_bits(norm_bits(kn), &st->maxk_bits);
 }
 
 // Step controller: one thread.  DESIGN.md R8.
@@ -432,6 +435,7 @@ static void configure(mm_sim* s)
     while (g.G > 1 && (size_t)smemA_elems(g) * cs > 100 * 1024) g.G /= 2;
     // pass B: TC columns per CTA
     int TC = s->prec == MM_F64 ? 4 : 8;
+    if (getenv("MM_TC")) TC = atoi(getenv("MM_TC"));       // tuning knob (power of two)
     g.TC = TC;
     while (g.TC > 1 && (size_t)smemB_elems(g) * cs > SMEM_CAP) g.TC /= 2;
     while (g.TC > 2 && ((g.nx + g.TC) / g.TC) * g.pz < target) g.TC /= 2;
@@ -444,6 +448,8 @@ static void configure(mm_sim* s)
     s->smemB = (size_t)smemB_elems(g) * cs;
     s->thrA = 256;
     s->thrB = (s->prec == MM_F32 && s->smemB > 64 * 1024) ? 512 : 256;
+    if (getenv("MM_THRB")) s->thrB = atoi(getenv("MM_THRB"));
+    if (getenv("MM_THRA")) s->thrA = atoi(getenv("MM_THRA"));
 }
 
 static void layout(mm_sim* s)
@@ -484,7 +490,7 @@ extern "C" int mm_create(mm_sim** out, int nx, int ny, int nz, double dx, double
     memset(&g, 0, sizeof(g));
     g.nx = nx; g.ny = ny; g.nz = nz;
     g.px = nx > 1 ? 2 * nx : 1; g.py = ny > 1 ? 2 * ny : 1; g.pz = nz > 1 ? 2 * nz : 1;
-    g.lognx = ilog2(nx); g.logpy = ilog2(g.py); g.logpz = ilog2(g.pz);
+    g.lognx = ilog2(nx); g.logny = ilog2(ny); g.logpy = ilog2(g.py); g.logpz = ilog2(g.pz);
     g.N = (long)nx * ny * nz;
     s->twN = g.px > g.py ? g.px : g.py;
     if (g.pz > s->twN) s->twN = g.pz;
@@ -816,19 +822,35 @@ template <typename T> static int demag_passes(mm_sim* s, const T* y)
 }
 
 // one evaluation: MODE 0 -> H, MODE 1 -> k (+ stage algebra)
+template <typename T, int MODE, int S, bool NEXT, bool ERR, bool MAXK>
+static void launch_stage(mm_sim* s, const LocalP<T>& lp, const T* y, const T* Hd, T* out, const StageArgs<T>& sa)
+{
+    const unsigned blocks = (unsigned)((s->g.N + 255) / 256);
+    llg_stage_kernel<T, MODE, S, NEXT, ERR, MAXK><<<blocks, 256, 0, s->stream>>>(s->g, lp, y, wsp<T>(s, s->off_Ms), Hd, out, sa, wsp<DevState>(s, s->off_st));
+}
+
 template <typename T, int MODE> static int eval(mm_sim* s, const T* y, T* out, const StageArgs<T>& sa, int terms)
 {
-    const Geom& g = s->g;
     const bool demag = s->demag_on && (terms & 16);
     if (demag) {
         if (!s->demag_ready) return fail(s, MM_ERR_STATE, "demag enabled but mm_init_demag not called");
         int rc = demag_passes<T>(s, y);
         if (rc) return rc;
     }
-    const unsigned blocks = (unsigned)((g.N + 255) / 256);
+    const LocalP<T> lp = make_local<T>(s, terms);
+    const T* Hd = demag ? wsp<T>(s, s->off_Hd) : (const T*)nullptr;
     prof_begin(s, 3);
-    llg_stage_kernel<T, MODE><<<blocks, 256, 0, s->stream>>>(g, make_local<T>(s, terms), y, wsp<T>(s, s->off_Ms),
-                                                              demag ? wsp<T>(s, s->off_Hd) : (const T*)nullptr, out, sa, wsp<DevState>(s, s->off_st));
+    if (MODE == 0) launch_stage<T, 0, 0, false, false, false>(s, lp, y, Hd, out, sa);
+    else if (sa.do_err) launch_stage<T, 1, 6, false, true, false>(s, lp, y, Hd, out, sa);          // DOPRI5 stage 7
+    else if (sa.ynext == nullptr) launch_stage<T, 1, 0, false, false, false>(s, lp, y, Hd, out, sa);
+    else switch (sa.s) {
+        case 0: launch_stage<T, 1, 0, true, false, true>(s, lp, y, Hd, out, sa); break;
+        case 1: launch_stage<T, 1, 1, true, false, false>(s, lp, y, Hd, out, sa); break;
+        case 2: launch_stage<T, 1, 2, true, false, false>(s, lp, y, Hd, out, sa); break;
+        case 3: launch_stage<T, 1, 3, true, false, false>(s, lp, y, Hd, out, sa); break;
+        case 4: launch_stage<T, 1, 4, true, false, false>(s, lp, y, Hd, out, sa); break;
+        default: launch_stage<T, 1, 5, true, false, false>(s, lp, y, Hd, out, sa); break;
+    }
     prof_end(s);
     s->launches++;
     MM_TRY(s, cudaGetLastError());
@@ -900,11 +922,11 @@ template <typename T> static int enqueue_step(mm_sim* s, T* m, int ctrl_mode)
         for (int j = 0; j < st && j < 6; j++) sa.kprev[j] = k[j];
         sa.do_maxk = st == 0;
         if (s->integ == MM_DOPRI5) {
-            if (st < 6) { sa.ynext = yb[st & 1]; for (int j = 0; j <= st; j++) sa.coef[j] = DP_A[st + 1][j]; }
-            else { sa.ynext = nullptr; sa.do_err = 1; for (int j = 0; j < 7; j++) sa.ecoef[j] = DP_E[j]; }
+            if (st < 6) { sa.ynext = yb[st & 1]; for (int j = 0; j <= st; j++) sa.coef[j] = (T)DP_A[st + 1][j]; }
+            else { sa.ynext = nullptr; sa.do_err = 1; for (int j = 0; j < 7; j++) sa.ecoef[j] = (T)DP_E[j]; }
         } else {
             sa.ynext = yb[st & 1];
-            for (int j = 0; j <= st; j++) sa.coef[j] = RK4_A[st][j];
+            for (int j = 0; j <= st; j++) sa.coef[j] = (T)RK4_A[st][j];
         }
         const T* y = st == 0 ? m : yb[(st - 1) & 1];
         int rc = eval<T, 1>(s, y, k[st], sa, 31);

@@ -23,7 +23,9 @@ template <typename T> struct LocalP {
 template <typename T> struct v3 { T x, y, z; };
 template <typename T> MM_HD v3<T> ld3(const T* p, long N, long q) { v3<T> r; r.x = p[q]; r.y = p[N + q]; r.z = p[2 * N + q]; return r; }
 
-// H_eff at cell (i,j,k) given H_d (or 0).  y = stage magnetisation.
+// H_eff at cell (i,j,k) given H_d (or 0).  y = stage magnetisation.  Branch-free in the data: every
+// neighbour is loaded (index clamped to the cell itself when outside the mesh) and then selected,
+// so all loads of a thread are in flight together.
 template <typename T>
 MM_HD v3<T> local_field(const Geom& g, const LocalP<T>& lp, const T* __restrict__ y, const T* __restrict__ Ms,
                         int i, int j, int k, long q, T Msi, v3<T> mi, v3<T> H)
@@ -31,32 +33,31 @@ MM_HD v3<T> local_field(const Geom& g, const LocalP<T>& lp, const T* __restrict_
     const long N = g.N;
     const T inv = (T)1 / Msi;
     if ((lp.terms & 3) != 0) {
-        v3<T> ex = { 0, 0, 0 };           // sum_a cex_a sum_{+-} (m_j - m_i)
-        v3<T> S[3];                        // S_a = m_{+a} - m_{-a} over present neighbours
         const long str[3] = { 1, g.nx, (long)g.nx * g.ny };
         const int pos[3] = { i, j, k }, lim[3] = { g.nx, g.ny, g.nz };
+        v3<T> nb[6];
+        bool ok[6];
 #pragma unroll
         for (int a = 0; a < 3; a++) {
-            v3<T> sm = { 0, 0, 0 };
-            v3<T> acc = { 0, 0, 0 };
-            if (pos[a] > 0) {
-                const long p = q - str[a];
-                if (Ms[p] != (T)0) {
-                    const v3<T> mj = ld3(y, N, p);
-                    acc.x += mj.x - mi.x; acc.y += mj.y - mi.y; acc.z += mj.z - mi.z;
-                    sm.x -= mj.x; sm.y -= mj.y; sm.z -= mj.z;
-                }
-            }
-            if (pos[a] < lim[a] - 1) {
-                const long p = q + str[a];
-                if (Ms[p] != (T)0) {
-                    const v3<T> mj = ld3(y, N, p);
-                    acc.x += mj.x - mi.x; acc.y += mj.y - mi.y; acc.z += mj.z - mi.z;
-                    sm.x += mj.x; sm.y += mj.y; sm.z += mj.z;
-                }
-            }
-            ex.x += lp.cex[a] * acc.x; ex.y += lp.cex[a] * acc.y; ex.z += lp.cex[a] * acc.z;
-            S[a] = sm;
+            const bool im = pos[a] > 0, ip = pos[a] < lim[a] - 1;
+            const long pm = im ? q - str[a] : q, pp = ip ? q + str[a] : q;
+            ok[2 * a] = im && (Ms[pm] != (T)0);
+            ok[2 * a + 1] = ip && (Ms[pp] != (T)0);
+            nb[2 * a] = ld3(y, N, pm);
+            nb[2 * a + 1] = ld3(y, N, pp);
+        }
+        v3<T> ex = { 0, 0, 0 };           // sum_a cex_a sum_{+-} (m_j - m_i)
+        v3<T> S[3];                        // S_a = m_{+a} - m_{-a} over present neighbours
+#pragma unroll
+        for (int a = 0; a < 3; a++) {
+            const v3<T> mm_ = nb[2 * a], mp = nb[2 * a + 1];
+            const bool bm = ok[2 * a], bp = ok[2 * a + 1];
+            const T dmx = bm ? mm_.x - mi.x : (T)0, dmy = bm ? mm_.y - mi.y : (T)0, dmz = bm ? mm_.z - mi.z : (T)0;
+            const T dpx = bp ? mp.x - mi.x : (T)0, dpy = bp ? mp.y - mi.y : (T)0, dpz = bp ? mp.z - mi.z : (T)0;
+            ex.x += lp.cex[a] * (dmx + dpx); ex.y += lp.cex[a] * (dmy + dpy); ex.z += lp.cex[a] * (dmz + dpz);
+            S[a].x = (bp ? mp.x : (T)0) - (bm ? mm_.x : (T)0);
+            S[a].y = (bp ? mp.y : (T)0) - (bm ? mm_.y : (T)0);
+            S[a].z = (bp ? mp.z : (T)0) - (bm ? mm_.z : (T)0);
         }
         if (lp.terms & 1) { H.x += inv * ex.x; H.y += inv * ex.y; H.z += inv * ex.z; }
         if ((lp.terms & 2) && lp.dmi != 0) {

@@ -27,7 +27,7 @@ static Geom make_geom(int nx, int ny, int nz, int G, int CH, int TC)
     memset(&g, 0, sizeof(g));
     g.nx = nx; g.ny = ny; g.nz = nz;
     g.px = 2 * nx; g.py = 2 * ny; g.pz = nz > 1 ? 2 * nz : 1;
-    g.lognx = ilog2(nx); g.logpy = ilog2(g.py); g.logpz = ilog2(g.pz);
+    g.lognx = ilog2(nx); g.logny = ilog2(ny); g.logpy = ilog2(g.py); g.logpz = ilog2(g.pz);
     g.N = (long)nx * ny * nz;
     g.G = G; g.CH = CH; g.TC = TC;
     g.Lx = ((nx + 1 + TC - 1) / TC) * TC;
