@@ -40,6 +40,41 @@ template <typename T> struct alignas(2 * sizeof(T)) cx {
 };
 
 template <typename T> MM_HD cx<T> mk(T a, T b) { cx<T> r; r.x = a; r.y = b; return r; }
+
+#if defined(__CUDA_ARCH__) && !defined(MM_NO_F32X2)
+// sm_100a packed fp32 arithmetic (add/mul/fma.rn.f32x2 -> FADD2 / FMUL2 / FFMA2): one instruction
+// per complex add, two per complex multiply.  A complex number is the register pair (re, im); ptxas
+// folds the swaps, broadcasts and sign patterns below into operand modifiers of the packed
+// instructions, so none of the pack / unpack moves survive into SASS.
+#define MM_F32X2 1
+typedef unsigned long long mm_u64;
+__device__ __forceinline__ mm_u64 pk2(float lo, float hi) { mm_u64 r; asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ cx<float> upk2(mm_u64 v) { cx<float> r; asm("mov.b64 {%0,%1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(v)); return r; }
+__device__ __forceinline__ mm_u64 add2(mm_u64 a, mm_u64 b) { mm_u64 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ mm_u64 sub2(mm_u64 a, mm_u64 b) { mm_u64 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ mm_u64 mul2(mm_u64 a, mm_u64 b) { mm_u64 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ mm_u64 fma2(mm_u64 a, mm_u64 b, mm_u64 c) { mm_u64 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+__device__ __forceinline__ cx<float> operator+(cx<float> a, cx<float> b) { return upk2(add2(pk2(a.x, a.y), pk2(b.x, b.y))); }
+__device__ __forceinline__ cx<float> operator-(cx<float> a, cx<float> b) { return upk2(sub2(pk2(a.x, a.y), pk2(b.x, b.y))); }
+__device__ __forceinline__ cx<float> cmul(cx<float> a, cx<float> b)
+{
+    return upk2(fma2(pk2(a.y, a.x), pk2(-b.y, b.y), mul2(pk2(a.x, a.y), pk2(b.x, b.x))));
+}
+__device__ __forceinline__ cx<float> cmulc(cx<float> a, cx<float> b)
+{
+    return upk2(fma2(pk2(a.y, a.x), pk2(b.y, -b.y), mul2(pk2(a.x, a.y), pk2(b.x, b.x))));
+}
+__device__ __forceinline__ cx<float> scale(cx<float> a, float s) { return upk2(mul2(pk2(a.x, a.y), pk2(s, s))); }
+// a*ka + b*kb (+ c*kc), real coefficients
+__device__ __forceinline__ cx<float> lin2(cx<float> a, float ka, cx<float> b, float kb)
+{
+    return upk2(fma2(pk2(b.x, b.y), pk2(kb, kb), mul2(pk2(a.x, a.y), pk2(ka, ka))));
+}
+__device__ __forceinline__ cx<float> lin3(cx<float> a, float ka, cx<float> b, float kb, cx<float> c, float kc)
+{
+    return upk2(fma2(pk2(c.x, c.y), pk2(kc, kc), fma2(pk2(b.x, b.y), pk2(kb, kb), mul2(pk2(a.x, a.y), pk2(ka, ka)))));
+}
+#endif
 template <typename T> MM_HD cx<T> operator+(cx<T> a, cx<T> b) { return mk<T>(a.x + b.x, a.y + b.y); }
 template <typename T> MM_HD cx<T> operator-(cx<T> a, cx<T> b) { return mk<T>(a.x - b.x, a.y - b.y); }
 template <typename T> MM_HD cx<T> cmul(cx<T> a, cx<T> b) { return mk<T>(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
@@ -49,6 +84,11 @@ template <typename T> MM_HD cx<T> conj(cx<T> a) { return mk<T>(a.x, -a.y); }
 template <typename T> MM_HD cx<T> mul_mi(cx<T> a) { return mk<T>(a.y, -a.x); }   // * (-i)
 template <typename T> MM_HD cx<T> mul_pi(cx<T> a) { return mk<T>(-a.y, a.x); }   // * (+i)
 template <typename T> MM_HD cx<T> scale(cx<T> a, T s) { return mk<T>(a.x * s, a.y * s); }
+template <typename T> MM_HD cx<T> lin2(cx<T> a, T ka, cx<T> b, T kb) { return mk<T>(ka * a.x + kb * b.x, ka * a.y + kb * b.y); }
+template <typename T> MM_HD cx<T> lin3(cx<T> a, T ka, cx<T> b, T kb, cx<T> c, T kc)
+{
+    return mk<T>(ka * a.x + kb * b.x + kc * c.x, ka * a.y + kb * b.y + kc * c.y);
+}
 template <typename T> MM_HD void bf2(cx<T>& a, cx<T>& b) { cx<T> t = a; a = t + b; b = t - b; }
 
 MM_HD int ilog2(int n) { int l = 0; while ((1 << l) < n) l++; return l; }
@@ -271,7 +311,13 @@ template <typename T, int V> MM_HD cvec<T, V> mul_pi(cvec<T, V> a)
     return r;
 }
 // multiplication by a compile-time-known constant (c + i s)
-template <typename T> MM_HD cx<T> crot(cx<T> a, T c, T s) { return mk<T>(c * a.x - s * a.y, c * a.y + s * a.x); }
+template <typename T> MM_HD cx<T> crot(cx<T> a, T c, T s)
+{
+#if defined(MM_F32X2)
+    if (sizeof(T) == 4) return cmul(a, mk<T>(c, s));
+#endif
+    return mk<T>(c * a.x - s * a.y, c * a.y + s * a.x);
+}
 template <typename T, int V> MM_HD cvec<T, V> crot(cvec<T, V> a, T c, T s)
 {
     cvec<T, V> r;

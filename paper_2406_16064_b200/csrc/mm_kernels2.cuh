@@ -152,13 +152,13 @@ MM_HD void yB_mul8(const Geom& g, cx<T>* s, const T* Kz, T sz, twiddles<T> tw, i
             const cx<T> Mx = M[0][r], My = M[1][r], Mz = M[2][r];
             if (IS3D) {
                 const T kxz = sz * Kp[4 * g.kcomp], kyz = sy * sz * Kp[5 * g.kcomp];
-                M[0][r] = mk<T>(-(kxx * Mx.x + kxy * My.x + kxz * Mz.x), -(kxx * Mx.y + kxy * My.y + kxz * Mz.y));
-                M[1][r] = mk<T>(-(kxy * Mx.x + kyy * My.x + kyz * Mz.x), -(kxy * Mx.y + kyy * My.y + kyz * Mz.y));
-                M[2][r] = mk<T>(-(kxz * Mx.x + kyz * My.x + kzz * Mz.x), -(kxz * Mx.y + kyz * My.y + kzz * Mz.y));
+                M[0][r] = lin3<T>(Mx, -kxx, My, -kxy, Mz, -kxz);
+                M[1][r] = lin3<T>(Mx, -kxy, My, -kyy, Mz, -kyz);
+                M[2][r] = lin3<T>(Mx, -kxz, My, -kyz, Mz, -kzz);
             } else {
-                M[0][r] = mk<T>(-(kxx * Mx.x + kxy * My.x), -(kxx * Mx.y + kxy * My.y));
-                M[1][r] = mk<T>(-(kxy * Mx.x + kyy * My.x), -(kxy * Mx.y + kyy * My.y));
-                M[2][r] = mk<T>(-(kzz * Mz.x), -(kzz * Mz.y));
+                M[0][r] = lin2<T>(Mx, -kxx, My, -kxy);
+                M[1][r] = lin2<T>(Mx, -kxy, My, -kyy);
+                M[2][r] = scale<T>(Mz, -kzz);
             }
         }
 #pragma unroll
@@ -179,6 +179,11 @@ MM_HD void y_conv_body2(const Geom g, cx<T>* __restrict__ S, const T* __restrict
     const int x0 = (bid % ntile) * g.TC, zq = bid / ntile;
     const int m = g.ny;
     cx<T>* Sz = S + (long)zq * g.plane + x0;
+    const int kz = (int)brev((unsigned)zq, g.logpz);
+    const bool is3d = g.nz > 1;
+    const int kzp = is3d ? (kz <= g.nz ? kz : g.pz - kz) : 0;
+    const T sz = (is3d && kz > g.nz) ? (T)-1 : (T)1;
+    const T* Kz = Kh + (long)kzp * g.kplane + x0;
     const int R1 = first_radix(m);
     if (R1 == 8) yB_first<T, V, 8>(g, Sz, s, tw, tid, nthr);
     else if (R1 == 4) yB_first<T, V, 4>(g, Sz, s, tw, tid, nthr);
@@ -186,11 +191,6 @@ MM_HD void y_conv_body2(const Geom g, cx<T>* __restrict__ S, const T* __restrict
     MM_SYNC();
     int Lc = m / R1;
     for (; Lc > 8; Lc >>= 3) { yB_mid8<T, V, 0>(g, s, Lc, tw, tid, nthr); MM_SYNC(); }
-    const int kz = (int)brev((unsigned)zq, g.logpz);
-    const bool is3d = g.nz > 1;
-    const int kzp = is3d ? (kz <= g.nz ? kz : g.pz - kz) : 0;
-    const T sz = (is3d && kz > g.nz) ? (T)-1 : (T)1;
-    const T* Kz = Kh + (long)kzp * g.kplane + x0;
     if (is3d) yB_mul8<T, true>(g, s, Kz, sz, tw, tid, nthr);
     else yB_mul8<T, false>(g, s, Kz, sz, tw, tid, nthr);
     MM_SYNC();
