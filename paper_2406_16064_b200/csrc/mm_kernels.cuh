@@ -31,9 +31,34 @@ struct Geom {
     long comp;             // pz * plane     (one component of S)
     long kplane;           // (ny+1) * Lx    (one kz' plane of K^)
     long kcomp;            // (nz>1 ? nz+1 : 1) * kplane
+    int flags;             // tuning bits (MM_FLAGS), 0 = defaults
 };
 
 MM_HD int odd_pitch(int n) { return n | 1; }
+
+// K^ in the order pass B (v2) consumes it, "Kc": one contiguous tile per (kz', x tile); inside a tile
+// element (b8, j, col) with j = r*NQ + q (r = row inside the radix-8 block b8, q = tensor component)
+// sits at ((b8*NJQ + j/EPL)*TC + col)*EPL + j%EPL, EPL = reals per 16-byte load.  Values are -K^ with
+// the ky mirror sign of the odd components baked in (all py positions are stored).
+MM_HD int kc_nq(const Geom& g) { return g.nz > 1 ? 6 : 4; }
+MM_HD long kc_tile_elems(const Geom& g) { return (long)g.py * kc_nq(g) * g.TC; }
+MM_HD long kc_elems(const Geom& g) { return (long)(g.nz > 1 ? g.nz + 1 : 1) * (g.Lx / g.TC) * kc_tile_elems(g); }
+template <typename T> MM_HD void kc_fill(const Geom& g, const T* Kh, T* Kc, long idx)
+{
+    const int NQ = kc_nq(g), EPL = 16 / (int)sizeof(T), NJQ = 8 * NQ / EPL, ntile = g.Lx / g.TC;
+    const long tile = kc_tile_elems(g);
+    const long t = idx / tile;
+    long o = idx - t * tile;
+    const int kzp = (int)(t / ntile), xt = (int)(t % ntile);
+    const int e = (int)(o % EPL); o /= EPL;
+    const int col = (int)(o % g.TC); o /= g.TC;
+    const int jq = (int)(o % NJQ), b8 = (int)(o / NJQ);
+    const int j = jq * EPL + e, r = j / NQ, q = j - r * NQ;
+    const int ky = (int)brev((unsigned)(b8 * 8 + r), g.logpy);
+    const int kyp = ky <= g.ny ? ky : g.py - ky;
+    const T v = Kh[(long)q * g.kcomp + (long)kzp * g.kplane + (long)kyp * g.Lx + xt * g.TC + col];
+    Kc[idx] = (ky > g.ny && (q == 3 || q == 5)) ? v : -v;
+}
 
 // shared memory (in complex elements) of passes A/C and B
 MM_HD long smemA_elems(const Geom& g)

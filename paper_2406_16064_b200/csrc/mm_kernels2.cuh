@@ -126,15 +126,36 @@ MM_HD void yB_mid8(const Geom& g, cx<T>* s, int Lc, twiddles<T> tw, int tid, int
     }
 }
 
-// last forward radix-8 stage (Lc = 8) + multiply by K^ + first inverse stage, three components in registers
-template <typename T, bool IS3D>
-MM_HD void yB_mul8(const Geom& g, cx<T>* s, const T* Kz, T sz, twiddles<T> tw, int tid, int nthr)
+template <typename T> struct alignas(16) kvec { T e[16 / sizeof(T)]; };
+
+MM_HD void prefetch_l2_bulk(const void* p, unsigned bytes)
 {
+#if defined(__CUDA_ARCH__)
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+#else
+    (void)p; (void)bytes;
+#endif
+}
+
+// last forward radix-8 stage (Lc = 8) + multiply by K^ + first inverse stage, three components in
+// registers.  Kt = this CTA's tile of Kc (mm_kernels.cuh): NJ/EPL 16-byte loads per thread.
+template <typename T, bool IS3D>
+MM_HD void yB_mul8(const Geom& g, cx<T>* s, const T* Kt, T sz, int tid, int nthr)
+{
+    constexpr int NQ = IS3D ? 6 : 4, NJ = 8 * NQ, EPL = 16 / (int)sizeof(T), NJQ = NJ / EPL;
     const int TC = g.TC, logTC = ilog2(TC), pitch = 3 * TC;
-    const int n = g.py, ny = g.ny;
+    const int n = g.py;
     for (int f = tid; f < (n >> 3) * TC; f += nthr) {
         const int col = f & (TC - 1), b8 = f >> logTC;
         cx<T>* p = s + (b8 * 8) * pitch + col;
+        const T* Kp = Kt + (long)b8 * (NJ * TC) + col * EPL;
+        T K[NJ];
+#pragma unroll
+        for (int jq = 0; jq < NJQ; jq++) {
+            const kvec<T> v = *reinterpret_cast<const kvec<T>*>(Kp + jq * TC * EPL);
+#pragma unroll
+            for (int e = 0; e < EPL; e++) K[jq * EPL + e] = v.e[e];
+        }
         cx<T> M[3][8];
 #pragma unroll
         for (int c = 0; c < 3; c++) {
@@ -144,21 +165,17 @@ MM_HD void yB_mul8(const Geom& g, cx<T>* s, const T* Kz, T sz, twiddles<T> tw, i
         }
 #pragma unroll
         for (int r = 0; r < 8; r++) {
-            const int ky = (int)brev((unsigned)(b8 * 8 + r), g.logpy);
-            const int kyp = ky <= ny ? ky : n - ky;
-            const T sy = ky > ny ? (T)-1 : (T)1;
-            const T* Kp = Kz + (long)kyp * g.Lx + col;
-            const T kxx = Kp[0], kyy = Kp[g.kcomp], kzz = Kp[2 * g.kcomp], kxy = sy * Kp[3 * g.kcomp];
+            const T kxx = K[r * NQ], kyy = K[r * NQ + 1], kzz = K[r * NQ + 2], kxy = K[r * NQ + 3];
             const cx<T> Mx = M[0][r], My = M[1][r], Mz = M[2][r];
             if (IS3D) {
-                const T kxz = sz * Kp[4 * g.kcomp], kyz = sy * sz * Kp[5 * g.kcomp];
-                M[0][r] = lin3<T>(Mx, -kxx, My, -kxy, Mz, -kxz);
-                M[1][r] = lin3<T>(Mx, -kxy, My, -kyy, Mz, -kyz);
-                M[2][r] = lin3<T>(Mx, -kxz, My, -kyz, Mz, -kzz);
+                const T kxz = sz * K[r * NQ + (IS3D ? 4 : 0)], kyz = sz * K[r * NQ + (IS3D ? 5 : 0)];
+                M[0][r] = lin3<T>(Mx, kxx, My, kxy, Mz, kxz);
+                M[1][r] = lin3<T>(Mx, kxy, My, kyy, Mz, kyz);
+                M[2][r] = lin3<T>(Mx, kxz, My, kyz, Mz, kzz);
             } else {
-                M[0][r] = lin2<T>(Mx, -kxx, My, -kxy);
-                M[1][r] = lin2<T>(Mx, -kxy, My, -kyy);
-                M[2][r] = scale<T>(Mz, -kzz);
+                M[0][r] = lin2<T>(Mx, kxx, My, kxy);
+                M[1][r] = lin2<T>(Mx, kxy, My, kyy);
+                M[2][r] = scale<T>(Mz, kzz);
             }
         }
 #pragma unroll
@@ -172,7 +189,7 @@ MM_HD void yB_mul8(const Geom& g, cx<T>* s, const T* Kz, T sz, twiddles<T> tw, i
 
 // requires ny >= 16 (so the schedule has >= 2 stages and ends with radix 8) and TC % V == 0
 template <typename T, int V>
-MM_HD void y_conv_body2(const Geom g, cx<T>* __restrict__ S, const T* __restrict__ Kh, twiddles<T> tw, cx<T>* s,
+MM_HD void y_conv_body2(const Geom g, cx<T>* __restrict__ S, const T* __restrict__ Kc, twiddles<T> tw, cx<T>* s,
                         int bid, int tid, int nthr)
 {
     const int ntile = g.Lx / g.TC;
@@ -183,16 +200,18 @@ MM_HD void y_conv_body2(const Geom g, cx<T>* __restrict__ S, const T* __restrict
     const bool is3d = g.nz > 1;
     const int kzp = is3d ? (kz <= g.nz ? kz : g.pz - kz) : 0;
     const T sz = (is3d && kz > g.nz) ? (T)-1 : (T)1;
-    const T* Kz = Kh + (long)kzp * g.kplane + x0;
+    const T* Kt = Kc + ((long)kzp * ntile + bid % ntile) * kc_tile_elems(g);
     const int R1 = first_radix(m);
     if (R1 == 8) yB_first<T, V, 8>(g, Sz, s, tw, tid, nthr);
     else if (R1 == 4) yB_first<T, V, 4>(g, Sz, s, tw, tid, nthr);
     else yB_first<T, V, 2>(g, Sz, s, tw, tid, nthr);
     MM_SYNC();
+    // the K^ tile of the multiply stage towards L2 while the middle stages run
+    if (!(g.flags & 1) && tid == 0) prefetch_l2_bulk(Kt, (unsigned)(kc_tile_elems(g) * sizeof(T)));
     int Lc = m / R1;
     for (; Lc > 8; Lc >>= 3) { yB_mid8<T, V, 0>(g, s, Lc, tw, tid, nthr); MM_SYNC(); }
-    if (is3d) yB_mul8<T, true>(g, s, Kz, sz, tw, tid, nthr);
-    else yB_mul8<T, false>(g, s, Kz, sz, tw, tid, nthr);
+    if (is3d) yB_mul8<T, true>(g, s, Kt, sz, tid, nthr);
+    else yB_mul8<T, false>(g, s, Kt, sz, tid, nthr);
     MM_SYNC();
     for (Lc = 64; Lc <= m / R1; Lc <<= 3) { yB_mid8<T, V, 1>(g, s, Lc, tw, tid, nthr); MM_SYNC(); }
     if (R1 == 8) yB_last<T, V, 8>(g, Sz, s, tw, tid, nthr);

@@ -13,8 +13,14 @@
 #include "mm_fft.cuh"
 #include "mm_kernels.cuh"
 #include "mm_kernels2.cuh"
-#include "mm_passB.cuh"
 #include "mm_llg.cuh"
+
+#ifndef MM_OCC_A
+#define MM_OCC_A 3      // resident CTAs per SM the fp32 pass A kernel is compiled for
+#endif
+#ifndef MM_OCC_C
+#define MM_OCC_C 2
+#endif
 
 extern "C" void mm_newell_near_box(int bx, int by, int bz, double dx, double dy, double dz, double* out);
 
@@ -56,7 +62,7 @@ __global__ void __launch_bounds__(256) inv_zx_kernel(Geom g, const cx<T>* S, T* 
 
 // v2 wrappers (mm_kernels2.cuh)
 template <typename T, int NZ>
-__global__ void __launch_bounds__(256) fwd_xz2_kernel(Geom g, const T* m, const T* Ms, cx<T>* S, twiddles<T> tw, const DevState* st)
+__global__ void __launch_bounds__(256, sizeof(T) == 8 ? 1 : MM_OCC_A) fwd_xz2_kernel(Geom g, const T* m, const T* Ms, cx<T>* S, twiddles<T> tw, const DevState* st)
 {
     if (st->done) return;
     fwd_xz_body2<T, NZ>(g, m, Ms, S, tw, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x);
@@ -67,14 +73,8 @@ __global__ void __launch_bounds__(sizeof(T) == 8 ? 256 : 512) y_conv2_kernel(Geo
     if (st->done) return;
     y_conv_body2<T, V>(g, S, Kh, tw, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x);
 }
-template <typename T, int V>
-__global__ void __launch_bounds__(256, 2) y_conv3_kernel(Geom g, const cx<T>* Sin, cx<T>* Sout, const T* Kh, twiddles<T> tw, const DevState* st)
-{
-    if (st->done) return;
-    y_conv_body3<T, V>(g, Sin, Sout, Kh, tw, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x);
-}
 template <typename T, int NZ>
-__global__ void __launch_bounds__(256) inv_zx2_kernel(Geom g, const cx<T>* S, T* Hd, twiddles<T> tw, T inv_scale, const DevState* st)
+__global__ void __launch_bounds__(256, sizeof(T) == 8 ? 1 : MM_OCC_C) inv_zx2_kernel(Geom g, const cx<T>* S, T* Hd, twiddles<T> tw, T inv_scale, const DevState* st)
 {
     if (st->done) return;
     inv_zx_body2<T, NZ>(g, S, Hd, tw, inv_scale, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x);
@@ -356,6 +356,12 @@ __global__ void __launch_bounds__(256) pack_khat_kernel(Geom g, int comp, const 
     block_max_bits(norm_bits(fabs(im)), maxbits + 1);
 }
 
+template <typename T> __global__ void __launch_bounds__(256) kc_fill_kernel(Geom g, const T* __restrict__ Kh, T* __restrict__ Kc, long total)
+{
+    const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx < total) kc_fill<T>(g, Kh, Kc, idx);
+}
+
 }  // namespace mm
 
 // ================================================================================================
@@ -374,16 +380,16 @@ struct mm_sim {
     // workspace
     void* ws;
     size_t ws_bytes, ws_need;
-    size_t off_Ms, off_S, off_S2, off_Kh, off_Hd, off_k[7], off_y[2], off_tw, off_Nr, off_st, off_part;
+    size_t off_Ms, off_S, off_Kh, off_Kc, off_Hd, off_k[7], off_y[2], off_tw, off_Nr, off_st, off_part;
     int twN;
-    size_t smemA, smemB;
+    size_t smemA, smemA2, smemB;
     int thrA, thrB;
     double khat_imag_ratio;
     double t_host;
     long launches;
     std::string err;
     // optional per-pass profiling (mm_set_profiling): event pairs around each kernel class
-    int use_v2, use_b3;
+    int use_v2;
     int prof_on;
     std::vector<cudaEvent_t> prof_ev;      // pairs
     std::vector<int> prof_cls;             // class of pair i: 0 pass A, 1 pass B, 2 pass C, 3 stage kernel
@@ -444,9 +450,7 @@ static void configure(mm_sim* s)
     int TC = s->prec == MM_F64 ? 4 : 8;
     if (getenv("MM_TC")) TC = atoi(getenv("MM_TC"));       // tuning knob (power of two)
     g.TC = TC;
-    s->use_b3 = s->use_v2 && g.ny >= 16 && getenv("MM_B3");
-    if (s->use_b3) { while (g.TC > 1 && (size_t)smemB3_elems(g) * cs > 100 * 1024) g.TC /= 2; }
-    else while (g.TC > 1 && (size_t)smemB_elems(g) * cs > SMEM_CAP) g.TC /= 2;
+    while (g.TC > 1 && (size_t)smemB_elems(g) * cs > SMEM_CAP) g.TC /= 2;
     while (g.TC > 2 && ((g.nx + g.TC) / g.TC) * g.pz < target) g.TC /= 2;
     g.Lx = ((g.nx + 1 + g.TC - 1) / g.TC) * g.TC;
     g.plane = (long)g.ny * g.Lx;
@@ -454,9 +458,11 @@ static void configure(mm_sim* s)
     g.kplane = (long)(g.ny + 1) * g.Lx;
     g.kcomp = (long)(g.nz > 1 ? g.nz + 1 : 1) * g.kplane;
     s->smemA = (size_t)smemA_elems(g) * cs;
-    s->smemB = (size_t)(s->use_b3 ? smemB3_elems(g) : smemB_elems(g)) * cs;
+    // the v2 bodies of passes A / C do the z transform in registers: no scratch tile
+    s->smemA2 = (size_t)(g.nx + 1) * odd_pitch(g.G * g.nz) * cs;
+    s->smemB = (size_t)smemB_elems(g) * cs;
     s->thrA = 256;
-    s->thrB = (!s->use_b3 && s->prec == MM_F32 && s->smemB > 64 * 1024) ? 512 : 256;
+    s->thrB = (s->prec == MM_F32 && s->smemB > 64 * 1024) ? 512 : 256;
     if (getenv("MM_THRB")) s->thrB = atoi(getenv("MM_THRB"));
 }
 
@@ -469,8 +475,8 @@ static void layout(mm_sim* s)
     s->off_st = take(sizeof(DevState));
     s->off_Ms = take(N * es);
     s->off_S = take((size_t)3 * g.comp * 2 * es);
-    s->off_S2 = s->use_b3 ? take((size_t)3 * g.comp * 2 * es) : s->off_S;      // pass B v3 output (in place otherwise)
     s->off_Kh = take((size_t)6 * g.kcomp * es);
+    s->off_Kc = take((s->use_v2 && g.ny >= 16 ? (size_t)kc_elems(g) : 0) * es);      // pass B v2: K^ in consumption order
     s->off_Hd = take(3 * N * es);
     for (int i = 0; i < 7; i++) s->off_k[i] = take(3 * N * es);
     for (int i = 0; i < 2; i++) s->off_y[i] = take(3 * N * es);
@@ -505,6 +511,7 @@ extern "C" int mm_create(mm_sim** out, int nx, int ny, int nz, double dx, double
     if (g.pz > s->twN) s->twN = g.pz;
     if (s->twN < 4) s->twN = 4;
     configure(s);
+    if (getenv("MM_FLAGS")) g.flags = atoi(getenv("MM_FLAGS"));
     layout(s);
     *out = s;
     return MM_OK;
@@ -701,6 +708,12 @@ template <typename T> static int init_demag_t(mm_sim* s)
         s->launches++;
         MM_TRY(s, cudaGetLastError());
     }
+    if (s->use_v2 && g.ny >= 16) {
+        const long total = kc_elems(g);
+        kc_fill_kernel<T><<<(unsigned)((total + 255) / 256), 256, 0, st>>>(g, Kh, wsp<T>(s, s->off_Kc), total);
+        s->launches++;
+        MM_TRY(s, cudaGetLastError());
+    }
     unsigned long long hmax[2];
     MM_TRY(s, cudaMemcpyAsync(hmax, d_max, sizeof(hmax), cudaMemcpyDeviceToHost, st));
     MM_TRY(s, cudaStreamSynchronize(st));
@@ -773,26 +786,19 @@ template <typename T, int NZ> static void launch_A2(mm_sim* s, unsigned grid, co
 {
     static bool attr = false;
     if (!attr) { cudaFuncSetAttribute(fwd_xz2_kernel<T, NZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_CAP); attr = true; }
-    fwd_xz2_kernel<T, NZ><<<grid, s->thrA, s->smemA, s->stream>>>(s->g, y, wsp<T>(s, s->off_Ms), S, tw, st);
+    fwd_xz2_kernel<T, NZ><<<grid, s->thrA, s->smemA2, s->stream>>>(s->g, y, wsp<T>(s, s->off_Ms), S, tw, st);
 }
 template <typename T, int NZ> static void launch_C2(mm_sim* s, unsigned grid, cx<T>* S, twiddles<T> tw, T sc, const DevState* st)
 {
     static bool attr = false;
     if (!attr) { cudaFuncSetAttribute(inv_zx2_kernel<T, NZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_CAP); attr = true; }
-    inv_zx2_kernel<T, NZ><<<grid, s->thrA, s->smemA, s->stream>>>(s->g, S, wsp<T>(s, s->off_Hd), tw, sc, st);
+    inv_zx2_kernel<T, NZ><<<grid, s->thrA, s->smemA2, s->stream>>>(s->g, S, wsp<T>(s, s->off_Hd), tw, sc, st);
 }
 template <typename T, int V> static void launch_B2(mm_sim* s, unsigned grid, cx<T>* S, twiddles<T> tw, const DevState* st)
 {
     static bool attr = false;
     if (!attr) { cudaFuncSetAttribute(y_conv2_kernel<T, V>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_CAP); attr = true; }
-    y_conv2_kernel<T, V><<<grid, s->thrB, s->smemB, s->stream>>>(s->g, S, wsp<T>(s, s->off_Kh), tw, st);
-}
-
-template <typename T, int V> static void launch_B3(mm_sim* s, unsigned grid, const cx<T>* S, cx<T>* S2, twiddles<T> tw, const DevState* st)
-{
-    static bool attr = false;
-    if (!attr) { cudaFuncSetAttribute(y_conv3_kernel<T, V>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_CAP); attr = true; }
-    y_conv3_kernel<T, V><<<grid, s->thrB, s->smemB, s->stream>>>(s->g, S, S2, wsp<T>(s, s->off_Kh), tw, st);
+    y_conv2_kernel<T, V><<<grid, s->thrB, s->smemB, s->stream>>>(s->g, S, wsp<T>(s, s->off_Kc), tw, st);
 }
 
 template <typename T> static int demag_passes(mm_sim* s, const T* y)
@@ -801,7 +807,6 @@ template <typename T> static int demag_passes(mm_sim* s, const T* y)
     twiddles<T> tw; tw.tw = wsp<cx<T>>(s, s->off_tw); tw.twN = s->twN;
     const DevState* st = wsp<DevState>(s, s->off_st);
     cx<T>* S = wsp<cx<T>>(s, s->off_S);
-    cx<T>* S2 = wsp<cx<T>>(s, s->off_S2);
     const unsigned gridA = 3u * (unsigned)(g.ny / g.G), gridB = (unsigned)(g.Lx / g.TC) * (unsigned)g.pz;
     const double P = (double)g.px * g.py * g.pz;
     const bool a2 = s->use_v2 && g.nx >= 32 && g.nz <= (sizeof(T) == 8 ? 16 : 32);
@@ -818,22 +823,19 @@ template <typename T> static int demag_passes(mm_sim* s, const T* y)
     }
     prof_end(s);
     prof_begin(s, 1);
-    if (s->use_b3) {
-        if (sizeof(T) == 4 && g.TC % 2 == 0) launch_B3<T, (sizeof(T) == 4 ? 2 : 1)>(s, gridB, S, S2, tw, st);
-        else launch_B3<T, 1>(s, gridB, S, S2, tw, st);
-    } else if (!b2) y_conv_kernel<T><<<gridB, s->thrB, s->smemB, s->stream>>>(g, S, wsp<T>(s, s->off_Kh), tw, st);
+    if (!b2) y_conv_kernel<T><<<gridB, s->thrB, s->smemB, s->stream>>>(g, S, wsp<T>(s, s->off_Kh), tw, st);
     else if (sizeof(T) == 4 && g.TC % 2 == 0) launch_B2<T, (sizeof(T) == 4 ? 2 : 1)>(s, gridB, S, tw, st);
     else launch_B2<T, 1>(s, gridB, S, tw, st);
     prof_end(s);
     prof_begin(s, 2);
-    if (!a2) inv_zx_kernel<T><<<gridA, s->thrA, s->smemA, s->stream>>>(g, S2, wsp<T>(s, s->off_Hd), tw, (T)(1.0 / P), st);
+    if (!a2) inv_zx_kernel<T><<<gridA, s->thrA, s->smemA, s->stream>>>(g, S, wsp<T>(s, s->off_Hd), tw, (T)(1.0 / P), st);
     else switch (g.nz) {
-        case 1: launch_C2<T, 1>(s, gridA, S2, tw, (T)(1.0 / P), st); break;
-        case 2: launch_C2<T, 2>(s, gridA, S2, tw, (T)(1.0 / P), st); break;
-        case 4: launch_C2<T, 4>(s, gridA, S2, tw, (T)(1.0 / P), st); break;
-        case 8: launch_C2<T, 8>(s, gridA, S2, tw, (T)(1.0 / P), st); break;
-        case 16: launch_C2<T, 16>(s, gridA, S2, tw, (T)(1.0 / P), st); break;
-        default: launch_C2<T, 32>(s, gridA, S2, tw, (T)(1.0 / P), st); break;
+        case 1: launch_C2<T, 1>(s, gridA, S, tw, (T)(1.0 / P), st); break;
+        case 2: launch_C2<T, 2>(s, gridA, S, tw, (T)(1.0 / P), st); break;
+        case 4: launch_C2<T, 4>(s, gridA, S, tw, (T)(1.0 / P), st); break;
+        case 8: launch_C2<T, 8>(s, gridA, S, tw, (T)(1.0 / P), st); break;
+        case 16: launch_C2<T, 16>(s, gridA, S, tw, (T)(1.0 / P), st); break;
+        default: launch_C2<T, 32>(s, gridA, S, tw, (T)(1.0 / P), st); break;
     }
     prof_end(s);
     s->launches += 3;

@@ -7,7 +7,6 @@
 #include <vector>
 #include "../../paper_2406_16064_b200/csrc/mm_kernels.cuh"
 #include "../../paper_2406_16064_b200/csrc/mm_kernels2.cuh"
-#include "../../paper_2406_16064_b200/csrc/mm_passB.cuh"
 #include "../../paper_2406_16064_b200/csrc/mm_llg.cuh"
 
 using namespace mm;
@@ -56,6 +55,8 @@ static void run(int ver, int nx, int ny, int nz, int G, int CH, int TC, const do
                     Kh[(size_t)c * g.kcomp + (size_t)kz * g.kplane + (size_t)ky * g.Lx + xp] =
                         (T)Kfull[(((size_t)c * g.pz + kz) * g.py + ky) * g.px + kx];
                 }
+    std::vector<T> Kc(ny >= 16 ? (size_t)kc_elems(g) : 0);
+    for (long i = 0; i < (long)Kc.size(); i++) kc_fill<T>(g, Kh.data(), Kc.data(), i);
     std::vector<T> mt(3 * g.N), Mst(g.N), Hdt(3 * g.N);
     for (long i = 0; i < 3 * g.N; i++) mt[i] = (T)m[i];
     for (long i = 0; i < g.N; i++) Mst[i] = (T)Ms[i];
@@ -64,9 +65,7 @@ static void run(int ver, int nx, int ny, int nz, int G, int CH, int TC, const do
     std::vector<cx<T>> smem((size_t)(smemA_elems(g) > smemB_elems(g) ? smemA_elems(g) : smemB_elems(g)) + 16);
     const int gridA = 3 * (ny / G), gridB = (g.Lx / TC) * g.pz;
     const double P = (double)g.px * g.py * g.pz;
-    const bool a2 = ver >= 2 && nx >= 32 && nz <= 32, b2 = ver == 2 && ny >= 16, b3 = ver == 3 && ny >= 16;
-    std::vector<cx<T>> S2v(b3 ? S.size() : 0);
-    cx<T>* S2 = b3 ? S2v.data() : S.data();
+    const bool a2 = ver == 2 && nx >= 32 && nz <= 32, b2 = ver == 2 && ny >= 16;
     for (int b = 0; b < gridA; b++) {
         if (!a2) fwd_xz_body<T>(g, mt.data(), Mst.data(), S.data(), tw, smem.data(), b, 0, 1);
         else switch (nz) {
@@ -75,17 +74,14 @@ static void run(int ver, int nx, int ny, int nz, int G, int CH, int TC, const do
         }
     }
     for (int b = 0; b < gridB; b++) {
-        if (b3) {
-            if (sizeof(T) == 4 && TC % 2 == 0) y_conv_body3<T, (sizeof(T) == 4 ? 2 : 1)>(g, S.data(), S2, Kh.data(), tw, smem.data(), b, 0, 1);
-            else y_conv_body3<T, 1>(g, S.data(), S2, Kh.data(), tw, smem.data(), b, 0, 1);
-        } else if (!b2) y_conv_body<T>(g, S.data(), Kh.data(), tw, smem.data(), b, 0, 1);
-        else if (sizeof(T) == 4 && TC % 2 == 0) y_conv_body2<T, (sizeof(T) == 4 ? 2 : 1)>(g, S.data(), Kh.data(), tw, smem.data(), b, 0, 1);
-        else y_conv_body2<T, 1>(g, S.data(), Kh.data(), tw, smem.data(), b, 0, 1);
+        if (!b2) y_conv_body<T>(g, S.data(), Kh.data(), tw, smem.data(), b, 0, 1);
+        else if (sizeof(T) == 4 && TC % 2 == 0) y_conv_body2<T, (sizeof(T) == 4 ? 2 : 1)>(g, S.data(), Kc.data(), tw, smem.data(), b, 0, 1);
+        else y_conv_body2<T, 1>(g, S.data(), Kc.data(), tw, smem.data(), b, 0, 1);
     }
     for (int b = 0; b < gridA; b++) {
-        if (!a2) inv_zx_body<T>(g, S2, Hdt.data(), tw, (T)(1.0 / P), smem.data(), b, 0, 1);
+        if (!a2) inv_zx_body<T>(g, S.data(), Hdt.data(), tw, (T)(1.0 / P), smem.data(), b, 0, 1);
         else switch (nz) {
-#define CASE_C(NZ) case NZ: inv_zx_body2<T, NZ>(g, S2, Hdt.data(), tw, (T)(1.0 / P), smem.data(), b, 0, 1); break;
+#define CASE_C(NZ) case NZ: inv_zx_body2<T, NZ>(g, S.data(), Hdt.data(), tw, (T)(1.0 / P), smem.data(), b, 0, 1); break;
             CASE_C(1) CASE_C(2) CASE_C(4) CASE_C(8) CASE_C(16) CASE_C(32)
         }
     }
