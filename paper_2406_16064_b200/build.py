@@ -24,7 +24,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     obj_cpp = os.path.join(CSRC, "mm_newell_host.o")
     cmds = [
         [NVCC, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
-         "-c", os.path.join(CSRC, "mm_lib.cu"), "-o", obj_cu] + (["-Xptxas", "-v"] if verbose else []),
+         "-c", os.path.join(CSRC, "mm_lib.cu"), "-o", obj_cu] + (["-Xptxas", "-v"] if verbose else []) + os.environ.get("MM_NVCC_FLAGS", "").split(),
         ["g++", "-O2", "-std=gnu++17", "-fPIC", "-c", os.path.join(CSRC, "mm_newell_host.cpp"), "-o", obj_cpp],
         [NVCC, "-shared", "-o", LIB, obj_cu, obj_cpp, "-lquadmath", "-lpthread"],
     ]

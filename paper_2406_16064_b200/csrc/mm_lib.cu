@@ -169,6 +169,153 @@ __global__ void __launch_bounds__(256) llg_stage_kernel(Geom g, LocalP<T> lp, co
     if (MODE == 1 && MAXK) block_max_bits(norm_bits(kn), &st->maxk_bits);
 }
 
+// Vectorised form of llg_stage_kernel: one thread owns CPT consecutive cells along x (16 bytes per
+// load: 4 fp32 / 2 fp64 cells), so every centre value, every earlier k_j and both outputs move as
+// 16-byte accesses; y / z neighbours are 16-byte loads of the neighbouring rows, x neighbours come
+// from the thread's own vector plus one scalar on each side.  Same per-cell arithmetic (and
+// operation order) as local_field() / ll_torque() in mm_llg.cuh.  Requires nx % CPT == 0.
+template <typename T, int CPT> struct alignas(CPT * sizeof(T)) cellvec { T e[CPT]; };
+template <typename T, int CPT> __device__ __forceinline__ cellvec<T, CPT> ldc(const T* p) { return *reinterpret_cast<const cellvec<T, CPT>*>(p); }
+template <typename T, int CPT> __device__ __forceinline__ void stc(T* p, const cellvec<T, CPT>& v) { *reinterpret_cast<cellvec<T, CPT>*>(p) = v; }
+
+#ifndef MM_STAGEV_THREADS
+#define MM_STAGEV_THREADS 128
+#endif
+#ifndef MM_STAGEV_CPT
+#define MM_STAGEV_CPT 2      // cells per thread (8-byte loads in fp32, 16-byte in fp64): measured best on B200
+#endif
+template <typename T, int CPT, int MODE, int S, bool NEXT, bool ERR, bool MAXK>
+__global__ void __launch_bounds__(MM_STAGEV_THREADS, sizeof(T) == 8 ? 1 : 4) llg_stagev_kernel(Geom g, LocalP<T> lp, const T* __restrict__ y, const T* __restrict__ Ms,
+                                                         const T* __restrict__ Hd, T* __restrict__ out, StageArgs<T> sa, DevState* st)
+{
+    if (st->done) return;
+    typedef cellvec<T, CPT> CV;
+    const long N = g.N;
+    const long q = ((long)blockIdx.x * blockDim.x + threadIdx.x) * CPT;
+    unsigned long long eb = 0ull, kb = 0ull;      // bit patterns: max keeps a NaN
+    if (q < N) {
+        const int i0 = (int)(q & (g.nx - 1)), j = (int)((q >> g.lognx) & (g.ny - 1)), k = (int)(q >> (g.lognx + g.logny));
+        const CV Msv = ldc<T, CPT>(Ms + q);
+        CV m[3], H[3];
+#pragma unroll
+        for (int c = 0; c < 3; c++) m[c] = ldc<T, CPT>(y + c * N + q);
+        if (Hd != nullptr) {
+#pragma unroll
+            for (int c = 0; c < 3; c++) H[c] = ldc<T, CPT>(Hd + c * N + q);
+        } else {
+#pragma unroll
+            for (int c = 0; c < 3; c++)
+#pragma unroll
+                for (int e = 0; e < CPT; e++) H[c].e[e] = 0;
+        }
+        CV kj[S > 0 ? S : 1][3];
+#pragma unroll
+        for (int jj = 0; jj < S; jj++)
+#pragma unroll
+            for (int c = 0; c < 3; c++) kj[jj][c] = ldc<T, CPT>(sa.kprev[jj] + c * N + q);
+        CV m0[3];
+        if (NEXT) {
+#pragma unroll
+            for (int c = 0; c < 3; c++) m0[c] = ldc<T, CPT>(sa.m0 + c * N + q);
+        }
+        if ((lp.terms & 3) != 0) {
+            // neighbour rows: index clamped to the own row when outside the mesh, then masked
+            const long sy = g.nx, szz = (long)g.nx * g.ny;
+            const bool oym = j > 0, oyp = j < g.ny - 1, ozm = k > 0, ozp = k < g.nz - 1, oxm = i0 > 0, oxp = i0 + CPT < g.nx;
+            const long qym = oym ? q - sy : q, qyp = oyp ? q + sy : q, qzm = ozm ? q - szz : q, qzp = ozp ? q + szz : q;
+            const long qxm = oxm ? q - 1 : q, qxp = oxp ? q + CPT : q;
+            CV nym[3], nyp[3], nzm[3], nzp[3];
+            const CV Mym = ldc<T, CPT>(Ms + qym), Myp = ldc<T, CPT>(Ms + qyp), Mzm = ldc<T, CPT>(Ms + qzm), Mzp = ldc<T, CPT>(Ms + qzp);
+            T xl[3], xr[3];
+            const T Mxl = Ms[qxm], Mxr = Ms[qxp];
+#pragma unroll
+            for (int c = 0; c < 3; c++) {
+                nym[c] = ldc<T, CPT>(y + c * N + qym); nyp[c] = ldc<T, CPT>(y + c * N + qyp);
+                nzm[c] = ldc<T, CPT>(y + c * N + qzm); nzp[c] = ldc<T, CPT>(y + c * N + qzp);
+                xl[c] = y[c * N + qxm]; xr[c] = y[c * N + qxp];
+            }
+#pragma unroll
+            for (int e = 0; e < CPT; e++) {
+                const T Msi = Msv.e[e];
+                const T inv = (T)1 / (Msi != (T)0 ? Msi : (T)1);
+                const v3<T> mi = { m[0].e[e], m[1].e[e], m[2].e[e] };
+                v3<T> nb[6];
+                bool ok[6];
+                // -x / +x
+                if (e > 0) { ok[0] = Msv.e[e > 0 ? e - 1 : 0] != (T)0; nb[0] = { m[0].e[e > 0 ? e - 1 : 0], m[1].e[e > 0 ? e - 1 : 0], m[2].e[e > 0 ? e - 1 : 0] }; }
+                else { ok[0] = oxm && Mxl != (T)0; nb[0] = { xl[0], xl[1], xl[2] }; }
+                if (e < CPT - 1) { ok[1] = Msv.e[e < CPT - 1 ? e + 1 : 0] != (T)0; nb[1] = { m[0].e[e < CPT - 1 ? e + 1 : 0], m[1].e[e < CPT - 1 ? e + 1 : 0], m[2].e[e < CPT - 1 ? e + 1 : 0] }; }
+                else { ok[1] = oxp && Mxr != (T)0; nb[1] = { xr[0], xr[1], xr[2] }; }
+                ok[2] = oym && Mym.e[e] != (T)0; nb[2] = { nym[0].e[e], nym[1].e[e], nym[2].e[e] };
+                ok[3] = oyp && Myp.e[e] != (T)0; nb[3] = { nyp[0].e[e], nyp[1].e[e], nyp[2].e[e] };
+                ok[4] = ozm && Mzm.e[e] != (T)0; nb[4] = { nzm[0].e[e], nzm[1].e[e], nzm[2].e[e] };
+                ok[5] = ozp && Mzp.e[e] != (T)0; nb[5] = { nzp[0].e[e], nzp[1].e[e], nzp[2].e[e] };
+                v3<T> h = { H[0].e[e], H[1].e[e], H[2].e[e] };
+                h = local_field_nb<T>(lp, inv, mi, nb, ok, h);
+                H[0].e[e] = h.x; H[1].e[e] = h.y; H[2].e[e] = h.z;
+            }
+        } else {
+#pragma unroll
+            for (int e = 0; e < CPT; e++) {
+                const T Msi = Msv.e[e];
+                const T inv = (T)1 / (Msi != (T)0 ? Msi : (T)1);
+                const v3<T> mi = { m[0].e[e], m[1].e[e], m[2].e[e] };
+                v3<T> h = { H[0].e[e], H[1].e[e], H[2].e[e] };
+                h = local_field_rest<T>(lp, inv, mi, h);
+                H[0].e[e] = h.x; H[1].e[e] = h.y; H[2].e[e] = h.z;
+            }
+        }
+        CV res[3];
+#pragma unroll
+        for (int e = 0; e < CPT; e++) {
+            const bool live = Msv.e[e] != (T)0;
+            const v3<T> mi = { m[0].e[e], m[1].e[e], m[2].e[e] };
+            const v3<T> h = { H[0].e[e], H[1].e[e], H[2].e[e] };
+            v3<T> r = MODE == 0 ? h : ll_torque<T>(lp, mi, h);
+            if (!live) { r.x = 0; r.y = 0; r.z = 0; }
+            res[0].e[e] = r.x; res[1].e[e] = r.y; res[2].e[e] = r.z;
+            if (MODE == 1 && MAXK && live) { const unsigned long long b = norm_bits(sqrt(r.x * r.x + r.y * r.y + r.z * r.z)); kb = b > kb ? b : kb; }
+        }
+#pragma unroll
+        for (int c = 0; c < 3; c++) stc<T, CPT>(out + c * N + q, res[c]);
+        if (MODE == 1 && (NEXT || ERR)) {
+            const T dt = (T)st->dt;
+            if (NEXT) {
+#pragma unroll
+                for (int c = 0; c < 3; c++) {
+                    CV yn;
+#pragma unroll
+                    for (int e = 0; e < CPT; e++) {
+                        T acc = sa.coef[S] * res[c].e[e];
+#pragma unroll
+                        for (int jj = 0; jj < S; jj++) acc += sa.coef[jj] * kj[jj][c].e[e];
+                        yn.e[e] = m0[c].e[e] + dt * acc;
+                    }
+                    stc<T, CPT>(sa.ynext + c * N + q, yn);
+                }
+            }
+            if (ERR) {
+#pragma unroll
+                for (int e = 0; e < CPT; e++) {
+                    T ea[3];
+#pragma unroll
+                    for (int c = 0; c < 3; c++) {
+                        ea[c] = sa.ecoef[S] * res[c].e[e];
+#pragma unroll
+                        for (int jj = 0; jj < S; jj++) ea[c] += sa.ecoef[jj] * kj[jj][c].e[e];
+                    }
+                    if (Msv.e[e] != (T)0) {
+                        const unsigned long long b = norm_bits(sqrt((dt * ea[0]) * (dt * ea[0]) + (dt * ea[1]) * (dt * ea[1]) + (dt * ea[2]) * (dt * ea[2])));
+                        eb = b > eb ? b : eb;
+                    }
+                }
+            }
+        }
+    }
+    if (MODE == 1 && ERR) block_max_bits(eb, &st->err_bits);
+    if (MODE == 1 && MAXK) block_max_bits(kb, &st->maxk_bits);
+}
+
 // Step controller: one thread.  DESIGN.md R8.
 __global__ void ctrl_kernel(DevState* st, int is_f64, int adaptive_mode)
 {
@@ -847,6 +994,12 @@ template <typename T> static int demag_passes(mm_sim* s, const T* y)
 template <typename T, int MODE, int S, bool NEXT, bool ERR, bool MAXK>
 static void launch_stage(mm_sim* s, const LocalP<T>& lp, const T* y, const T* Hd, T* out, const StageArgs<T>& sa)
 {
+    constexpr int CPT = MM_STAGEV_CPT;
+    if (s->g.nx % CPT == 0 && !getenv("MM_NO_STAGEV")) {
+        const unsigned blocks = (unsigned)((s->g.N / CPT + MM_STAGEV_THREADS - 1) / MM_STAGEV_THREADS);
+        llg_stagev_kernel<T, CPT, MODE, S, NEXT, ERR, MAXK><<<blocks, MM_STAGEV_THREADS, 0, s->stream>>>(s->g, lp, y, wsp<T>(s, s->off_Ms), Hd, out, sa, wsp<DevState>(s, s->off_st));
+        return;
+    }
     const unsigned blocks = (unsigned)((s->g.N + 255) / 256);
     llg_stage_kernel<T, MODE, S, NEXT, ERR, MAXK><<<blocks, 256, 0, s->stream>>>(s->g, lp, y, wsp<T>(s, s->off_Ms), Hd, out, sa, wsp<DevState>(s, s->off_st));
 }

@@ -23,6 +23,50 @@ template <typename T> struct LocalP {
 template <typename T> struct v3 { T x, y, z; };
 template <typename T> MM_HD v3<T> ld3(const T* p, long N, long q) { v3<T> r; r.x = p[q]; r.y = p[N + q]; r.z = p[2 * N + q]; return r; }
 
+// anisotropy + Zeeman part of H_eff (inv = 1/Ms_i)
+template <typename T> MM_HD v3<T> local_field_rest(const LocalP<T>& lp, T inv, v3<T> mi, v3<T> H)
+{
+    if (lp.terms & 4) {
+        const T f = inv * lp.cku * (mi.x * lp.u[0] + mi.y * lp.u[1] + mi.z * lp.u[2]);
+        H.x += f * lp.u[0]; H.y += f * lp.u[1]; H.z += f * lp.u[2];
+    }
+    if (lp.terms & 8) { H.x += lp.hext[0]; H.y += lp.hext[1]; H.z += lp.hext[2]; }
+    return H;
+}
+
+// H_eff from the six neighbour values nb[-x,+x,-y,+y,-z,+z] (ok[] = neighbour present) added to H
+template <typename T> MM_HD v3<T> local_field_nb(const LocalP<T>& lp, T inv, v3<T> mi, const v3<T>* nb, const bool* ok, v3<T> H)
+{
+    v3<T> ex = { 0, 0, 0 };           // sum_a cex_a sum_{+-} (m_j - m_i)
+    v3<T> S[3];                        // S_a = m_{+a} - m_{-a} over present neighbours
+#pragma unroll
+    for (int a = 0; a < 3; a++) {
+        const v3<T> mm_ = nb[2 * a], mp = nb[2 * a + 1];
+        const bool bm = ok[2 * a], bp = ok[2 * a + 1];
+        const T dmx = bm ? mm_.x - mi.x : (T)0, dmy = bm ? mm_.y - mi.y : (T)0, dmz = bm ? mm_.z - mi.z : (T)0;
+        const T dpx = bp ? mp.x - mi.x : (T)0, dpy = bp ? mp.y - mi.y : (T)0, dpz = bp ? mp.z - mi.z : (T)0;
+        ex.x += lp.cex[a] * (dmx + dpx); ex.y += lp.cex[a] * (dmy + dpy); ex.z += lp.cex[a] * (dmz + dpz);
+        S[a].x = (bp ? mp.x : (T)0) - (bm ? mm_.x : (T)0);
+        S[a].y = (bp ? mp.y : (T)0) - (bm ? mm_.y : (T)0);
+        S[a].z = (bp ? mp.z : (T)0) - (bm ? mm_.z : (T)0);
+    }
+    if (lp.terms & 1) { H.x += inv * ex.x; H.y += inv * ex.y; H.z += inv * ex.z; }
+    if ((lp.terms & 2) && lp.dmi != 0) {
+        v3<T> d;
+        if (lp.dmi == 1) {      // bulk: e_ij = r^_ij  =>  sum_a cdm_a (a^ x S_a)
+            d.x = lp.cdm[1] * S[1].z - lp.cdm[2] * S[2].y;
+            d.y = -lp.cdm[0] * S[0].z + lp.cdm[2] * S[2].x;
+            d.z = lp.cdm[0] * S[0].y - lp.cdm[1] * S[1].x;
+        } else {                // interfacial: e_ij = z^ x r^_ij : (y^ x S_x) - (x^ x S_y)
+            d.x = lp.cdm[0] * S[0].z;
+            d.y = lp.cdm[1] * S[1].z;
+            d.z = -lp.cdm[0] * S[0].x - lp.cdm[1] * S[1].y;
+        }
+        H.x -= inv * d.x; H.y -= inv * d.y; H.z -= inv * d.z;
+    }
+    return local_field_rest<T>(lp, inv, mi, H);
+}
+
 // H_eff at cell (i,j,k) given H_d (or 0).  y = stage magnetisation.  Branch-free in the data: every
 // neighbour is loaded (index clamped to the cell itself when outside the mesh) and then selected,
 // so all loads of a thread are in flight together.
@@ -32,54 +76,21 @@ MM_HD v3<T> local_field(const Geom& g, const LocalP<T>& lp, const T* __restrict_
 {
     const long N = g.N;
     const T inv = (T)1 / Msi;
-    if ((lp.terms & 3) != 0) {
-        const long str[3] = { 1, g.nx, (long)g.nx * g.ny };
-        const int pos[3] = { i, j, k }, lim[3] = { g.nx, g.ny, g.nz };
-        v3<T> nb[6];
-        bool ok[6];
+    if ((lp.terms & 3) == 0) return local_field_rest<T>(lp, inv, mi, H);
+    const long str[3] = { 1, g.nx, (long)g.nx * g.ny };
+    const int pos[3] = { i, j, k }, lim[3] = { g.nx, g.ny, g.nz };
+    v3<T> nb[6];
+    bool ok[6];
 #pragma unroll
-        for (int a = 0; a < 3; a++) {
-            const bool im = pos[a] > 0, ip = pos[a] < lim[a] - 1;
-            const long pm = im ? q - str[a] : q, pp = ip ? q + str[a] : q;
-            ok[2 * a] = im && (Ms[pm] != (T)0);
-            ok[2 * a + 1] = ip && (Ms[pp] != (T)0);
-            nb[2 * a] = ld3(y, N, pm);
-            nb[2 * a + 1] = ld3(y, N, pp);
-        }
-        v3<T> ex = { 0, 0, 0 };           // sum_a cex_a sum_{+-} (m_j - m_i)
-        v3<T> S[3];                        // S_a = m_{+a} - m_{-a} over present neighbours
-#pragma unroll
-        for (int a = 0; a < 3; a++) {
-            const v3<T> mm_ = nb[2 * a], mp = nb[2 * a + 1];
-            const bool bm = ok[2 * a], bp = ok[2 * a + 1];
-            const T dmx = bm ? mm_.x - mi.x : (T)0, dmy = bm ? mm_.y - mi.y : (T)0, dmz = bm ? mm_.z - mi.z : (T)0;
-            const T dpx = bp ? mp.x - mi.x : (T)0, dpy = bp ? mp.y - mi.y : (T)0, dpz = bp ? mp.z - mi.z : (T)0;
-            ex.x += lp.cex[a] * (dmx + dpx); ex.y += lp.cex[a] * (dmy + dpy); ex.z += lp.cex[a] * (dmz + dpz);
-            S[a].x = (bp ? mp.x : (T)0) - (bm ? mm_.x : (T)0);
-            S[a].y = (bp ? mp.y : (T)0) - (bm ? mm_.y : (T)0);
-            S[a].z = (bp ? mp.z : (T)0) - (bm ? mm_.z : (T)0);
-        }
-        if (lp.terms & 1) { H.x += inv * ex.x; H.y += inv * ex.y; H.z += inv * ex.z; }
-        if ((lp.terms & 2) && lp.dmi != 0) {
-            v3<T> d;
-            if (lp.dmi == 1) {      // bulk: e_ij = r^_ij  =>  sum_a cdm_a (a^ x S_a)
-                d.x = lp.cdm[1] * S[1].z - lp.cdm[2] * S[2].y;
-                d.y = -lp.cdm[0] * S[0].z + lp.cdm[2] * S[2].x;
-                d.z = lp.cdm[0] * S[0].y - lp.cdm[1] * S[1].x;
-            } else {                // interfacial: e_ij = z^ x r^_ij : (y^ x S_x) - (x^ x S_y)
-                d.x = lp.cdm[0] * S[0].z;
-                d.y = lp.cdm[1] * S[1].z;
-                d.z = -lp.cdm[0] * S[0].x - lp.cdm[1] * S[1].y;
-            }
-            H.x -= inv * d.x; H.y -= inv * d.y; H.z -= inv * d.z;
-        }
+    for (int a = 0; a < 3; a++) {
+        const bool im = pos[a] > 0, ip = pos[a] < lim[a] - 1;
+        const long pm = im ? q - str[a] : q, pp = ip ? q + str[a] : q;
+        ok[2 * a] = im && (Ms[pm] != (T)0);
+        ok[2 * a + 1] = ip && (Ms[pp] != (T)0);
+        nb[2 * a] = ld3(y, N, pm);
+        nb[2 * a + 1] = ld3(y, N, pp);
     }
-    if (lp.terms & 4) {
-        const T f = inv * lp.cku * (mi.x * lp.u[0] + mi.y * lp.u[1] + mi.z * lp.u[2]);
-        H.x += f * lp.u[0]; H.y += f * lp.u[1]; H.z += f * lp.u[2];
-    }
-    if (lp.terms & 8) { H.x += lp.hext[0]; H.y += lp.hext[1]; H.z += lp.hext[2]; }
-    return H;
+    return local_field_nb<T>(lp, inv, mi, nb, ok, H);
 }
 
 template <typename T> MM_HD v3<T> ll_torque(const LocalP<T>& lp, v3<T> m, v3<T> H)
