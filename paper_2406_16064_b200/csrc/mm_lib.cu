@@ -13,6 +13,7 @@
 #include "mm_fft.cuh"
 #include "mm_kernels.cuh"
 #include "mm_kernels2.cuh"
+#include "mm_passAC.cuh"
 #include "mm_llg.cuh"
 
 #ifndef MM_OCC_A
@@ -65,7 +66,7 @@ template <typename T, int NZ>
 __global__ void __launch_bounds__(256, sizeof(T) == 8 ? 1 : MM_OCC_A) fwd_xz2_kernel(Geom g, const T* m, const T* Ms, cx<T>* S, twiddles<T> tw, const DevState* st)
 {
     if (st->done) return;
-    fwd_xz_body2<T, NZ>(g, m, Ms, S, tw, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x);
+    fwd_xz_body3<T, NZ>(g, m, Ms, S, tw, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x);
 }
 template <typename T, int V>
 __global__ void __launch_bounds__(sizeof(T) == 8 ? 256 : 512) y_conv2_kernel(Geom g, cx<T>* S, const T* Kh, twiddles<T> tw, const DevState* st)
@@ -77,7 +78,7 @@ template <typename T, int NZ>
 __global__ void __launch_bounds__(256, sizeof(T) == 8 ? 1 : MM_OCC_C) inv_zx2_kernel(Geom g, const cx<T>* S, T* Hd, twiddles<T> tw, T inv_scale, const DevState* st)
 {
     if (st->done) return;
-    inv_zx_body2<T, NZ>(g, S, Hd, tw, inv_scale, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x);
+    inv_zx_body3<T, NZ>(g, S, Hd, tw, inv_scale, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x);
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -20,7 +20,7 @@ _dp = C.POINTER(C.c_double)
 
 @pytest.fixture(scope="module")
 def emul():
-    deps = [SRC] + [os.path.join(ROOT, "paper_2406_16064_b200", "csrc", f) for f in ("mm_fft.cuh", "mm_kernels.cuh", "mm_kernels2.cuh", "mm_llg.cuh")]
+    deps = [SRC] + [os.path.join(ROOT, "paper_2406_16064_b200", "csrc", f) for f in ("mm_fft.cuh", "mm_kernels.cuh", "mm_kernels2.cuh", "mm_passAC.cuh", "mm_llg.cuh")]
     if not os.path.exists(LIB) or os.path.getmtime(LIB) < max(os.path.getmtime(d) for d in deps):
         subprocess.run(["g++", "-O1", "-std=c++17", "-fPIC", "-shared", "-o", LIB, SRC], check=True)
     L = C.CDLL(LIB)
