@@ -16,6 +16,17 @@
 
 namespace mm {
 
+// Pass B tile: row pitch 3*TC complex plus MM_PADB bytes after every 8 rows.  MM_PADB = 64 makes the
+// multiply stage (one column per lane, 8-byte accesses, 8-row blocks) bank-conflict free, but on
+// cfg4 the tile then exceeds the 196 KB shared-memory carve-out, the SM falls to the 228 KB one
+// with no L1 left for the twiddle / K^ loads, and the pass gets 6 % SLOWER (measured, B200) — so 0.
+#ifndef MM_PADB
+#define MM_PADB 0
+#endif
+template <typename T> MM_HD int padB() { return MM_PADB / (int)sizeof(cx<T>); }
+template <typename T> MM_HD int rowB(int row, int pitch) { return row * pitch + (row >> 3) * padB<T>(); }
+template <typename T> MM_HD long smemB2_elems(const Geom& g) { return (long)g.py * 3 * g.TC + (g.py >> 3) * padB<T>(); }
+
 template <typename E, typename T> MM_HD E ldv(const cx<T>* p) { return *reinterpret_cast<const E*>(p); }
 template <typename E, typename T> MM_HD void stv(cx<T>* p, const E& v) { *reinterpret_cast<E*>(p) = v; }
 
@@ -38,7 +49,8 @@ MM_HD void yB_first(const Geom& g, const cx<T>* Sz, cx<T>* s, twiddles<T> tw, in
 #pragma unroll
         for (int c = 0; c < 3; c++) {
             const cx<T>* src = Sz + (long)c * g.comp + (long)i * g.Lx + lc * V;
-            cx<T>* dst = s + i * pitch + c * TC + lc * V;
+            cx<T>* dst = s + rowB<T>(i, pitch) + c * TC + lc * V;
+            const int rs = rowB<T>(sub, pitch), mo = rowB<T>(m, pitch);
             E a[R], u[R];
 #pragma unroll
             for (int r = 0; r < R; r++) a[r] = ldv<E, T>(src + (long)r * sub * g.Lx);
@@ -51,7 +63,7 @@ MM_HD void yB_first(const Geom& g, const cx<T>* Sz, cx<T>* s, twiddles<T> tw, in
                 for (int r = 1; r < R; r++) { a[r] = cmul(a[r], pw[r]); u[r] = cmul(u[r], pw[r]); }
             }
 #pragma unroll
-            for (int r = 0; r < R; r++) { stv<E, T>(dst + r * sub * pitch, a[r]); stv<E, T>(dst + (m + r * sub) * pitch, u[r]); }
+            for (int r = 0; r < R; r++) { stv<E, T>(dst + r * rs, a[r]); stv<E, T>(dst + mo + r * rs, u[r]); }
         }
     }
 }
@@ -72,10 +84,11 @@ MM_HD void yB_last(const Geom& g, cx<T>* Sz, const cx<T>* s, twiddles<T> tw, int
 #pragma unroll
         for (int c = 0; c < 3; c++) {
             cx<T>* dstg = Sz + (long)c * g.comp + (long)i * g.Lx + lc * V;
-            const cx<T>* src = s + i * pitch + c * TC + lc * V;
+            const cx<T>* src = s + rowB<T>(i, pitch) + c * TC + lc * V;
+            const int rs = rowB<T>(sub, pitch), mo = rowB<T>(m, pitch);
             E a[R], u[R];
 #pragma unroll
-            for (int r = 0; r < R; r++) { a[r] = ldv<E, T>(src + r * sub * pitch); u[r] = ldv<E, T>(src + (m + r * sub) * pitch); }
+            for (int r = 0; r < R; r++) { a[r] = ldv<E, T>(src + r * rs); u[r] = ldv<E, T>(src + mo + r * rs); }
             if (i != 0) {
 #pragma unroll
                 for (int r = 1; r < R; r++) { a[r] = cmulc(a[r], pw[r]); u[r] = cmulc(u[r], pw[r]); }
@@ -100,13 +113,14 @@ MM_HD void yB_mid8(const Geom& g, cx<T>* s, int Lc, twiddles<T> tw, int tid, int
         const int blk = b >> logsub, i = b & (sub - 1);
         cx<T> pw[8];
         if (i != 0) twiddle_powers<T, 8>(tw.get(i, Lc), pw);
-        cx<T>* base = s + (blk * Lc + i) * pitch + lc * V;
+        cx<T>* base = s + rowB<T>(blk * Lc + i, pitch) + lc * V;
+        const int rs = rowB<T>(sub, pitch);
 #pragma unroll
         for (int c = 0; c < 3; c++) {
             cx<T>* p = base + c * TC;
             E v[8];
 #pragma unroll
-            for (int r = 0; r < 8; r++) v[r] = ldv<E, T>(p + r * sub * pitch);
+            for (int r = 0; r < 8; r++) v[r] = ldv<E, T>(p + r * rs);
             if (DIR == 0) {
                 rad<E, 8>::fwd(v);
                 if (i != 0) {
@@ -121,7 +135,7 @@ MM_HD void yB_mid8(const Geom& g, cx<T>* s, int Lc, twiddles<T> tw, int tid, int
                 rad<E, 8>::inv(v);
             }
 #pragma unroll
-            for (int r = 0; r < 8; r++) stv<E, T>(p + r * sub * pitch, v[r]);
+            for (int r = 0; r < 8; r++) stv<E, T>(p + r * rs, v[r]);
         }
     }
 }
@@ -147,7 +161,7 @@ MM_HD void yB_mul8(const Geom& g, cx<T>* s, const T* Kt, T sz, int tid, int nthr
     const int n = g.py;
     for (int f = tid; f < (n >> 3) * TC; f += nthr) {
         const int col = f & (TC - 1), b8 = f >> logTC;
-        cx<T>* p = s + (b8 * 8) * pitch + col;
+        cx<T>* p = s + rowB<T>(b8 * 8, pitch) + col;
         const T* Kp = Kt + (long)b8 * (NJ * TC) + col * EPL;
         T K[NJ];
 #pragma unroll
@@ -222,42 +236,6 @@ MM_HD void y_conv_body2(const Geom g, cx<T>* __restrict__ S, const T* __restrict
 // ------------------------------------------------------------------------------------------------
 // Passes A / C v2 (x transform of packed pairs with m = nx/2, n = nx; z transform in registers)
 // ------------------------------------------------------------------------------------------------
-// generic radix-8 middle stage for the x tile: lines fastest in groups of LG lines sharing twiddles
-template <typename T, int DIR>
-MM_HD void xs_mid8(cx<T>* s, int pitch, int L, int n, int Lc, twiddles<T> tw, int tid, int nthr)
-{
-    const int LG = L < 4 ? L : 4, NG = L / LG, logNG = ilog2(NG);
-    const int sub = Lc >> 3, logsub = ilog2(sub);
-    for (int f = tid; f < (n >> 3) * NG; f += nthr) {
-        const int lg = f & (NG - 1), b = f >> logNG;
-        const int blk = b >> logsub, i = b & (sub - 1);
-        cx<T> pw[8];
-        if (i != 0) twiddle_powers<T, 8>(tw.get(i, Lc), pw);
-        cx<T>* base = s + (blk * Lc + i) * pitch + lg * LG;
-        for (int t = 0; t < LG; t++) {
-            cx<T>* p = base + t;
-            cx<T> v[8];
-#pragma unroll
-            for (int r = 0; r < 8; r++) v[r] = p[r * sub * pitch];
-            if (DIR == 0) {
-                rad<cx<T>, 8>::fwd(v);
-                if (i != 0) {
-#pragma unroll
-                    for (int r = 1; r < 8; r++) v[r] = cmul(v[r], pw[r]);
-                }
-            } else {
-                if (i != 0) {
-#pragma unroll
-                    for (int r = 1; r < 8; r++) v[r] = cmulc(v[r], pw[r]);
-                }
-                rad<cx<T>, 8>::inv(v);
-            }
-#pragma unroll
-            for (int r = 0; r < 8; r++) p[r * sub * pitch] = v[r];
-        }
-    }
-}
-
 // first x stage: load Ms*m pairs from global (i fastest: coalesced), pad twiddle, radix R, both blocks
 template <typename T, int R>
 MM_HD void xA_first(const Geom& g, const T* mc, const T* Ms, cx<T>* s, int pitch, int j0, twiddles<T> tw, int tid, int nthr)
@@ -355,34 +333,6 @@ MM_HD void x_split_merge(const Geom& g, cx<T>* s, int pitch, twiddles<T> tw, int
     }
 }
 
-// z transform in registers, forward: tile -> S.  One item per (x position, row gg).
-template <typename T, int NZ>
-MM_HD void zA_regs(const Geom& g, cx<T>* Sc, const cx<T>* s, int pitch, int j0, twiddles<T> tw, int tid, int nthr)
-{
-    const int np = g.nx + 1;
-    for (int f = tid; f < np * g.G; f += nthr) {
-        const int xp = f % np, gg = f / np;
-        const cx<T>* src = s + xp * pitch + gg * NZ;
-        cx<T>* dst = Sc + (long)(j0 + gg) * g.Lx + xp;
-        cx<T> a[NZ];
-#pragma unroll
-        for (int z = 0; z < NZ; z++) a[z] = src[z];
-        {
-            cx<T> v[NZ];
-#pragma unroll
-            for (int z = 0; z < NZ; z++) v[z] = a[z];
-            rad<cx<T>, NZ>::fwd(v);
-#pragma unroll
-            for (int z = 0; z < NZ; z++) dst[(long)z * g.plane] = v[z];
-        }
-#pragma unroll
-        for (int z = 1; z < NZ; z++) a[z] = cmul(a[z], tw.get(z, 2 * NZ));
-        rad<cx<T>, NZ>::fwd(a);
-#pragma unroll
-        for (int z = 0; z < NZ; z++) dst[(long)(NZ + z) * g.plane] = a[z];
-    }
-}
-
 // z transform in registers, inverse + crop: S -> tile
 template <typename T, int NZ>
 MM_HD void zC_regs(const Geom& g, const cx<T>* Sc, cx<T>* s, int pitch, int j0, twiddles<T> tw, int tid, int nthr)
@@ -401,59 +351,6 @@ MM_HD void zC_regs(const Geom& g, const cx<T>* Sc, cx<T>* s, int pitch, int j0, 
 #pragma unroll
         for (int z = 1; z < NZ; z++) dst[z] = a[z] + cmulc(u[z], tw.get(z, 2 * NZ));
     }
-}
-
-// NZ = 0: nz > 32 (not supported by v2; host falls back to v1).  Requires nx >= 32.
-template <typename T, int NZ>
-MM_HD void fwd_xz_body2(const Geom g, const T* __restrict__ mvec, const T* __restrict__ Ms, cx<T>* __restrict__ S,
-                        twiddles<T> tw, cx<T>* s, int bid, int tid, int nthr)
-{
-    const int c = bid % 3, j0 = (bid / 3) * g.G;
-    const int n = g.nx, m = n / 2, L = g.G * g.nz, pitch = odd_pitch(L);
-    const T* mc = mvec + (long)c * g.N;
-    const int R1 = first_radix(m);
-    if (R1 == 8) xA_first<T, 8>(g, mc, Ms, s, pitch, j0, tw, tid, nthr);
-    else if (R1 == 4) xA_first<T, 4>(g, mc, Ms, s, pitch, j0, tw, tid, nthr);
-    else xA_first<T, 2>(g, mc, Ms, s, pitch, j0, tw, tid, nthr);
-    MM_SYNC();
-    for (int Lc = m / R1; Lc > 1; Lc >>= 3) { xs_mid8<T, 0>(s, pitch, L, n, Lc, tw, tid, nthr); MM_SYNC(); }
-    x_split_merge<T, 0>(g, s, pitch, tw, tid, nthr);
-    MM_SYNC();
-    cx<T>* Sc = S + (long)c * g.comp;
-    if (NZ == 1) {
-        for (int f = tid; f < L * (n + 1); f += nthr) {
-            const int xp = f % (n + 1), l = f / (n + 1);
-            Sc[(long)(j0 + l) * g.Lx + xp] = s[xp * pitch + l];
-        }
-    } else {
-        zA_regs<T, NZ>(g, Sc, s, pitch, j0, tw, tid, nthr);
-    }
-}
-
-template <typename T, int NZ>
-MM_HD void inv_zx_body2(const Geom g, const cx<T>* __restrict__ S, T* __restrict__ Hd, twiddles<T> tw, T inv_scale,
-                        cx<T>* s, int bid, int tid, int nthr)
-{
-    const int c = bid % 3, j0 = (bid / 3) * g.G;
-    const int n = g.nx, m = n / 2, L = g.G * g.nz, pitch = odd_pitch(L);
-    const cx<T>* Sc = S + (long)c * g.comp;
-    if (NZ == 1) {
-        for (int f = tid; f < L * (n + 1); f += nthr) {
-            const int xp = f % (n + 1), l = f / (n + 1);
-            s[xp * pitch + l] = Sc[(long)(j0 + l) * g.Lx + xp];
-        }
-    } else {
-        zC_regs<T, NZ>(g, Sc, s, pitch, j0, tw, tid, nthr);
-    }
-    MM_SYNC();
-    x_split_merge<T, 1>(g, s, pitch, tw, tid, nthr);
-    MM_SYNC();
-    const int R1 = first_radix(m);
-    for (int Lc = 8; Lc <= m / R1; Lc <<= 3) { xs_mid8<T, 1>(s, pitch, L, n, Lc, tw, tid, nthr); MM_SYNC(); }
-    T* Hc = Hd + (long)c * g.N;
-    if (R1 == 8) xC_last<T, 8>(g, Hc, s, pitch, j0, inv_scale, tw, tid, nthr);
-    else if (R1 == 4) xC_last<T, 4>(g, Hc, s, pitch, j0, inv_scale, tw, tid, nthr);
-    else xC_last<T, 2>(g, Hc, s, pitch, j0, inv_scale, tw, tid, nthr);
 }
 
 }  // namespace mm

@@ -598,7 +598,7 @@ static void configure(mm_sim* s)
     int TC = s->prec == MM_F64 ? 4 : 8;
     if (getenv("MM_TC")) TC = atoi(getenv("MM_TC"));       // tuning knob (power of two)
     g.TC = TC;
-    while (g.TC > 1 && (size_t)smemB_elems(g) * cs > SMEM_CAP) g.TC /= 2;
+    while (g.TC > 1 && (size_t)smemB_elems(g) * cs + (size_t)(g.py / 8) * MM_PADB > SMEM_CAP) g.TC /= 2;
     while (g.TC > 2 && ((g.nx + g.TC) / g.TC) * g.pz < target) g.TC /= 2;
     g.Lx = ((g.nx + 1 + g.TC - 1) / g.TC) * g.TC;
     g.plane = (long)g.ny * g.Lx;
@@ -608,7 +608,7 @@ static void configure(mm_sim* s)
     s->smemA = (size_t)smemA_elems(g) * cs;
     // the v2 bodies of passes A / C do the z transform in registers: no scratch tile
     s->smemA2 = (size_t)(g.nx + 1) * odd_pitch(g.G * g.nz) * cs;
-    s->smemB = (size_t)smemB_elems(g) * cs;
+    s->smemB = (size_t)smemB_elems(g) * cs + (s->use_v2 && g.ny >= 16 ? (size_t)(g.py / 8) * MM_PADB : 0);      // v2: padded 8-row blocks
     s->thrA = 256;
     s->thrB = (s->prec == MM_F32 && s->smemB > 64 * 1024) ? 512 : 256;
     if (getenv("MM_THRB")) s->thrB = atoi(getenv("MM_THRB"));

@@ -63,7 +63,7 @@ static void run(int ver, int nx, int ny, int nz, int G, int CH, int TC, const do
     for (long i = 0; i < g.N; i++) Mst[i] = (T)Ms[i];
     std::vector<cx<T>> S((size_t)3 * g.comp);
     memset(S.data(), 0, S.size() * sizeof(cx<T>));
-    std::vector<cx<T>> smem((size_t)(smemA_elems(g) > smemB_elems(g) ? smemA_elems(g) : smemB_elems(g)) + 16);
+    std::vector<cx<T>> smem((size_t)(smemA_elems(g) > smemB2_elems<T>(g) ? smemA_elems(g) : smemB2_elems<T>(g)) + 16);
     const int gridA = 3 * (ny / G), gridB = (g.Lx / TC) * g.pz;
     const double P = (double)g.px * g.py * g.pz;
     const bool a2 = ver == 2 && nx >= 32 && nz <= 32, b2 = ver == 2 && ny >= 16;
