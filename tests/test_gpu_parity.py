@@ -256,3 +256,68 @@ def test_edge_cases_and_errors():
     bad[0, 0, 3, 3] = float("nan")
     with pytest.raises(MMError):
         s2.step(bad, 1e-14, 1e-6)
+
+
+# ---------------------------------------------------------------------------------------------
+# Full BASELINE.json sizes, in the launch configuration bench.py times (default Sim of the workload)
+# ---------------------------------------------------------------------------------------------
+def test_cfg4_full_size_sampled_direct_sum():
+    """configs[3] (512x512x16): the demag field of Eq. 8 at sampled cells, each computed by the oracle as
+    the plain O(N) sum over all source cells with its quad-precision tensor; fp64 and fp32."""
+    from paper_2406_16064_b200 import Sim
+    w = wl.cfg4()
+    o = oracle.Oracle(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz)
+    o.set_Ms(w.Ms_array())
+    o.init_demag()
+    m = np.ascontiguousarray(w.m0)
+    rng = np.random.default_rng(4004)
+    cells = [0, w.nx - 1, w.N - 1, (w.nx * w.ny) * 7 + w.nx * 255 + 256] + [int(c) for c in rng.integers(0, w.N, 20)]
+    ref = np.array([o.demag_direct_at(m, c) for c in cells])
+    for prec in (F64, F32):
+        s = Sim(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, prec=prec)
+        wl.apply(s, w)
+        s.set_A(0.0); s.set_D(0.0, 0); s.set_Ku(0.0); s.set_H_ext(0, 0, 0)      # demag term alone
+        H = to_np(s.effective_field(s.to_device(m))).reshape(3, -1)
+        got = np.array([H[:, c] for c in cells])
+        assert np.abs(got - ref).max() / w.Ms_max <= HTOL[prec], (prec, np.abs(got - ref).max() / w.Ms_max)
+        del s
+
+
+@pytest.mark.parametrize("case", ["cfg4", "film4096_f32", "film2048_f64", "film1024_f64"])
+def test_full_size_block_aggregation_identity(case):
+    """Uniformly magnetised full mesh: the MEAN demag field is -Ms N_self(block) m exactly, with N_self the
+    Newell self term of the whole block as one cell (SURVEY.md §8c pins; holds at any size)."""
+    from paper_2406_16064_b200 import Sim
+    if case == "cfg4":
+        w, precs = wl.cfg4(with_m=False), (F64, F32)
+    else:
+        n = int(case.split("_")[0][4:])
+        w, precs = wl.cfg5(n, with_m=False), ((F32,) if case.endswith("f32") else (F64,))
+    nself = oracle.newell_point(0, 0, 0, w.nx * w.dx, w.ny * w.dy, w.nz * w.dz)[:3]
+    u = np.array([0.36, -0.48, 0.8])
+    m = np.ascontiguousarray(np.broadcast_to(u.reshape(3, 1, 1, 1), (3, w.nz, w.ny, w.nx)))
+    for prec in precs:
+        s = Sim(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, prec=prec)
+        wl.apply(s, w)
+        s.set_A(0.0); s.set_D(0.0, 0); s.set_Ku(0.0); s.set_H_ext(0, 0, 0)
+        H = s.effective_field(s.to_device(m)).double().reshape(3, -1).mean(dim=1).cpu().numpy()
+        ref = -w.Ms_max * np.array(nself) * u
+        assert np.abs(H - ref).max() / w.Ms_max <= (1e-10 if prec == F64 else 2e-5), (case, prec, H, ref)
+        del s
+
+
+def test_cfg4_full_size_step_invariants():
+    """configs[3] in bench.py's configuration (fp32, fixed-dt DOPRI5): |m| = 1 after every step, finite,
+    and the energy does not increase (alpha > 0, constant field)."""
+    from paper_2406_16064_b200 import Sim
+    import torch
+    w = wl.cfg4()
+    s = Sim(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, prec=F32)
+    wl.apply(s, w)
+    dm = s.to_device(w.m0)
+    E0 = s.energy(dm)[0]
+    for _ in range(5):
+        s.step(dm, w.dt, sync=False)
+    nrm = torch.sqrt((dm.double() ** 2).sum(dim=0))
+    assert bool(torch.isfinite(dm).all()) and float((nrm - 1).abs().max()) < 1e-5
+    assert s.energy(dm)[0] < E0
