@@ -26,6 +26,13 @@ UNIT = "cell-updates/s"
 RHS_PER_STEP = 7
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
+# (profiles/r01_ncu_full_v3.md); None where no capture of that kernel / workload / precision exists.
+NCU_TRAFFIC = {("cfg4_slab_512x512x16", "f32", "y_conv"): 526.2e6 + 181.7e6,
+               ("cfg4_slab_512x512x16", "f32", "fwd_xz"): 68.3e6 + 160.6e6,
+               ("cfg4_slab_512x512x16", "f32", "inv_zx"): 204.6e6 + 30.7e6}
+
+
 def measured_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -236,8 +243,10 @@ def run_mm(args):
     dom = max(range(4), key=lambda i: prof_ms[i])
     # algorithmic bytes of each kernel class per launch (units of N*s): SURVEY.md §8(d) rows
     three_d = w.nz > 1
-    alg_units = {"fwd_xz": 10 + (18 if three_d else 0) // 2, "y_conv": 30 if three_d else 16,
-                 "inv_zx": 13 + (18 if three_d else 0) // 2, "llg_stage": 13}
+    # y_conv is SURVEY's "last forward + multiply + first inverse (+K^)" row; the other rows are DESIGN.md §5's
+    # (this build does z inside the x passes: A = 4 + 12 (film 4 + 6), C = 12 + 3 (film 6 + 3))
+    alg_units = {"fwd_xz": 16 if three_d else 10, "y_conv": 30 if three_d else 16,
+                 "inv_zx": 15 if three_d else 9, "llg_stage": 13}
     dom_name = names[dom]
     dom_bytes = alg_units[dom_name] * w.N * esize
     achieved = dom_bytes / (per[dom_name] * 1e-3) / 1e9
@@ -264,7 +273,7 @@ def run_mm(args):
         "gpu_launches": launches,
         "clocks": clocks,
         "roofline": {"bound": "hbm", "kernel": dom_name, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "peak_kind": peak_kind, "traffic": None, "algorithmic_bytes_per_launch": dom_bytes,
+                     "peak_kind": peak_kind, "traffic": NCU_TRAFFIC.get((w.name, args.prec, dom_name)), "algorithmic_bytes_per_launch": dom_bytes,
                      "avg_launch_ms": per[dom_name], "kernel_ms": per,
                      "kernel_share": {n: prof_ms[i] / sum(prof_ms) for i, n in enumerate(names)},
                      "step_algorithmic_gbs": step_gbs, "step_frac": step_gbs / peak,

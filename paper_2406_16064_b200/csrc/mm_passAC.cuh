@@ -138,6 +138,69 @@ MM_HD void fwd_xz_body3(const Geom g, const T* __restrict__ mvec, const T* __res
     zA_split_regs<T, NZ>(g, S + (long)c * g.comp, s, pitch, j0, tw, tid, nthr);
 }
 
+// Pass C head: merge of the packed real transform (pairs k, n-k) fused with the first inverse radix-8
+// stage (Lc = 8).  Position p = blk*8 + r holds k = brev3(r)*nb + beta, beta = brev(blk), nb = n/8; the
+// partner n-k sits at r' = 7-r of block blk' = brev(nb - beta): blocks pair up, so one thread merges
+// and transforms BOTH blocks of a pair in place (no cross-thread hazard, no separate merge sweep):
+//   Z'[k] = (X[k] + conj X[n-k]) + i conj(w_2n^k) (X[k] - conj X[n-k]),  Z'[n-k] = conj(E) + i conj(O);
+//   Z'[0] = (X[0] + conj X[n]) + i (X[0] - conj X[n])   (X[n] is stored at position n).
+template <typename T>
+MM_HD void xC_merge8(const Geom& g, cx<T>* s, int pitch, int L, twiddles<T> tw, int tid, int nthr)
+{
+    const int n = g.nx, nb = n >> 3, logb = g.lognx - 3, logL = ilog2(L);
+    for (int f = tid; f < (nb / 2 + 1) * L; f += nthr) {
+        const int l = f & (L - 1), beta = f >> logL;
+        cx<T>* pA = s + (int)brev((unsigned)beta, logb) * 8 * pitch + l;
+        cx<T> w[8];
+#pragma unroll
+        for (int r = 0; r < 8; r++) w[r] = tw.get((int)brev((unsigned)r, 3) * nb + beta, 2 * n);
+        cx<T> ZA[8];
+#pragma unroll
+        for (int r = 0; r < 8; r++) ZA[r] = pA[r * pitch];
+        if (beta != 0 && beta != nb / 2) {
+            cx<T>* pB = s + (int)brev((unsigned)(nb - beta), logb) * 8 * pitch + l;
+            cx<T> ZB[8];
+#pragma unroll
+            for (int r = 0; r < 8; r++) ZB[r] = pB[r * pitch];
+#pragma unroll
+            for (int r = 0; r < 8; r++) {
+                const cx<T> A = ZA[r], B = conj(ZB[7 - r]);
+                const cx<T> E = A + B, O = cmulc(A - B, w[r]);
+                ZA[r] = E + mul_pi(O);
+                ZB[7 - r] = conj(E) + mul_pi(conj(O));
+            }
+            rad<cx<T>, 8>::inv(ZB);
+#pragma unroll
+            for (int r = 0; r < 8; r++) pB[r * pitch] = ZB[r];
+        } else if (beta != 0) {      // self-paired block: r <-> 7-r
+#pragma unroll
+            for (int r = 0; r < 4; r++) {
+                const cx<T> A = ZA[r], B = conj(ZA[7 - r]);
+                const cx<T> E = A + B, O = cmulc(A - B, w[r]);
+                ZA[r] = E + mul_pi(O);
+                ZA[7 - r] = conj(E) + mul_pi(conj(O));
+            }
+        } else {                     // block 0: k = rho*nb; r=0 <-> Nyquist slot, r=1 is k = n/2, pairs (4,7) (2,3) (6,5)
+            {
+                const cx<T> A = ZA[0], B = conj(s[n * pitch + l]);
+                ZA[0] = (A + B) + mul_pi(A - B);
+            }
+            ZA[1] = scale(conj(ZA[1]), (T)2);
+            const int ra[3] = { 4, 2, 6 }, rb[3] = { 7, 3, 5 };
+#pragma unroll
+            for (int q = 0; q < 3; q++) {
+                const cx<T> A = ZA[ra[q]], B = conj(ZA[rb[q]]);
+                const cx<T> E = A + B, O = cmulc(A - B, w[ra[q]]);
+                ZA[ra[q]] = E + mul_pi(O);
+                ZA[rb[q]] = conj(E) + mul_pi(conj(O));
+            }
+        }
+        rad<cx<T>, 8>::inv(ZA);
+#pragma unroll
+        for (int r = 0; r < 8; r++) pA[r * pitch] = ZA[r];
+    }
+}
+
 template <typename T, int NZ>
 MM_HD void inv_zx_body3(const Geom g, const cx<T>* __restrict__ S, T* __restrict__ Hd, twiddles<T> tw, T inv_scale,
                         cx<T>* s, int bid, int tid, int nthr)
@@ -154,10 +217,10 @@ MM_HD void inv_zx_body3(const Geom g, const cx<T>* __restrict__ S, T* __restrict
         zC_regs<T, NZ>(g, Sc, s, pitch, j0, tw, tid, nthr);
     }
     MM_SYNC();
-    x_split_merge<T, 1>(g, s, pitch, tw, tid, nthr);
+    xC_merge8<T>(g, s, pitch, L, tw, tid, nthr);
     MM_SYNC();
     const int R1 = first_radix(m);
-    for (int Lc = 8; Lc <= m / R1; Lc <<= 3) { xs_mid8_any<T, 1>(s, pitch, L, n, Lc, tw, tid, nthr); MM_SYNC(); }
+    for (int Lc = 64; Lc <= m / R1; Lc <<= 3) { xs_mid8_any<T, 1>(s, pitch, L, n, Lc, tw, tid, nthr); MM_SYNC(); }
     T* Hc = Hd + (long)c * g.N;
     if (R1 == 8) xC_last<T, 8>(g, Hc, s, pitch, j0, inv_scale, tw, tid, nthr);
     else if (R1 == 4) xC_last<T, 4>(g, Hc, s, pitch, j0, inv_scale, tw, tid, nthr);
