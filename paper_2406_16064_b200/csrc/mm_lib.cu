@@ -122,6 +122,19 @@ __device__ __forceinline__ void block_max_bits(unsigned long long v, unsigned lo
     __syncthreads();
 }
 
+// Warp-level form of block_max_bits for the vectorised stage kernel: no shared memory, no block barrier; a
+// warp touches the global word only when it can raise it (the plain read may be stale, which only costs
+// a redundant atomicMax).
+__device__ __forceinline__ void warp_max_bits(unsigned long long v, unsigned long long* dst)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        unsigned long long w = __shfl_xor_sync(0xffffffffu, v, o);
+        v = w > v ? w : v;
+    }
+    if ((threadIdx.x & 31) == 0 && v != 0ull && v > *reinterpret_cast<volatile unsigned long long*>(dst)) atomicMax(dst, v);
+}
+
 // MODE 0: out = H_eff ; MODE 1: out = k = LL torque, then the RK stage algebra selected at compile
 // time: S earlier stages, NEXT (write the next stage input), ERR (embedded error norm), MAXK (max |k|).
 // One thread per cell; indices by shifts (all mesh sizes are powers of two).
@@ -313,8 +326,8 @@ __global__ void __launch_bounds__(MM_STAGEV_THREADS, sizeof(T) == 8 ? 1 : 4) llg
             }
         }
     }
-    if (MODE == 1 && ERR) block_max_bits(eb, &st->err_bits);
-    if (MODE == 1 && MAXK) block_max_bits(kb, &st->maxk_bits);
+    if (MODE == 1 && ERR) warp_max_bits(eb, &st->err_bits);
+    if (MODE == 1 && MAXK) warp_max_bits(kb, &st->maxk_bits);
 }
 
 // Step controller: one thread.  DESIGN.md R8.
