@@ -161,7 +161,14 @@ MM_HD void yB_mul8(const Geom& g, cx<T>* s, const T* Kt, T sz, int tid, int nthr
     const int n = g.py;
     for (int f = tid; f < (n >> 3) * TC; f += nthr) {
         const int col = f & (TC - 1), b8 = f >> logTC;
+        // Rows of the 8-point block are taken cyclically rotated by g = b8 & 3: register slot r holds row
+        // (r + g) & 7.  DFT_8 -> per-frequency real multiply -> IDFT_8 commutes with a cyclic shift (the
+        // phase factors w8^(-g k) cancel), so the result lands in the right rows, and lanes that work on
+        // neighbouring blocks (block stride = 0 mod 128 bytes) now hit different bank windows.
         cx<T>* p = s + rowB<T>(b8 * 8, pitch) + col;
+        int ro[8];
+#pragma unroll
+        for (int r = 0; r < 8; r++) ro[r] = ((r + b8) & 7) * pitch;
         const T* Kp = Kt + (long)b8 * (NJ * TC) + col * EPL;
         T K[NJ];
 #pragma unroll
@@ -174,7 +181,7 @@ MM_HD void yB_mul8(const Geom& g, cx<T>* s, const T* Kt, T sz, int tid, int nthr
 #pragma unroll
         for (int c = 0; c < 3; c++) {
 #pragma unroll
-            for (int r = 0; r < 8; r++) M[c][r] = p[r * pitch + c * TC];
+            for (int r = 0; r < 8; r++) M[c][r] = p[ro[r] + c * TC];
             rad<cx<T>, 8>::fwd(M[c]);
         }
 #pragma unroll
@@ -196,7 +203,7 @@ MM_HD void yB_mul8(const Geom& g, cx<T>* s, const T* Kt, T sz, int tid, int nthr
         for (int c = 0; c < 3; c++) {
             rad<cx<T>, 8>::inv(M[c]);
 #pragma unroll
-            for (int r = 0; r < 8; r++) p[r * pitch + c * TC] = M[c][r];
+            for (int r = 0; r < 8; r++) p[ro[r] + c * TC] = M[c][r];
         }
     }
 }

@@ -612,6 +612,9 @@ static void configure(mm_sim* s)
     if (getenv("MM_TC")) TC = atoi(getenv("MM_TC"));       // tuning knob (power of two)
     g.TC = TC;
     while (g.TC > 1 && (size_t)smemB_elems(g) * cs + (size_t)(g.py / 8) * MM_PADB > SMEM_CAP) g.TC /= 2;
+    // fp32: two resident CTAs per SM (tile <= 98 KB) beat one CTA with a tile twice as wide — one CTA's
+    // shared-memory-bound stages overlap the other's FP32-bound ones (measured, profiles/r01_experiments.md)
+    if (s->prec == MM_F32 && !getenv("MM_TC") && g.TC >= 4 && (size_t)smemB_elems(g) * cs > 98 * 1024) g.TC /= 2;
     while (g.TC > 2 && ((g.nx + g.TC) / g.TC) * g.pz < target) g.TC /= 2;
     g.Lx = ((g.nx + 1 + g.TC - 1) / g.TC) * g.TC;
     g.plane = (long)g.ny * g.Lx;
@@ -623,7 +626,7 @@ static void configure(mm_sim* s)
     s->smemA2 = (size_t)(g.nx + 1) * odd_pitch(g.G * g.nz) * cs;
     s->smemB = (size_t)smemB_elems(g) * cs + (s->use_v2 && g.ny >= 16 ? (size_t)(g.py / 8) * MM_PADB : 0);      // v2: padded 8-row blocks
     s->thrA = 256;
-    s->thrB = (s->prec == MM_F32 && s->smemB > 64 * 1024) ? 512 : 256;
+    s->thrB = (s->prec == MM_F32 && s->smemB > 98 * 1024) ? 512 : 256;
     if (getenv("MM_THRB")) s->thrB = atoi(getenv("MM_THRB"));
 }
 
