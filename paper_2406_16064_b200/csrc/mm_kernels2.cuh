@@ -223,7 +223,13 @@ MM_HD void y_conv_body2(const Geom g, cx<T>* __restrict__ S, const T* __restrict
     const T sz = (is3d && kz > g.nz) ? (T)-1 : (T)1;
     const T* Kt = Kc + ((long)kzp * ntile + bid % ntile) * kc_tile_elems(g);
     const int R1 = first_radix(m);
-    if (R1 == 8) yB_first<T, V, 8>(g, Sz, s, tw, tid, nthr);
+    // first / last stage: one column per item when column pairs would leave threads without an item
+    const bool narrow = V > 1 && (m / R1) * (g.TC / V) < nthr;
+    if (narrow) {
+        if (R1 == 8) yB_first<T, 1, 8>(g, Sz, s, tw, tid, nthr);
+        else if (R1 == 4) yB_first<T, 1, 4>(g, Sz, s, tw, tid, nthr);
+        else yB_first<T, 1, 2>(g, Sz, s, tw, tid, nthr);
+    } else if (R1 == 8) yB_first<T, V, 8>(g, Sz, s, tw, tid, nthr);
     else if (R1 == 4) yB_first<T, V, 4>(g, Sz, s, tw, tid, nthr);
     else yB_first<T, V, 2>(g, Sz, s, tw, tid, nthr);
     MM_SYNC();
@@ -235,7 +241,11 @@ MM_HD void y_conv_body2(const Geom g, cx<T>* __restrict__ S, const T* __restrict
     else yB_mul8<T, false>(g, s, Kt, sz, tid, nthr);
     MM_SYNC();
     for (Lc = 64; Lc <= m / R1; Lc <<= 3) { yB_mid8<T, V, 1>(g, s, Lc, tw, tid, nthr); MM_SYNC(); }
-    if (R1 == 8) yB_last<T, V, 8>(g, Sz, s, tw, tid, nthr);
+    if (narrow) {
+        if (R1 == 8) yB_last<T, 1, 8>(g, Sz, s, tw, tid, nthr);
+        else if (R1 == 4) yB_last<T, 1, 4>(g, Sz, s, tw, tid, nthr);
+        else yB_last<T, 1, 2>(g, Sz, s, tw, tid, nthr);
+    } else if (R1 == 8) yB_last<T, V, 8>(g, Sz, s, tw, tid, nthr);
     else if (R1 == 4) yB_last<T, V, 4>(g, Sz, s, tw, tid, nthr);
     else yB_last<T, V, 2>(g, Sz, s, tw, tid, nthr);
 }
