@@ -27,10 +27,10 @@ RHS_PER_STEP = 7
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
-# (profiles/r01_ncu_full_v3.md); None where no capture of that kernel / workload / precision exists.
-NCU_TRAFFIC = {("cfg4_slab_512x512x16", "f32", "y_conv"): 526.2e6 + 181.7e6,
-               ("cfg4_slab_512x512x16", "f32", "fwd_xz"): 68.3e6 + 160.6e6,
-               ("cfg4_slab_512x512x16", "f32", "inv_zx"): 204.6e6 + 30.7e6}
+# (profiles/r01_ncu_full_v4.md); None where no capture of that kernel / workload / precision exists.
+NCU_TRAFFIC = {("cfg4_slab_512x512x16", "f32", "y_conv"): 510.1e6 + 178.6e6,
+               ("cfg4_slab_512x512x16", "f32", "fwd_xz"): 68.2e6 + 161.8e6,
+               ("cfg4_slab_512x512x16", "f32", "inv_zx"): 202.9e6 + 31.5e6}
 
 
 def measured_peaks():
@@ -288,7 +288,7 @@ def run_mm(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="mm", choices=["mm", "reference"])
     ap.add_argument("--prec", default="f32", choices=["f32", "f64"])
