@@ -253,63 +253,73 @@ MM_HD void y_conv_body2(const Geom g, cx<T>* __restrict__ S, const T* __restrict
 // ------------------------------------------------------------------------------------------------
 // Passes A / C v2 (x transform of packed pairs with m = nx/2, n = nx; z transform in registers)
 // ------------------------------------------------------------------------------------------------
-// first x stage: load Ms*m pairs from global (i fastest: coalesced), pad twiddle, radix R, both blocks
+// first x stage: load Ms*m pairs from global (i fastest: coalesced), pad twiddle, radix R, both blocks.
+// A thread keeps one i (butterfly index) and walks the lines: the pad twiddles w_n^(i + r sub) and the
+// stage twiddles are loaded / formed once per thread, not once per line.
 template <typename T, int R>
 MM_HD void xA_first(const Geom& g, const T* mc, const T* Ms, cx<T>* s, int pitch, int j0, twiddles<T> tw, int tid, int nthr)
 {
-    const int n = g.nx, m = n / 2, sub = m / R, logsub = ilog2(sub), L = g.G * g.nz, lognz = ilog2(g.nz);
-    for (int f = tid; f < sub * L; f += nthr) {
-        const int i = f & (sub - 1), l = f >> logsub;
-        const int gg = l >> lognz, z = l & (g.nz - 1);
-        const long row = ((long)z * g.ny + (j0 + gg)) * g.nx;
-        cx<T> a[R], u[R];
+    const int n = g.nx, m = n / 2, sub = m / R, L = g.G * g.nz, lognz = ilog2(g.nz);
+    const int isub = sub < nthr ? sub : nthr, logisub = ilog2(isub), lstep = nthr >> logisub;
+    for (int i = tid & (isub - 1); i < sub; i += isub) {
+        cx<T> wp[R], pw[R];
 #pragma unroll
-        for (int r = 0; r < R; r++) {
-            const long cell = row + 2 * (i + r * sub);
-            const cx<T> mm2 = *reinterpret_cast<const cx<T>*>(mc + cell);
-            const cx<T> ms2 = *reinterpret_cast<const cx<T>*>(Ms + cell);
-            a[r] = mk<T>(ms2.x == (T)0 ? (T)0 : ms2.x * mm2.x, ms2.y == (T)0 ? (T)0 : ms2.y * mm2.y);
-            u[r] = cmul(a[r], tw.get(i + r * sub, n));
+        for (int r = 0; r < R; r++) wp[r] = tw.get(i + r * sub, n);
+        if (R > 1 && i != 0) twiddle_powers<T, R>(tw.get(i, m), pw);
+        for (int l = tid >> logisub; l < L; l += lstep) {
+            const int gg = l >> lognz, z = l & (g.nz - 1);
+            const long row = ((long)z * g.ny + (j0 + gg)) * g.nx + 2 * i;
+            const T* mrow = mc + row;
+            const T* srow = Ms + row;
+            cx<T> a[R], u[R];
+#pragma unroll
+            for (int r = 0; r < R; r++) {
+                const cx<T> mm2 = *reinterpret_cast<const cx<T>*>(mrow + 2 * r * sub);
+                const cx<T> ms2 = *reinterpret_cast<const cx<T>*>(srow + 2 * r * sub);
+                a[r] = mk<T>(ms2.x == (T)0 ? (T)0 : ms2.x * mm2.x, ms2.y == (T)0 ? (T)0 : ms2.y * mm2.y);
+                u[r] = cmul(a[r], wp[r]);
+            }
+            rad<cx<T>, R>::fwd(a);
+            rad<cx<T>, R>::fwd(u);
+            if (R > 1 && i != 0) {
+#pragma unroll
+                for (int r = 1; r < R; r++) { a[r] = cmul(a[r], pw[r]); u[r] = cmul(u[r], pw[r]); }
+            }
+            cx<T>* dst = s + i * pitch + l;
+#pragma unroll
+            for (int r = 0; r < R; r++) { dst[r * sub * pitch] = a[r]; dst[(m + r * sub) * pitch] = u[r]; }
         }
-        rad<cx<T>, R>::fwd(a);
-        rad<cx<T>, R>::fwd(u);
-        if (R > 1 && i != 0) {
-            cx<T> pw[R];
-            twiddle_powers<T, R>(tw.get(i, m), pw);
-#pragma unroll
-            for (int r = 1; r < R; r++) { a[r] = cmul(a[r], pw[r]); u[r] = cmul(u[r], pw[r]); }
-        }
-        cx<T>* dst = s + i * pitch + l;
-#pragma unroll
-        for (int r = 0; r < R; r++) { dst[r * sub * pitch] = a[r]; dst[(m + r * sub) * pitch] = u[r]; }
     }
 }
 
-// last x stage of pass C: inverse radix R on both blocks, crop combine, scale, store H_d pairs
+// last x stage of pass C: inverse radix R on both blocks, crop combine, scale, store H_d pairs (same
+// thread -> (i, lines) mapping as xA_first)
 template <typename T, int R>
 MM_HD void xC_last(const Geom& g, T* Hc, const cx<T>* s, int pitch, int j0, T inv_scale, twiddles<T> tw, int tid, int nthr)
 {
-    const int n = g.nx, m = n / 2, sub = m / R, logsub = ilog2(sub), L = g.G * g.nz, lognz = ilog2(g.nz);
-    for (int f = tid; f < sub * L; f += nthr) {
-        const int i = f & (sub - 1), l = f >> logsub;
-        const int gg = l >> lognz, z = l & (g.nz - 1);
-        const long row = ((long)z * g.ny + (j0 + gg)) * g.nx;
-        const cx<T>* src = s + i * pitch + l;
-        cx<T> a[R], u[R];
+    const int n = g.nx, m = n / 2, sub = m / R, L = g.G * g.nz, lognz = ilog2(g.nz);
+    const int isub = sub < nthr ? sub : nthr, logisub = ilog2(isub), lstep = nthr >> logisub;
+    for (int i = tid & (isub - 1); i < sub; i += isub) {
+        cx<T> wp[R], pw[R];
 #pragma unroll
-        for (int r = 0; r < R; r++) { a[r] = src[r * sub * pitch]; u[r] = src[(m + r * sub) * pitch]; }
-        if (R > 1 && i != 0) {
-            cx<T> pw[R];
-            twiddle_powers<T, R>(tw.get(i, m), pw);
+        for (int r = 0; r < R; r++) wp[r] = scale(tw.get(i + r * sub, n), inv_scale);      // 1/P folded into the crop twiddle
+        if (R > 1 && i != 0) twiddle_powers<T, R>(tw.get(i, m), pw);
+        for (int l = tid >> logisub; l < L; l += lstep) {
+            const int gg = l >> lognz, z = l & (g.nz - 1);
+            T* hrow = Hc + ((long)z * g.ny + (j0 + gg)) * g.nx + 2 * i;
+            const cx<T>* src = s + i * pitch + l;
+            cx<T> a[R], u[R];
 #pragma unroll
-            for (int r = 1; r < R; r++) { a[r] = cmulc(a[r], pw[r]); u[r] = cmulc(u[r], pw[r]); }
-        }
-        rad<cx<T>, R>::inv(a);
-        rad<cx<T>, R>::inv(u);
+            for (int r = 0; r < R; r++) { a[r] = src[r * sub * pitch]; u[r] = src[(m + r * sub) * pitch]; }
+            if (R > 1 && i != 0) {
 #pragma unroll
-        for (int r = 0; r < R; r++) {
-            const cx<T> o = a[r] + cmulc(u[r], tw.get(i + r * sub, n));
-            *reinterpret_cast<cx<T>*>(Hc + row + 2 * (i + r * sub)) = scale(o, inv_scale);
+                for (int r = 1; r < R; r++) { a[r] = cmulc(a[r], pw[r]); u[r] = cmulc(u[r], pw[r]); }
+            }
+            rad<cx<T>, R>::inv(a);
+            rad<cx<T>, R>::inv(u);
+#pragma unroll
+            for (int r = 0; r < R; r++)
+                *reinterpret_cast<cx<T>*>(hrow + 2 * r * sub) = scale(a[r], inv_scale) + cmulc(u[r], wp[r]);
         }
     }
 }
