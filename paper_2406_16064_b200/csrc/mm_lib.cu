@@ -596,7 +596,8 @@ static void configure(mm_sim* s)
 {
     Geom& g = s->g;
     const size_t cs = 2 * esize(s);
-    const int target = 2 * 148;
+    int target = 2 * 148;
+    if (getenv("MM_TARGET")) target = atoi(getenv("MM_TARGET"));       // tuning knob: minimum grid size aimed at
     // passes A/C: G rows per CTA
     int G = 1;
     if (g.nz < 8) {
