@@ -541,7 +541,7 @@ struct mm_sim {
     // workspace
     void* ws;
     size_t ws_bytes, ws_need;
-    size_t off_Ms, off_S, off_Kh, off_Kc, off_Hd, off_k[7], off_y[2], off_tw, off_Nr, off_st, off_part;
+    size_t off_Ms, off_S, off_Kh, off_Kc, off_mh, off_Hd, off_k[7], off_y[2], off_tw, off_Nr, off_st, off_part;
     int twN;
     size_t smemA, smemA2, smemB;
     int thrA, thrB;
@@ -645,6 +645,7 @@ static void layout(mm_sim* s)
     s->off_Hd = take(3 * N * es);
     for (int i = 0; i < 7; i++) s->off_k[i] = take(3 * N * es);
     for (int i = 0; i < 2; i++) s->off_y[i] = take(3 * N * es);
+    s->off_mh = take(3 * N * es);      // staging slot of the host-buffer entry points
     s->off_tw = take((size_t)(s->twN / 2 + 1) * 2 * es);
     s->off_Nr = take(6 * N * sizeof(double));
     s->off_part = take(4 * 1024 * sizeof(double));
@@ -1231,10 +1232,8 @@ extern "C" int mm_run_host(mm_sim* s, void* host_m, int nsteps, double dt, doubl
     NEED_READY(s);
     if (!host_m || nsteps < 0 || !(dt > 0)) return MM_ERR_ARG;
     const size_t bytes = 3 * (size_t)s->g.N * esize(s);
-    // stage through k[6]'s neighbour-free slot: y buffers are used by the step, so m lives in Hd's
-    // sibling — the workspace has no spare 3N slot, take one transiently
-    void* dm = nullptr;
-    MM_TRY(s, cudaMallocAsync(&dm, bytes, s->stream));
+    // m lives in the workspace's own staging slot for the duration of the call
+    void* dm = wsp<char>(s, s->off_mh);
     MM_TRY(s, cudaMemcpyAsync(dm, host_m, bytes, cudaMemcpyHostToDevice, s->stream));
     int rc = set_state(s, dt, s->integ == MM_RK4 ? 0.0 : tol, 0, 0, 0, 1);
     for (int i = 0; i < nsteps && !rc; i++) rc = enqueue_step_any(s, dm, 0);
@@ -1242,7 +1241,6 @@ extern "C" int mm_run_host(mm_sim* s, void* host_m, int nsteps, double dt, doubl
         cudaError_t e = cudaMemcpyAsync(host_m, dm, bytes, cudaMemcpyDeviceToHost, s->stream);
         if (e != cudaSuccess) { s->err = cudaGetErrorString(e); rc = MM_ERR_CUDA; }
     }
-    cudaFreeAsync(dm, s->stream);
     DevState h;
     int rc2 = read_state(s, &h);
     return rc ? rc : rc2;
