@@ -183,6 +183,25 @@ __global__ void __launch_bounds__(256) llg_stage_kernel(Geom g, LocalP<T> lp, co
     if (MODE == 1 && MAXK) block_max_bits(norm_bits(kn), &st->maxk_bits);
 }
 
+// Neighbour-presence mask, one byte per cell: bit 0..5 = the -x +x -y +y -z +z neighbour is inside the mesh
+// and has Ms != 0 (R4).  Rebuilt whenever Ms is set; read by the vectorised stage kernel.
+template <typename T>
+__global__ void __launch_bounds__(256) nbmask_kernel(Geom g, const T* __restrict__ Ms, unsigned char* __restrict__ nbm)
+{
+    const long q = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= g.N) return;
+    const int i = (int)(q & (g.nx - 1)), j = (int)((q >> g.lognx) & (g.ny - 1)), k = (int)(q >> (g.lognx + g.logny));
+    const long sy = g.nx, sz = (long)g.nx * g.ny;
+    unsigned b = 0;
+    if (i > 0 && Ms[q - 1] != (T)0) b |= 1u;
+    if (i < g.nx - 1 && Ms[q + 1] != (T)0) b |= 2u;
+    if (j > 0 && Ms[q - sy] != (T)0) b |= 4u;
+    if (j < g.ny - 1 && Ms[q + sy] != (T)0) b |= 8u;
+    if (k > 0 && Ms[q - sz] != (T)0) b |= 16u;
+    if (k < g.nz - 1 && Ms[q + sz] != (T)0) b |= 32u;
+    nbm[q] = (unsigned char)b;
+}
+
 // Vectorised form of llg_stage_kernel: one thread owns CPT consecutive cells along x (16 bytes per
 // load: 4 fp32 / 2 fp64 cells), so every centre value, every earlier k_j and both outputs move as
 // 16-byte accesses; y / z neighbours are 16-byte loads of the neighbouring rows, x neighbours come
@@ -200,10 +219,11 @@ template <typename T, int CPT> __device__ __forceinline__ void stc(T* p, const c
 #endif
 template <typename T, int CPT, int MODE, int S, bool NEXT, bool ERR, bool MAXK>
 __global__ void __launch_bounds__(MM_STAGEV_THREADS, sizeof(T) == 8 ? 1 : 4) llg_stagev_kernel(Geom g, LocalP<T> lp, const T* __restrict__ y, const T* __restrict__ Ms,
-                                                         const T* __restrict__ Hd, T* __restrict__ out, StageArgs<T> sa, DevState* st)
+                                                         const unsigned char* __restrict__ nbm, const T* __restrict__ Hd, T* __restrict__ out, StageArgs<T> sa, DevState* st)
 {
     if (st->done) return;
     typedef cellvec<T, CPT> CV;
+    constexpr unsigned ALLNB = CPT == 1 ? 0x3fu : (CPT == 2 ? 0x3f3fu : 0x3f3f3f3fu);
     const long N = g.N;
     const long q = ((long)blockIdx.x * blockDim.x + threadIdx.x) * CPT;
     unsigned long long eb = 0ull, kb = 0ull;      // bit patterns: max keeps a NaN
@@ -239,33 +259,43 @@ __global__ void __launch_bounds__(MM_STAGEV_THREADS, sizeof(T) == 8 ? 1 : 4) llg
             const long qym = oym ? q - sy : q, qyp = oyp ? q + sy : q, qzm = ozm ? q - szz : q, qzp = ozp ? q + szz : q;
             const long qxm = oxm ? q - 1 : q, qxp = oxp ? q + CPT : q;
             CV nym[3], nyp[3], nzm[3], nzp[3];
-            const CV Mym = ldc<T, CPT>(Ms + qym), Myp = ldc<T, CPT>(Ms + qyp), Mzm = ldc<T, CPT>(Ms + qzm), Mzp = ldc<T, CPT>(Ms + qzp);
             T xl[3], xr[3];
-            const T Mxl = Ms[qxm], Mxr = Ms[qxp];
 #pragma unroll
             for (int c = 0; c < 3; c++) {
                 nym[c] = ldc<T, CPT>(y + c * N + qym); nyp[c] = ldc<T, CPT>(y + c * N + qyp);
                 nzm[c] = ldc<T, CPT>(y + c * N + qzm); nzp[c] = ldc<T, CPT>(y + c * N + qzp);
                 xl[c] = y[c * N + qxm]; xr[c] = y[c * N + qxp];
             }
+            // neighbour-presence bits of the thread's cells (nbmask_kernel, written when Ms is set):
+            // bit 0..5 = -x +x -y +y -z +z present (inside the mesh and Ms != 0)
+            unsigned mk = 0;
+#pragma unroll
+            for (int e = 0; e < CPT; e++) mk |= (unsigned)nbm[q + e] << (8 * e);
+            const bool all_present = (mk & ALLNB) == ALLNB;
 #pragma unroll
             for (int e = 0; e < CPT; e++) {
                 const T Msi = Msv.e[e];
                 const T inv = (T)1 / (Msi != (T)0 ? Msi : (T)1);
                 const v3<T> mi = { m[0].e[e], m[1].e[e], m[2].e[e] };
                 v3<T> nb[6];
-                bool ok[6];
-                // -x / +x
-                if (e > 0) { ok[0] = Msv.e[e > 0 ? e - 1 : 0] != (T)0; nb[0] = { m[0].e[e > 0 ? e - 1 : 0], m[1].e[e > 0 ? e - 1 : 0], m[2].e[e > 0 ? e - 1 : 0] }; }
-                else { ok[0] = oxm && Mxl != (T)0; nb[0] = { xl[0], xl[1], xl[2] }; }
-                if (e < CPT - 1) { ok[1] = Msv.e[e < CPT - 1 ? e + 1 : 0] != (T)0; nb[1] = { m[0].e[e < CPT - 1 ? e + 1 : 0], m[1].e[e < CPT - 1 ? e + 1 : 0], m[2].e[e < CPT - 1 ? e + 1 : 0] }; }
-                else { ok[1] = oxp && Mxr != (T)0; nb[1] = { xr[0], xr[1], xr[2] }; }
-                ok[2] = oym && Mym.e[e] != (T)0; nb[2] = { nym[0].e[e], nym[1].e[e], nym[2].e[e] };
-                ok[3] = oyp && Myp.e[e] != (T)0; nb[3] = { nyp[0].e[e], nyp[1].e[e], nyp[2].e[e] };
-                ok[4] = ozm && Mzm.e[e] != (T)0; nb[4] = { nzm[0].e[e], nzm[1].e[e], nzm[2].e[e] };
-                ok[5] = ozp && Mzp.e[e] != (T)0; nb[5] = { nzp[0].e[e], nzp[1].e[e], nzp[2].e[e] };
+                if (e > 0) nb[0] = { m[0].e[e > 0 ? e - 1 : 0], m[1].e[e > 0 ? e - 1 : 0], m[2].e[e > 0 ? e - 1 : 0] };
+                else nb[0] = { xl[0], xl[1], xl[2] };
+                if (e < CPT - 1) nb[1] = { m[0].e[e < CPT - 1 ? e + 1 : 0], m[1].e[e < CPT - 1 ? e + 1 : 0], m[2].e[e < CPT - 1 ? e + 1 : 0] };
+                else nb[1] = { xr[0], xr[1], xr[2] };
+                nb[2] = { nym[0].e[e], nym[1].e[e], nym[2].e[e] };
+                nb[3] = { nyp[0].e[e], nyp[1].e[e], nyp[2].e[e] };
+                nb[4] = { nzm[0].e[e], nzm[1].e[e], nzm[2].e[e] };
+                nb[5] = { nzp[0].e[e], nzp[1].e[e], nzp[2].e[e] };
                 v3<T> h = { H[0].e[e], H[1].e[e], H[2].e[e] };
-                h = local_field_nb<T>(lp, inv, mi, nb, ok, h);
+                if (all_present) {      // interior of the magnetic region: no masking arithmetic at all
+                    const bool ok[6] = { true, true, true, true, true, true };
+                    h = local_field_nb<T>(lp, inv, mi, nb, ok, h);
+                } else {
+                    bool ok[6];
+#pragma unroll
+                    for (int b = 0; b < 6; b++) ok[b] = (mk >> (8 * e + b)) & 1u;
+                    h = local_field_nb<T>(lp, inv, mi, nb, ok, h);
+                }
                 H[0].e[e] = h.x; H[1].e[e] = h.y; H[2].e[e] = h.z;
             }
         } else {
@@ -541,7 +571,7 @@ struct mm_sim {
     // workspace
     void* ws;
     size_t ws_bytes, ws_need;
-    size_t off_Ms, off_S, off_Kh, off_Kc, off_mh, off_Hd, off_k[7], off_y[2], off_tw, off_Nr, off_st, off_part;
+    size_t off_Ms, off_nbm, off_S, off_Kh, off_Kc, off_mh, off_Hd, off_k[7], off_y[2], off_tw, off_Nr, off_st, off_part;
     int twN;
     size_t smemA, smemA2, smemB;
     int thrA, thrB;
@@ -639,6 +669,7 @@ static void layout(mm_sim* s)
     auto take = [&](size_t bytes) { size_t r = o; o = align256(o + bytes); return r; };
     s->off_st = take(sizeof(DevState));
     s->off_Ms = take(N * es);
+    s->off_nbm = take(N);
     s->off_S = take((size_t)3 * g.comp * 2 * es);
     s->off_Kh = take((size_t)6 * g.kcomp * es);
     s->off_Kc = take((s->use_v2 && g.ny >= 16 ? (size_t)kc_elems(g) : 0) * es);      // pass B v2: K^ in consumption order
@@ -748,6 +779,17 @@ extern "C" int mm_set_workspace(mm_sim* s, void* dev_ptr, size_t bytes)
 
 #define NEED_WS(s) do { if (!(s)) return MM_ERR_ARG; if (!(s)->ws) return fail((s), MM_ERR_STATE, "mm_set_workspace not called"); } while (0)
 
+static int build_nbmask(mm_sim* s)
+{
+    const long N = s->g.N;
+    const unsigned blocks = (unsigned)((N + 255) / 256);
+    if (s->prec == MM_F64) nbmask_kernel<double><<<blocks, 256, 0, s->stream>>>(s->g, wsp<double>(s, s->off_Ms), wsp<unsigned char>(s, s->off_nbm));
+    else nbmask_kernel<float><<<blocks, 256, 0, s->stream>>>(s->g, wsp<float>(s, s->off_Ms), wsp<unsigned char>(s, s->off_nbm));
+    s->launches++;
+    MM_TRY(s, cudaGetLastError());
+    return MM_OK;
+}
+
 extern "C" int mm_set_Ms_uniform(mm_sim* s, double Ms)
 {
     NEED_WS(s);
@@ -758,6 +800,7 @@ extern "C" int mm_set_Ms_uniform(mm_sim* s, double Ms)
     else fill_kernel<float><<<blocks, 256, 0, s->stream>>>(N, wsp<float>(s, s->off_Ms), (float)Ms);
     s->launches++;
     MM_TRY(s, cudaGetLastError());
+    { int rc = build_nbmask(s); if (rc) return rc; }
     s->Ms_set = 1;
     return MM_OK;
 }
@@ -766,6 +809,7 @@ extern "C" int mm_set_Ms(mm_sim* s, const void* dev_Ms)
     NEED_WS(s);
     if (!dev_Ms) return MM_ERR_ARG;
     MM_TRY(s, cudaMemcpyAsync(wsp<char>(s, s->off_Ms), dev_Ms, s->g.N * esize(s), cudaMemcpyDeviceToDevice, s->stream));
+    { int rc = build_nbmask(s); if (rc) return rc; }
     s->Ms_set = 1;
     return MM_OK;
 }
@@ -1016,7 +1060,7 @@ static void launch_stage(mm_sim* s, const LocalP<T>& lp, const T* y, const T* Hd
     constexpr int CPT = MM_STAGEV_CPT;
     if (s->g.nx % CPT == 0 && !getenv("MM_NO_STAGEV")) {
         const unsigned blocks = (unsigned)((s->g.N / CPT + MM_STAGEV_THREADS - 1) / MM_STAGEV_THREADS);
-        llg_stagev_kernel<T, CPT, MODE, S, NEXT, ERR, MAXK><<<blocks, MM_STAGEV_THREADS, 0, s->stream>>>(s->g, lp, y, wsp<T>(s, s->off_Ms), Hd, out, sa, wsp<DevState>(s, s->off_st));
+        llg_stagev_kernel<T, CPT, MODE, S, NEXT, ERR, MAXK><<<blocks, MM_STAGEV_THREADS, 0, s->stream>>>(s->g, lp, y, wsp<T>(s, s->off_Ms), wsp<unsigned char>(s, s->off_nbm), Hd, out, sa, wsp<DevState>(s, s->off_st));
         return;
     }
     const unsigned blocks = (unsigned)((s->g.N + 255) / 256);
