@@ -16,16 +16,12 @@
 
 namespace mm {
 
-// Pass B tile: row pitch 3*TC complex plus MM_PADB bytes after every 8 rows.  MM_PADB = 64 makes the
-// multiply stage (one column per lane, 8-byte accesses, 8-row blocks) bank-conflict free, but on
-// cfg4 the tile then exceeds the 196 KB shared-memory carve-out, the SM falls to the 228 KB one
-// with no L1 left for the twiddle / K^ loads, and the pass gets 6 % SLOWER (measured, B200) — so 0.
-#ifndef MM_PADB
-#define MM_PADB 0
-#endif
-template <typename T> MM_HD int padB() { return MM_PADB / (int)sizeof(cx<T>); }
-template <typename T> MM_HD int rowB(int row, int pitch) { return row * pitch + (row >> 3) * padB<T>(); }
-template <typename T> MM_HD long smemB2_elems(const Geom& g) { return (long)g.py * 3 * g.TC + (g.py >> 3) * padB<T>(); }
+// Pass B tile layouts.  Row-major (CM = false): element (row, comp, col) at row*3*TC + comp*TC + col — rows
+// are loaded / stored by the threads with plain global accesses.  Component-major (CM = true):
+// comp*py*TC + row*TC + col — each component's rows are dense, which is the box shape a TMA tensor-map
+// copy deposits and picks up; used by the TMA form of the kernel.
+template <bool CM> MM_HD int rsB(const Geom& g) { return CM ? g.TC : 3 * g.TC; }
+template <bool CM> MM_HD int csB(const Geom& g) { return CM ? g.py * g.TC : g.TC; }
 
 template <typename E, typename T> MM_HD E ldv(const cx<T>* p) { return *reinterpret_cast<const E*>(p); }
 template <typename E, typename T> MM_HD void stv(cx<T>* p, const E& v) { *reinterpret_cast<E*>(p) = v; }
@@ -33,12 +29,13 @@ template <typename E, typename T> MM_HD void stv(cx<T>* p, const E& v) { *reinte
 // ------------------------------------------------------------------------------------------------
 // Pass B v2
 // ------------------------------------------------------------------------------------------------
-// first stage: global load + zero-pad twiddle + radix R on both blocks
-template <typename T, int V, int R>
+// first stage: load (global, or CM: the rows a TMA copy left in the first m rows of the tile) + zero-pad
+// twiddle + radix R on both blocks
+template <typename T, int V, int R, bool CM>
 MM_HD void yB_first(const Geom& g, const cx<T>* Sz, cx<T>* s, twiddles<T> tw, int tid, int nthr)
 {
     typedef cvec<T, V> E;
-    const int TC = g.TC, LC = TC / V, logLC = ilog2(LC), pitch = 3 * TC;
+    const int TC = g.TC, LC = TC / V, logLC = ilog2(LC), pitch = rsB<CM>(g), cs = csB<CM>(g);
     const int m = g.ny, n = g.py, sub = m / R;
     for (int f = tid; f < sub * LC; f += nthr) {
         const int lc = f & (LC - 1), i = f >> logLC;
@@ -49,7 +46,7 @@ MM_HD void yB_first(const Geom& g, const cx<T>* Sz, cx<T>* s, twiddles<T> tw, in
         // fp64 (one column per item, 255-register kernel): the global loads of all three components are in
         // flight before the first butterfly; fp32 (128-register kernel) loads component by component —
         // preloading there costs registers and measured 1.5 % slower
-        constexpr bool PRE = V == 1 && sizeof(T) == 8;
+        constexpr bool PRE = !CM && V == 1 && sizeof(T) == 8;
         constexpr int NA = PRE ? 3 : 1;
         E av[NA][R];
         const cx<T>* src0 = Sz + (long)i * g.Lx + lc * V;
@@ -61,11 +58,11 @@ MM_HD void yB_first(const Geom& g, const cx<T>* Sz, cx<T>* s, twiddles<T> tw, in
         }
 #pragma unroll
         for (int c = 0; c < 3; c++) {
-            cx<T>* dst = s + rowB<T>(i, pitch) + c * TC + lc * V;
-            const int rs = rowB<T>(sub, pitch), mo = rowB<T>(m, pitch);
+            cx<T>* dst = s + (i) * pitch + c * cs + lc * V;
+            const int rs = (sub) * pitch, mo = (m) * pitch;
             E a[R], u[R];
 #pragma unroll
-            for (int r = 0; r < R; r++) a[r] = PRE ? av[c % NA][r] : ldv<E, T>(src0 + (long)c * g.comp + (long)r * sub * g.Lx);
+            for (int r = 0; r < R; r++) a[r] = CM ? ldv<E, T>(dst + r * rs) : (PRE ? av[c % NA][r] : ldv<E, T>(src0 + (long)c * g.comp + (long)r * sub * g.Lx));
 #pragma unroll
             for (int r = 0; r < R; r++) u[r] = cmul(a[r], wp[r]);
             rad<E, R>::fwd(a);
@@ -80,12 +77,12 @@ MM_HD void yB_first(const Geom& g, const cx<T>* Sz, cx<T>* s, twiddles<T> tw, in
     }
 }
 
-// last stage: inverse radix R on both blocks + crop combine + global store
-template <typename T, int V, int R>
-MM_HD void yB_last(const Geom& g, cx<T>* Sz, const cx<T>* s, twiddles<T> tw, int tid, int nthr)
+// last stage: inverse radix R on both blocks + crop combine + store (global, or CM: in place in the tile)
+template <typename T, int V, int R, bool CM>
+MM_HD void yB_last(const Geom& g, cx<T>* Sz, cx<T>* s, twiddles<T> tw, int tid, int nthr)
 {
     typedef cvec<T, V> E;
-    const int TC = g.TC, LC = TC / V, logLC = ilog2(LC), pitch = 3 * TC;
+    const int TC = g.TC, LC = TC / V, logLC = ilog2(LC), pitch = rsB<CM>(g), cs = csB<CM>(g);
     const int m = g.ny, n = g.py, sub = m / R;
     for (int f = tid; f < sub * LC; f += nthr) {
         const int lc = f & (LC - 1), i = f >> logLC;
@@ -96,8 +93,8 @@ MM_HD void yB_last(const Geom& g, cx<T>* Sz, const cx<T>* s, twiddles<T> tw, int
 #pragma unroll
         for (int c = 0; c < 3; c++) {
             cx<T>* dstg = Sz + (long)c * g.comp + (long)i * g.Lx + lc * V;
-            const cx<T>* src = s + rowB<T>(i, pitch) + c * TC + lc * V;
-            const int rs = rowB<T>(sub, pitch), mo = rowB<T>(m, pitch);
+            cx<T>* src = s + (i) * pitch + c * cs + lc * V;
+            const int rs = (sub) * pitch, mo = (m) * pitch;
             E a[R], u[R];
 #pragma unroll
             for (int r = 0; r < R; r++) { a[r] = ldv<E, T>(src + r * rs); u[r] = ldv<E, T>(src + mo + r * rs); }
@@ -108,28 +105,32 @@ MM_HD void yB_last(const Geom& g, cx<T>* Sz, const cx<T>* s, twiddles<T> tw, int
             rad<E, R>::inv(a);
             rad<E, R>::inv(u);
 #pragma unroll
-            for (int r = 0; r < R; r++) stv<E, T>(dstg + (long)r * sub * g.Lx, a[r] + cmulc(u[r], wp[r]));
+            for (int r = 0; r < R; r++) {
+                const E o = a[r] + cmulc(u[r], wp[r]);
+                if (CM) stv<E, T>(src + r * rs, o);      // back into the first m rows: a TMA copy stores them
+                else stv<E, T>(dstg + (long)r * sub * g.Lx, o);
+            }
         }
     }
 }
 
 // middle radix-8 stage (DIR = 0 forward DIF, 1 inverse DIT) on blocks of length Lc over all n points
-template <typename T, int V, int DIR>
+template <typename T, int V, int DIR, bool CM>
 MM_HD void yB_mid8(const Geom& g, cx<T>* s, int Lc, twiddles<T> tw, int tid, int nthr)
 {
     typedef cvec<T, V> E;
-    const int TC = g.TC, LC = TC / V, logLC = ilog2(LC), pitch = 3 * TC;
+    const int TC = g.TC, LC = TC / V, logLC = ilog2(LC), pitch = rsB<CM>(g), cs = csB<CM>(g);
     const int n = g.py, sub = Lc >> 3, logsub = ilog2(sub);
     for (int f = tid; f < (n >> 3) * LC; f += nthr) {
         const int lc = f & (LC - 1), b = f >> logLC;
         const int blk = b >> logsub, i = b & (sub - 1);
         cx<T> pw[8];
         if (i != 0) twiddle_powers<T, 8>(tw.get(i, Lc), pw);
-        cx<T>* base = s + rowB<T>(blk * Lc + i, pitch) + lc * V;
-        const int rs = rowB<T>(sub, pitch);
+        cx<T>* base = s + (blk * Lc + i) * pitch + lc * V;
+        const int rs = (sub) * pitch;
 #pragma unroll
         for (int c = 0; c < 3; c++) {
-            cx<T>* p = base + c * TC;
+            cx<T>* p = base + c * cs;
             E v[8];
 #pragma unroll
             for (int r = 0; r < 8; r++) v[r] = ldv<E, T>(p + r * rs);
@@ -165,11 +166,11 @@ MM_HD void prefetch_l2_bulk(const void* p, unsigned bytes)
 
 // last forward radix-8 stage (Lc = 8) + multiply by K^ + first inverse stage, three components in
 // registers.  Kt = this CTA's tile of Kc (mm_kernels.cuh): NJ/EPL 16-byte loads per thread.
-template <typename T, bool IS3D>
+template <typename T, bool IS3D, bool CM>
 MM_HD void yB_mul8(const Geom& g, cx<T>* s, const T* Kt, T sz, int tid, int nthr)
 {
     constexpr int NQ = IS3D ? 6 : 4, NJ = 8 * NQ, EPL = 16 / (int)sizeof(T), NJQ = NJ / EPL;
-    const int TC = g.TC, logTC = ilog2(TC), pitch = 3 * TC;
+    const int TC = g.TC, logTC = ilog2(TC), pitch = rsB<CM>(g), cs = csB<CM>(g);
     const int n = g.py;
     for (int f = tid; f < (n >> 3) * TC; f += nthr) {
         const int col = f & (TC - 1), b8 = f >> logTC;
@@ -177,7 +178,7 @@ MM_HD void yB_mul8(const Geom& g, cx<T>* s, const T* Kt, T sz, int tid, int nthr
         // (r + g) & 7.  DFT_8 -> per-frequency real multiply -> IDFT_8 commutes with a cyclic shift (the
         // phase factors w8^(-g k) cancel), so the result lands in the right rows, and lanes that work on
         // neighbouring blocks (block stride = 0 mod 128 bytes) now hit different bank windows.
-        cx<T>* p = s + rowB<T>(b8 * 8, pitch) + col;
+        cx<T>* p = s + (b8 * 8) * pitch + col;
         int ro[8];
 #pragma unroll
         for (int r = 0; r < 8; r++) ro[r] = ((r + b8) & 7) * pitch;
@@ -193,7 +194,7 @@ MM_HD void yB_mul8(const Geom& g, cx<T>* s, const T* Kt, T sz, int tid, int nthr
 #pragma unroll
         for (int c = 0; c < 3; c++) {
 #pragma unroll
-            for (int r = 0; r < 8; r++) M[c][r] = p[ro[r] + c * TC];
+            for (int r = 0; r < 8; r++) M[c][r] = p[ro[r] + c * cs];
             rad<cx<T>, 8>::fwd(M[c]);
         }
 #pragma unroll
@@ -215,9 +216,43 @@ MM_HD void yB_mul8(const Geom& g, cx<T>* s, const T* Kt, T sz, int tid, int nthr
         for (int c = 0; c < 3; c++) {
             rad<cx<T>, 8>::inv(M[c]);
 #pragma unroll
-            for (int r = 0; r < 8; r++) p[ro[r] + c * TC] = M[c][r];
+            for (int r = 0; r < 8; r++) p[ro[r] + c * cs] = M[c][r];
         }
     }
+}
+
+// stages of one tile; CM = false: first / last stage move the rows from / to Sz themselves
+template <typename T, int V, bool CM>
+MM_HD void y_conv_stages(const Geom& g, cx<T>* Sz, const T* Kt, T sz, twiddles<T> tw, cx<T>* s, int tid, int nthr)
+{
+    const int m = g.ny;
+    const bool is3d = g.nz > 1;
+    const int R1 = first_radix(m);
+    // first / last stage: one column per item when column pairs would leave threads without an item
+    const bool narrow = V > 1 && (m / R1) * (g.TC / V) < nthr;
+    if (narrow) {
+        if (R1 == 8) yB_first<T, 1, 8, CM>(g, Sz, s, tw, tid, nthr);
+        else if (R1 == 4) yB_first<T, 1, 4, CM>(g, Sz, s, tw, tid, nthr);
+        else yB_first<T, 1, 2, CM>(g, Sz, s, tw, tid, nthr);
+    } else if (R1 == 8) yB_first<T, V, 8, CM>(g, Sz, s, tw, tid, nthr);
+    else if (R1 == 4) yB_first<T, V, 4, CM>(g, Sz, s, tw, tid, nthr);
+    else yB_first<T, V, 2, CM>(g, Sz, s, tw, tid, nthr);
+    MM_SYNC();
+    // the K^ tile of the multiply stage towards L2 while the middle stages run
+    if (!CM && !(g.flags & 1) && tid == 0) prefetch_l2_bulk(Kt, (unsigned)(kc_tile_elems(g) * sizeof(T)));
+    int Lc = m / R1;
+    for (; Lc > 8; Lc >>= 3) { yB_mid8<T, V, 0, CM>(g, s, Lc, tw, tid, nthr); MM_SYNC(); }
+    if (is3d) yB_mul8<T, true, CM>(g, s, Kt, sz, tid, nthr);
+    else yB_mul8<T, false, CM>(g, s, Kt, sz, tid, nthr);
+    MM_SYNC();
+    for (Lc = 64; Lc <= m / R1; Lc <<= 3) { yB_mid8<T, V, 1, CM>(g, s, Lc, tw, tid, nthr); MM_SYNC(); }
+    if (narrow) {
+        if (R1 == 8) yB_last<T, 1, 8, CM>(g, Sz, s, tw, tid, nthr);
+        else if (R1 == 4) yB_last<T, 1, 4, CM>(g, Sz, s, tw, tid, nthr);
+        else yB_last<T, 1, 2, CM>(g, Sz, s, tw, tid, nthr);
+    } else if (R1 == 8) yB_last<T, V, 8, CM>(g, Sz, s, tw, tid, nthr);
+    else if (R1 == 4) yB_last<T, V, 4, CM>(g, Sz, s, tw, tid, nthr);
+    else yB_last<T, V, 2, CM>(g, Sz, s, tw, tid, nthr);
 }
 
 // requires ny >= 16 (so the schedule has >= 2 stages and ends with radix 8) and TC % V == 0
@@ -227,39 +262,77 @@ MM_HD void y_conv_body2(const Geom g, cx<T>* __restrict__ S, const T* __restrict
 {
     const int ntile = g.Lx / g.TC;
     const int x0 = (bid % ntile) * g.TC, zq = bid / ntile;
-    const int m = g.ny;
-    cx<T>* Sz = S + (long)zq * g.plane + x0;
     const int kz = (int)brev((unsigned)zq, g.logpz);
     const bool is3d = g.nz > 1;
     const int kzp = is3d ? (kz <= g.nz ? kz : g.pz - kz) : 0;
     const T sz = (is3d && kz > g.nz) ? (T)-1 : (T)1;
     const T* Kt = Kc + ((long)kzp * ntile + bid % ntile) * kc_tile_elems(g);
-    const int R1 = first_radix(m);
-    // first / last stage: one column per item when column pairs would leave threads without an item
-    const bool narrow = V > 1 && (m / R1) * (g.TC / V) < nthr;
-    if (narrow) {
-        if (R1 == 8) yB_first<T, 1, 8>(g, Sz, s, tw, tid, nthr);
-        else if (R1 == 4) yB_first<T, 1, 4>(g, Sz, s, tw, tid, nthr);
-        else yB_first<T, 1, 2>(g, Sz, s, tw, tid, nthr);
-    } else if (R1 == 8) yB_first<T, V, 8>(g, Sz, s, tw, tid, nthr);
-    else if (R1 == 4) yB_first<T, V, 4>(g, Sz, s, tw, tid, nthr);
-    else yB_first<T, V, 2>(g, Sz, s, tw, tid, nthr);
-    MM_SYNC();
-    // the K^ tile of the multiply stage towards L2 while the middle stages run
-    if (!(g.flags & 1) && tid == 0) prefetch_l2_bulk(Kt, (unsigned)(kc_tile_elems(g) * sizeof(T)));
-    int Lc = m / R1;
-    for (; Lc > 8; Lc >>= 3) { yB_mid8<T, V, 0>(g, s, Lc, tw, tid, nthr); MM_SYNC(); }
-    if (is3d) yB_mul8<T, true>(g, s, Kt, sz, tid, nthr);
-    else yB_mul8<T, false>(g, s, Kt, sz, tid, nthr);
-    MM_SYNC();
-    for (Lc = 64; Lc <= m / R1; Lc <<= 3) { yB_mid8<T, V, 1>(g, s, Lc, tw, tid, nthr); MM_SYNC(); }
-    if (narrow) {
-        if (R1 == 8) yB_last<T, 1, 8>(g, Sz, s, tw, tid, nthr);
-        else if (R1 == 4) yB_last<T, 1, 4>(g, Sz, s, tw, tid, nthr);
-        else yB_last<T, 1, 2>(g, Sz, s, tw, tid, nthr);
-    } else if (R1 == 8) yB_last<T, V, 8>(g, Sz, s, tw, tid, nthr);
-    else if (R1 == 4) yB_last<T, V, 4>(g, Sz, s, tw, tid, nthr);
-    else yB_last<T, V, 2>(g, Sz, s, tw, tid, nthr);
+    y_conv_stages<T, V, false>(g, S + (long)zq * g.plane + x0, Kt, sz, tw, s, tid, nthr);
+}
+
+// TMA form: the rows of the tile travel as tensor-map box copies (cp.async.bulk.tensor, boxes of TC columns x
+// <= 256 rows of one component) between S and the component-major tile; no thread issues a global load or
+// store of S.  `tmap` = CUtensorMap of S as (x, j, zpos, comp) in 8-byte (fp32) / 2 x 8-byte (fp64) elements,
+// `bar` = an 8-byte shared-memory mbarrier.  On the host (emulation) the copies are plain loops.
+template <typename T, int V>
+MM_HD void y_conv_body5(const Geom g, cx<T>* __restrict__ S, const T* __restrict__ Kc, twiddles<T> tw, cx<T>* s,
+                        int bid, int tid, int nthr, const void* tmap, unsigned long long* bar)
+{
+    const int ntile = g.Lx / g.TC;
+    const int x0 = (bid % ntile) * g.TC, zq = bid / ntile;
+    const int kz = (int)brev((unsigned)zq, g.logpz);
+    const bool is3d = g.nz > 1;
+    const int kzp = is3d ? (kz <= g.nz ? kz : g.pz - kz) : 0;
+    const T sz = (is3d && kz > g.nz) ? (T)-1 : (T)1;
+    const T* Kt = Kc + ((long)kzp * ntile + bid % ntile) * kc_tile_elems(g);
+    const int RB = g.ny < 256 ? g.ny : 256, cs = csB<true>(g);
+    constexpr int EW = (int)sizeof(cx<T>) / 8;      // 8-byte tensor-map elements per complex number
+#if defined(__CUDA_ARCH__)
+    const unsigned b32 = (unsigned)__cvta_generic_to_shared(bar);
+    if (tid == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(b32));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(b32), "r"(3 * g.ny * g.TC * (int)sizeof(cx<T>)) : "memory");
+        for (int c = 0; c < 3; c++)
+            for (int r0 = 0; r0 < g.ny; r0 += RB) {
+                const unsigned dst = (unsigned)__cvta_generic_to_shared(s + c * cs + r0 * g.TC);
+                asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+                             ::"r"(dst), "l"(tmap), "r"(x0 * EW), "r"(r0), "r"(zq), "r"(c), "r"(b32) : "memory");
+            }
+        // the K^ tile of the multiply stage follows the rows towards L2
+        if (!(g.flags & 1)) prefetch_l2_bulk(Kt, (unsigned)(kc_tile_elems(g) * sizeof(T)));
+    }
+    __syncthreads();      // the barrier word is initialised before anyone polls it
+    {
+        unsigned done = 0;
+        while (!done)
+            asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }" : "=r"(done) : "r"(b32), "r"(0) : "memory");
+    }
+#else
+    (void)tmap; (void)bar; (void)RB; (void)EW;
+    for (int c = 0; c < 3; c++)
+        for (int j = 0; j < g.ny; j++)
+            for (int col = 0; col < g.TC; col++) s[c * cs + j * g.TC + col] = S[(long)c * g.comp + (long)zq * g.plane + (long)j * g.Lx + x0 + col];
+#endif
+    y_conv_stages<T, V, true>(g, (cx<T>*)nullptr, Kt, sz, tw, s, tid, nthr);
+#if defined(__CUDA_ARCH__)
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // the threads' tile writes before the async-proxy reads
+    __syncthreads();
+    if (tid == 0) {
+        for (int c = 0; c < 3; c++)
+            for (int r0 = 0; r0 < g.ny; r0 += RB) {
+                const unsigned src = (unsigned)__cvta_generic_to_shared(s + c * cs + r0 * g.TC);
+                asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.bulk_group [%0, {%1, %2, %3, %4}], [%5];"
+                             ::"l"(tmap), "r"(x0 * EW), "r"(r0), "r"(zq), "r"(c), "r"(src) : "memory");
+            }
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");      // the tile must outlive the copies
+    }
+#else
+    for (int c = 0; c < 3; c++)
+        for (int j = 0; j < g.ny; j++)
+            for (int col = 0; col < g.TC; col++) S[(long)c * g.comp + (long)zq * g.plane + (long)j * g.Lx + x0 + col] = s[c * cs + j * g.TC + col];
+#endif
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -1,5 +1,6 @@
 // mm_lib.cu — libmm.so: the C ABI of include/mm.h, its host runtime and the __global__ kernels.
 // Hand-written CUDA for sm_100a; no cuFFT, no cuBLAS, no CPU fallback.
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdint.h>
@@ -40,7 +41,7 @@ struct DevState {
 // ------------------------------------------------------------------------------------------------
 // __global__ wrappers of the convolution passes
 // ------------------------------------------------------------------------------------------------
-extern __shared__ __align__(16) unsigned char mm_smem[];
+extern __shared__ __align__(128) unsigned char mm_smem[];
 
 template <typename T>
 __global__ void __launch_bounds__(256) fwd_xz_kernel(Geom g, const T* m, const T* Ms, cx<T>* S, twiddles<T> tw, const DevState* st)
@@ -73,6 +74,15 @@ __global__ void __launch_bounds__(sizeof(T) == 8 ? 256 : 512) y_conv2_kernel(Geo
 {
     if (st->done) return;
     y_conv_body2<T, V>(g, S, Kh, tw, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x);
+}
+// TMA form of pass B: tile rows move as tensor-map box copies (y_conv_body5)
+template <typename T, int V>
+__global__ void __launch_bounds__(sizeof(T) == 8 ? 256 : 512) y_conv5_kernel(Geom g, cx<T>* S, const T* Kh, twiddles<T> tw, const DevState* st,
+                                                                             const __grid_constant__ CUtensorMap tmS)
+{
+    __shared__ __align__(8) unsigned long long bar;
+    if (st->done) return;
+    y_conv_body5<T, V>(g, S, Kh, tw, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x, &tmS, &bar);
 }
 template <typename T, int NZ>
 __global__ void __launch_bounds__(256, sizeof(T) == 8 ? 1 : MM_OCC_C) inv_zx2_kernel(Geom g, const cx<T>* S, T* Hd, twiddles<T> tw, T inv_scale, const DevState* st)
@@ -581,6 +591,8 @@ struct mm_sim {
     std::string err;
     // optional per-pass profiling (mm_set_profiling): event pairs around each kernel class
     int use_v2;
+    int use_tma;            // pass B moves its tile rows with TMA tensor-map copies
+    CUtensorMap tmS;        // S as (x, j, zpos, comp)
     int prof_on;
     std::vector<cudaEvent_t> prof_ev;      // pairs
     std::vector<int> prof_cls;             // class of pair i: 0 pass A, 1 pass B, 2 pass C, 3 stage kernel
@@ -642,7 +654,7 @@ static void configure(mm_sim* s)
     int TC = s->prec == MM_F64 ? 4 : 8;
     if (getenv("MM_TC")) TC = atoi(getenv("MM_TC"));       // tuning knob (power of two)
     g.TC = TC;
-    while (g.TC > 1 && (size_t)smemB_elems(g) * cs + (size_t)(g.py / 8) * MM_PADB > SMEM_CAP) g.TC /= 2;
+    while (g.TC > 1 && (size_t)smemB_elems(g) * cs > SMEM_CAP) g.TC /= 2;
     // fp32: two resident CTAs per SM (tile <= 98 KB) beat one CTA with a tile twice as wide — one CTA's
     // shared-memory-bound stages overlap the other's FP32-bound ones (measured, profiles/r01_experiments.md)
     if (s->prec == MM_F32 && !getenv("MM_TC") && g.TC >= 4 && (size_t)smemB_elems(g) * cs > 98 * 1024) g.TC /= 2;
@@ -655,7 +667,7 @@ static void configure(mm_sim* s)
     s->smemA = (size_t)smemA_elems(g) * cs;
     // the v2 bodies of passes A / C do the z transform in registers: no scratch tile
     s->smemA2 = (size_t)(g.nx + 1) * odd_pitch(g.G * g.nz) * cs;
-    s->smemB = (size_t)smemB_elems(g) * cs + (s->use_v2 && g.ny >= 16 ? (size_t)(g.py / 8) * MM_PADB : 0);      // v2: padded 8-row blocks
+    s->smemB = (size_t)smemB_elems(g) * cs;
     s->thrA = 256;
     s->thrB = (s->prec == MM_F32 && s->smemB > 98 * 1024) ? 512 : 256;
     if (getenv("MM_THRB")) s->thrB = atoi(getenv("MM_THRB"));
@@ -935,6 +947,8 @@ template <typename T> static int init_demag_t(mm_sim* s)
     return MM_OK;
 }
 
+static int make_tmap(mm_sim* s);
+
 extern "C" int mm_init_demag(mm_sim* s)
 {
     NEED_WS(s);
@@ -954,6 +968,7 @@ extern "C" int mm_init_demag(mm_sim* s)
         MM_TRY(s, cudaFuncSetAttribute(y_conv_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_CAP));
         MM_TRY(s, cudaFuncSetAttribute(inv_zx_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_CAP));
     }
+    if ((rc = make_tmap(s))) return rc;
     s->demag_ready = 1;
     return MM_OK;
 }
@@ -1011,6 +1026,42 @@ template <typename T, int V> static void launch_B2(mm_sim* s, unsigned grid, cx<
     y_conv2_kernel<T, V><<<grid, s->thrB, s->smemB, s->stream>>>(s->g, S, wsp<T>(s, s->off_Kc), tw, st);
 }
 
+template <typename T, int V> static void launch_B5(mm_sim* s, unsigned grid, cx<T>* S, twiddles<T> tw, const DevState* st)
+{
+    static bool attr = false;
+    if (!attr) { cudaFuncSetAttribute(y_conv5_kernel<T, V>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_CAP); attr = true; }
+    y_conv5_kernel<T, V><<<grid, s->thrB, s->smemB, s->stream>>>(s->g, S, wsp<T>(s, s->off_Kc), tw, st, s->tmS);
+}
+
+// Tensor map of the spectrum S[comp][zpos][j][xpos] for pass B's box copies (TC columns x <= 256 rows).
+// cuTensorMapEncodeTiled comes from the driver through the runtime's entry-point query (no -lcuda).
+static int make_tmap(mm_sim* s)
+{
+    typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                 const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    const Geom& g = s->g;
+    const size_t cs = 2 * esize(s);
+    s->use_tma = 0;
+    // measured (cfg4, B200): fp32, two CTAs per SM: TMA form 0.248 ms vs 0.254; fp64, one CTA per SM: 0.560 vs
+    // 0.523 (nothing overlaps the wait for the whole tile) -> on for fp32 only; MM_TMA=0/1 overrides
+    int want = s->prec == MM_F32;
+    if (getenv("MM_TMA")) want = atoi(getenv("MM_TMA"));
+    if (!want || !s->use_v2 || g.ny < 16) return MM_OK;
+    if ((g.Lx * cs) % 16 || g.TC * cs < 16 || g.ny > 256 * 64) return MM_OK;
+    EncodeFn enc = nullptr;
+    cudaDriverEntryPointQueryResult qr;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", (void**)&enc, cudaEnableDefault, &qr) != cudaSuccess || !enc) { cudaGetLastError(); return MM_OK; }
+    const cuuint64_t ew = cs / 8;      // 8-byte tensor-map elements per complex number
+    cuuint64_t dims[4] = { (cuuint64_t)g.Lx * ew, (cuuint64_t)g.ny, (cuuint64_t)g.pz, 3 };
+    cuuint64_t strides[3] = { (cuuint64_t)g.Lx * cs, (cuuint64_t)g.plane * cs, (cuuint64_t)g.comp * cs };
+    cuuint32_t box[4] = { (cuuint32_t)(g.TC * ew), (cuuint32_t)(g.ny < 256 ? g.ny : 256), 1, 1 };
+    cuuint32_t es[4] = { 1, 1, 1, 1 };
+    const CUresult r = enc(&s->tmS, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, wsp<char>(s, s->off_S), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                           CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r == CUDA_SUCCESS) s->use_tma = 1;
+    return MM_OK;
+}
+
 template <typename T> static int demag_passes(mm_sim* s, const T* y)
 {
     const Geom& g = s->g;
@@ -1033,7 +1084,10 @@ template <typename T> static int demag_passes(mm_sim* s, const T* y)
     }
     prof_end(s);
     prof_begin(s, 1);
-    if (!b2) y_conv_kernel<T><<<gridB, s->thrB, s->smemB, s->stream>>>(g, S, wsp<T>(s, s->off_Kh), tw, st);
+    if (b2 && s->use_tma) {
+        if (sizeof(T) == 4 && g.TC % 2 == 0) launch_B5<T, (sizeof(T) == 4 ? 2 : 1)>(s, gridB, S, tw, st);
+        else launch_B5<T, 1>(s, gridB, S, tw, st);
+    } else if (!b2) y_conv_kernel<T><<<gridB, s->thrB, s->smemB, s->stream>>>(g, S, wsp<T>(s, s->off_Kh), tw, st);
     else if (sizeof(T) == 4 && g.TC % 2 == 0) launch_B2<T, (sizeof(T) == 4 ? 2 : 1)>(s, gridB, S, tw, st);
     else launch_B2<T, 1>(s, gridB, S, tw, st);
     prof_end(s);

@@ -63,10 +63,10 @@ static void run(int ver, int nx, int ny, int nz, int G, int CH, int TC, const do
     for (long i = 0; i < g.N; i++) Mst[i] = (T)Ms[i];
     std::vector<cx<T>> S((size_t)3 * g.comp);
     memset(S.data(), 0, S.size() * sizeof(cx<T>));
-    std::vector<cx<T>> smem((size_t)(smemA_elems(g) > smemB2_elems<T>(g) ? smemA_elems(g) : smemB2_elems<T>(g)) + 16);
+    std::vector<cx<T>> smem((size_t)(smemA_elems(g) > smemB_elems(g) ? smemA_elems(g) : smemB_elems(g)) + 16);
     const int gridA = 3 * (ny / G), gridB = (g.Lx / TC) * g.pz;
     const double P = (double)g.px * g.py * g.pz;
-    const bool a2 = ver == 2 && nx >= 32 && nz <= 32, b2 = ver == 2 && ny >= 16;
+    const bool a2 = ver >= 2 && nx >= 32 && nz <= 32, b2 = ver >= 2 && ny >= 16, b5 = ver == 5 && ny >= 16;
     for (int b = 0; b < gridA; b++) {
         if (!a2) fwd_xz_body<T>(g, mt.data(), Mst.data(), S.data(), tw, smem.data(), b, 0, 1);
         else switch (nz) {
@@ -75,7 +75,10 @@ static void run(int ver, int nx, int ny, int nz, int G, int CH, int TC, const do
         }
     }
     for (int b = 0; b < gridB; b++) {
-        if (!b2) y_conv_body<T>(g, S.data(), Kh.data(), tw, smem.data(), b, 0, 1);
+        if (b5) {
+            if (sizeof(T) == 4 && TC % 2 == 0) y_conv_body5<T, (sizeof(T) == 4 ? 2 : 1)>(g, S.data(), Kc.data(), tw, smem.data(), b, 0, 1, nullptr, nullptr);
+            else y_conv_body5<T, 1>(g, S.data(), Kc.data(), tw, smem.data(), b, 0, 1, nullptr, nullptr);
+        } else if (!b2) y_conv_body<T>(g, S.data(), Kh.data(), tw, smem.data(), b, 0, 1);
         else if (sizeof(T) == 4 && TC % 2 == 0) y_conv_body2<T, (sizeof(T) == 4 ? 2 : 1)>(g, S.data(), Kc.data(), tw, smem.data(), b, 0, 1);
         else y_conv_body2<T, 1>(g, S.data(), Kc.data(), tw, smem.data(), b, 0, 1);
     }

@@ -56,7 +56,7 @@ def khat_full(o, nx, ny, nz):
                                        ((32, 16, 1), (4, 8, 8)), ((64, 32, 2), (2, 8, 4)), ((32, 64, 16), (1, 8, 8)),
                                        ((128, 128, 1), (2, 8, 2)), ((256, 16, 4), (1, 8, 1)), ((32, 32, 32), (1, 8, 4))])
 @pytest.mark.parametrize("prec64", [1, 0])
-@pytest.mark.parametrize("ver", [1, 2])
+@pytest.mark.parametrize("ver", [1, 2, 5])
 def test_demag_passes_match_oracle(emul, shape, cfg, prec64, ver):
     nx, ny, nz = shape
     G, CH, TC = cfg
