@@ -321,3 +321,22 @@ def test_cfg4_full_size_step_invariants():
     nrm = torch.sqrt((dm.double() ** 2).sum(dim=0))
     assert bool(torch.isfinite(dm).all()) and float((nrm - 1).abs().max()) < 1e-5
     assert s.energy(dm)[0] < E0
+
+
+@pytest.mark.parametrize("prec", [F64, F32])
+@pytest.mark.parametrize("tma", ["0", "1"])
+def test_pass_b_tma_and_register_forms(monkeypatch, prec, tma):
+    """Pass B has two forms (TMA box copies into a component-major tile / thread-issued loads into a row-major
+    tile); the library picks one per precision.  Both are checked against the oracle here (MM_TMA forces one)."""
+    monkeypatch.setenv("MM_TMA", tma)
+    w = small3d(64, 64, 16)
+    o, s = make_pair(w, prec)
+    m = masked_m(w)
+    H = to_np(s.effective_field(s.to_device(m)))
+    Href = o.effective_field(m)
+    assert np.abs(H - Href).max() / w.Ms_max <= HTOL[prec]
+    wf = film(512)
+    o, s = make_pair(wf, prec)
+    H = to_np(s.effective_field(s.to_device(wf.m0)))
+    Href = o.effective_field(np.ascontiguousarray(wf.m0))
+    assert np.abs(H - Href).max() / wf.Ms_max <= HTOL[prec]
