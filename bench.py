@@ -27,10 +27,10 @@ RHS_PER_STEP = 7
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
-# (profiles/r01_ncu_full_v5.md); None where no capture of that kernel / workload / precision exists.
-NCU_TRAFFIC = {("cfg4_slab_512x512x16", "f32", "y_conv"): 512.2e6 + 179.0e6,
-               ("cfg4_slab_512x512x16", "f32", "fwd_xz"): 68.2e6 + 159.4e6,
-               ("cfg4_slab_512x512x16", "f32", "inv_zx"): 202.9e6 + 30.7e6}
+# (profiles/r01_ncu_full_v6.md); None where no capture of that kernel / workload / precision exists.
+NCU_TRAFFIC = {("cfg4_slab_512x512x16", "f32", "y_conv"): 520.2e6 + 187.2e6,
+               ("cfg4_slab_512x512x16", "f32", "fwd_xz"): 68.2e6 + 159.6e6,
+               ("cfg4_slab_512x512x16", "f32", "inv_zx"): 202.9e6 + 31.4e6}
 
 
 def measured_peaks():
