@@ -129,7 +129,9 @@ int mm_get_demag_kernel(mm_sim* sim, int comp, void* dev_out);
  * kernel with CUDA events on the handle's stream; mm_get_profile synchronises the stream, sums the
  * elapsed milliseconds and launch counts per kernel class since the last call — [0] pass A
  * fwd_xz, [1] pass B y_conv, [2] pass C inv_zx, [3] fused local-field/torque/RK-stage kernel —
- * and clears the record.  Off by default (no events are recorded). */
+ * and clears the record.  Off by default (no events are recorded).  on = 1: all four classes; any other
+ * value is a bit mask (bit c+1 = class c, e.g. 4 = pass B only), so that a benchmark can bracket only its dominant kernel and keep
+ * the event overhead (two stream operations per kernel) out of the rest of the step. */
 int mm_set_profiling(mm_sim* sim, int on);
 int mm_get_profile(mm_sim* sim, double ms_out[4], long count_out[4]);
 /* Number of kernel launches issued by this handle so far (for bench accounting). */

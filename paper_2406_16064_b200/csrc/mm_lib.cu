@@ -593,7 +593,7 @@ struct mm_sim {
     int use_v2;
     int use_tma;            // pass B moves its tile rows with TMA tensor-map copies
     CUtensorMap tmS;        // S as (x, j, zpos, comp)
-    int prof_on;
+    int prof_on, prof_open;      // prof_on: bit c = kernel class c is bracketed with events
     std::vector<cudaEvent_t> prof_ev;      // pairs
     std::vector<int> prof_cls;             // class of pair i: 0 pass A, 1 pass B, 2 pass C, 3 stage kernel
     size_t prof_used;
@@ -601,7 +601,8 @@ struct mm_sim {
 
 static void prof_begin(mm_sim* s, int cls)
 {
-    if (!s->prof_on) return;
+    s->prof_open = (s->prof_on >> cls) & 1;
+    if (!s->prof_open) return;
     if (s->prof_used + 1 > s->prof_cls.size()) {
         cudaEvent_t a, b;
         cudaEventCreate(&a); cudaEventCreate(&b);
@@ -612,7 +613,8 @@ static void prof_begin(mm_sim* s, int cls)
 }
 static void prof_end(mm_sim* s)
 {
-    if (!s->prof_on) return;
+    if (!s->prof_open) return;
+    s->prof_open = 0;
     cudaEventRecord(s->prof_ev[2 * s->prof_used + 1], s->stream);
     s->prof_used++;
 }
@@ -709,7 +711,7 @@ extern "C" int mm_create(mm_sim** out, int nx, int ny, int nz, double dx, double
     s->dx = dx; s->dy = dy; s->dz = dz;
     s->A = s->D = s->Ku = 0; s->u[0] = s->u[1] = 0; s->u[2] = 1; s->hext[0] = s->hext[1] = s->hext[2] = 0;
     s->alpha = 0.5; s->gamma = 2.211e5; s->dmi_kind = 0; s->integ = MM_DOPRI5; s->demag_on = 1; s->demag_ready = 0; s->Ms_set = 0;
-    s->ws = nullptr; s->ws_bytes = 0; s->khat_imag_ratio = -1; s->t_host = 0; s->launches = 0; s->prof_on = 0; s->prof_used = 0; s->use_v2 = getenv("MM_FORCE_V1") ? 0 : 1;
+    s->ws = nullptr; s->ws_bytes = 0; s->khat_imag_ratio = -1; s->t_host = 0; s->launches = 0; s->prof_on = 0; s->prof_open = 0; s->prof_used = 0; s->use_v2 = getenv("MM_FORCE_V1") ? 0 : 1;
     Geom& g = s->g;
     memset(&g, 0, sizeof(g));
     g.nx = nx; g.ny = ny; g.nz = nz;
@@ -736,7 +738,7 @@ extern "C" int mm_destroy(mm_sim* s)
 extern "C" int mm_set_profiling(mm_sim* s, int on)
 {
     if (!s) return MM_ERR_ARG;
-    s->prof_on = on ? 1 : 0;
+    s->prof_on = on == 1 ? 15 : ((on >> 1) & 15);      // 1 = all four classes, otherwise bit c+1 = class c
     s->prof_used = 0;
     return MM_OK;
 }
