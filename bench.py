@@ -121,12 +121,14 @@ def algorithmic_bytes(w, esize):
             "passB": (30 if three_d else 16) * N * esize}
 
 
-def oracle_sample(w):
-    """Bounded sample of the workload for the CPU legs: same cells/material, fewer cells."""
+def oracle_sample(w, shrink=0):
+    """Bounded sample of the workload for the CPU legs: same cells/material, fewer cells (shrink halves the
+    in-plane size again)."""
     from paper_2406_16064_b200 import workloads as wl
     if w.nz > 1:
-        return wl.cfg4(64, 64, w.nz)
-    n = min(w.nx, 256)
+        n = max(16, 64 >> shrink)
+        return wl.cfg4(n, n, w.nz)
+    n = max(16, min(w.nx, 256) >> shrink)
     return wl.cfg5(n)
 
 
@@ -156,8 +158,14 @@ def run_reference(args):
     if rank != 0:
         return
     w = get_workload(args.workload)
-    ws = oracle_sample(w)
     cores = os.cpu_count()
+    # bound the whole run to a few minutes on whatever host this is: one probe step decides the sample size
+    budget = float(os.environ.get("MM_REF_BUDGET_S", "150"))
+    for shrink in range(3):
+        ws = oracle_sample(w, shrink)
+        probe, _ = time_oracle(ws, 1, 0, RHS_PER_STEP)
+        if probe * (args.steps + args.warmup) <= budget or shrink == 2:
+            break
     sec, units = time_oracle(ws, args.steps, args.warmup, RHS_PER_STEP)
     value = units / sec
     sample = f"{ws.nx}x{ws.ny}x{ws.nz} sub-mesh of the workload (same cells and material), {args.steps} DOPRI5 steps"
