@@ -428,6 +428,20 @@ template <typename E> struct rad<E, 32> {
     }
 };
 
+// w0 * exp(-i pi r / R), r = 0..R-1: the pad / crop twiddles w_n^(i + r n/(2R)) of a pruned first / last
+// stage derived from the single table value w0 = w_n^i (one load per butterfly instead of R)
+template <typename T, int R> MM_HD void pad_twiddles(cx<T> w0, cx<T>* wp)
+{
+    const T c1 = (T)0.92387953251128675613, s1 = (T)0.38268343236508977173, c = (T)0.70710678118654752440;
+    wp[0] = w0;
+    if (R == 2) { wp[1] = mul_mi(w0); }
+    else if (R == 4) { wp[1] = crot(w0, c, -c); wp[2] = mul_mi(w0); wp[3] = crot(w0, -c, -c); }
+    else if (R == 8) {
+        wp[1] = crot(w0, c1, -s1); wp[2] = crot(w0, c, -c); wp[3] = crot(w0, s1, -c1); wp[4] = mul_mi(w0);
+        wp[5] = crot(w0, -s1, -c1); wp[6] = crot(w0, -c, -c); wp[7] = crot(w0, -c1, -s1);
+    }
+}
+
 // first radix of the v2 schedule for block length m >= 16: remainder first, then 8s
 MM_HD int first_radix(int m) { int r = m; while (r > 8) r >>= 3; return r; }
 

@@ -36,12 +36,16 @@ struct Geom {
 
 MM_HD int odd_pitch(int n) { return n | 1; }
 
-// K^ in the order pass B (v2) consumes it, "Kc": one contiguous tile per (kz', x tile); inside a tile
-// element (b8, j, col) with j = r*NQ + q (r = row inside the radix-8 block b8, q = tensor component)
-// sits at ((b8*NJQ + j/EPL)*TC + col)*EPL + j%EPL, EPL = reals per 16-byte load.  Values are -K^ with
-// the ky mirror sign of the odd components baked in (all py positions are stored).
+// K^ in the order pass B (v2) consumes it, "Kc": one contiguous tile per (kz', x tile).  The multiply stage
+// works on radix-8 blocks b8 of the bit-reversed y spectrum: slot r of block b8 holds ky = brev3(r)*nbk + beta,
+// beta = brev(b8), nbk = py/8.  The tensor spectrum is even or odd in ky, and the mirror py - ky of (beta, r) is
+// (nbk - beta, 7 - r): blocks pair up, so only the sets beta = 0 .. nbk/2 are stored (half the rows; beta = 0
+// and beta = nbk/2 are their own mirrors) and a thread that owns a pair reads one set for both blocks.
+// Inside a tile, element (beta, j, col) with j = r*NQ + q (q = tensor component) sits at
+// ((beta*NJQ + j/EPL)*TC + col)*EPL + j%EPL, EPL = reals per 16-byte load.  Values are -K^ with the ky mirror
+// sign of the odd components (xy, yz) baked in.
 MM_HD int kc_nq(const Geom& g) { return g.nz > 1 ? 6 : 4; }
-MM_HD long kc_tile_elems(const Geom& g) { return (long)g.py * kc_nq(g) * g.TC; }
+MM_HD long kc_tile_elems(const Geom& g) { return (long)(g.py / 16 + 1) * 8 * kc_nq(g) * g.TC; }
 MM_HD long kc_elems(const Geom& g) { return (long)(g.nz > 1 ? g.nz + 1 : 1) * (g.Lx / g.TC) * kc_tile_elems(g); }
 template <typename T> MM_HD void kc_fill(const Geom& g, const T* Kh, T* Kc, long idx)
 {
@@ -52,12 +56,17 @@ template <typename T> MM_HD void kc_fill(const Geom& g, const T* Kh, T* Kc, long
     const int kzp = (int)(t / ntile), xt = (int)(t % ntile);
     const int e = (int)(o % EPL); o /= EPL;
     const int col = (int)(o % g.TC); o /= g.TC;
-    const int jq = (int)(o % NJQ), b8 = (int)(o / NJQ);
-    const int j = jq * EPL + e, r = j / NQ, q = j - r * NQ;
-    const int ky = (int)brev((unsigned)(b8 * 8 + r), g.logpy);
+    const int jq = (int)(o % NJQ), beta = (int)(o / NJQ);
+    const int j = jq * EPL + e, q = j % NQ;
+    // the set beta = nbk/2 is consumed as the mirror of itself: stored row-reversed with the odd components negated
+    const bool self = beta == g.py / 16;
+    const int r = self ? 7 - j / NQ : j / NQ;
+    const bool odd = q == 3 || q == 5;
+    const int ky = (int)brev((unsigned)r, 3) * (g.py / 8) + beta;
     const int kyp = ky <= g.ny ? ky : g.py - ky;
     const T v = Kh[(long)q * g.kcomp + (long)kzp * g.kplane + (long)kyp * g.Lx + xt * g.TC + col];
-    Kc[idx] = (ky > g.ny && (q == 3 || q == 5)) ? v : -v;
+    const T w = (ky > g.ny && odd) ? v : -v;      // -K^(ky)
+    Kc[idx] = (self && odd) ? -w : w;
 }
 
 // shared memory (in complex elements) of passes A/C and B

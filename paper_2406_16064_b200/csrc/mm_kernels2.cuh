@@ -31,8 +31,23 @@ template <typename E, typename T> MM_HD void stv(cx<T>* p, const E& v) { *reinte
 // ------------------------------------------------------------------------------------------------
 // first stage: load (global, or CM: the rows a TMA copy left in the first m rows of the tile) + zero-pad
 // twiddle + radix R on both blocks
+// spin until phase 0 of the shared-memory mbarrier has completed (a TMA load has landed); host: no-op
+MM_HD void mbar_wait0(unsigned long long* bar)
+{
+#if defined(__CUDA_ARCH__)
+    const unsigned b32 = (unsigned)__cvta_generic_to_shared(bar);
+    unsigned done = 0;
+    while (!done)
+        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }" : "=r"(done) : "r"(b32), "r"(0) : "memory");
+#else
+    (void)bar;
+#endif
+}
+
+// `bars` (CM only, may be null): one mbarrier per component; the rows of component c are in the tile once
+// bars[c] has completed, so the stage starts on component 0 while the other two are still in flight
 template <typename T, int V, int R, bool CM>
-MM_HD void yB_first(const Geom& g, const cx<T>* Sz, cx<T>* s, twiddles<T> tw, int tid, int nthr)
+MM_HD void yB_first(const Geom& g, const cx<T>* Sz, cx<T>* s, twiddles<T> tw, int tid, int nthr, unsigned long long* bars = nullptr)
 {
     typedef cvec<T, V> E;
     const int TC = g.TC, LC = TC / V, logLC = ilog2(LC), pitch = rsB<CM>(g), cs = csB<CM>(g);
@@ -40,9 +55,8 @@ MM_HD void yB_first(const Geom& g, const cx<T>* Sz, cx<T>* s, twiddles<T> tw, in
     for (int f = tid; f < sub * LC; f += nthr) {
         const int lc = f & (LC - 1), i = f >> logLC;
         cx<T> pw[R], wp[R];
-        if (R > 1 && i != 0) twiddle_powers<T, R>(tw.get(i, m), pw);
-#pragma unroll
-        for (int r = 0; r < R; r++) wp[r] = tw.get(i + r * sub, n);
+        pad_twiddles<T, R>(tw.get(i, n), wp);
+        if (R > 1 && i != 0) twiddle_powers<T, R>(cmul(wp[0], wp[0]), pw);      // w_m^i = (w_n^i)^2
         // fp64 (one column per item, 255-register kernel): the global loads of all three components are in
         // flight before the first butterfly; fp32 (128-register kernel) loads component by component —
         // preloading there costs registers and measured 1.5 % slower
@@ -61,6 +75,7 @@ MM_HD void yB_first(const Geom& g, const cx<T>* Sz, cx<T>* s, twiddles<T> tw, in
             cx<T>* dst = s + (i) * pitch + c * cs + lc * V;
             const int rs = (sub) * pitch, mo = (m) * pitch;
             E a[R], u[R];
+            if (CM && bars != nullptr) mbar_wait0(bars + c);
 #pragma unroll
             for (int r = 0; r < R; r++) a[r] = CM ? ldv<E, T>(dst + r * rs) : (PRE ? av[c % NA][r] : ldv<E, T>(src0 + (long)c * g.comp + (long)r * sub * g.Lx));
 #pragma unroll
@@ -87,9 +102,8 @@ MM_HD void yB_last(const Geom& g, cx<T>* Sz, cx<T>* s, twiddles<T> tw, int tid, 
     for (int f = tid; f < sub * LC; f += nthr) {
         const int lc = f & (LC - 1), i = f >> logLC;
         cx<T> pw[R], wp[R];
-        if (R > 1 && i != 0) twiddle_powers<T, R>(tw.get(i, m), pw);
-#pragma unroll
-        for (int r = 0; r < R; r++) wp[r] = tw.get(i + r * sub, n);
+        pad_twiddles<T, R>(tw.get(i, n), wp);
+        if (R > 1 && i != 0) twiddle_powers<T, R>(cmul(wp[0], wp[0]), pw);
 #pragma unroll
         for (int c = 0; c < 3; c++) {
             cx<T>* dstg = Sz + (long)c * g.comp + (long)i * g.Lx + lc * V;
@@ -165,65 +179,89 @@ MM_HD void prefetch_l2_bulk(const void* p, unsigned bytes)
 }
 
 // last forward radix-8 stage (Lc = 8) + multiply by K^ + first inverse stage, three components in
-// registers.  Kt = this CTA's tile of Kc (mm_kernels.cuh): NJ/EPL 16-byte loads per thread.
+// registers.  An item is a column and a PAIR of 8-row blocks whose frequencies mirror each other (ky <-> py - ky,
+// see kc_fill): t = 1 .. nbk/2 - 1 owns the blocks beta = t and nbk - t and reads ONE set of K^ (NJ/EPL 16-byte
+// loads) for both — the second block uses it with the rows reversed and the odd components (xy, yz) negated;
+// t = 0 owns the two self-mirrored blocks beta = 0 and nbk/2 and reads a set for each.  Kt = this CTA's tile of Kc.
 template <typename T, bool IS3D, bool CM>
 MM_HD void yB_mul8(const Geom& g, cx<T>* s, const T* Kt, T sz, int tid, int nthr)
 {
     constexpr int NQ = IS3D ? 6 : 4, NJ = 8 * NQ, EPL = 16 / (int)sizeof(T), NJQ = NJ / EPL;
     const int TC = g.TC, logTC = ilog2(TC), pitch = rsB<CM>(g), cs = csB<CM>(g);
-    const int n = g.py;
-    for (int f = tid; f < (n >> 3) * TC; f += nthr) {
-        const int col = f & (TC - 1), b8 = f >> logTC;
-        // Rows of the 8-point block are taken cyclically rotated by g = b8 & 3: register slot r holds row
-        // (r + g) & 7.  DFT_8 -> per-frequency real multiply -> IDFT_8 commutes with a cyclic shift (the
-        // phase factors w8^(-g k) cancel), so the result lands in the right rows, and lanes that work on
-        // neighbouring blocks (block stride = 0 mod 128 bytes) now hit different bank windows.
-        cx<T>* p = s + (b8 * 8) * pitch + col;
+    const int nbk = g.py >> 3, lognbk = g.logpy - 3;
+    for (int f = tid; f < (nbk >> 1) * TC; f += nthr) {
+        const int col = f & (TC - 1), t = f >> logTC;
+        // Rows of an 8-point block are taken cyclically rotated by t & 7: register slot r holds row
+        // (r + t) & 7.  DFT_8 -> per-frequency real multiply -> IDFT_8 commutes with a cyclic shift (the
+        // phase factors w8^(-g k) cancel), so the result lands in the right rows, and the lanes of a warp
+        // (block offsets = 0 mod 256 bytes) hit different bank windows.
         int ro[8];
 #pragma unroll
-        for (int r = 0; r < 8; r++) ro[r] = ((r + b8) & 7) * pitch;
-        const T* Kp = Kt + (long)b8 * (NJ * TC) + col * EPL;
+        for (int r = 0; r < 8; r++) ro[r] = ((r + t) & 7) * pitch;
         T K[NJ];
+        {
+            const T* Kp = Kt + (long)t * (NJ * TC) + col * EPL;
 #pragma unroll
-        for (int jq = 0; jq < NJQ; jq++) {
-            const kvec<T> v = *reinterpret_cast<const kvec<T>*>(Kp + jq * TC * EPL);
+            for (int jq = 0; jq < NJQ; jq++) {
+                const kvec<T> v = *reinterpret_cast<const kvec<T>*>(Kp + jq * TC * EPL);
 #pragma unroll
-            for (int e = 0; e < EPL; e++) K[jq * EPL + e] = v.e[e];
-        }
-        cx<T> M[3][8];
-#pragma unroll
-        for (int c = 0; c < 3; c++) {
-#pragma unroll
-            for (int r = 0; r < 8; r++) M[c][r] = p[ro[r] + c * cs];
-            rad<cx<T>, 8>::fwd(M[c]);
-        }
-#pragma unroll
-        for (int r = 0; r < 8; r++) {
-            const T kxx = K[r * NQ], kyy = K[r * NQ + 1], kzz = K[r * NQ + 2], kxy = K[r * NQ + 3];
-            const cx<T> Mx = M[0][r], My = M[1][r], Mz = M[2][r];
-            if (IS3D) {
-                const T kxz = sz * K[r * NQ + (IS3D ? 4 : 0)], kyz = sz * K[r * NQ + (IS3D ? 5 : 0)];
-                M[0][r] = lin3<T>(Mx, kxx, My, kxy, Mz, kxz);
-                M[1][r] = lin3<T>(Mx, kxy, My, kyy, Mz, kyz);
-                M[2][r] = lin3<T>(Mx, kxz, My, kyz, Mz, kzz);
-            } else {
-                M[0][r] = lin2<T>(Mx, kxx, My, kxy);
-                M[1][r] = lin2<T>(Mx, kxy, My, kyy);
-                M[2][r] = scale<T>(Mz, kzz);
+                for (int e = 0; e < EPL; e++) K[jq * EPL + e] = v.e[e];
             }
         }
 #pragma unroll
-        for (int c = 0; c < 3; c++) {
-            rad<cx<T>, 8>::inv(M[c]);
+        for (int h = 0; h < 2; h++) {
+            const int beta = h == 0 ? t : (t == 0 ? (nbk >> 1) : nbk - t);
+            if (h == 1 && t == 0) {      // the second self-mirrored block has its own set (stored row-reversed and signed like a mirror)
+                const T* Kp = Kt + (long)(nbk >> 1) * (NJ * TC) + col * EPL;
 #pragma unroll
-            for (int r = 0; r < 8; r++) p[ro[r] + c * cs] = M[c][r];
+                for (int jq = 0; jq < NJQ; jq++) {
+                    const kvec<T> v = *reinterpret_cast<const kvec<T>*>(Kp + jq * TC * EPL);
+#pragma unroll
+                    for (int e = 0; e < EPL; e++) K[jq * EPL + e] = v.e[e];
+                }
+            }
+            cx<T>* p = s + ((int)brev((unsigned)beta, lognbk) * 8) * pitch + col;
+            cx<T> M[3][8];
+#pragma unroll
+            for (int c = 0; c < 3; c++) {
+#pragma unroll
+                for (int r = 0; r < 8; r++) M[c][r] = p[ro[r] + c * cs];
+                rad<cx<T>, 8>::fwd(M[c]);
+            }
+#pragma unroll
+            for (int r = 0; r < 8; r++) {
+                // second block: K_B[r][q] = +-K_A[7 - r][q] (odd components xy, yz change sign)
+                const int kr = (h == 0 ? r : 7 - r) * NQ;
+                const T so = h == 0 ? (T)1 : (T)-1;
+                const T kxx = K[kr], kyy = K[kr + 1], kzz = K[kr + 2], kxy = so * K[kr + 3];
+                const cx<T> Mx = M[0][r], My = M[1][r], Mz = M[2][r];
+                if (IS3D) {
+                    const T kxz = sz * K[kr + (IS3D ? 4 : 0)], kyz = (so * sz) * K[kr + (IS3D ? 5 : 0)];
+                    M[0][r] = lin3<T>(Mx, kxx, My, kxy, Mz, kxz);
+                    M[1][r] = lin3<T>(Mx, kxy, My, kyy, Mz, kyz);
+                    M[2][r] = lin3<T>(Mx, kxz, My, kyz, Mz, kzz);
+                } else {
+                    M[0][r] = lin2<T>(Mx, kxx, My, kxy);
+                    M[1][r] = lin2<T>(Mx, kxy, My, kyy);
+                    M[2][r] = scale<T>(Mz, kzz);
+                }
+            }
+#pragma unroll
+            for (int c = 0; c < 3; c++) {
+                rad<cx<T>, 8>::inv(M[c]);
+#pragma unroll
+                for (int r = 0; r < 8; r++) p[ro[r] + c * cs] = M[c][r];
+            }
         }
     }
 }
 
 // stages of one tile; CM = false: first / last stage move the rows from / to Sz themselves
+// returns false when `done` (the step controller's flag, read by the caller; tested only after the first stage so
+// that the load is off the critical path) stops the pass early
 template <typename T, int V, bool CM>
-MM_HD void y_conv_stages(const Geom& g, cx<T>* Sz, const T* Kt, T sz, twiddles<T> tw, cx<T>* s, int tid, int nthr)
+MM_HD bool y_conv_stages(const Geom& g, cx<T>* Sz, const T* Kt, T sz, twiddles<T> tw, cx<T>* s, int tid, int nthr, unsigned long long* bars = nullptr,
+                         int done = 0)
 {
     const int m = g.ny;
     const bool is3d = g.nz > 1;
@@ -231,12 +269,13 @@ MM_HD void y_conv_stages(const Geom& g, cx<T>* Sz, const T* Kt, T sz, twiddles<T
     // first / last stage: one column per item when column pairs would leave threads without an item
     const bool narrow = V > 1 && (m / R1) * (g.TC / V) < nthr;
     if (narrow) {
-        if (R1 == 8) yB_first<T, 1, 8, CM>(g, Sz, s, tw, tid, nthr);
-        else if (R1 == 4) yB_first<T, 1, 4, CM>(g, Sz, s, tw, tid, nthr);
-        else yB_first<T, 1, 2, CM>(g, Sz, s, tw, tid, nthr);
-    } else if (R1 == 8) yB_first<T, V, 8, CM>(g, Sz, s, tw, tid, nthr);
-    else if (R1 == 4) yB_first<T, V, 4, CM>(g, Sz, s, tw, tid, nthr);
-    else yB_first<T, V, 2, CM>(g, Sz, s, tw, tid, nthr);
+        if (R1 == 8) yB_first<T, 1, 8, CM>(g, Sz, s, tw, tid, nthr, bars);
+        else if (R1 == 4) yB_first<T, 1, 4, CM>(g, Sz, s, tw, tid, nthr, bars);
+        else yB_first<T, 1, 2, CM>(g, Sz, s, tw, tid, nthr, bars);
+    } else if (R1 == 8) yB_first<T, V, 8, CM>(g, Sz, s, tw, tid, nthr, bars);
+    else if (R1 == 4) yB_first<T, V, 4, CM>(g, Sz, s, tw, tid, nthr, bars);
+    else yB_first<T, V, 2, CM>(g, Sz, s, tw, tid, nthr, bars);
+    if (done) return false;
     MM_SYNC();
     // the K^ tile of the multiply stage towards L2 while the middle stages run
     if (!CM && !(g.flags & 1) && tid == 0) prefetch_l2_bulk(Kt, (unsigned)(kc_tile_elems(g) * sizeof(T)));
@@ -253,6 +292,7 @@ MM_HD void y_conv_stages(const Geom& g, cx<T>* Sz, const T* Kt, T sz, twiddles<T
     } else if (R1 == 8) yB_last<T, V, 8, CM>(g, Sz, s, tw, tid, nthr);
     else if (R1 == 4) yB_last<T, V, 4, CM>(g, Sz, s, tw, tid, nthr);
     else yB_last<T, V, 2, CM>(g, Sz, s, tw, tid, nthr);
+    return true;
 }
 
 // requires ny >= 16 (so the schedule has >= 2 stages and ends with radix 8) and TC % V == 0
@@ -276,7 +316,7 @@ MM_HD void y_conv_body2(const Geom g, cx<T>* __restrict__ S, const T* __restrict
 // `bar` = an 8-byte shared-memory mbarrier.  On the host (emulation) the copies are plain loops.
 template <typename T, int V>
 MM_HD void y_conv_body5(const Geom g, cx<T>* __restrict__ S, const T* __restrict__ Kc, twiddles<T> tw, cx<T>* s,
-                        int bid, int tid, int nthr, const void* tmap, unsigned long long* bar)
+                        int bid, int tid, int nthr, const void* tmap, unsigned long long* bar, const int* done_flag = nullptr)
 {
     const int ntile = g.Lx / g.TC;
     const int x0 = (bid % ntile) * g.TC, zq = bid / ntile;
@@ -288,33 +328,33 @@ MM_HD void y_conv_body5(const Geom g, cx<T>* __restrict__ S, const T* __restrict
     const int RB = g.ny < 256 ? g.ny : 256, cs = csB<true>(g);
     constexpr int EW = (int)sizeof(cx<T>) / 8;      // 8-byte tensor-map elements per complex number
 #if defined(__CUDA_ARCH__)
-    const unsigned b32 = (unsigned)__cvta_generic_to_shared(bar);
+    // one mbarrier per component (bar[0..2]); the loads are issued before the step controller's `done` flag
+    // has arrived (a kernel enqueued after the stop condition loads its tile for nothing and returns)
     if (tid == 0) {
-        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(b32));
+        for (int c = 0; c < 3; c++) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"((unsigned)__cvta_generic_to_shared(bar + c)));
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(b32), "r"(3 * g.ny * g.TC * (int)sizeof(cx<T>)) : "memory");
-        for (int c = 0; c < 3; c++)
+        for (int c = 0; c < 3; c++) {
+            const unsigned b32 = (unsigned)__cvta_generic_to_shared(bar + c);
+            asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(b32), "r"(g.ny * g.TC * (int)sizeof(cx<T>)) : "memory");
             for (int r0 = 0; r0 < g.ny; r0 += RB) {
                 const unsigned dst = (unsigned)__cvta_generic_to_shared(s + c * cs + r0 * g.TC);
                 asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
                              ::"r"(dst), "l"(tmap), "r"(x0 * EW), "r"(r0), "r"(zq), "r"(c), "r"(b32) : "memory");
             }
+        }
         // the K^ tile of the multiply stage follows the rows towards L2
         if (!(g.flags & 1)) prefetch_l2_bulk(Kt, (unsigned)(kc_tile_elems(g) * sizeof(T)));
     }
-    __syncthreads();      // the barrier word is initialised before anyone polls it
-    {
-        unsigned done = 0;
-        while (!done)
-            asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }" : "=r"(done) : "r"(b32), "r"(0) : "memory");
-    }
+    const int done = done_flag ? *reinterpret_cast<const volatile int*>(done_flag) : 0;
+    __syncthreads();      // the barrier words are initialised before anyone polls them
 #else
+    const int done = 0; (void)done_flag;
     (void)tmap; (void)bar; (void)RB; (void)EW;
     for (int c = 0; c < 3; c++)
         for (int j = 0; j < g.ny; j++)
             for (int col = 0; col < g.TC; col++) s[c * cs + j * g.TC + col] = S[(long)c * g.comp + (long)zq * g.plane + (long)j * g.Lx + x0 + col];
 #endif
-    y_conv_stages<T, V, true>(g, (cx<T>*)nullptr, Kt, sz, tw, s, tid, nthr);
+    if (!y_conv_stages<T, V, true>(g, (cx<T>*)nullptr, Kt, sz, tw, s, tid, nthr, bar, done)) return;      // every thread has seen all three loads land
 #if defined(__CUDA_ARCH__)
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // the threads' tile writes before the async-proxy reads
     __syncthreads();

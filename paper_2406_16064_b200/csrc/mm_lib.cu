@@ -80,9 +80,8 @@ template <typename T, int V>
 __global__ void __launch_bounds__(sizeof(T) == 8 ? 256 : 512) y_conv5_kernel(Geom g, cx<T>* S, const T* Kh, twiddles<T> tw, const DevState* st,
                                                                              const __grid_constant__ CUtensorMap tmS)
 {
-    __shared__ __align__(8) unsigned long long bar;
-    if (st->done) return;
-    y_conv_body5<T, V>(g, S, Kh, tw, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x, &tmS, &bar);
+    __shared__ __align__(8) unsigned long long bar[3];
+    y_conv_body5<T, V>(g, S, Kh, tw, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x, &tmS, bar, &st->done);
 }
 template <typename T, int NZ>
 __global__ void __launch_bounds__(256, sizeof(T) == 8 ? 1 : MM_OCC_C) inv_zx2_kernel(Geom g, const cx<T>* S, T* Hd, twiddles<T> tw, T inv_scale, const DevState* st)
