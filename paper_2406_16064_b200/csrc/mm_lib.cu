@@ -15,10 +15,15 @@
 #include "mm_kernels.cuh"
 #include "mm_kernels2.cuh"
 #include "mm_passAC.cuh"
+#include "mm_passB7.cuh"
 #include "mm_llg.cuh"
 
 #ifndef MM_OCC_A
 #define MM_OCC_A 3      // resident CTAs per SM the fp32 pass A kernel is compiled for
+#endif
+#ifndef MM_B5_THR
+#define MM_B5_THR 512
+#define MM_B5_OCC 1
 #endif
 #ifndef MM_OCC_C
 #define MM_OCC_C 2
@@ -77,11 +82,19 @@ __global__ void __launch_bounds__(sizeof(T) == 8 ? 256 : 512) y_conv2_kernel(Geo
 }
 // TMA form of pass B: tile rows move as tensor-map box copies (y_conv_body5)
 template <typename T, int V>
-__global__ void __launch_bounds__(sizeof(T) == 8 ? 256 : 512) y_conv5_kernel(Geom g, cx<T>* S, const T* Kh, twiddles<T> tw, const DevState* st,
+__global__ void __launch_bounds__(MM_B5_THR, MM_B5_OCC) y_conv5_kernel(Geom g, cx<T>* S, const T* Kh, twiddles<T> tw, const DevState* st,
                                                                              const __grid_constant__ CUtensorMap tmS)
 {
     __shared__ __align__(8) unsigned long long bar[3];
     y_conv_body5<T, V>(g, S, Kh, tw, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x, &tmS, bar, &st->done);
+}
+// compile-time specialised form of the TMA pass B (mm_passB7.cuh): fp32, ny = 2^LOGM, TC = 4, 256 threads
+template <int LOGM, bool IS3D>
+__global__ void __launch_bounds__(256, 2) y_conv7_kernel(Geom g, cx<float>* S, const float* Kc, twiddles<float> tw, int logtw, const DevState* st,
+                                                         const __grid_constant__ CUtensorMap tmS)
+{
+    __shared__ __align__(8) unsigned long long bar[3];
+    y_conv_body7<LOGM, IS3D, float>(g, S, Kc, tw, logtw, reinterpret_cast<cx<float>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x, &tmS, bar, &st->done);
 }
 template <typename T, int NZ>
 __global__ void __launch_bounds__(256, sizeof(T) == 8 ? 1 : MM_OCC_C) inv_zx2_kernel(Geom g, const cx<T>* S, T* Hd, twiddles<T> tw, T inv_scale, const DevState* st)
@@ -591,6 +604,7 @@ struct mm_sim {
     // optional per-pass profiling (mm_set_profiling): event pairs around each kernel class
     int use_v2;
     int use_tma;            // pass B moves its tile rows with TMA tensor-map copies
+    int no_b7;              // MM_NO_B7: keep the generic TMA pass B (A/B comparisons)
     CUtensorMap tmS;        // S as (x, j, zpos, comp)
     int prof_on, prof_open;      // prof_on: bit c = kernel class c is bracketed with events
     std::vector<cudaEvent_t> prof_ev;      // pairs
@@ -710,7 +724,7 @@ extern "C" int mm_create(mm_sim** out, int nx, int ny, int nz, double dx, double
     s->dx = dx; s->dy = dy; s->dz = dz;
     s->A = s->D = s->Ku = 0; s->u[0] = s->u[1] = 0; s->u[2] = 1; s->hext[0] = s->hext[1] = s->hext[2] = 0;
     s->alpha = 0.5; s->gamma = 2.211e5; s->dmi_kind = 0; s->integ = MM_DOPRI5; s->demag_on = 1; s->demag_ready = 0; s->Ms_set = 0;
-    s->ws = nullptr; s->ws_bytes = 0; s->khat_imag_ratio = -1; s->t_host = 0; s->launches = 0; s->prof_on = 0; s->prof_open = 0; s->prof_used = 0; s->use_v2 = getenv("MM_FORCE_V1") ? 0 : 1;
+    s->ws = nullptr; s->ws_bytes = 0; s->khat_imag_ratio = -1; s->t_host = 0; s->launches = 0; s->prof_on = 0; s->prof_open = 0; s->prof_used = 0; s->use_v2 = getenv("MM_FORCE_V1") ? 0 : 1; s->no_b7 = getenv("MM_NO_B7") ? 1 : 0;
     Geom& g = s->g;
     memset(&g, 0, sizeof(g));
     g.nx = nx; g.ny = ny; g.nz = nz;
@@ -1034,6 +1048,26 @@ template <typename T, int V> static void launch_B5(mm_sim* s, unsigned grid, cx<
     y_conv5_kernel<T, V><<<grid, s->thrB, s->smemB, s->stream>>>(s->g, S, wsp<T>(s, s->off_Kc), tw, st, s->tmS);
 }
 
+template <int LOGM, bool IS3D> static void launch_B7(mm_sim* s, unsigned grid, cx<float>* S, twiddles<float> tw, const DevState* st)
+{
+    static bool attr = false;
+    if (!attr) { cudaFuncSetAttribute(y_conv7_kernel<LOGM, IS3D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_CAP); attr = true; }
+    y_conv7_kernel<LOGM, IS3D><<<grid, 256, s->smemB, s->stream>>>(s->g, S, wsp<float>(s, s->off_Kc), tw, ilog2(s->twN), st, s->tmS);
+}
+// ny = 2^4 .. 2^9 with TC = 4 and the TMA tile: the specialised kernel; false = not covered
+static bool try_launch_B7(mm_sim* s, unsigned grid, cx<float>* S, twiddles<float> tw, const DevState* st)
+{
+    const Geom& g = s->g;
+    if (!s->use_tma || s->prec != MM_F32 || g.TC != 4 || s->thrB != 256 || s->no_b7) return false;
+    const bool d3 = g.nz > 1;
+    switch (g.logny) {
+#define MM_B7_CASE(L) case L: if (d3) launch_B7<L, true>(s, grid, S, tw, st); else launch_B7<L, false>(s, grid, S, tw, st); return true;
+        MM_B7_CASE(4) MM_B7_CASE(5) MM_B7_CASE(6) MM_B7_CASE(7) MM_B7_CASE(8) MM_B7_CASE(9)
+#undef MM_B7_CASE
+        default: return false;
+    }
+}
+
 // Tensor map of the spectrum S[comp][zpos][j][xpos] for pass B's box copies (TC columns x <= 256 rows).
 // cuTensorMapEncodeTiled comes from the driver through the runtime's entry-point query (no -lcuda).
 static int make_tmap(mm_sim* s)
@@ -1085,7 +1119,8 @@ template <typename T> static int demag_passes(mm_sim* s, const T* y)
     }
     prof_end(s);
     prof_begin(s, 1);
-    if (b2 && s->use_tma) {
+    if (b2 && sizeof(T) == 4 && try_launch_B7(s, gridB, reinterpret_cast<cx<float>*>(S), *reinterpret_cast<twiddles<float>*>(&tw), st)) {
+    } else if (b2 && s->use_tma) {
         if (sizeof(T) == 4 && g.TC % 2 == 0) launch_B5<T, (sizeof(T) == 4 ? 2 : 1)>(s, gridB, S, tw, st);
         else launch_B5<T, 1>(s, gridB, S, tw, st);
     } else if (!b2) y_conv_kernel<T><<<gridB, s->thrB, s->smemB, s->stream>>>(g, S, wsp<T>(s, s->off_Kh), tw, st);

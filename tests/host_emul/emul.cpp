@@ -8,6 +8,7 @@
 #include "../../paper_2406_16064_b200/csrc/mm_kernels.cuh"
 #include "../../paper_2406_16064_b200/csrc/mm_kernels2.cuh"
 #include "../../paper_2406_16064_b200/csrc/mm_passAC.cuh"
+#include "../../paper_2406_16064_b200/csrc/mm_passB7.cuh"
 #include "../../paper_2406_16064_b200/csrc/mm_llg.cuh"
 
 using namespace mm;
@@ -66,7 +67,7 @@ static void run(int ver, int nx, int ny, int nz, int G, int CH, int TC, const do
     std::vector<cx<T>> smem((size_t)(smemA_elems(g) > smemB_elems(g) ? smemA_elems(g) : smemB_elems(g)) + 16);
     const int gridA = 3 * (ny / G), gridB = (g.Lx / TC) * g.pz;
     const double P = (double)g.px * g.py * g.pz;
-    const bool a2 = ver >= 2 && nx >= 32 && nz <= 32, b2 = ver >= 2 && ny >= 16, b5 = ver == 5 && ny >= 16;
+    const bool a2 = ver >= 2 && nx >= 32 && nz <= 32, b2 = ver >= 2 && ny >= 16, b5 = (ver == 5 || ver == 7) && ny >= 16;
     for (int b = 0; b < gridA; b++) {
         if (!a2) fwd_xz_body<T>(g, mt.data(), Mst.data(), S.data(), tw, smem.data(), b, 0, 1);
         else switch (nz) {
@@ -74,8 +75,20 @@ static void run(int ver, int nx, int ny, int nz, int G, int CH, int TC, const do
             CASE_A(1) CASE_A(2) CASE_A(4) CASE_A(8) CASE_A(16) CASE_A(32)
         }
     }
+    const bool b7 = ver == 7 && sizeof(T) == 4 && TC == 4 && ny >= 16 && ny <= 512;
+    unsigned long long* nobar = nullptr;
     for (int b = 0; b < gridB; b++) {
-        if (b5) {
+        if (b7) {
+            float* Kcf = reinterpret_cast<float*>(Kc.data());
+            cx<float>* Sf = reinterpret_cast<cx<float>*>(S.data());
+            cx<float>* sm = reinterpret_cast<cx<float>*>(smem.data());
+            twiddles<float> twf; twf.tw = reinterpret_cast<const cx<float>*>(tw.tw); twf.twN = twN;
+            switch (g.logny * 2 + (nz > 1)) {
+#define CASE_B7(L) case 2 * L: y_conv_body7<L, false, float>(g, Sf, Kcf, twf, ilog2(twN), sm, b, 0, 1, nullptr, nobar, nullptr); break; \
+                   case 2 * L + 1: y_conv_body7<L, true, float>(g, Sf, Kcf, twf, ilog2(twN), sm, b, 0, 1, nullptr, nobar, nullptr); break;
+                CASE_B7(4) CASE_B7(5) CASE_B7(6) CASE_B7(7) CASE_B7(8) CASE_B7(9)
+            }
+        } else if (b5) {
             if (sizeof(T) == 4 && TC % 2 == 0) y_conv_body5<T, (sizeof(T) == 4 ? 2 : 1)>(g, S.data(), Kc.data(), tw, smem.data(), b, 0, 1, nullptr, nullptr);
             else y_conv_body5<T, 1>(g, S.data(), Kc.data(), tw, smem.data(), b, 0, 1, nullptr, nullptr);
         } else if (!b2) y_conv_body<T>(g, S.data(), Kh.data(), tw, smem.data(), b, 0, 1);

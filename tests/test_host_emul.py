@@ -20,7 +20,7 @@ _dp = C.POINTER(C.c_double)
 
 @pytest.fixture(scope="module")
 def emul():
-    deps = [SRC] + [os.path.join(ROOT, "paper_2406_16064_b200", "csrc", f) for f in ("mm_fft.cuh", "mm_kernels.cuh", "mm_kernels2.cuh", "mm_passAC.cuh", "mm_llg.cuh")]
+    deps = [SRC] + [os.path.join(ROOT, "paper_2406_16064_b200", "csrc", f) for f in ("mm_fft.cuh", "mm_kernels.cuh", "mm_kernels2.cuh", "mm_passAC.cuh", "mm_passB7.cuh", "mm_llg.cuh")]
     if not os.path.exists(LIB) or os.path.getmtime(LIB) < max(os.path.getmtime(d) for d in deps):
         subprocess.run(["g++", "-O1", "-std=c++17", "-fPIC", "-shared", "-o", LIB, SRC], check=True)
     L = C.CDLL(LIB)
@@ -97,3 +97,22 @@ def test_local_field_and_torque_match_oracle(emul, kind):
         emul.emul_local(nx, ny, nz, par.ctypes.data_as(_dp), kind, 15, Msf.ctypes.data_as(_dp), m.ctypes.data_as(_dp),
                         None, torque, out.ctypes.data_as(_dp))
         assert np.abs(out.reshape(ref.shape) - ref).max() <= 1e-12 * np.abs(ref).max()
+
+
+@pytest.mark.parametrize("shape", [(16, 16, 1), (8, 32, 2), (32, 64, 1), (8, 128, 2), (4, 256, 1), (4, 512, 1), (4, 512, 2), (16, 64, 4)])
+def test_specialised_pass_B_matches_oracle(emul, shape):
+    """mm_passB7.cuh (fp32, TC = 4, compile-time ny): every instantiated ny, films and 3-D."""
+    nx, ny, nz = shape
+    cell = (2e-9, 1.5e-9, 3e-9)
+    Ms = 8e5 * wl.random_mask(23, nx, ny, nz, 0.8)
+    m = np.ascontiguousarray(wl.random_unit(24, nx, ny, nz) * (Ms > 0))
+    o = oracle.Oracle(nx, ny, nz, *cell)
+    o.set_Ms(Ms)
+    o.init_demag()
+    Href = o.field_terms(m, oracle.TERM_DEMAG)
+    K = khat_full(o, nx, ny, nz)
+    Hd = np.zeros(3 * nx * ny * nz)
+    Msf = np.ascontiguousarray(Ms.reshape(-1))
+    emul.emul_demag(7, 0, nx, ny, nz, 1, 8, 4, K.ctypes.data_as(_dp), Msf.ctypes.data_as(_dp), m.ctypes.data_as(_dp), Hd.ctypes.data_as(_dp))
+    Hd = Hd.reshape(3, nz, ny, nx) * (Ms > 0)
+    assert np.abs(Hd - Href).max() / 8e5 < 2e-5
