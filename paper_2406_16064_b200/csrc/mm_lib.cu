@@ -94,7 +94,7 @@ __global__ void __launch_bounds__(256, 2) y_conv7_kernel(Geom g, cx<float>* S, c
                                                          const __grid_constant__ CUtensorMap tmS)
 {
     __shared__ __align__(8) unsigned long long bar[3];
-    y_conv_body7<LOGM, IS3D, float>(g, S, Kc, tw, logtw, reinterpret_cast<cx<float>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x, &tmS, bar, &st->done);
+    y_conv_body7<LOGM, IS3D, 256, float>(g, S, Kc, tw, logtw, reinterpret_cast<cx<float>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x, &tmS, bar, &st->done);
 }
 template <typename T, int NZ>
 __global__ void __launch_bounds__(256, sizeof(T) == 8 ? 1 : MM_OCC_C) inv_zx2_kernel(Geom g, const cx<T>* S, T* Hd, twiddles<T> tw, T inv_scale, const DevState* st)

@@ -9,8 +9,9 @@
 //     are derived from it) and the K^ set of the multiply stage are loaded BEFORE the block barrier that ends
 //     the previous stage, so their latency is covered by the barrier wait instead of heading the next stage;
 //   * the first stage's twiddles are formed while the TMA loads of the tile are in flight.
-// Everything is __host__ __device__ (thread loops run with tid = 0, nthr = 1 on the CPU; the prefetched
-// values are then recomputed per item) so tests/host_emul can check the index arithmetic without a GPU.
+// Everything is __host__ __device__ (NTHR = 256 on the device, where every stage has at most one item per
+// thread and the item loops fold away; tid = 0, NTHR = 1 on the CPU, where the prefetched values are
+// recomputed per item) so tests/host_emul can check the index arithmetic without a GPU.
 #pragma once
 #include "mm_fft.cuh"
 #include "mm_kernels.cuh"
@@ -52,13 +53,13 @@ template <typename T, int R> MM_HD twfl<T, R> b7_fl_tw(twiddles<T> tw, int logtw
 
 // ---- stages ------------------------------------------------------------------------------------------------
 // first: rows i + r*SUB1 of the TMA-deposited lower half -> radix R1 of (a) and of (a * pad twiddle), both halves
-template <int LOGM, typename T>
+template <int LOGM, int NTHR, typename T>
 MM_HD void b7_first(cx<T>* s, const twfl<T, B7<LOGM>::R1>& pre, twiddles<T> tw, int logtw, int tid, int nthr, unsigned long long* bars)
 {
     typedef B7<LOGM> P;
     constexpr int R = P::R1, TC = P::TC;
     bool first = true;
-    for (int f = tid; f < P::SUB1 * TC; f += nthr, first = false) {
+    for (int f = tid; f < P::SUB1 * TC; f += NTHR, first = false) {
         const int col = f & (TC - 1), i = f >> 2;
         const twfl<T, R> t = first ? pre : b7_fl_tw<T, R>(tw, logtw, LOGM + 1, i);
         cx<T>* base = s + i * TC + col;
@@ -82,13 +83,13 @@ MM_HD void b7_first(cx<T>* s, const twfl<T, B7<LOGM>::R1>& pre, twiddles<T> tw, 
 }
 
 // last: inverse radix R1 on both halves, crop combine a + conj(w) u -> the lower half of the tile
-template <int LOGM, typename T>
+template <int LOGM, int NTHR, typename T>
 MM_HD void b7_last(cx<T>* s, const twfl<T, B7<LOGM>::R1>& pre, twiddles<T> tw, int logtw, int tid, int nthr)
 {
     typedef B7<LOGM> P;
     constexpr int R = P::R1, TC = P::TC;
     bool first = true;
-    for (int f = tid; f < P::SUB1 * TC; f += nthr, first = false) {
+    for (int f = tid; f < P::SUB1 * TC; f += NTHR, first = false) {
         const int col = f & (TC - 1), i = f >> 2;
         const twfl<T, R> t = first ? pre : b7_fl_tw<T, R>(tw, logtw, LOGM + 1, i);
         cx<T>* base = s + i * TC + col;
@@ -109,14 +110,14 @@ MM_HD void b7_last(cx<T>* s, const twfl<T, B7<LOGM>::R1>& pre, twiddles<T> tw, i
 }
 
 // middle radix-8 stage on blocks of length 2^LOGLC, two columns (16 bytes) per access
-template <int LOGM, int LOGLC, int DIR, typename T>
+template <int LOGM, int LOGLC, int DIR, int NTHR, typename T>
 MM_HD void b7_mid8(cx<T>* s, const tw8<T>& pre, twiddles<T> tw, int logtw, int tid, int nthr)
 {
     typedef B7<LOGM> P;
     typedef cvec<T, 2> E;
     constexpr int TC = P::TC, SUB = 1 << (LOGLC - 3), RS = SUB * TC;
     bool first = true;
-    for (int f = tid; f < (P::N >> 3) * 2; f += nthr, first = false) {
+    for (int f = tid; f < (P::N >> 3) * 2; f += NTHR, first = false) {
         const int lc = f & 1, b = f >> 1;
         const int blk = b >> (LOGLC - 3), i = b & (SUB - 1);
         const tw8<T> t = first ? pre : b7_mid_tw<T>(tw, logtw, LOGLC, i);
@@ -159,13 +160,13 @@ template <typename T, bool IS3D> MM_HD kset<T, IS3D ? 48 : 32> b7_kload(const T*
 }
 
 // multiply stage: item = (column, mirror pair of 8-row blocks), see yB_mul8 in mm_kernels2.cuh
-template <int LOGM, bool IS3D, typename T>
+template <int LOGM, bool IS3D, int NTHR, typename T>
 MM_HD void b7_mul8(cx<T>* s, const kset<T, IS3D ? 48 : 32>& pre, const T* Kt, T sz, int tid, int nthr)
 {
     typedef B7<LOGM> P;
     constexpr int NQ = IS3D ? 6 : 4, NJ = 8 * NQ, TC = P::TC, NBK = P::NBK, LOGNBK = LOGM - 2;
     bool first = true;
-    for (int f = tid; f < (NBK >> 1) * TC; f += nthr, first = false) {
+    for (int f = tid; f < (NBK >> 1) * TC; f += NTHR, first = false) {
         const int col = f & (TC - 1), t = f >> 2;
         kset<T, NJ> K = first ? pre : b7_kload<T, IS3D>(Kt, t, col);
         int ro[8];
@@ -212,33 +213,33 @@ MM_HD void b7_mul8(cx<T>* s, const kset<T, IS3D ? 48 : 32>& pre, const T* Kt, T 
 
 // forward middle stages Lc = 2^LOGLC, 2^(LOGLC-3), ..., 64 ; each one ends with the block barrier and, before
 // it, the loads of what the following stage needs first (its twiddle; the K^ set of the multiply stage)
-template <int LOGM, int LOGLC, bool IS3D, typename T>
+template <int LOGM, int LOGLC, bool IS3D, int NTHR, typename T>
 MM_HD void b7_fwd_mids(cx<T>* s, twiddles<T> tw, int logtw, const T* Kt, int tid, int nthr, kset<T, IS3D ? 48 : 32>& kpre)
 {
     if constexpr (LOGLC > 3) {
         const tw8<T> t = b7_mid_tw<T>(tw, logtw, LOGLC, b7_mid_i<LOGM, T>(tid, LOGLC));
         MM_SYNC();
-        b7_mid8<LOGM, LOGLC, 0, T>(s, t, tw, logtw, tid, nthr);
-        b7_fwd_mids<LOGM, LOGLC - 3, IS3D, T>(s, tw, logtw, Kt, tid, nthr, kpre);
+        b7_mid8<LOGM, LOGLC, 0, NTHR, T>(s, t, tw, logtw, tid, nthr);
+        b7_fwd_mids<LOGM, LOGLC - 3, IS3D, NTHR, T>(s, tw, logtw, Kt, tid, nthr, kpre);
     } else {
         if (tid < (B7<LOGM>::NBK >> 1) * B7<LOGM>::TC) kpre = b7_kload<T, IS3D>(Kt, tid >> 2, tid & 3);      // K^ set of the thread's first multiply item
         MM_SYNC();
     }
 }
 // inverse middle stages Lc = 2^LOGLC, ..., 2^LOGTOP
-template <int LOGM, int LOGLC, int LOGTOP, typename T>
+template <int LOGM, int LOGLC, int LOGTOP, int NTHR, typename T>
 MM_HD void b7_inv_mids(cx<T>* s, twiddles<T> tw, int logtw, int tid, int nthr)
 {
     if constexpr (LOGLC <= LOGTOP) {
         const tw8<T> t = b7_mid_tw<T>(tw, logtw, LOGLC, b7_mid_i<LOGM, T>(tid, LOGLC));
         MM_SYNC();
-        b7_mid8<LOGM, LOGLC, 1, T>(s, t, tw, logtw, tid, nthr);
-        b7_inv_mids<LOGM, LOGLC + 3, LOGTOP, T>(s, tw, logtw, tid, nthr);
+        b7_mid8<LOGM, LOGLC, 1, NTHR, T>(s, t, tw, logtw, tid, nthr);
+        b7_inv_mids<LOGM, LOGLC + 3, LOGTOP, NTHR, T>(s, tw, logtw, tid, nthr);
     }
 }
 
 // One tile.  `tmap` = CUtensorMap of S as (x, j, zpos, comp); `bar` = three 8-byte shared-memory mbarriers.
-template <int LOGM, bool IS3D, typename T>
+template <int LOGM, bool IS3D, int NTHR, typename T>
 MM_HD void y_conv_body7(const Geom g, cx<T>* __restrict__ S, const T* __restrict__ Kc, twiddles<T> tw, int logtw, cx<T>* s,
                         int bid, int tid, int nthr, const void* tmap, unsigned long long* bar, const int* done_flag)
 {
@@ -277,15 +278,15 @@ MM_HD void y_conv_body7(const Geom g, cx<T>* __restrict__ S, const T* __restrict
     // twiddles of the first stage while the tile is in flight
     const twfl<T, P::R1> tf = b7_fl_tw<T, P::R1>(tw, logtw, LOGM + 1, (tid >> 2) & (P::SUB1 - 1));
     MM_SYNC();      // the barrier words are initialised before anyone polls them
-    b7_first<LOGM, T>(s, tf, tw, logtw, tid, nthr, bar);
+    b7_first<LOGM, NTHR, T>(s, tf, tw, logtw, tid, nthr, bar);
     if (done) return;      // every thread that owns an item has seen all three loads land
     kset<T, IS3D ? 48 : 32> kpre;
-    b7_fwd_mids<LOGM, LOGTOP, IS3D, T>(s, tw, logtw, Kt, tid, nthr, kpre);
-    b7_mul8<LOGM, IS3D, T>(s, kpre, Kt, sz, tid, nthr);
-    b7_inv_mids<LOGM, 6, LOGTOP, T>(s, tw, logtw, tid, nthr);
+    b7_fwd_mids<LOGM, LOGTOP, IS3D, NTHR, T>(s, tw, logtw, Kt, tid, nthr, kpre);
+    b7_mul8<LOGM, IS3D, NTHR, T>(s, kpre, Kt, sz, tid, nthr);
+    b7_inv_mids<LOGM, 6, LOGTOP, NTHR, T>(s, tw, logtw, tid, nthr);
     const twfl<T, P::R1> tl = b7_fl_tw<T, P::R1>(tw, logtw, LOGM + 1, (tid >> 2) & (P::SUB1 - 1));
     MM_SYNC();
-    b7_last<LOGM, T>(s, tl, tw, logtw, tid, nthr);
+    b7_last<LOGM, NTHR, T>(s, tl, tw, logtw, tid, nthr);
 #if defined(__CUDA_ARCH__)
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // the threads' tile writes before the async-proxy reads
     __syncthreads();

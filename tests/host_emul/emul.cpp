@@ -84,8 +84,8 @@ static void run(int ver, int nx, int ny, int nz, int G, int CH, int TC, const do
             cx<float>* sm = reinterpret_cast<cx<float>*>(smem.data());
             twiddles<float> twf; twf.tw = reinterpret_cast<const cx<float>*>(tw.tw); twf.twN = twN;
             switch (g.logny * 2 + (nz > 1)) {
-#define CASE_B7(L) case 2 * L: y_conv_body7<L, false, float>(g, Sf, Kcf, twf, ilog2(twN), sm, b, 0, 1, nullptr, nobar, nullptr); break; \
-                   case 2 * L + 1: y_conv_body7<L, true, float>(g, Sf, Kcf, twf, ilog2(twN), sm, b, 0, 1, nullptr, nobar, nullptr); break;
+#define CASE_B7(L) case 2 * L: y_conv_body7<L, false, 1, float>(g, Sf, Kcf, twf, ilog2(twN), sm, b, 0, 1, nullptr, nobar, nullptr); break; \
+                   case 2 * L + 1: y_conv_body7<L, true, 1, float>(g, Sf, Kcf, twf, ilog2(twN), sm, b, 0, 1, nullptr, nobar, nullptr); break;
                 CASE_B7(4) CASE_B7(5) CASE_B7(6) CASE_B7(7) CASE_B7(8) CASE_B7(9)
             }
         } else if (b5) {
