@@ -48,7 +48,8 @@ typedef enum {
                               /* or workspace not set                                           */
     MM_ERR_CUDA = -4,         /* a CUDA runtime call or kernel launch failed                    */
     MM_ERR_NOMEM = -5,        /* workspace too small / allocation failed                        */
-    MM_ERR_NAN = -6           /* non-finite error norm met in mm_step / mm_relax                */
+    MM_ERR_NAN = -6,          /* non-finite error norm met in mm_step / mm_relax                */
+    MM_ERR_INTERNAL = -7      /* a self-check of the library failed (e.g. K^ not real at setup)   */
 } mm_status;
 typedef enum { MM_DMI_NONE = 0, MM_DMI_BULK = 1, MM_DMI_INTERFACIAL = 2 } mm_dmi_kind;
 typedef enum { MM_RK4 = 0, MM_DOPRI5 = 1 } mm_integrator;
@@ -63,7 +64,11 @@ int mm_destroy(mm_sim* sim);
 /* Persistent device memory the library needs (cached tensor spectrum K^, FFT spectra, RK stage
  * vectors, Ms).  The CALLER allocates it (e.g. torch.empty) and keeps it alive until mm_destroy;
  * the library only carves it up.  Must be called before mm_set_Ms / mm_init_demag / any compute.
- * mm_init_demag additionally uses transient cudaMalloc'ed scratch that it frees before returning. */
+ * mm_init_demag builds the padded tensor inside this workspace (in slots that hold nothing before the first
+ * evaluation); it cudaMallocs only the real-space tensor (6N doubles) and small tables, and frees them on
+ * every exit path.
+ * Alignment: every device pointer handed to the library (m, H, dm/dt, Ms) must be 16-byte aligned (the
+ * kernels use 16-byte vector accesses); torch allocations are, offset views of them may not be. */
 size_t mm_workspace_bytes(const mm_sim* sim);
 int mm_set_workspace(mm_sim* sim, void* dev_ptr, size_t bytes);   /* dev_ptr 256-byte aligned */
 
@@ -100,8 +105,10 @@ int mm_step(mm_sim* sim, void* dev_m, double dt, double tol,
             int* accepted, double* err, double* dt_next, double* max_dmdt);
 
 /* Adaptive steps (DOPRI5) from dt0 until max|dm/dt| < stop_dmdt (rad/s) or max_steps steps
- * (accepted + rejected).  The step controller runs on the device; the host polls every
- * `poll` steps (<=0: library default). */
+ * (accepted + rejected).  dt0 (the first trial step, seconds) is an addition to SURVEY.md 8(b)'s
+ * signature: the paper gives no rule for it and the caller knows the time scale.
+ * The step controller runs on the device; the host reads the device state back every 16 steps,
+ * kernels enqueued after the stop condition return at once. */
 int mm_relax(mm_sim* sim, void* dev_m, double tol, double stop_dmdt, long max_steps, double dt0,
              long* steps_done, double* max_dmdt);
 
@@ -115,7 +122,7 @@ int mm_run_host(mm_sim* sim, void* host_m, int nsteps, double dt, double tol);
 /* Same for one RHS evaluation: host_m in, host_dmdt out. */
 int mm_llg_rhs_host(mm_sim* sim, const void* host_m, void* host_dmdt);
 
-double mm_time(const mm_sim* sim);
+double mm_time(mm_sim* sim);                                      /* synchronises the stream to read the device clock */
 int mm_set_time(mm_sim* sim, double t);
 
 /* Diagnostics, off the hot path (synchronous). */

@@ -9,7 +9,7 @@ F32, F64 = 0, 1
 RK4, DOPRI5 = 0, 1
 DMI_NONE, DMI_BULK, DMI_INTERFACIAL = 0, 1, 2
 _STATUS = {0: "MM_OK", -1: "MM_ERR_ARG", -2: "MM_ERR_UNSUPPORTED", -3: "MM_ERR_STATE", -4: "MM_ERR_CUDA",
-           -5: "MM_ERR_NOMEM", -6: "MM_ERR_NAN"}
+           -5: "MM_ERR_NOMEM", -6: "MM_ERR_NAN", -7: "MM_ERR_INTERNAL"}
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libmm.so")
 _lib = None
@@ -112,6 +112,7 @@ class Sim:
 
     def _dev(self, t, n):
         assert t.is_cuda and t.dtype == self.dtype and t.is_contiguous() and t.numel() == n, "bad device tensor"
+        assert t.data_ptr() % 16 == 0, "device pointers must be 16-byte aligned (include/mm.h)"
         return _vp(t.data_ptr())
 
     def empty_field(self):

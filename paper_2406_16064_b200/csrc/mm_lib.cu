@@ -417,7 +417,7 @@ __global__ void ctrl_kernel(DevState* st, int is_f64, int adaptive_mode)
 
 // On acceptance: m <- y / |y| on cells with Ms > 0 (projection)
 template <typename T>
-__global__ void __launch_bounds__(256) accept_kernel(long N, const DevState* st, const T* __restrict__ ysol, const T* __restrict__ Ms, T* __restrict__ m, int check_done_before)
+__global__ void __launch_bounds__(256) accept_kernel(long N, const DevState* st, const T* __restrict__ ysol, const T* __restrict__ Ms, T* __restrict__ m)
 {
     if (!st->accepted) return;
     const long q = (long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -593,7 +593,7 @@ struct mm_sim {
     // workspace
     void* ws;
     size_t ws_bytes, ws_need;
-    size_t off_Ms, off_nbm, off_S, off_Kh, off_Kc, off_mh, off_Hd, off_k[7], off_y[2], off_tw, off_Nr, off_st, off_part;
+    size_t off_Ms, off_nbm, off_S, off_Kh, off_Kc, off_mh, off_Hd, off_k[7], off_y[2], off_tw, off_st, off_part;
     int twN;
     size_t smemA, smemA2, smemB;
     int thrA, thrB;
@@ -606,29 +606,36 @@ struct mm_sim {
     int use_tma;            // pass B moves its tile rows with TMA tensor-map copies
     int no_b7;              // MM_NO_B7: keep the generic TMA pass B (A/B comparisons)
     CUtensorMap tmS;        // S as (x, j, zpos, comp)
+    int no_stagev;          // MM_NO_STAGEV: one-cell-per-thread stage kernel (A/B comparisons)
+    std::vector<const void*> smem_attr;      // kernels whose dynamic shared-memory limit has been raised on s->device
     int prof_on, prof_open;      // prof_on: bit c = kernel class c is bracketed with events
     std::vector<cudaEvent_t> prof_ev;      // pairs
     std::vector<int> prof_cls;             // class of pair i: 0 pass A, 1 pass B, 2 pass C, 3 stage kernel
     size_t prof_used;
 };
 
+static const size_t PROF_MAX_PAIRS = 1 << 14;      // brackets kept between two mm_get_profile calls; later kernels run unbracketed
 static void prof_begin(mm_sim* s, int cls)
 {
     s->prof_open = (s->prof_on >> cls) & 1;
     if (!s->prof_open) return;
+    if (s->prof_used >= PROF_MAX_PAIRS) { s->prof_open = 0; return; }
     if (s->prof_used + 1 > s->prof_cls.size()) {
-        cudaEvent_t a, b;
-        cudaEventCreate(&a); cudaEventCreate(&b);
+        cudaEvent_t a = nullptr, b = nullptr;
+        if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) {
+            if (a) cudaEventDestroy(a);
+            cudaGetLastError(); s->prof_open = 0; return;
+        }
         s->prof_ev.push_back(a); s->prof_ev.push_back(b); s->prof_cls.push_back(cls);
     }
     s->prof_cls[s->prof_used] = cls;
-    cudaEventRecord(s->prof_ev[2 * s->prof_used], s->stream);
+    if (cudaEventRecord(s->prof_ev[2 * s->prof_used], s->stream) != cudaSuccess) { cudaGetLastError(); s->prof_open = 0; }
 }
 static void prof_end(mm_sim* s)
 {
     if (!s->prof_open) return;
     s->prof_open = 0;
-    cudaEventRecord(s->prof_ev[2 * s->prof_used + 1], s->stream);
+    if (cudaEventRecord(s->prof_ev[2 * s->prof_used + 1], s->stream) != cudaSuccess) { cudaGetLastError(); return; }
     s->prof_used++;
 }
 
@@ -640,6 +647,17 @@ static void prof_end(mm_sim* s)
             return MM_ERR_CUDA;                                                                    \
         }                                                                                          \
     } while (0)
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a per-device setting: recorded per handle (a handle lives on one
+// device), not per process.  Returns false (and leaves the CUDA error in s->err) when the driver refuses.
+static bool raise_smem_limit(mm_sim* s, const void* func)
+{
+    for (const void* f : s->smem_attr) if (f == func) return true;
+    const cudaError_t e = cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    if (e != cudaSuccess) { s->err = std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e); cudaGetLastError(); return false; }
+    s->smem_attr.push_back(func);
+    return true;
+}
 
 static int fail(mm_sim* s, int code, const char* msg) { if (s) s->err = msg; return code; }
 static size_t esize(const mm_sim* s) { return s->prec == MM_F64 ? sizeof(double) : sizeof(float); }
@@ -653,8 +671,7 @@ static void configure(mm_sim* s)
 {
     Geom& g = s->g;
     const size_t cs = 2 * esize(s);
-    int target = 2 * 148;
-    if (getenv("MM_TARGET")) target = atoi(getenv("MM_TARGET"));       // tuning knob: minimum grid size aimed at
+    const int target = 2 * 148;      // minimum grid size aimed at
     // passes A/C: G rows per CTA
     int G = 1;
     if (g.nz < 8) {
@@ -705,7 +722,6 @@ static void layout(mm_sim* s)
     for (int i = 0; i < 2; i++) s->off_y[i] = take(3 * N * es);
     s->off_mh = take(3 * N * es);      // staging slot of the host-buffer entry points
     s->off_tw = take((size_t)(s->twN / 2 + 1) * 2 * es);
-    s->off_Nr = take(6 * N * sizeof(double));
     s->off_part = take(4 * 1024 * sizeof(double));
     s->ws_need = o;
 }
@@ -724,7 +740,7 @@ extern "C" int mm_create(mm_sim** out, int nx, int ny, int nz, double dx, double
     s->dx = dx; s->dy = dy; s->dz = dz;
     s->A = s->D = s->Ku = 0; s->u[0] = s->u[1] = 0; s->u[2] = 1; s->hext[0] = s->hext[1] = s->hext[2] = 0;
     s->alpha = 0.5; s->gamma = 2.211e5; s->dmi_kind = 0; s->integ = MM_DOPRI5; s->demag_on = 1; s->demag_ready = 0; s->Ms_set = 0;
-    s->ws = nullptr; s->ws_bytes = 0; s->khat_imag_ratio = -1; s->t_host = 0; s->launches = 0; s->prof_on = 0; s->prof_open = 0; s->prof_used = 0; s->use_v2 = getenv("MM_FORCE_V1") ? 0 : 1; s->no_b7 = getenv("MM_NO_B7") ? 1 : 0;
+    s->ws = nullptr; s->ws_bytes = 0; s->khat_imag_ratio = -1; s->t_host = 0; s->launches = 0; s->prof_on = 0; s->prof_open = 0; s->prof_used = 0; s->use_v2 = getenv("MM_FORCE_V1") ? 0 : 1; s->no_b7 = getenv("MM_NO_B7") ? 1 : 0; s->no_stagev = getenv("MM_NO_STAGEV") ? 1 : 0;
     Geom& g = s->g;
     memset(&g, 0, sizeof(g));
     g.nx = nx; g.ny = ny; g.nz = nz;
@@ -879,10 +895,18 @@ static void make_rule(double d, int* n_out, double* s_out, double* w_out)
     *n_out = n;
 }
 
-template <typename T> static int init_demag_t(mm_sim* s)
+// device scratch that is released on every exit path
+struct DevBuf {
+    void* p = nullptr;
+    ~DevBuf() { if (p) cudaFree(p); }
+    cudaError_t alloc(size_t bytes) { return cudaMalloc(&p, bytes); }
+    template <typename U> U* as() const { return static_cast<U*>(p); }
+};
+
+// Real-space tensor N_ab(r) at offsets i, j, k >= 0 (6 components x N doubles) into Nr.
+static int build_real_tensor(mm_sim* s, double* Nr)
 {
     const Geom& g = s->g;
-    const long N = g.N, P = (long)g.px * g.py * g.pz;
     cudaStream_t st = s->stream;
     // near box: 8 largest-cell-edges in every direction (quadrature error there < 1e-16)
     const double dmax = fmax(s->dx, fmax(s->dy, s->dz));
@@ -891,22 +915,37 @@ template <typename T> static int init_demag_t(mm_sim* s)
     const size_t Bn = (size_t)bx * by * bz;
     std::vector<double> near(6 * Bn);
     mm_newell_near_box(bx, by, bz, s->dx, s->dy, s->dz, near.data());
-    double* d_near = nullptr;
-    cx<double>* A = nullptr;
-    unsigned long long* d_max = nullptr;
-    MM_TRY(s, cudaMalloc(&d_near, 6 * Bn * sizeof(double)));
-    MM_TRY(s, cudaMalloc(&A, (size_t)P * sizeof(cx<double>)));
-    MM_TRY(s, cudaMalloc(&d_max, 2 * sizeof(unsigned long long)));
-    MM_TRY(s, cudaMemcpyAsync(d_near, near.data(), 6 * Bn * sizeof(double), cudaMemcpyHostToDevice, st));
-    MM_TRY(s, cudaMemsetAsync(d_max, 0, 2 * sizeof(unsigned long long), st));
+    DevBuf d_near;
+    MM_TRY(s, d_near.alloc(6 * Bn * sizeof(double)));
+    MM_TRY(s, cudaMemcpyAsync(d_near.p, near.data(), 6 * Bn * sizeof(double), cudaMemcpyHostToDevice, st));
     QuadRule rule;
     make_rule(s->dx, &rule.n[0], rule.s[0], rule.w[0]);
     make_rule(s->dy, &rule.n[1], rule.s[1], rule.w[1]);
     make_rule(s->dz, &rule.n[2], rule.s[2], rule.w[2]);
-    double* Nr = wsp<double>(s, s->off_Nr);
-    tensor_real_kernel<<<(unsigned)((N + 127) / 128), 128, 0, st>>>(g.nx, g.ny, g.nz, s->dx, s->dy, s->dz, rule, bx, by, bz, d_near, Nr);
+    tensor_real_kernel<<<(unsigned)((g.N + 127) / 128), 128, 0, st>>>(g.nx, g.ny, g.nz, s->dx, s->dy, s->dz, rule, bx, by, bz, d_near.as<double>(), Nr);
     s->launches++;
     MM_TRY(s, cudaGetLastError());
+    MM_TRY(s, cudaStreamSynchronize(st));      // d_near and `near` are released on return
+    return MM_OK;
+}
+
+template <typename T> static int init_demag_t(mm_sim* s)
+{
+    const Geom& g = s->g;
+    const long N = g.N, P = (long)g.px * g.py * g.pz;
+    cudaStream_t st = s->stream;
+    // Transient arrays.  The padded complex tensor A (P fp64 complex numbers, 128 N bytes at most) lives in the
+    // caller's workspace, in the slots of H_d and the RK stage vectors (11 x 3N reals >= 132 N bytes), which hold
+    // nothing before the first evaluation; the real-space tensor (6N doubles) and three small tables are
+    // cudaMalloc'ed here and freed on every exit path.
+    if ((size_t)P * sizeof(cx<double>) > s->off_tw - s->off_Hd) return fail(s, MM_ERR_NOMEM, "workspace scratch smaller than the padded tensor");
+    cx<double>* A = wsp<cx<double>>(s, s->off_Hd);
+    DevBuf d_Nr, d_max, d_tw;
+    MM_TRY(s, d_Nr.alloc((size_t)6 * N * sizeof(double)));
+    MM_TRY(s, d_max.alloc(2 * sizeof(unsigned long long)));
+    MM_TRY(s, cudaMemsetAsync(d_max.p, 0, 2 * sizeof(unsigned long long), st));
+    double* Nr = d_Nr.as<double>();
+    { int rc = build_real_tensor(s, Nr); if (rc) return rc; }
     // fp64 twiddles for the setup transforms
     const int twN = s->twN, ntw = twN / 2 + 1;
     std::vector<cx<double>> htw(ntw);
@@ -914,10 +953,9 @@ template <typename T> static int init_demag_t(mm_sim* s)
         const long double a = -2.0L * 3.14159265358979323846264338327950288L * (long double)k / (long double)twN;
         htw[k].x = (double)cosl(a); htw[k].y = (double)sinl(a);
     }
-    cx<double>* d_tw = nullptr;
-    MM_TRY(s, cudaMalloc(&d_tw, ntw * sizeof(cx<double>)));
-    MM_TRY(s, cudaMemcpyAsync(d_tw, htw.data(), ntw * sizeof(cx<double>), cudaMemcpyHostToDevice, st));
-    twiddles<double> tw; tw.tw = d_tw; tw.twN = twN;
+    MM_TRY(s, d_tw.alloc(ntw * sizeof(cx<double>)));
+    MM_TRY(s, cudaMemcpyAsync(d_tw.p, htw.data(), ntw * sizeof(cx<double>), cudaMemcpyHostToDevice, st));
+    twiddles<double> tw; tw.tw = d_tw.as<cx<double>>(); tw.twN = twN;
     MM_TRY(s, cudaFuncSetAttribute(setup_fft_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_CAP));
     T* Kh = wsp<T>(s, s->off_Kh);
     MM_TRY(s, cudaMemsetAsync(Kh, 0, (size_t)6 * g.kcomp * sizeof(T), st));
@@ -941,7 +979,7 @@ template <typename T> static int init_demag_t(mm_sim* s)
         if ((rc = line_fft(g.py, g.px, (long)g.px * g.pz, g.px, 1, (long)g.px * g.py, 0))) return rc;
         if ((rc = line_fft(g.pz, (long)g.px * g.py, (long)g.px * g.py, g.px * g.py, 1, 0, 0))) return rc;
         const long total = g.kcomp;
-        pack_khat_kernel<T><<<(unsigned)((total + 255) / 256), 256, 0, st>>>(g, c, A, Kh, d_max);
+        pack_khat_kernel<T><<<(unsigned)((total + 255) / 256), 256, 0, st>>>(g, c, A, Kh, d_max.as<unsigned long long>());
         s->launches++;
         MM_TRY(s, cudaGetLastError());
     }
@@ -952,13 +990,13 @@ template <typename T> static int init_demag_t(mm_sim* s)
         MM_TRY(s, cudaGetLastError());
     }
     unsigned long long hmax[2];
-    MM_TRY(s, cudaMemcpyAsync(hmax, d_max, sizeof(hmax), cudaMemcpyDeviceToHost, st));
+    MM_TRY(s, cudaMemcpyAsync(hmax, d_max.p, sizeof(hmax), cudaMemcpyDeviceToHost, st));
     MM_TRY(s, cudaStreamSynchronize(st));
     double re, im;
     memcpy(&re, &hmax[0], 8); memcpy(&im, &hmax[1], 8);
     s->khat_imag_ratio = re > 0 ? im / re : -1;
-    cudaFree(d_near); cudaFree(A); cudaFree(d_max); cudaFree(d_tw);
-    if (!(s->khat_imag_ratio < 1e-10)) return fail(s, MM_ERR_CUDA, "demag tensor spectrum is not real: setup failed");
+    // a numerical self-check, not a CUDA failure: every component is even, or odd in exactly two axes, so K^ is real
+    if (!(s->khat_imag_ratio < 1e-10)) return fail(s, MM_ERR_INTERNAL, "demag tensor spectrum is not real: setup failed its symmetry check");
     return MM_OK;
 }
 
@@ -993,7 +1031,14 @@ extern "C" int mm_get_demag_kernel(mm_sim* s, int comp, void* dev_out)
     NEED_WS(s);
     if (!s->demag_ready) return fail(s, MM_ERR_STATE, "mm_init_demag not called");
     if (comp < 0 || comp > 5 || !dev_out) return MM_ERR_ARG;
-    MM_TRY(s, cudaMemcpyAsync(dev_out, wsp<double>(s, s->off_Nr) + (size_t)comp * s->g.N, s->g.N * sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
+    // a test hook, off every hot path: the tensor is not kept resident (6N doubles), it is rebuilt on request
+    MM_TRY(s, cudaSetDevice(s->device));
+    DevBuf d_Nr;
+    MM_TRY(s, d_Nr.alloc((size_t)6 * s->g.N * sizeof(double)));
+    int rc = build_real_tensor(s, d_Nr.as<double>());
+    if (rc) return rc;
+    MM_TRY(s, cudaMemcpyAsync(dev_out, d_Nr.as<double>() + (size_t)comp * s->g.N, s->g.N * sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
+    MM_TRY(s, cudaStreamSynchronize(s->stream));
     return MM_OK;
 }
 
@@ -1024,34 +1069,29 @@ template <typename T> static LocalP<T> make_local(const mm_sim* s, int terms)
 // demag passes A, B, C: y -> Hd.  v2 kernels where the mesh allows, v1 otherwise (tiny meshes).
 template <typename T, int NZ> static void launch_A2(mm_sim* s, unsigned grid, const T* y, cx<T>* S, twiddles<T> tw, const DevState* st)
 {
-    static bool attr = false;
-    if (!attr) { cudaFuncSetAttribute(fwd_xz2_kernel<T, NZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_CAP); attr = true; }
+    if (!raise_smem_limit(s, (const void*)fwd_xz2_kernel<T, NZ>)) return;
     fwd_xz2_kernel<T, NZ><<<grid, s->thrA, s->smemA2, s->stream>>>(s->g, y, wsp<T>(s, s->off_Ms), S, tw, st);
 }
 template <typename T, int NZ> static void launch_C2(mm_sim* s, unsigned grid, cx<T>* S, twiddles<T> tw, T sc, const DevState* st)
 {
-    static bool attr = false;
-    if (!attr) { cudaFuncSetAttribute(inv_zx2_kernel<T, NZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_CAP); attr = true; }
+    if (!raise_smem_limit(s, (const void*)inv_zx2_kernel<T, NZ>)) return;
     inv_zx2_kernel<T, NZ><<<grid, s->thrA, s->smemA2, s->stream>>>(s->g, S, wsp<T>(s, s->off_Hd), tw, sc, st);
 }
 template <typename T, int V> static void launch_B2(mm_sim* s, unsigned grid, cx<T>* S, twiddles<T> tw, const DevState* st)
 {
-    static bool attr = false;
-    if (!attr) { cudaFuncSetAttribute(y_conv2_kernel<T, V>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_CAP); attr = true; }
+    if (!raise_smem_limit(s, (const void*)y_conv2_kernel<T, V>)) return;
     y_conv2_kernel<T, V><<<grid, s->thrB, s->smemB, s->stream>>>(s->g, S, wsp<T>(s, s->off_Kc), tw, st);
 }
 
 template <typename T, int V> static void launch_B5(mm_sim* s, unsigned grid, cx<T>* S, twiddles<T> tw, const DevState* st)
 {
-    static bool attr = false;
-    if (!attr) { cudaFuncSetAttribute(y_conv5_kernel<T, V>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_CAP); attr = true; }
+    if (!raise_smem_limit(s, (const void*)y_conv5_kernel<T, V>)) return;
     y_conv5_kernel<T, V><<<grid, s->thrB, s->smemB, s->stream>>>(s->g, S, wsp<T>(s, s->off_Kc), tw, st, s->tmS);
 }
 
 template <int LOGM, bool IS3D> static void launch_B7(mm_sim* s, unsigned grid, cx<float>* S, twiddles<float> tw, const DevState* st)
 {
-    static bool attr = false;
-    if (!attr) { cudaFuncSetAttribute(y_conv7_kernel<LOGM, IS3D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_CAP); attr = true; }
+    if (!raise_smem_limit(s, (const void*)y_conv7_kernel<LOGM, IS3D>)) return;
     y_conv7_kernel<LOGM, IS3D><<<grid, 256, s->smemB, s->stream>>>(s->g, S, wsp<float>(s, s->off_Kc), tw, ilog2(s->twN), st, s->tmS);
 }
 // ny = 2^4 .. 2^9 with TC = 4 and the TMA tile: the specialised kernel; false = not covered
@@ -1148,7 +1188,7 @@ template <typename T, int MODE, int S, bool NEXT, bool ERR, bool MAXK>
 static void launch_stage(mm_sim* s, const LocalP<T>& lp, const T* y, const T* Hd, T* out, const StageArgs<T>& sa)
 {
     constexpr int CPT = MM_STAGEV_CPT;
-    if (s->g.nx % CPT == 0 && !getenv("MM_NO_STAGEV")) {
+    if (s->g.nx % CPT == 0 && !s->no_stagev) {
         const unsigned blocks = (unsigned)((s->g.N / CPT + MM_STAGEV_THREADS - 1) / MM_STAGEV_THREADS);
         llg_stagev_kernel<T, CPT, MODE, S, NEXT, ERR, MAXK><<<blocks, MM_STAGEV_THREADS, 0, s->stream>>>(s->g, lp, y, wsp<T>(s, s->off_Ms), wsp<unsigned char>(s, s->off_nbm), Hd, out, sa, wsp<DevState>(s, s->off_st));
         return;
@@ -1263,7 +1303,7 @@ template <typename T> static int enqueue_step(mm_sim* s, T* m, int ctrl_mode)
     DevState* ds = wsp<DevState>(s, s->off_st);
     ctrl_kernel<<<1, 1, 0, s->stream>>>(ds, s->prec == MM_F64, ctrl_mode);
     const T* ysol = yb[1];     // DOPRI5: y_6 written at stage 5 ; RK4: solution written at stage 3
-    accept_kernel<T><<<(unsigned)((N + 255) / 256), 256, 0, s->stream>>>(N, ds, ysol, wsp<T>(s, s->off_Ms), m, 0);
+    accept_kernel<T><<<(unsigned)((N + 255) / 256), 256, 0, s->stream>>>(N, ds, ysol, wsp<T>(s, s->off_Ms), m);
     s->launches += 2;
     MM_TRY(s, cudaGetLastError());
     return MM_OK;
@@ -1335,14 +1375,18 @@ extern "C" int mm_relax(mm_sim* s, void* dev_m, double tol, double stop_dmdt, lo
 extern "C" int mm_run_until(mm_sim* s, void* dev_m, double t_end, double tol, double dt0, long max_steps, long* steps_done)
 {
     NEED_READY(s);
+    {   // steps enqueued without a host read-back (mm_step with NULL out-pointers) have advanced the device clock
+        DevState h;
+        int rc = read_state(s, &h);
+        if (rc) return rc;
+    }
     if (!(t_end > s->t_host)) return fail(s, MM_ERR_ARG, "t_end must be later than the current time");
     const double left = t_end - s->t_host;
     return adaptive_loop(s, dev_m, tol, dt0 < left ? dt0 : left, t_end, 0.0, 2, max_steps, steps_done, nullptr);
 }
 
-extern "C" double mm_time(const mm_sim* cs)
+extern "C" double mm_time(mm_sim* s)
 {
-    mm_sim* s = const_cast<mm_sim*>(cs);
     if (!s || !s->ws) return 0.0;
     DevState h;
     if (read_state(s, &h)) return s->t_host;
