@@ -3,15 +3,21 @@
 Dormand-Prince step (7 RHS evaluations: demag FFT convolution + local field + torque + RK stage
 algebra) of a 512x512x16 mesh.  Metric: cell-updates/s per RHS evaluation = N * 7 * steps / seconds.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--prec f32|f64] [--workload cfg4|cfg5_<n>]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--prec f32|f64|both] [--workload cfg4|cfg5_<n>]
   python bench.py --impl reference ...      # the CPU oracle on a bounded sample of the same workload
 
-N > 1 (torchrun): independent replicas, one per GPU, no data-path collective ("replicas only",
-DESIGN.md); value = cells all ranks processed / max-over-ranks time.
+One JSON line.  Its top-level fields are the fp32 run (the arithmetic the paper's throughput figure is quoted in,
+PAPER.md:495); with --prec both (the default) the same line carries an "fp64" object with the fp64 run's value,
+ms_per_step, roofline and e2e.  N > 1: independent replicas, one per GPU, no data-path collective ("replicas
+only"); value = cells all ranks processed / max-over-ranks time.  Started without torchrun,
+`--gpus N` launches the N ranks itself (torch.distributed.run on 127.0.0.1).
 """
 import argparse
+import csv
+import ctypes
 import json
 import os
+import socket
 import subprocess
 import sys
 import threading
@@ -24,13 +30,8 @@ if ROOT not in sys.path:
 METRIC = "cell_updates_per_sec_per_rhs_eval"
 UNIT = "cell-updates/s"
 RHS_PER_STEP = 7
-
-
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
-# (profiles/r01_ncu_full_v6.md); None where no capture of that kernel / workload / precision exists.
-NCU_TRAFFIC = {("cfg4_slab_512x512x16", "f32", "y_conv"): 520.2e6 + 187.2e6,
-               ("cfg4_slab_512x512x16", "f32", "fwd_xz"): 68.2e6 + 159.6e6,
-               ("cfg4_slab_512x512x16", "f32", "inv_zx"): 202.9e6 + 31.4e6}
+CLASSES = ["fwd_xz", "y_conv", "inv_zx", "llg_stage"]
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
 
 
 def measured_peaks():
@@ -41,6 +42,20 @@ def measured_peaks():
         except Exception:
             pass
     return 6650.0, "fallback"
+
+
+def ncu_traffic(version, workload, prec, cls):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of kernel class `cls`, from the committed table of
+    `ncu --set full` captures (profiles/ncu_traffic.csv).  A row counts only if it was captured from THIS library
+    version (mm_version()), workload and precision; otherwise None — a stale capture is not a measurement."""
+    try:
+        with open(TRAFFIC_CSV) as f:
+            for row in csv.DictReader(r for r in f if not r.startswith("#")):
+                if (row["mm_version"], row["workload"], row["prec"], row["class"]) == (version, workload, prec, cls):
+                    return float(row["dram_read_bytes"]) + float(row["dram_write_bytes"])
+    except Exception:
+        pass
+    return None
 
 
 def get_workload(name):
@@ -56,47 +71,89 @@ def get_workload(name):
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md)."""
+    """SM clock and throttle reasons of one GPU, polled through NVML every ~5 ms with a timestamp per sample
+    (nvidia-smi -lms as the fallback), so that the samples inside the timed region can be picked out."""
+
+    REASONS = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20, "sw_power_cap": 0x4}
 
     def __init__(self, index):
-        self.index, self.rows, self.proc = index, [], None
+        self.index, self.rows, self.stop_flag, self.th, self.mode = index, [], False, None, None
 
     def start(self):
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.mode = "nvml"
+            self.th = threading.Thread(target=self._poll_nvml, daemon=True)
+            self.th.start()
+            return
+        except Exception:
+            self.mode = None
         q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits", "-lms", "100",
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits", "-lms", "20",
                                           "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
-            self.th = threading.Thread(target=self._read, daemon=True)
+            self.mode = "smi"
+            self.th = threading.Thread(target=self._read_smi, daemon=True)
             self.th.start()
         except Exception:
-            self.proc = None
+            self.mode = None
 
-    def _read(self):
-        for line in self.proc.stdout:
-            self.rows.append([c.strip() for c in line.split(",")])
-
-    def stop(self):
-        if not self.proc:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        self.proc.terminate()
-        try:
-            self.proc.wait(timeout=2)
-        except Exception:
-            self.proc.kill()
-        sm, mx, reasons = [], [], set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for r in self.rows:
+    def _poll_nvml(self):
+        nv = self.nv
+        while not self.stop_flag:
             try:
-                sm.append(float(r[0])); mx.append(float(r[1]))
-                for n, v in zip(names, r[2:6]):
-                    if v.lower().startswith("active"):
-                        reasons.add(n)
+                mhz = float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    mask = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:
+                    mask = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                self.rows.append((time.perf_counter(), mhz, self.max_mhz, mask))
             except Exception:
                 pass
-        sm.sort()
-        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "reasons": sorted(reasons), "samples": len(sm)}
+            time.sleep(0.004)
+
+    def _read_smi(self):
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.proc.stdout:
+            r = [c.strip() for c in line.split(",")]
+            try:
+                mask = 0
+                for n, v in zip(names, r[2:6]):
+                    if v.lower().startswith("active"):
+                        mask |= self.REASONS[n]
+                self.rows.append((time.perf_counter(), float(r[0]), float(r[1]), mask))
+            except Exception:
+                pass
+
+    def stop(self, t0=None, t1=None):
+        """Summary of the samples with t0 <= timestamp <= t1 (all samples when the window holds none)."""
+        self.stop_flag = True
+        if self.mode == "smi":
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                self.proc.kill()
+        if self.th is not None:
+            self.th.join(timeout=1)
+        if not self.mode:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["clock sampling unavailable"], "samples": 0}
+        rows = [r for r in self.rows if t0 is None or (t0 <= r[0] <= t1)]
+        window = "timed region"
+        if not rows:
+            rows, window = list(self.rows), "whole run (no sample fell inside the timed region)"
+        sm = sorted(r[1] for r in rows)
+        mask = 0
+        for r in rows:
+            mask |= r[3]
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max((r[2] for r in rows), default=None),
+                "reasons": sorted(n for n, b in self.REASONS.items() if mask & b), "samples": len(sm), "window": window,
+                "source": self.mode}
 
 
 def aggregate_over_ranks(local_seconds, local_units, device=None):
@@ -114,15 +171,30 @@ def aggregate_over_ranks(local_seconds, local_units, device=None):
 
 def algorithmic_bytes(w, esize):
     """per RHS 39 N s (film) / 89 N s (3-D); DOPRI5 step = 7 RHS + 102 N s.
-    Pass B ("last forward + multiply + first inverse"): 16 N s (film) / 30 N s (3-D)."""
+    Per kernel class (units of N s): pass B is SURVEY's "last forward + multiply + first inverse (+K^)" row,
+    16 (film) / 30 (3-D); this build does z inside the x passes, so A = 4 + 6 / 4 + 12 and C = 6 + 3 / 12 + 3
+    (DESIGN.md §5); the stage kernel reads H_d, m, Ms and writes k: 13 (+3 per earlier k_j it reads)."""
     N = w.N
     three_d = w.nz > 1
+    per_class = {"fwd_xz": 16 if three_d else 10, "y_conv": 30 if three_d else 16, "inv_zx": 15 if three_d else 9, "llg_stage": 13}
     return {"rhs": (89 if three_d else 39) * N * esize, "step": (7 * (89 if three_d else 39) + 102) * N * esize,
-            "passB": (30 if three_d else 16) * N * esize}
+            "class": {k: v * N * esize for k, v in per_class.items()}}
+
+
+# ------------------------------------------------------------------------------------------------------------
+# CPU legs: the oracle, as it stands, on the host cores
+# ------------------------------------------------------------------------------------------------------------
+def omp_set_threads(n):
+    """Thread count of the oracle's OpenMP loops for the calls that follow (the runtime libmo.so is linked with)."""
+    try:
+        ctypes.CDLL("libgomp.so.1").omp_set_num_threads(int(n))
+        return True
+    except Exception:
+        return False
 
 
 def oracle_sample(w, shrink=0):
-    """Bounded sample of the workload for the CPU legs: same cells/material, fewer cells (shrink halves the
+    """Bounded sample of the workload for the reference arm: same cells/material, fewer cells (shrink halves the
     in-plane size again)."""
     from paper_2406_16064_b200 import workloads as wl
     if w.nz > 1:
@@ -153,6 +225,38 @@ def time_oracle(ws, steps, warmup, per_step_rhs):
     return dt, ws.N * per_step_rhs * steps
 
 
+def cpu_baseline_full_mesh(w):
+    """BASELINE.md's plan: the oracle's FFT-path RHS on the benchmark's OWN mesh (no sub-mesh), one evaluation with
+    all host cores and one with a single thread.  `value` is the all-cores figure."""
+    import numpy as np
+    import oracle
+    from paper_2406_16064_b200 import workloads as wl
+    cores = os.cpu_count()
+    t_setup = time.perf_counter()
+    o = oracle.Oracle(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz)
+    wl.apply(o, w)
+    m = np.ascontiguousarray(w.m0)
+    o.llg_rhs(m)                       # first call: builds the cached spectrum (setup, untimed) and warms up
+    t_setup = time.perf_counter() - t_setup
+    t0 = time.perf_counter()
+    o.llg_rhs(m)
+    t_all = time.perf_counter() - t0
+    one = None
+    # single thread only when it stays a bounded sample (~30 s): estimated from the all-cores time
+    if omp_set_threads(1) and t_all * cores <= 60.0:
+        t0 = time.perf_counter()
+        o.llg_rhs(m)
+        one = time.perf_counter() - t0
+    omp_set_threads(cores)
+    out = {"value": w.N / t_all, "unit": UNIT, "cores": cores, "kind": "oracle",
+           "sample": f"1 RHS evaluation (oracle FFT path, fp64) on the full {w.nx}x{w.ny}x{w.nz} mesh, all {cores} host cores; "
+                     f"setup (quad-precision tensor + spectrum) {t_setup:.1f} s untimed",
+           "seconds_per_rhs": t_all}
+    if one is not None:
+        out["single_thread"] = {"value": w.N / one, "unit": UNIT, "cores": 1, "seconds_per_rhs": one}
+    return out
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -178,59 +282,61 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
-def run_mm(args):
+# ------------------------------------------------------------------------------------------------------------
+# The CUDA path
+# ------------------------------------------------------------------------------------------------------------
+def measure(args, w, prec_name, rank, world, local, barrier, dev, sample_clocks):
+    """One precision: warm-up, K timed steps (device events, max over ranks), a profiled pass for the per-kernel
+    times, and the end-to-end leg through mm_run_host.  Returns the fields of the JSON line for this precision."""
     import numpy as np
     import torch
-    import torch.distributed as dist
     from paper_2406_16064_b200 import Sim, F32, F64, workloads as wl
+    from paper_2406_16064_b200.binding import load_library
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if world > 1:
-        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", rank=rank, world_size=world, device_id=torch.device("cuda", local))
-    torch.cuda.set_device(local)
-    dev = torch.device("cuda", local)
-    prec = F64 if args.prec == "f64" else F32
+    prec = F64 if prec_name == "f64" else F32
     esize = 8 if prec == F64 else 4
-    w = get_workload(args.workload)
-    w.seed += rank
     s = Sim(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, prec=prec, device=local)
     wl.apply(s, w)
     dm = s.to_device(w.m0)
     host_m = torch.from_numpy(np.ascontiguousarray(w.m0)).to(s.dtype).pin_memory()
+    warm = max(args.warmup, 3)
 
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    # warm-up with every kernel class bracketed by events: per-class times, and which class dominates
+    # which kernel class dominates: every class bracketed by events over the warm-up steps
     s.set_profiling(True)
-    for _ in range(max(args.warmup, 3)):
+    for _ in range(warm):
         s.step(dm, w.dt, sync=False)
     barrier()
     warm_ms, warm_cnt = s.get_profile()
     dom = max(range(4), key=lambda i: warm_ms[i])
     # timed region: only the dominant class keeps its events (2 stream operations per bracketed kernel)
     s.set_profiling(2 << dom)
-    sampler = ClockSampler(local)
-    if rank == 0:
+    sampler = ClockSampler(local) if sample_clocks else None
+    if sampler:
         sampler.start()
+        time.sleep(0.02)
     l0 = s.launch_count()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    t_host0 = time.perf_counter()
     e0.record()
     for _ in range(args.steps):
         s.step(dm, w.dt, sync=False)
     e1.record()
     barrier()
+    t_host1 = time.perf_counter()
     sec = e0.elapsed_time(e1) * 1e-3
     launches = s.launch_count() - l0
+    dom_ms, dom_cnt = s.get_profile()
+    clocks = sampler.stop(t_host0, t_host1) if sampler else None
+    assert bool(torch.isfinite(dm).all()), "non-finite magnetisation after the timed region"
+
+    # per-kernel times of every class: a separate profiled pass over the same number of steps (not part of `value`)
+    s.set_profiling(True)
+    for _ in range(min(args.steps, 20)):
+        s.step(dm, w.dt, sync=False)
+    barrier()
     prof_ms, prof_cnt = s.get_profile()
     s.set_profiling(False)
-    clocks = sampler.stop() if rank == 0 else None
-    assert bool(torch.isfinite(dm).all()), "non-finite magnetisation after the timed region"
 
     # end to end: host buffers through the C ABI, H2D + step + D2H inside the timed region
     e2e_steps = max(1, min(args.steps, 5))
@@ -245,58 +351,89 @@ def run_mm(args):
     units = w.N * RHS_PER_STEP * args.steps
     sec_max, units_all = aggregate_over_ranks(sec, units, dev)
     e2e_max, e2e_units = aggregate_over_ranks(e2e_sec, w.N * RHS_PER_STEP * e2e_steps, dev)
+    version = load_library().mm_version().decode()
+    del s, dm
+    torch.cuda.empty_cache()
     if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
-        return
+        return None
     peak, peak_kind = measured_peaks()
     ab = algorithmic_bytes(w, esize)
-    names = ["fwd_xz", "y_conv", "inv_zx", "llg_stage"]
-    # the dominant class is timed in the timed region, the others come from the warm-up steps
-    per = {n: ((prof_ms[i] / prof_cnt[i]) if prof_cnt[i] else (warm_ms[i] / warm_cnt[i] if warm_cnt[i] else None)) for i, n in enumerate(names)}
-    # algorithmic bytes of each kernel class per launch (units of N*s): SURVEY.md §8(d) rows
-    three_d = w.nz > 1
-    # y_conv is SURVEY's "last forward + multiply + first inverse (+K^)" row; the other rows are DESIGN.md §5's
-    # (this build does z inside the x passes: A = 4 + 12 (film 4 + 6), C = 12 + 3 (film 6 + 3))
-    alg_units = {"fwd_xz": 16 if three_d else 10, "y_conv": 30 if three_d else 16,
-                 "inv_zx": 15 if three_d else 9, "llg_stage": 13}
-    dom_name = names[dom]
-    dom_bytes = alg_units[dom_name] * w.N * esize
-    achieved = dom_bytes / (per[dom_name] * 1e-3) / 1e9
+    per = {n: (prof_ms[i] / prof_cnt[i] if prof_cnt[i] else None) for i, n in enumerate(CLASSES)}
+    dom_name = CLASSES[dom]
+    dom_avg = dom_ms[dom] / dom_cnt[dom]      # the dominant kernel's average launch, measured inside the timed region
+    per[dom_name] = dom_avg
+    dom_bytes = ab["class"][dom_name]
+    achieved = dom_bytes / (dom_avg * 1e-3) / 1e9
     step_gbs = ab["step"] * args.steps / sec / 1e9
-    cpu = None
-    if not args.no_cpu_baseline:
-        ws = oracle_sample(w)
-        csec, cunits = time_oracle(ws, 1, 0, 1)
-        reps = 1
-        while csec < 5.0 and reps < 64:
-            reps *= 2
-            csec, cunits = time_oracle(ws, reps, 0, 1)
-        cpu = {"value": cunits / csec, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle",
-               "sample": f"{reps} RHS evaluation(s) (oracle FFT path, fp64) on a {ws.nx}x{ws.ny}x{ws.nz} sub-mesh of the workload"}
-    line = {
-        "metric": METRIC, "value": units_all / sec_max, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": max(args.warmup, 3), "ms_per_step": 1e3 * sec_max / args.steps, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": args.prec, "data": "synthetic",
-        "config": {"workload": w.name, "mesh": [w.nx, w.ny, w.nz], "integrator": "dopri5_fixed_dt", "dt": w.dt,
-                   "rhs_per_step": RHS_PER_STEP, "parallelism": f"replicas x{world}",
-                   "l2": "working set (spectra + stage vectors > 1 GB) exceeds the 126 MB L2; no explicit flush"},
+    tot = sum(prof_ms)
+    return {
+        "value": units_all / sec_max, "ms_per_step": 1e3 * sec_max / args.steps, "dtype": prec_name,
         "e2e": {"value": e2e_units / e2e_max, "unit": UNIT, "h2d_bytes_per_step": 3 * w.N * esize, "d2h_bytes_per_step": 3 * w.N * esize,
                 "api": "mm_run_host (pinned host m in, one DOPRI5 step, m out)"},
-        "gpu_launches": launches,
-        "clocks": clocks,
+        "gpu_launches": launches, "clocks": clocks,
         "roofline": {"bound": "hbm", "kernel": dom_name, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "peak_kind": peak_kind, "traffic": NCU_TRAFFIC.get((w.name, args.prec, dom_name)), "algorithmic_bytes_per_launch": dom_bytes,
-                     "avg_launch_ms": per[dom_name], "kernel_ms": per,
-                     "kernel_share": {n: warm_ms[i] / sum(warm_ms) for i, n in enumerate(names)},
-                     "kernel_ms_source": f"{dom_name}: CUDA events in the timed region; other classes and kernel_share: the warm-up steps",
-                     "step_algorithmic_gbs": step_gbs, "step_frac": step_gbs / peak,
-                     "step_frac_nominal_8TBs": step_gbs / 8000.0},
-        "cpu_baseline": cpu,
+                     "peak_kind": peak_kind, "traffic": ncu_traffic(version, w.name, prec_name, dom_name),
+                     "traffic_source": "profiles/ncu_traffic.csv row of this mm_version / workload / precision, else null",
+                     "algorithmic_bytes_per_launch": dom_bytes, "avg_launch_ms": dom_avg, "kernel_ms": per,
+                     "kernel_frac": {n: (ab["class"][n] / (per[n] * 1e-3) / 1e9 / peak if per[n] else None) for n in CLASSES},
+                     "kernel_share": {n: prof_ms[i] / tot for i, n in enumerate(CLASSES)},
+                     "kernel_ms_source": f"{dom_name}: CUDA events inside the timed region; the other classes and kernel_share: a profiled "
+                                         "pass of the same steps after it (all classes bracketed, ~3 % slower)",
+                     "step_algorithmic_gbs": step_gbs, "step_frac": step_gbs / peak, "step_frac_nominal_8TBs": step_gbs / 8000.0,
+                     "mm_version": version},
     }
-    print(json.dumps(line), flush=True)
+
+
+def run_mm(args):
+    import torch
+    import torch.distributed as dist
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", rank=rank, world_size=world, device_id=torch.device("cuda", local))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    w = get_workload(args.workload)
+    w.seed += rank
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    precs = ["f32", "f64"] if args.prec == "both" else [args.prec]
+    res = {p: measure(args, w, p, rank, world, local, barrier, dev, sample_clocks=(rank == 0)) for p in precs}
+    if rank == 0:
+        top = res[precs[0]]
+        cpu = None
+        if not args.no_cpu_baseline:
+            cpu = cpu_baseline_full_mesh(w)
+        line = {
+            "metric": METRIC, "value": top["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": top["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": top["dtype"], "data": "synthetic",
+            "config": {"workload": w.name, "mesh": [w.nx, w.ny, w.nz], "integrator": "dopri5_fixed_dt", "dt": w.dt,
+                       "rhs_per_step": RHS_PER_STEP, "parallelism": f"replicas x{world}",
+                       "l2": "working set (spectra + stage vectors > 1 GB) exceeds the 126 MB L2; no explicit flush"},
+            "e2e": top["e2e"], "gpu_launches": top["gpu_launches"], "clocks": top["clocks"], "roofline": top["roofline"],
+            "cpu_baseline": cpu,
+        }
+        if len(precs) > 1:
+            o = res["f64"]
+            line["fp64"] = {k: o[k] for k in ("value", "ms_per_step", "dtype", "e2e", "gpu_launches", "clocks", "roofline")}
+            line["fp64"]["unit"] = UNIT
+        print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
+
+
+def free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
 
 
 def main():
@@ -305,10 +442,19 @@ def main():
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="mm", choices=["mm", "reference"])
-    ap.add_argument("--prec", default="f32", choices=["f32", "f64"])
+    ap.add_argument("--prec", default="both", choices=["f32", "f64", "both"])
     ap.add_argument("--workload", default="cfg4")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
+    world_env = os.environ.get("WORLD_SIZE")
+    if world_env is None and args.gpus > 1:
+        # not under torchrun: start the N ranks ourselves, one process per GPU
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(free_port()), os.path.abspath(__file__)] + sys.argv[1:]
+        raise SystemExit(subprocess.run(cmd).returncode)
+    if world_env is not None and int(world_env) != args.gpus:
+        print(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world_env}: launch one rank per GPU", file=sys.stderr)
+        raise SystemExit(2)
     if args.impl == "reference":
         run_reference(args)
     else:

@@ -50,10 +50,10 @@ def test_algorithmic_bytes_model():
     from paper_2406_16064_b200 import workloads as wl
     w = wl.cfg4(with_m=False)
     ab = bench.algorithmic_bytes(w, 4)
-    assert ab["rhs"] == 89 * w.N * 4 and ab["step"] == (7 * 89 + 102) * w.N * 4 and ab["passB"] == 30 * w.N * 4
+    assert ab["rhs"] == 89 * w.N * 4 and ab["step"] == (7 * 89 + 102) * w.N * 4 and ab["class"]["y_conv"] == 30 * w.N * 4
     f = wl.cfg5(256, with_m=False)
     ab = bench.algorithmic_bytes(f, 8)
-    assert ab["rhs"] == 39 * f.N * 8 and ab["passB"] == 16 * f.N * 8
+    assert ab["rhs"] == 39 * f.N * 8 and ab["class"]["y_conv"] == 16 * f.N * 8
 
 
 def test_reference_arm_json_contract():
@@ -66,3 +66,35 @@ def test_reference_arm_json_contract():
     assert line["cpu_baseline"]["kind"] == "oracle" and line["cpu_baseline"]["value"] == line["value"]
     assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["e2e"]["d2h_bytes_per_step"] == 0
     assert line["higher_is_better"] is True and line["vs_baseline"] is None
+
+
+def test_gpus_flag_launches_the_ranks_itself():
+    """`bench.py --gpus 2` outside torchrun starts two ranks (torch.distributed.run on 127.0.0.1); in the reference arm
+    rank 0 alone works and prints the line with n_gpus = 2, the other rank exits 0."""
+    env = dict(os.environ, MM_REF_BUDGET_S="20")
+    env.pop("WORLD_SIZE", None); env.pop("RANK", None)
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2", "--steps", "1", "--warmup", "0",
+                          "--workload", "cfg5_64"], capture_output=True, text=True, timeout=900, env=env)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [json.loads(l) for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1 and lines[0]["n_gpus"] == 2 and lines[0]["impl"] == "reference"
+
+
+def test_world_size_mismatch_is_an_error():
+    env = dict(os.environ, WORLD_SIZE="4", RANK="0")
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2", "--steps", "1", "--warmup", "0"],
+                         capture_output=True, text=True, timeout=120, env=env)
+    assert out.returncode == 2 and "WORLD_SIZE" in out.stderr
+
+
+def test_ncu_traffic_lookup_is_keyed_by_version(tmp_path, monkeypatch):
+    """roofline.traffic comes from the committed capture table and only for the library version it was captured from."""
+    sys.path.insert(0, ROOT)
+    import bench
+    f = tmp_path / "t.csv"
+    f.write_text("# comment\nmm_version,workload,prec,class,kernel,dram_read_bytes,dram_write_bytes,duration_us,capture\n"
+                 "v1,cfg4_slab_512x512x16,f32,y_conv,k,100,50,1,c\n")
+    monkeypatch.setattr(bench, "TRAFFIC_CSV", str(f))
+    assert bench.ncu_traffic("v1", "cfg4_slab_512x512x16", "f32", "y_conv") == 150.0
+    assert bench.ncu_traffic("v2", "cfg4_slab_512x512x16", "f32", "y_conv") is None
+    assert bench.ncu_traffic("v1", "cfg4_slab_512x512x16", "f64", "y_conv") is None
