@@ -88,13 +88,15 @@ __global__ void __launch_bounds__(MM_B5_THR, MM_B5_OCC) y_conv5_kernel(Geom g, c
     __shared__ __align__(8) unsigned long long bar[3];
     y_conv_body5<T, V>(g, S, Kh, tw, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x, &tmS, bar, &st->done);
 }
-// compile-time specialised form of the TMA pass B (mm_passB7.cuh): fp32, ny = 2^LOGM, TC = 4, 256 threads
-template <int LOGM, bool IS3D>
-__global__ void __launch_bounds__(256, 2) y_conv7_kernel(Geom g, cx<float>* S, const float* Kc, twiddles<float> tw, int logtw, const DevState* st,
-                                                         const __grid_constant__ CUtensorMap tmS)
+// compile-time specialised form of the TMA pass B (mm_passB7.cuh): ny = 2^LOGM; fp32: TC = 4, 256 threads; fp64: TC = 2,
+// 128 threads (rows of 32 bytes and tiles of py * 96 bytes in both; two CTAs per SM)
+template <typename T, int LOGM, bool IS3D>
+__global__ void __launch_bounds__(sizeof(T) == 8 ? 128 : 256, 2) y_conv7_kernel(Geom g, cx<T>* S, const T* Kc, twiddles<T> tw, int logtw, const DevState* st,
+                                                                                const __grid_constant__ CUtensorMap tmS)
 {
     __shared__ __align__(8) unsigned long long bar[3];
-    y_conv_body7<LOGM, IS3D, 256, float>(g, S, Kc, tw, logtw, reinterpret_cast<cx<float>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x, &tmS, bar, &st->done);
+    constexpr int LOGTC = sizeof(T) == 8 ? 1 : 2, NTHR = sizeof(T) == 8 ? 128 : 256;
+    y_conv_body7<LOGM, LOGTC, IS3D, NTHR, T>(g, S, Kc, tw, logtw, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, NTHR, &tmS, bar, &st->done);
 }
 template <typename T, int NZ>
 __global__ void __launch_bounds__(256, sizeof(T) == 8 ? 1 : MM_OCC_C) inv_zx2_kernel(Geom g, const cx<T>* S, T* Hd, twiddles<T> tw, T inv_scale, const DevState* st)
@@ -691,6 +693,9 @@ static void configure(mm_sim* s)
     // shared-memory-bound stages overlap the other's FP32-bound ones (measured, profiles/r01_experiments.md)
     if (s->prec == MM_F32 && !getenv("MM_TC") && g.TC >= 4 && (size_t)smemB_elems(g) * cs > 98 * 1024) g.TC /= 2;
     while (g.TC > 2 && ((g.nx + g.TC) / g.TC) * g.pz < target) g.TC /= 2;
+    // fp64: the specialised pass B (mm_passB7.cuh) wants rows of 32 bytes = two columns, tiles of py * 96 bytes
+    const bool b7_f64 = s->prec == MM_F64 && !getenv("MM_TC") && !s->no_b7 && s->use_v2 && g.logny >= 4 && g.logny <= 9 && g.TC >= 2;
+    if (b7_f64) g.TC = 2;
     g.Lx = ((g.nx + 1 + g.TC - 1) / g.TC) * g.TC;
     g.plane = (long)g.ny * g.Lx;
     g.comp = (long)g.pz * g.plane;
@@ -702,6 +707,7 @@ static void configure(mm_sim* s)
     s->smemB = (size_t)smemB_elems(g) * cs;
     s->thrA = 256;
     s->thrB = (s->prec == MM_F32 && s->smemB > 98 * 1024) ? 512 : 256;
+    if (b7_f64) s->thrB = 128;
     if (getenv("MM_THRB")) s->thrB = atoi(getenv("MM_THRB"));
 }
 
@@ -1089,19 +1095,24 @@ template <typename T, int V> static void launch_B5(mm_sim* s, unsigned grid, cx<
     y_conv5_kernel<T, V><<<grid, s->thrB, s->smemB, s->stream>>>(s->g, S, wsp<T>(s, s->off_Kc), tw, st, s->tmS);
 }
 
-template <int LOGM, bool IS3D> static void launch_B7(mm_sim* s, unsigned grid, cx<float>* S, twiddles<float> tw, const DevState* st)
-{
-    if (!raise_smem_limit(s, (const void*)y_conv7_kernel<LOGM, IS3D>)) return;
-    y_conv7_kernel<LOGM, IS3D><<<grid, 256, s->smemB, s->stream>>>(s->g, S, wsp<float>(s, s->off_Kc), tw, ilog2(s->twN), st, s->tmS);
-}
-// ny = 2^4 .. 2^9 with TC = 4 and the TMA tile: the specialised kernel; false = not covered
-static bool try_launch_B7(mm_sim* s, unsigned grid, cx<float>* S, twiddles<float> tw, const DevState* st)
+template <typename T> static bool b7_applies(const mm_sim* s)
 {
     const Geom& g = s->g;
-    if (!s->use_tma || s->prec != MM_F32 || g.TC != 4 || s->thrB != 256 || s->no_b7) return false;
+    return s->use_v2 && !s->no_b7 && g.logny >= 4 && g.logny <= 9 && g.TC == (sizeof(T) == 8 ? 2 : 4) && s->thrB == (sizeof(T) == 8 ? 128 : 256);
+}
+template <typename T, int LOGM, bool IS3D> static void launch_B7(mm_sim* s, unsigned grid, cx<T>* S, twiddles<T> tw, const DevState* st)
+{
+    if (!raise_smem_limit(s, (const void*)y_conv7_kernel<T, LOGM, IS3D>)) return;
+    y_conv7_kernel<T, LOGM, IS3D><<<grid, s->thrB, s->smemB, s->stream>>>(s->g, S, wsp<T>(s, s->off_Kc), tw, ilog2(s->twN), st, s->tmS);
+}
+// ny = 2^4 .. 2^9 with the TMA tile of 32-byte rows: the specialised kernel; false = not covered
+template <typename T> static bool try_launch_B7(mm_sim* s, unsigned grid, cx<T>* S, twiddles<T> tw, const DevState* st)
+{
+    const Geom& g = s->g;
+    if (!s->use_tma || !b7_applies<T>(s)) return false;
     const bool d3 = g.nz > 1;
     switch (g.logny) {
-#define MM_B7_CASE(L) case L: if (d3) launch_B7<L, true>(s, grid, S, tw, st); else launch_B7<L, false>(s, grid, S, tw, st); return true;
+#define MM_B7_CASE(L) case L: if (d3) launch_B7<T, L, true>(s, grid, S, tw, st); else launch_B7<T, L, false>(s, grid, S, tw, st); return true;
         MM_B7_CASE(4) MM_B7_CASE(5) MM_B7_CASE(6) MM_B7_CASE(7) MM_B7_CASE(8) MM_B7_CASE(9)
 #undef MM_B7_CASE
         default: return false;
@@ -1119,7 +1130,7 @@ static int make_tmap(mm_sim* s)
     s->use_tma = 0;
     // measured (cfg4, B200): fp32, two CTAs per SM: TMA form 0.248 ms vs 0.254; fp64, one CTA per SM: 0.560 vs
     // 0.523 (nothing overlaps the wait for the whole tile) -> on for fp32 only; MM_TMA=0/1 overrides
-    int want = s->prec == MM_F32;
+    int want = s->prec == MM_F32 || b7_applies<double>(s);
     if (getenv("MM_TMA")) want = atoi(getenv("MM_TMA"));
     if (!want || !s->use_v2 || g.ny < 16) return MM_OK;
     if ((g.Lx * cs) % 16 || g.TC * cs < 16 || g.ny > 256 * 64) return MM_OK;
@@ -1159,7 +1170,7 @@ template <typename T> static int demag_passes(mm_sim* s, const T* y)
     }
     prof_end(s);
     prof_begin(s, 1);
-    if (b2 && sizeof(T) == 4 && try_launch_B7(s, gridB, reinterpret_cast<cx<float>*>(S), *reinterpret_cast<twiddles<float>*>(&tw), st)) {
+    if (b2 && try_launch_B7<T>(s, gridB, S, tw, st)) {
     } else if (b2 && s->use_tma) {
         if (sizeof(T) == 4 && g.TC % 2 == 0) launch_B5<T, (sizeof(T) == 4 ? 2 : 1)>(s, gridB, S, tw, st);
         else launch_B5<T, 1>(s, gridB, S, tw, st);

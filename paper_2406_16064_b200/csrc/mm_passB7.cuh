@@ -1,6 +1,6 @@
 // mm_passB7.cuh — pass B (pad + FFT y, H^ = -K^ M^ of Eq. 8 in k-space, inverse FFT y, crop)
-// specialised at compile time: ny = 2^LOGM, TC = 4 columns, 256 threads, fp32, component-major tile moved
-// by TMA box copies.  Same math, tile layout and K^ layout ("Kc", mm_kernels.cuh) as y_conv_body5 in
+// specialised at compile time: ny = 2^LOGM, TC = 2^LOGTC columns of 32 bytes per row (fp32: TC = 4, 256 threads;
+// fp64: TC = 2, 128 threads with twice the registers), component-major tile moved by TMA box copies.  Same math, tile layout and K^ layout ("Kc", mm_kernels.cuh) as y_conv_body5 in
 // mm_kernels2.cuh; what changes is how the work is issued (profiles/r02_*: the generic body spends a quarter
 // of its warp time on exposed global-load latency and on index arithmetic):
 //   * every stride and trip count is a constant, so the shared-memory accesses of a stage are base + immediate
@@ -19,15 +19,16 @@
 
 namespace mm {
 
-template <int LOGM> struct B7 {
-    static constexpr int M = 1 << LOGM, N = 2 * M, TC = 4, NT = 256;
+template <int LOGM, int LOGTC> struct B7 {
+    static constexpr int M = 1 << LOGM, N = 2 * M, TC = 1 << LOGTC;
+    static constexpr int LOGLCV = LOGTC - 1, LCV = TC / 2;      // column pairs (16 / 32-byte accesses of the middle stages)
     static constexpr int R1 = (LOGM % 3 == 0) ? 8 : ((LOGM % 3 == 2) ? 4 : 2);      // first_radix(M)
     static constexpr int LOGR1 = (LOGM % 3 == 0) ? 3 : (LOGM % 3);
     static constexpr int SUB1 = M / R1;                 // butterflies of the first / last stage per column
     static constexpr int CS = N * TC;                   // component stride of the tile (complex elements)
     static constexpr int NBK = N / 8;                   // radix-8 blocks of the multiply stage
     static constexpr int RB = M < 256 ? M : 256;        // rows per TMA box
-    static_assert(LOGM >= 4, "ny >= 16");
+    static_assert(LOGM >= 4 && LOGTC >= 1, "ny >= 16, TC >= 2");
 };
 
 template <typename T> struct tw8 { cx<T> p[8]; };      // p[r] = w^brev3(r), p[0] unused
@@ -53,14 +54,14 @@ template <typename T, int R> MM_HD twfl<T, R> b7_fl_tw(twiddles<T> tw, int logtw
 
 // ---- stages ------------------------------------------------------------------------------------------------
 // first: rows i + r*SUB1 of the TMA-deposited lower half -> radix R1 of (a) and of (a * pad twiddle), both halves
-template <int LOGM, int NTHR, typename T>
-MM_HD void b7_first(cx<T>* s, const twfl<T, B7<LOGM>::R1>& pre, twiddles<T> tw, int logtw, int tid, int nthr, unsigned long long* bars)
+template <int LOGM, int LOGTC, int NTHR, typename T>
+MM_HD void b7_first(cx<T>* s, const twfl<T, B7<LOGM, LOGTC>::R1>& pre, twiddles<T> tw, int logtw, int tid, int nthr, unsigned long long* bars)
 {
-    typedef B7<LOGM> P;
+    typedef B7<LOGM, LOGTC> P;
     constexpr int R = P::R1, TC = P::TC;
     bool first = true;
     for (int f = tid; f < P::SUB1 * TC; f += NTHR, first = false) {
-        const int col = f & (TC - 1), i = f >> 2;
+        const int col = f & (TC - 1), i = f >> LOGTC;
         const twfl<T, R> t = first ? pre : b7_fl_tw<T, R>(tw, logtw, LOGM + 1, i);
         cx<T>* base = s + i * TC + col;
 #pragma unroll
@@ -83,14 +84,14 @@ MM_HD void b7_first(cx<T>* s, const twfl<T, B7<LOGM>::R1>& pre, twiddles<T> tw, 
 }
 
 // last: inverse radix R1 on both halves, crop combine a + conj(w) u -> the lower half of the tile
-template <int LOGM, int NTHR, typename T>
-MM_HD void b7_last(cx<T>* s, const twfl<T, B7<LOGM>::R1>& pre, twiddles<T> tw, int logtw, int tid, int nthr)
+template <int LOGM, int LOGTC, int NTHR, typename T>
+MM_HD void b7_last(cx<T>* s, const twfl<T, B7<LOGM, LOGTC>::R1>& pre, twiddles<T> tw, int logtw, int tid, int nthr)
 {
-    typedef B7<LOGM> P;
+    typedef B7<LOGM, LOGTC> P;
     constexpr int R = P::R1, TC = P::TC;
     bool first = true;
     for (int f = tid; f < P::SUB1 * TC; f += NTHR, first = false) {
-        const int col = f & (TC - 1), i = f >> 2;
+        const int col = f & (TC - 1), i = f >> LOGTC;
         const twfl<T, R> t = first ? pre : b7_fl_tw<T, R>(tw, logtw, LOGM + 1, i);
         cx<T>* base = s + i * TC + col;
 #pragma unroll
@@ -110,15 +111,15 @@ MM_HD void b7_last(cx<T>* s, const twfl<T, B7<LOGM>::R1>& pre, twiddles<T> tw, i
 }
 
 // middle radix-8 stage on blocks of length 2^LOGLC, two columns (16 bytes) per access
-template <int LOGM, int LOGLC, int DIR, int NTHR, typename T>
+template <int LOGM, int LOGTC, int LOGLC, int DIR, int NTHR, typename T>
 MM_HD void b7_mid8(cx<T>* s, const tw8<T>& pre, twiddles<T> tw, int logtw, int tid, int nthr)
 {
-    typedef B7<LOGM> P;
+    typedef B7<LOGM, LOGTC> P;
     typedef cvec<T, 2> E;
     constexpr int TC = P::TC, SUB = 1 << (LOGLC - 3), RS = SUB * TC;
     bool first = true;
-    for (int f = tid; f < (P::N >> 3) * 2; f += NTHR, first = false) {
-        const int lc = f & 1, b = f >> 1;
+    for (int f = tid; f < (P::N >> 3) * P::LCV; f += NTHR, first = false) {
+        const int lc = f & (P::LCV - 1), b = f >> P::LOGLCV;
         const int blk = b >> (LOGLC - 3), i = b & (SUB - 1);
         const tw8<T> t = first ? pre : b7_mid_tw<T>(tw, logtw, LOGLC, i);
         cx<T>* base = s + ((blk << LOGLC) + i) * TC + lc * 2;
@@ -142,12 +143,12 @@ MM_HD void b7_mid8(cx<T>* s, const tw8<T>& pre, twiddles<T> tw, int logtw, int t
         }
     }
 }
-template <int LOGM, typename T> MM_HD int b7_mid_i(int f, int logLc) { return (f >> 1) & ((1 << (logLc - 3)) - 1); }
+template <int LOGTC> MM_HD int b7_mid_i(int f, int logLc) { return (f >> (LOGTC - 1)) & ((1 << (logLc - 3)) - 1); }
 
 template <typename T, int NJ> struct kset { T k[NJ]; };
-template <typename T, bool IS3D> MM_HD kset<T, IS3D ? 48 : 32> b7_kload(const T* Kt, int set, int col)
+template <typename T, bool IS3D, int TC> MM_HD kset<T, IS3D ? 48 : 32> b7_kload(const T* Kt, int set, int col)
 {
-    constexpr int NQ = IS3D ? 6 : 4, NJ = 8 * NQ, EPL = 16 / (int)sizeof(T), NJQ = NJ / EPL, TC = 4;
+    constexpr int NQ = IS3D ? 6 : 4, NJ = 8 * NQ, EPL = 16 / (int)sizeof(T), NJQ = NJ / EPL;
     kset<T, NJ> r;
     const T* Kp = Kt + (long)set * (NJ * TC) + col * EPL;
 #pragma unroll
@@ -160,22 +161,22 @@ template <typename T, bool IS3D> MM_HD kset<T, IS3D ? 48 : 32> b7_kload(const T*
 }
 
 // multiply stage: item = (column, mirror pair of 8-row blocks), see yB_mul8 in mm_kernels2.cuh
-template <int LOGM, bool IS3D, int NTHR, typename T>
+template <int LOGM, int LOGTC, bool IS3D, int NTHR, typename T>
 MM_HD void b7_mul8(cx<T>* s, const kset<T, IS3D ? 48 : 32>& pre, const T* Kt, T sz, int tid, int nthr)
 {
-    typedef B7<LOGM> P;
+    typedef B7<LOGM, LOGTC> P;
     constexpr int NQ = IS3D ? 6 : 4, NJ = 8 * NQ, TC = P::TC, NBK = P::NBK, LOGNBK = LOGM - 2;
     bool first = true;
     for (int f = tid; f < (NBK >> 1) * TC; f += NTHR, first = false) {
-        const int col = f & (TC - 1), t = f >> 2;
-        kset<T, NJ> K = first ? pre : b7_kload<T, IS3D>(Kt, t, col);
+        const int col = f & (TC - 1), t = f >> LOGTC;
+        kset<T, NJ> K = first ? pre : b7_kload<T, IS3D, TC>(Kt, t, col);
         int ro[8];
 #pragma unroll
         for (int r = 0; r < 8; r++) ro[r] = ((r + t) & 7) * TC;
 #pragma unroll
         for (int h = 0; h < 2; h++) {
             const int beta = h == 0 ? t : (t == 0 ? (NBK >> 1) : NBK - t);
-            if (h == 1 && t == 0) K = b7_kload<T, IS3D>(Kt, NBK >> 1, col);
+            if (h == 1 && t == 0) K = b7_kload<T, IS3D, TC>(Kt, NBK >> 1, col);
             cx<T>* p = s + ((int)brev((unsigned)beta, LOGNBK) * 8) * TC + col;
             cx<T> Mv[3][8];
 #pragma unroll
@@ -213,37 +214,37 @@ MM_HD void b7_mul8(cx<T>* s, const kset<T, IS3D ? 48 : 32>& pre, const T* Kt, T 
 
 // forward middle stages Lc = 2^LOGLC, 2^(LOGLC-3), ..., 64 ; each one ends with the block barrier and, before
 // it, the loads of what the following stage needs first (its twiddle; the K^ set of the multiply stage)
-template <int LOGM, int LOGLC, bool IS3D, int NTHR, typename T>
+template <int LOGM, int LOGTC, int LOGLC, bool IS3D, int NTHR, typename T>
 MM_HD void b7_fwd_mids(cx<T>* s, twiddles<T> tw, int logtw, const T* Kt, int tid, int nthr, kset<T, IS3D ? 48 : 32>& kpre)
 {
     if constexpr (LOGLC > 3) {
-        const tw8<T> t = b7_mid_tw<T>(tw, logtw, LOGLC, b7_mid_i<LOGM, T>(tid, LOGLC));
+        const tw8<T> t = b7_mid_tw<T>(tw, logtw, LOGLC, b7_mid_i<LOGTC>(tid, LOGLC));
         MM_SYNC();
-        b7_mid8<LOGM, LOGLC, 0, NTHR, T>(s, t, tw, logtw, tid, nthr);
-        b7_fwd_mids<LOGM, LOGLC - 3, IS3D, NTHR, T>(s, tw, logtw, Kt, tid, nthr, kpre);
+        b7_mid8<LOGM, LOGTC, LOGLC, 0, NTHR, T>(s, t, tw, logtw, tid, nthr);
+        b7_fwd_mids<LOGM, LOGTC, LOGLC - 3, IS3D, NTHR, T>(s, tw, logtw, Kt, tid, nthr, kpre);
     } else {
-        if (tid < (B7<LOGM>::NBK >> 1) * B7<LOGM>::TC) kpre = b7_kload<T, IS3D>(Kt, tid >> 2, tid & 3);      // K^ set of the thread's first multiply item
+        if (tid < (B7<LOGM, LOGTC>::NBK >> 1) * B7<LOGM, LOGTC>::TC) kpre = b7_kload<T, IS3D, B7<LOGM, LOGTC>::TC>(Kt, tid >> LOGTC, tid & (B7<LOGM, LOGTC>::TC - 1));      // K^ set of the thread's first multiply item
         MM_SYNC();
     }
 }
 // inverse middle stages Lc = 2^LOGLC, ..., 2^LOGTOP
-template <int LOGM, int LOGLC, int LOGTOP, int NTHR, typename T>
+template <int LOGM, int LOGTC, int LOGLC, int LOGTOP, int NTHR, typename T>
 MM_HD void b7_inv_mids(cx<T>* s, twiddles<T> tw, int logtw, int tid, int nthr)
 {
     if constexpr (LOGLC <= LOGTOP) {
-        const tw8<T> t = b7_mid_tw<T>(tw, logtw, LOGLC, b7_mid_i<LOGM, T>(tid, LOGLC));
+        const tw8<T> t = b7_mid_tw<T>(tw, logtw, LOGLC, b7_mid_i<LOGTC>(tid, LOGLC));
         MM_SYNC();
-        b7_mid8<LOGM, LOGLC, 1, NTHR, T>(s, t, tw, logtw, tid, nthr);
-        b7_inv_mids<LOGM, LOGLC + 3, LOGTOP, NTHR, T>(s, tw, logtw, tid, nthr);
+        b7_mid8<LOGM, LOGTC, LOGLC, 1, NTHR, T>(s, t, tw, logtw, tid, nthr);
+        b7_inv_mids<LOGM, LOGTC, LOGLC + 3, LOGTOP, NTHR, T>(s, tw, logtw, tid, nthr);
     }
 }
 
 // One tile.  `tmap` = CUtensorMap of S as (x, j, zpos, comp); `bar` = three 8-byte shared-memory mbarriers.
-template <int LOGM, bool IS3D, int NTHR, typename T>
+template <int LOGM, int LOGTC, bool IS3D, int NTHR, typename T>
 MM_HD void y_conv_body7(const Geom g, cx<T>* __restrict__ S, const T* __restrict__ Kc, twiddles<T> tw, int logtw, cx<T>* s,
                         int bid, int tid, int nthr, const void* tmap, unsigned long long* bar, const int* done_flag)
 {
-    typedef B7<LOGM> P;
+    typedef B7<LOGM, LOGTC> P;
     constexpr int TC = P::TC, LOGTOP = LOGM - P::LOGR1;      // first middle stage: blocks of M / R1
     const int ntile = g.Lx / TC;
     const int x0 = (bid % ntile) * TC, zq = bid / ntile;
@@ -276,17 +277,17 @@ MM_HD void y_conv_body7(const Geom g, cx<T>* __restrict__ S, const T* __restrict
             for (int col = 0; col < TC; col++) s[c * P::CS + j * TC + col] = S[(long)c * g.comp + (long)zq * g.plane + (long)j * g.Lx + x0 + col];
 #endif
     // twiddles of the first stage while the tile is in flight
-    const twfl<T, P::R1> tf = b7_fl_tw<T, P::R1>(tw, logtw, LOGM + 1, (tid >> 2) & (P::SUB1 - 1));
+    const twfl<T, P::R1> tf = b7_fl_tw<T, P::R1>(tw, logtw, LOGM + 1, (tid >> LOGTC) & (P::SUB1 - 1));
     MM_SYNC();      // the barrier words are initialised before anyone polls them
-    b7_first<LOGM, NTHR, T>(s, tf, tw, logtw, tid, nthr, bar);
+    b7_first<LOGM, LOGTC, NTHR, T>(s, tf, tw, logtw, tid, nthr, bar);
     if (done) return;      // every thread that owns an item has seen all three loads land
     kset<T, IS3D ? 48 : 32> kpre;
-    b7_fwd_mids<LOGM, LOGTOP, IS3D, NTHR, T>(s, tw, logtw, Kt, tid, nthr, kpre);
-    b7_mul8<LOGM, IS3D, NTHR, T>(s, kpre, Kt, sz, tid, nthr);
-    b7_inv_mids<LOGM, 6, LOGTOP, NTHR, T>(s, tw, logtw, tid, nthr);
-    const twfl<T, P::R1> tl = b7_fl_tw<T, P::R1>(tw, logtw, LOGM + 1, (tid >> 2) & (P::SUB1 - 1));
+    b7_fwd_mids<LOGM, LOGTC, LOGTOP, IS3D, NTHR, T>(s, tw, logtw, Kt, tid, nthr, kpre);
+    b7_mul8<LOGM, LOGTC, IS3D, NTHR, T>(s, kpre, Kt, sz, tid, nthr);
+    b7_inv_mids<LOGM, LOGTC, 6, LOGTOP, NTHR, T>(s, tw, logtw, tid, nthr);
+    const twfl<T, P::R1> tl = b7_fl_tw<T, P::R1>(tw, logtw, LOGM + 1, (tid >> LOGTC) & (P::SUB1 - 1));
     MM_SYNC();
-    b7_last<LOGM, NTHR, T>(s, tl, tw, logtw, tid, nthr);
+    b7_last<LOGM, LOGTC, NTHR, T>(s, tl, tw, logtw, tid, nthr);
 #if defined(__CUDA_ARCH__)
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // the threads' tile writes before the async-proxy reads
     __syncthreads();

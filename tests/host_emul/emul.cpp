@@ -75,17 +75,14 @@ static void run(int ver, int nx, int ny, int nz, int G, int CH, int TC, const do
             CASE_A(1) CASE_A(2) CASE_A(4) CASE_A(8) CASE_A(16) CASE_A(32)
         }
     }
-    const bool b7 = ver == 7 && sizeof(T) == 4 && TC == 4 && ny >= 16 && ny <= 512;
+    const bool b7 = ver == 7 && TC == (sizeof(T) == 8 ? 2 : 4) && ny >= 16 && ny <= 512;
     unsigned long long* nobar = nullptr;
+    constexpr int LOGTC7 = sizeof(T) == 8 ? 1 : 2;
     for (int b = 0; b < gridB; b++) {
         if (b7) {
-            float* Kcf = reinterpret_cast<float*>(Kc.data());
-            cx<float>* Sf = reinterpret_cast<cx<float>*>(S.data());
-            cx<float>* sm = reinterpret_cast<cx<float>*>(smem.data());
-            twiddles<float> twf; twf.tw = reinterpret_cast<const cx<float>*>(tw.tw); twf.twN = twN;
             switch (g.logny * 2 + (nz > 1)) {
-#define CASE_B7(L) case 2 * L: y_conv_body7<L, false, 1, float>(g, Sf, Kcf, twf, ilog2(twN), sm, b, 0, 1, nullptr, nobar, nullptr); break; \
-                   case 2 * L + 1: y_conv_body7<L, true, 1, float>(g, Sf, Kcf, twf, ilog2(twN), sm, b, 0, 1, nullptr, nobar, nullptr); break;
+#define CASE_B7(L) case 2 * L: y_conv_body7<L, LOGTC7, false, 1, T>(g, S.data(), Kc.data(), tw, ilog2(twN), smem.data(), b, 0, 1, nullptr, nobar, nullptr); break; \
+                   case 2 * L + 1: y_conv_body7<L, LOGTC7, true, 1, T>(g, S.data(), Kc.data(), tw, ilog2(twN), smem.data(), b, 0, 1, nullptr, nobar, nullptr); break;
                 CASE_B7(4) CASE_B7(5) CASE_B7(6) CASE_B7(7) CASE_B7(8) CASE_B7(9)
             }
         } else if (b5) {

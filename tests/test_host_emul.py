@@ -99,9 +99,10 @@ def test_local_field_and_torque_match_oracle(emul, kind):
         assert np.abs(out.reshape(ref.shape) - ref).max() <= 1e-12 * np.abs(ref).max()
 
 
+@pytest.mark.parametrize("prec64", [0, 1])
 @pytest.mark.parametrize("shape", [(16, 16, 1), (8, 32, 2), (32, 64, 1), (8, 128, 2), (4, 256, 1), (4, 512, 1), (4, 512, 2), (16, 64, 4)])
-def test_specialised_pass_B_matches_oracle(emul, shape):
-    """mm_passB7.cuh (fp32, TC = 4, compile-time ny): every instantiated ny, films and 3-D."""
+def test_specialised_pass_B_matches_oracle(emul, shape, prec64):
+    """mm_passB7.cuh (compile-time ny; fp32 with TC = 4, fp64 with TC = 2): every instantiated ny, films and 3-D."""
     nx, ny, nz = shape
     cell = (2e-9, 1.5e-9, 3e-9)
     Ms = 8e5 * wl.random_mask(23, nx, ny, nz, 0.8)
@@ -113,6 +114,7 @@ def test_specialised_pass_B_matches_oracle(emul, shape):
     K = khat_full(o, nx, ny, nz)
     Hd = np.zeros(3 * nx * ny * nz)
     Msf = np.ascontiguousarray(Ms.reshape(-1))
-    emul.emul_demag(7, 0, nx, ny, nz, 1, 8, 4, K.ctypes.data_as(_dp), Msf.ctypes.data_as(_dp), m.ctypes.data_as(_dp), Hd.ctypes.data_as(_dp))
+    emul.emul_demag(7, prec64, nx, ny, nz, 1, 8, 2 if prec64 else 4, K.ctypes.data_as(_dp), Msf.ctypes.data_as(_dp), m.ctypes.data_as(_dp),
+                    Hd.ctypes.data_as(_dp))
     Hd = Hd.reshape(3, nz, ny, nx) * (Ms > 0)
-    assert np.abs(Hd - Href).max() / 8e5 < 2e-5
+    assert np.abs(Hd - Href).max() / 8e5 < (1e-12 if prec64 else 2e-5)
