@@ -21,7 +21,6 @@ namespace mm {
 
 template <int LOGM, int LOGTC> struct B7 {
     static constexpr int M = 1 << LOGM, N = 2 * M, TC = 1 << LOGTC;
-    static constexpr int LOGLCV = LOGTC - 1, LCV = TC / 2;      // column pairs (16 / 32-byte accesses of the middle stages)
     static constexpr int R1 = (LOGM % 3 == 0) ? 8 : ((LOGM % 3 == 2) ? 4 : 2);      // first_radix(M)
     static constexpr int LOGR1 = (LOGM % 3 == 0) ? 3 : (LOGM % 3);
     static constexpr int SUB1 = M / R1;                 // butterflies of the first / last stage per column
@@ -110,19 +109,22 @@ MM_HD void b7_last(cx<T>* s, const twfl<T, B7<LOGM, LOGTC>::R1>& pre, twiddles<T
     }
 }
 
-// middle radix-8 stage on blocks of length 2^LOGLC, two columns (16 bytes) per access
+// middle radix-8 stage on blocks of length 2^LOGLC, 16 bytes per shared-memory access (fp32: two columns, fp64: one —
+// the lanes of a warp then cover consecutive 16-byte words: conflict-free in both precisions)
+template <typename T> struct b7_v { static constexpr int LOGV = sizeof(T) == 8 ? 0 : 1, V = 1 << LOGV; };
 template <int LOGM, int LOGTC, int LOGLC, int DIR, int NTHR, typename T>
 MM_HD void b7_mid8(cx<T>* s, const tw8<T>& pre, twiddles<T> tw, int logtw, int tid, int nthr)
 {
     typedef B7<LOGM, LOGTC> P;
-    typedef cvec<T, 2> E;
+    constexpr int V = b7_v<T>::V, LOGLCV = LOGTC - b7_v<T>::LOGV, LCV = 1 << LOGLCV;
+    typedef cvec<T, V> E;
     constexpr int TC = P::TC, SUB = 1 << (LOGLC - 3), RS = SUB * TC;
     bool first = true;
-    for (int f = tid; f < (P::N >> 3) * P::LCV; f += NTHR, first = false) {
-        const int lc = f & (P::LCV - 1), b = f >> P::LOGLCV;
+    for (int f = tid; f < (P::N >> 3) * LCV; f += NTHR, first = false) {
+        const int lc = f & (LCV - 1), b = f >> LOGLCV;
         const int blk = b >> (LOGLC - 3), i = b & (SUB - 1);
         const tw8<T> t = first ? pre : b7_mid_tw<T>(tw, logtw, LOGLC, i);
-        cx<T>* base = s + ((blk << LOGLC) + i) * TC + lc * 2;
+        cx<T>* base = s + ((blk << LOGLC) + i) * TC + lc * V;
 #pragma unroll
         for (int c = 0; c < 3; c++) {
             cx<T>* p = base + c * P::CS;
@@ -143,7 +145,7 @@ MM_HD void b7_mid8(cx<T>* s, const tw8<T>& pre, twiddles<T> tw, int logtw, int t
         }
     }
 }
-template <int LOGTC> MM_HD int b7_mid_i(int f, int logLc) { return (f >> (LOGTC - 1)) & ((1 << (logLc - 3)) - 1); }
+template <int LOGTC, typename T> MM_HD int b7_mid_i(int f, int logLc) { return (f >> (LOGTC - b7_v<T>::LOGV)) & ((1 << (logLc - 3)) - 1); }
 
 template <typename T, int NJ> struct kset { T k[NJ]; };
 template <typename T, bool IS3D, int TC> MM_HD kset<T, IS3D ? 48 : 32> b7_kload(const T* Kt, int set, int col)
@@ -218,7 +220,7 @@ template <int LOGM, int LOGTC, int LOGLC, bool IS3D, int NTHR, typename T>
 MM_HD void b7_fwd_mids(cx<T>* s, twiddles<T> tw, int logtw, const T* Kt, int tid, int nthr, kset<T, IS3D ? 48 : 32>& kpre)
 {
     if constexpr (LOGLC > 3) {
-        const tw8<T> t = b7_mid_tw<T>(tw, logtw, LOGLC, b7_mid_i<LOGTC>(tid, LOGLC));
+        const tw8<T> t = b7_mid_tw<T>(tw, logtw, LOGLC, b7_mid_i<LOGTC, T>(tid, LOGLC));
         MM_SYNC();
         b7_mid8<LOGM, LOGTC, LOGLC, 0, NTHR, T>(s, t, tw, logtw, tid, nthr);
         b7_fwd_mids<LOGM, LOGTC, LOGLC - 3, IS3D, NTHR, T>(s, tw, logtw, Kt, tid, nthr, kpre);
@@ -232,7 +234,7 @@ template <int LOGM, int LOGTC, int LOGLC, int LOGTOP, int NTHR, typename T>
 MM_HD void b7_inv_mids(cx<T>* s, twiddles<T> tw, int logtw, int tid, int nthr)
 {
     if constexpr (LOGLC <= LOGTOP) {
-        const tw8<T> t = b7_mid_tw<T>(tw, logtw, LOGLC, b7_mid_i<LOGTC>(tid, LOGLC));
+        const tw8<T> t = b7_mid_tw<T>(tw, logtw, LOGLC, b7_mid_i<LOGTC, T>(tid, LOGLC));
         MM_SYNC();
         b7_mid8<LOGM, LOGTC, LOGLC, 1, NTHR, T>(s, t, tw, logtw, tid, nthr);
         b7_inv_mids<LOGM, LOGTC, LOGLC + 3, LOGTOP, NTHR, T>(s, tw, logtw, tid, nthr);
