@@ -442,6 +442,25 @@ template <typename T, int R> MM_HD void pad_twiddles(cx<T> w0, cx<T>* wp)
     }
 }
 
+// a * w_n^k for compile-time n <= 64 and k < n/2 (the pad / crop twiddles of the register z transform): the twiddle is
+// an immediate, not a table load.  w_64^j = cos(pi j / 32) - i sin(pi j / 32).
+template <typename T> MM_HD void w64(int j, T& c, T& s)
+{
+    const T C[32] = { (T)1.00000000000000000000, (T)0.99518472667219692873, (T)0.98078528040323043058, (T)0.95694033573220882438, (T)0.92387953251128673848, (T)0.88192126434835504956, (T)0.83146961230254523567, (T)0.77301045336273699338, (T)0.70710678118654757274, (T)0.63439328416364548779, (T)0.55557023301960228867, (T)0.47139673682599780857, (T)0.38268343236508983729, (T)0.29028467725446233105, (T)0.19509032201612833135, (T)0.09801714032956077016, (T)0.00000000000000006123, (T)-0.09801714032956064526, (T)-0.19509032201612819257, (T)-0.29028467725446216452, (T)-0.38268343236508972627, (T)-0.47139673682599769755, (T)-0.55557023301960195560, (T)-0.63439328416364537677, (T)-0.70710678118654746172, (T)-0.77301045336273699338, (T)-0.83146961230254534669, (T)-0.88192126434835493853, (T)-0.92387953251128673848, (T)-0.95694033573220882438, (T)-0.98078528040323043058, (T)-0.99518472667219681771 };
+    const T S[32] = { (T)0.00000000000000000000, (T)0.09801714032956060363, (T)0.19509032201612824808, (T)0.29028467725446233105, (T)0.38268343236508978178, (T)0.47139673682599764204, (T)0.55557023301960217765, (T)0.63439328416364548779, (T)0.70710678118654746172, (T)0.77301045336273699338, (T)0.83146961230254523567, (T)0.88192126434835493853, (T)0.92387953251128673848, (T)0.95694033573220893540, (T)0.98078528040323043058, (T)0.99518472667219681771, (T)1.00000000000000000000, (T)0.99518472667219692873, (T)0.98078528040323043058, (T)0.95694033573220893540, (T)0.92387953251128673848, (T)0.88192126434835504956, (T)0.83146961230254545772, (T)0.77301045336273710440, (T)0.70710678118654757274, (T)0.63439328416364548779, (T)0.55557023301960217765, (T)0.47139673682599786408, (T)0.38268343236508989280, (T)0.29028467725446238656, (T)0.19509032201612860891, (T)0.09801714032956082567 };
+    c = C[j]; s = S[j];
+}
+template <typename T, int N> MM_HD cx<T> rot_w(cx<T> a, int k)      // a * w_N^k
+{
+    T c, s; w64<T>(k * (64 / N), c, s);
+    return crot(a, c, -s);
+}
+template <typename T, int N> MM_HD cx<T> rot_wc(cx<T> a, int k)     // a * conj(w_N^k)
+{
+    T c, s; w64<T>(k * (64 / N), c, s);
+    return crot(a, c, s);
+}
+
 // first radix of the v2 schedule for block length m >= 16: remainder first, then 8s
 MM_HD int first_radix(int m) { int r = m; while (r > 8) r >>= 3; return r; }
 

@@ -501,7 +501,7 @@ MM_HD void zC_regs(const Geom& g, const cx<T>* Sc, cx<T>* s, int pitch, int j0, 
         rad<cx<T>, NZ>::inv(u);
         dst[0] = a[0] + u[0];
 #pragma unroll
-        for (int z = 1; z < NZ; z++) dst[z] = a[z] + cmulc(u[z], tw.get(z, 2 * NZ));
+        for (int z = 1; z < NZ; z++) dst[z] = a[z] + rot_wc<T, 2 * NZ>(u[z], z);      // conj(w_2NZ^z), an immediate
     }
 }
 

@@ -76,7 +76,7 @@ MM_HD void zfft_store(const Geom& g, cx<T>* dst, cx<T>* a, twiddles<T> tw)
         for (int z = 0; z < NZ; z++) dst[(long)z * g.plane] = v[z];
     }
 #pragma unroll
-    for (int z = 1; z < NZ; z++) a[z] = cmul(a[z], tw.get(z, 2 * NZ));
+    for (int z = 1; z < NZ; z++) a[z] = rot_w<T, 2 * NZ>(a[z], z);      // * w_2NZ^z, an immediate
     rad<cx<T>, NZ>::fwd(a);
 #pragma unroll
     for (int z = 0; z < NZ; z++) dst[(long)(NZ + z) * g.plane] = a[z];
