@@ -44,6 +44,10 @@ def lib():
         L.mo_step.argtypes = [C.c_void_p, _dp, C.c_double, C.c_double, C.POINTER(C.c_int), _dp, _dp, _dp]
         L.mo_relax.argtypes = [C.c_void_p, _dp, C.c_double, C.c_double, C.c_long, C.c_double,
                                C.POINTER(C.c_long), _dp]
+        L.mo_minimize.argtypes = [C.c_void_p, _dp, C.c_double, C.c_double, C.c_double, C.c_double, C.c_long,
+                                  C.POINTER(C.c_long), _dp, _dp]
+        L.mo_sd_update.argtypes = [C.c_void_p, _dp, _dp, C.c_double]
+        L.mo_sd_update.restype = None
         L.mo_energy.argtypes = [C.c_void_p, _dp, _dp, _dp]
         L.mo_average_m.argtypes = [C.c_void_p, _dp, _dp]
         L.mo_get_demag_kernel.argtypes = [C.c_void_p, C.c_int, _dp]
@@ -153,6 +157,21 @@ class Oracle:
         md = np.zeros(1)
         _chk(self.L.mo_relax(self.h, _p(m.reshape(-1)), tol, stop_dmdt, max_steps, dt0, C.byref(n), _p(md)), "relax")
         return n.value, float(md[0])
+
+    def minimize(self, m, tau0, tau_min, tau_max, stop_torque, max_steps):
+        """Steepest descent with Barzilai-Borwein steps, in place.
+        Returns (updates done, max|m x (m x H)| at the last evaluation, last tau)."""
+        assert m.dtype == np.float64 and m.flags["C_CONTIGUOUS"] and m.size == 3 * self.N
+        n = C.c_long()
+        mg, tl = np.zeros(1), np.zeros(1)
+        _chk(self.L.mo_minimize(self.h, _p(m.reshape(-1)), tau0, tau_min, tau_max, stop_torque, max_steps, C.byref(n), _p(mg), _p(tl)),
+             "minimize")
+        return n.value, float(mg[0]), float(tl[0])
+
+    def sd_update(self, m, H, tau):
+        """One update of Eq. 51 with the given tau, in place on m."""
+        assert m.dtype == np.float64 and m.flags["C_CONTIGUOUS"] and m.size == 3 * self.N
+        self.L.mo_sd_update(self.h, _p(m.reshape(-1)), _p(np.ascontiguousarray(H, dtype=np.float64).reshape(-1)), tau)
 
     def energy(self, m):
         a = self._m(m)

@@ -22,6 +22,7 @@
  *   LL right-hand side Eq. 37
  *   RK4 + projection  PAPER.md:425; Dormand-Prince + projection PAPER.md:298, ref [37]
  *   energy            Eq. 1, 2, 6/7, 10, 12 summed per cell
+ *   mo_minimize       steepest descent with Barzilai-Borwein steps, Eq. 50-52
  *
  * Layout: x fastest, idx = i + nx*(j + ny*k); vector fields are SoA, v[c*N + idx].
  * A neighbour is absent when outside the mesh or when its Ms is 0 (R4);
@@ -579,6 +580,85 @@ int mo_relax(mo_sim *s, double *m, double tol, double stop_dmdt, long max_steps,
     if (steps_done) *steps_done = it;
     if (max_dmdt_out) *max_dmdt_out = md;
     return 0;
+}
+
+/* ------------------------------------------------------------------------------------
+ * Steepest-descent energy minimisation with Barzilai-Borwein steps, PAPER.md:376-393 (§VI).
+ *   f_k = m_k x H_eff(m_k),  g_k = m_k x (m_k x H_eff(m_k))            (text under Eq. 51)
+ *   (1 + tau^2 f_k^2 / 4) m_{k+1} = (1 - tau^2 f_k^2 / 4) m_k - tau g_k      (Eq. 51, per cell)
+ *   s_{k-1} = m_k - m_{k-1},  y_{k-1} = g_k - g_{k-1}
+ *   tau^1 = sum_i s.s / sum_i s.y ,  tau^2 = sum_i s.y / sum_i y.y           (Eq. 52, sums over cells)
+ * Readings where the paper is silent (R16): the first step uses the caller's tau0; afterwards
+ * tau^1 on odd k and tau^2 on even k (the alternation of ref [44]); |tau| is used, clamped to
+ * [tau_min, tau_max]; a vanishing or non-finite quotient falls back to tau0; iteration stops BEFORE the
+ * update when max_i |g_k,i| < stop_torque (A/m) or after max_steps updates.  Cells with Ms = 0 are
+ * left untouched and do not enter the sums.  No projection: Eq. 50 preserves |m| by itself.
+ * mo_sd_update is the single update of Eq. 51 with a given tau (exposed for the pins). */
+void mo_sd_update(const mo_sim *s, double *m, const double *H, double tau)
+{
+    const long N = s->N;
+    for (long q = 0; q < N; q++) {
+        if (s->Ms[q] == 0.0) continue;
+        const double mx = m[q], my = m[N + q], mz = m[2 * N + q];
+        const double hx = H[q], hy = H[N + q], hz = H[2 * N + q];
+        const double fx = my * hz - mz * hy, fy = mz * hx - mx * hz, fz = mx * hy - my * hx;       /* f = m x H */
+        const double gx = my * fz - mz * fy, gy = mz * fx - mx * fz, gz = mx * fy - my * fx;       /* g = m x f */
+        const double a = 0.25 * tau * tau * (fx * fx + fy * fy + fz * fz);
+        m[q] = ((1.0 - a) * mx - tau * gx) / (1.0 + a);
+        m[N + q] = ((1.0 - a) * my - tau * gy) / (1.0 + a);
+        m[2 * N + q] = ((1.0 - a) * mz - tau * gz) / (1.0 + a);
+    }
+}
+
+int mo_minimize(mo_sim *s, double *m, double tau0, double tau_min, double tau_max, double stop_torque, long max_steps,
+                long *steps_done, double *max_torque_out, double *tau_last)
+{
+    const long N = s->N;
+    double *H = (double *)malloc(sizeof(double) * 3 * N), *g = (double *)malloc(sizeof(double) * 3 * N);
+    double *gp = (double *)malloc(sizeof(double) * 3 * N), *mp = (double *)malloc(sizeof(double) * 3 * N);
+    double tau = tau0, maxg = INFINITY;
+    long k = 0;
+    int rc = 0;
+    for (;; k++) {
+        if ((rc = mo_effective_field(s, m, H))) break;
+        maxg = 0.0;
+        for (long q = 0; q < N; q++) {
+            double gx = 0, gy = 0, gz = 0;
+            if (s->Ms[q] != 0.0) {
+                const double mx = m[q], my = m[N + q], mz = m[2 * N + q];
+                const double hx = H[q], hy = H[N + q], hz = H[2 * N + q];
+                const double fx = my * hz - mz * hy, fy = mz * hx - mx * hz, fz = mx * hy - my * hx;
+                gx = my * fz - mz * fy; gy = mz * fx - mx * fz; gz = mx * fy - my * fx;
+                const double n = sqrt(gx * gx + gy * gy + gz * gz);
+                if (!(n <= maxg)) maxg = n;      /* keeps a NaN */
+            }
+            g[q] = gx; g[N + q] = gy; g[2 * N + q] = gz;
+        }
+        if (!(maxg == maxg)) { rc = -6; break; }
+        if (maxg < stop_torque || k >= max_steps) break;
+        if (k > 0) {                              /* Eq. 52 */
+            double ss = 0, sy = 0, yy = 0;
+            for (long q = 0; q < N; q++) {
+                if (s->Ms[q] == 0.0) continue;
+                for (int c = 0; c < 3; c++) {
+                    const double sv = m[c * N + q] - mp[c * N + q], yv = g[c * N + q] - gp[c * N + q];
+                    ss += sv * sv; sy += sv * yv; yy += yv * yv;
+                }
+            }
+            double t = (k & 1) ? ss / sy : sy / yy;
+            t = fabs(t);
+            if (!(t > 0.0) || isinf(t)) t = tau0;
+            tau = t < tau_min ? tau_min : (t > tau_max ? tau_max : t);
+        }
+        memcpy(mp, m, sizeof(double) * 3 * N);
+        memcpy(gp, g, sizeof(double) * 3 * N);
+        mo_sd_update(s, m, H, tau);               /* Eq. 51 */
+    }
+    if (steps_done) *steps_done = k;
+    if (max_torque_out) *max_torque_out = maxg;
+    if (tau_last) *tau_last = tau;
+    free(H); free(g); free(gp); free(mp);
+    return rc;
 }
 
 /* E = - mu0 sum_i V Ms_i m_i . (1/2 H_d + 1/2 H_ex + 1/2 H_dmi + 1/2 H_an + H_ext)_i
