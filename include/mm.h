@@ -112,6 +112,17 @@ int mm_step(mm_sim* sim, void* dev_m, double dt, double tol,
 int mm_relax(mm_sim* sim, void* dev_m, double tol, double stop_dmdt, long max_steps, double dt0,
              long* steps_done, double* max_dmdt);
 
+/* Energy minimisation by steepest descent with Barzilai-Borwein steps (§VI).  Per iteration k:
+ * f_k = m x H_eff(m_k), g_k = m x (m x H_eff(m_k)); the modulus-preserving update of Eq. 51,
+ * (1 + tau^2 f_k^2/4) m_{k+1} = (1 - tau^2 f_k^2/4) m_k - tau g_k, per cell; step size by Eq. 52 with
+ * s = m_k - m_{k-1}, y = g_k - g_{k-1}: tau^1 = sum s.s / sum s.y on odd k, tau^2 = sum s.y / sum y.y on even k
+ * (sums over cells with Ms > 0, fp64, fixed order).  Readings where the paper is silent (R16): tau0 (m/A)
+ * for the first update, |tau| clamped to [tau_min, tau_max], a vanishing / non-finite quotient falls back to tau0.
+ * Stops before the update when max_i |g_k,i| < stop_torque (A/m) or after max_steps updates.  dev_m (3N reals) is
+ * updated in place; no projection is applied (Eq. 50 keeps |m|).  Out-pointers may be NULL.  Synchronous. */
+int mm_minimize(mm_sim* sim, void* dev_m, double tau0, double tau_min, double tau_max, double stop_torque, long max_steps,
+                long* steps_done, double* max_torque, double* tau_last);
+
 /* Advance by adaptive DOPRI5 steps until exactly t_end (last step clipped). */
 int mm_run_until(mm_sim* sim, void* dev_m, double t_end, double tol, double dt0, long max_steps,
                  long* steps_done);

@@ -39,6 +39,7 @@ SIGNATURES = {
     "mm_step": (_i, [_vp, _vp, _d, _d, _ip, _dp, _dp, _dp]),
     "mm_relax": (_i, [_vp, _vp, _d, _d, _l, _d, _lp, _dp]),
     "mm_run_until": (_i, [_vp, _vp, _d, _d, _d, _l, _lp]),
+    "mm_minimize": (_i, [_vp, _vp, _d, _d, _d, _d, _l, _lp, _dp, _dp]),
     "mm_run_host": (_i, [_vp, _vp, _i, _d, _d]),
     "mm_llg_rhs_host": (_i, [_vp, _vp, _vp]),
     "mm_time": (_d, [_vp]),
@@ -172,6 +173,15 @@ class Sim:
         n = C.c_long()
         self._chk(self.L.mm_run_until(self.h, self._dev(m, 3 * self.N), t_end, tol, dt0, max_steps, C.byref(n)), "mm_run_until")
         return n.value
+
+    def minimize(self, m, tau0, tau_min, tau_max, stop_torque, max_steps):
+        """Steepest descent with Barzilai-Borwein steps (mm_minimize), in place on m.
+        Returns (updates done, max|m x (m x H)| at the last evaluation, last tau)."""
+        n = C.c_long()
+        mg, tl = C.c_double(), C.c_double()
+        self._chk(self.L.mm_minimize(self.h, self._dev(m, 3 * self.N), tau0, tau_min, tau_max, stop_torque, max_steps,
+                                     C.byref(n), C.byref(mg), C.byref(tl)), "mm_minimize")
+        return n.value, mg.value, tl.value
 
     def run_host(self, host_m, nsteps, dt, tol=0.0):
         """host_m: pinned (or pageable) CPU tensor [3,nz,ny,nx] of the sim dtype, updated in place."""

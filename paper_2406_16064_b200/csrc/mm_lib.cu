@@ -458,6 +458,114 @@ __global__ void __launch_bounds__(256) dot_kernel(long N, const T* __restrict__ 
     if (threadIdx.x == 0) for (int c = 0; c < 4; c++) out[4 * blockIdx.x + c] = red[c][0];
 }
 
+// ------------------------------------------------------------------------------------------------
+// Steepest-descent minimiser with Barzilai-Borwein steps (Eq. 50-52; R16)
+// ------------------------------------------------------------------------------------------------
+struct MinState {
+    double tau, tau0, tau_min, tau_max, stop, maxg;
+    unsigned long long maxg_bits;
+    long long iter, max_steps;      // updates done so far / allowed
+    int done, nan;
+};
+
+// g_k = m x (m x H_eff(m_k)) and f_k^2 per cell (text under Eq. 51); partial sums of Eq. 52 per block in fp64,
+// combined in a fixed order (deterministic); max |g_k| by the bit-pattern maximum.
+template <typename T>
+__global__ void __launch_bounds__(256) sd_field_kernel(Geom g, LocalP<T> lp, const T* __restrict__ m, const T* __restrict__ Ms, const T* __restrict__ Hd,
+                                                       T* __restrict__ gcur, const T* __restrict__ gprev, const T* __restrict__ sprev, T* __restrict__ f2,
+                                                       double* __restrict__ part, MinState* ms)
+{
+    if (ms->done) return;
+    const long N = g.N;
+    const long q = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    double ss = 0, sy = 0, yy = 0;
+    T gn = 0;
+    if (q < N) {
+        const T Msi = Ms[q];
+        v3<T> gk = { 0, 0, 0 };
+        T ff = 0;
+        if (Msi != (T)0) {
+            const int i = (int)(q & (g.nx - 1)), j = (int)((q >> g.lognx) & (g.ny - 1)), k = (int)(q >> (g.lognx + g.logny));
+            const v3<T> mi = ld3(m, N, q);
+            v3<T> H = { 0, 0, 0 };
+            if (Hd != nullptr) H = ld3(Hd, N, q);
+            H = local_field<T>(g, lp, m, Ms, i, j, k, q, Msi, mi, H);
+            const T fx = mi.y * H.z - mi.z * H.y, fy = mi.z * H.x - mi.x * H.z, fz = mi.x * H.y - mi.y * H.x;       // f = m x H
+            gk.x = mi.y * fz - mi.z * fy; gk.y = mi.z * fx - mi.x * fz; gk.z = mi.x * fy - mi.y * fx;               // g = m x f
+            ff = fx * fx + fy * fy + fz * fz;
+            gn = sqrt(gk.x * gk.x + gk.y * gk.y + gk.z * gk.z);
+            if (ms->iter > 0) {
+                const v3<T> sv = ld3(sprev, N, q), gp = ld3(gprev, N, q);
+                const double yx = (double)(gk.x - gp.x), yyv = (double)(gk.y - gp.y), yz = (double)(gk.z - gp.z);
+                ss = (double)sv.x * sv.x + (double)sv.y * sv.y + (double)sv.z * sv.z;
+                sy = (double)sv.x * yx + (double)sv.y * yyv + (double)sv.z * yz;
+                yy = yx * yx + yyv * yyv + yz * yz;
+            }
+        }
+        gcur[q] = gk.x; gcur[N + q] = gk.y; gcur[2 * N + q] = gk.z;
+        f2[q] = ff;
+    }
+    __shared__ double red[3][256];
+    red[0][threadIdx.x] = ss; red[1][threadIdx.x] = sy; red[2][threadIdx.x] = yy;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) for (int c = 0; c < 3; c++) red[c][threadIdx.x] += red[c][threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) for (int c = 0; c < 3; c++) part[3 * (long)blockIdx.x + c] = red[c][0];
+    block_max_bits(norm_bits(gn), &ms->maxg_bits);
+}
+
+// One block: sums the per-block partials in a fixed order, takes the stop decision and the next tau (Eq. 52).
+__global__ void __launch_bounds__(256) sd_ctrl_kernel(const double* __restrict__ part, long nblk, int is_f64, MinState* ms)
+{
+    if (ms->done) return;
+    __shared__ double red[3][256];
+    double v[3] = { 0, 0, 0 };
+    for (long b = threadIdx.x; b < nblk; b += 256) for (int c = 0; c < 3; c++) v[c] += part[3 * b + c];
+    for (int c = 0; c < 3; c++) red[c][threadIdx.x] = v[c];
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) for (int c = 0; c < 3; c++) red[c][threadIdx.x] += red[c][threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x != 0) return;
+    const double maxg = is_f64 ? __longlong_as_double((long long)ms->maxg_bits) : (double)__uint_as_float((unsigned)ms->maxg_bits);
+    ms->maxg_bits = 0ull;
+    ms->maxg = maxg;
+    if (!(maxg == maxg)) { ms->nan = 1; ms->done = 1; return; }
+    if (maxg < ms->stop || ms->iter >= ms->max_steps) { ms->done = 1; return; }
+    if (ms->iter > 0) {
+        const double ss = red[0][0], sy = red[1][0], yy = red[2][0];
+        double t = (ms->iter & 1) ? ss / sy : sy / yy;
+        t = fabs(t);
+        if (!(t > 0.0) || isinf(t)) t = ms->tau0;
+        ms->tau = t < ms->tau_min ? ms->tau_min : (t > ms->tau_max ? ms->tau_max : t);
+    }
+}
+
+// Eq. 51, per cell; keeps s_k = m_{k+1} - m_k for the next Eq. 52.
+template <typename T>
+__global__ void __launch_bounds__(256) sd_update_kernel(long N, T* __restrict__ m, const T* __restrict__ gcur, const T* __restrict__ f2, const T* __restrict__ Ms,
+                                                        T* __restrict__ sprev, MinState* ms)
+{
+    if (ms->done) return;
+    const long q = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    const T tau = (T)ms->tau;
+    if (q < N && Ms[q] != (T)0) {
+        const T a = (T)0.25 * tau * tau * f2[q];
+#pragma unroll
+        for (int c = 0; c < 3; c++) {
+            const T mo = m[c * N + q];
+            const T mn = (((T)1 - a) * mo - tau * gcur[c * N + q]) / ((T)1 + a);
+            m[c * N + q] = mn;
+            sprev[c * N + q] = mn - mo;
+        }
+    }
+}
+// separate launch: every block of sd_update_kernel must have read ms->iter-independent state before it moves on
+__global__ void sd_count_kernel(MinState* ms) { if (!ms->done) ms->iter++; }
+
 template <typename T> __global__ void fill_kernel(long n, T* p, T v)
 {
     const long q = (long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -595,7 +703,7 @@ struct mm_sim {
     // workspace
     void* ws;
     size_t ws_bytes, ws_need;
-    size_t off_Ms, off_nbm, off_S, off_Kh, off_Kc, off_mh, off_Hd, off_k[7], off_y[2], off_tw, off_st, off_part;
+    size_t off_Ms, off_nbm, off_S, off_Kh, off_Kc, off_mh, off_Hd, off_k[7], off_y[2], off_tw, off_st, off_part, off_min;
     int twN;
     size_t smemA, smemA2, smemB;
     int thrA, thrB;
@@ -728,7 +836,8 @@ static void layout(mm_sim* s)
     for (int i = 0; i < 2; i++) s->off_y[i] = take(3 * N * es);
     s->off_mh = take(3 * N * es);      // staging slot of the host-buffer entry points
     s->off_tw = take((size_t)(s->twN / 2 + 1) * 2 * es);
-    s->off_part = take(4 * 1024 * sizeof(double));
+    s->off_part = take(3 * (size_t)((N + 255) / 256) * sizeof(double) > 4 * 1024 * sizeof(double) ? 3 * (size_t)((N + 255) / 256) * sizeof(double) : 4 * 1024 * sizeof(double));
+    s->off_min = take(sizeof(MinState));
     s->ws_need = o;
 }
 
@@ -1411,6 +1520,63 @@ extern "C" int mm_set_time(mm_sim* s, double t)
     MM_TRY(s, cudaStreamSynchronize(s->stream));
     s->t_host = t;
     return MM_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// mm_minimize: steepest descent with Barzilai-Borwein steps.  Per iteration: demag passes,
+// sd_field (field, g_k, Eq. 52 partial sums), sd_ctrl (stop decision, tau_k), sd_update (Eq. 51).  The controller
+// lives on the device; the host reads it back every 16 iterations.
+// ------------------------------------------------------------------------------------------------
+template <typename T> static int minimize_t(mm_sim* s, T* m, double tau0, double tau_min, double tau_max, double stop, long max_steps,
+                                            long* steps_done, double* max_torque, double* tau_last)
+{
+    const long N = s->g.N;
+    MinState h;
+    memset(&h, 0, sizeof(h));
+    h.tau = tau0; h.tau0 = tau0; h.tau_min = tau_min; h.tau_max = tau_max; h.stop = stop; h.max_steps = max_steps;
+    MinState* ms = wsp<MinState>(s, s->off_min);
+    MM_TRY(s, cudaMemcpyAsync(ms, &h, sizeof(h), cudaMemcpyHostToDevice, s->stream));
+    int rc = set_state(s, 0, 0, 0, 0, 0, 1);      // the demag passes look at the step controller's `done`: cleared
+    if (rc) return rc;
+    T* G[2] = { wsp<T>(s, s->off_k[0]), wsp<T>(s, s->off_k[1]) };
+    T* sprev = wsp<T>(s, s->off_k[2]);
+    T* f2 = wsp<T>(s, s->off_k[3]);
+    double* part = wsp<double>(s, s->off_part);
+    const bool demag = s->demag_on != 0;
+    if (demag && !s->demag_ready) return fail(s, MM_ERR_STATE, "demag enabled but mm_init_demag not called");
+    const LocalP<T> lp = make_local<T>(s, 31);
+    const unsigned nblk = (unsigned)((N + 255) / 256);
+    long issued = 0;
+    while (issued <= max_steps) {
+        const long batch = (max_steps + 1 - issued) < 16 ? (max_steps + 1 - issued) : 16;
+        for (long i = 0; i < batch; i++, issued++) {
+            if (demag && (rc = demag_passes<T>(s, m))) return rc;
+            sd_field_kernel<T><<<nblk, 256, 0, s->stream>>>(s->g, lp, m, wsp<T>(s, s->off_Ms), demag ? wsp<T>(s, s->off_Hd) : (const T*)nullptr,
+                                                            G[issued & 1], G[(issued + 1) & 1], sprev, f2, part, ms);
+            sd_ctrl_kernel<<<1, 256, 0, s->stream>>>(part, (long)nblk, s->prec == MM_F64, ms);
+            sd_update_kernel<T><<<nblk, 256, 0, s->stream>>>(N, m, G[issued & 1], f2, wsp<T>(s, s->off_Ms), sprev, ms);
+            sd_count_kernel<<<1, 1, 0, s->stream>>>(ms);
+            s->launches += 4;
+            MM_TRY(s, cudaGetLastError());
+        }
+        MM_TRY(s, cudaMemcpyAsync(&h, ms, sizeof(h), cudaMemcpyDeviceToHost, s->stream));
+        MM_TRY(s, cudaStreamSynchronize(s->stream));
+        if (h.done) break;
+    }
+    if (steps_done) *steps_done = (long)h.iter;
+    if (max_torque) *max_torque = h.maxg;
+    if (tau_last) *tau_last = h.tau;
+    if (h.nan) return fail(s, MM_ERR_NAN, "non-finite torque in mm_minimize");
+    return MM_OK;
+}
+
+extern "C" int mm_minimize(mm_sim* s, void* dev_m, double tau0, double tau_min, double tau_max, double stop_torque, long max_steps,
+                           long* steps_done, double* max_torque, double* tau_last)
+{
+    NEED_READY(s);
+    if (!dev_m || !(tau0 > 0) || !(tau_min > 0) || !(tau_max >= tau_min) || max_steps < 0) return MM_ERR_ARG;
+    return s->prec == MM_F64 ? minimize_t<double>(s, (double*)dev_m, tau0, tau_min, tau_max, stop_torque, max_steps, steps_done, max_torque, tau_last)
+                             : minimize_t<float>(s, (float*)dev_m, tau0, tau_min, tau_max, stop_torque, max_steps, steps_done, max_torque, tau_last);
 }
 
 // ------------------------------------------------------------------------------------------------
