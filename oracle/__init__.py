@@ -11,10 +11,10 @@ from .build import build as _build
 
 _lib = None
 
-DMI_NONE, DMI_BULK, DMI_INTERFACIAL = 0, 1, 2
+DMI_NONE, DMI_BULK, DMI_INTERFACIAL, DMI_D2D = 0, 1, 2, 3
 RK4, DOPRI5 = 0, 1
 DEMAG_OFF, DEMAG_FFT, DEMAG_DIRECT = 0, 1, 2
-TERM_EXCHANGE, TERM_DMI, TERM_ANIS, TERM_ZEEMAN, TERM_DEMAG = 1, 2, 4, 8, 16
+TERM_EXCHANGE, TERM_DMI, TERM_ANIS, TERM_ZEEMAN, TERM_DEMAG, TERM_CUBIC = 1, 2, 4, 8, 16, 32
 
 _dp = C.POINTER(C.c_double)
 
@@ -26,7 +26,7 @@ def lib():
         L.mo_time.restype = C.c_double
         L.mo_khat_imag_ratio.restype = C.c_double
         L.mo_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double]
-        for name in ("mo_set_Ms_uniform", "mo_set_A", "mo_set_Ku", "mo_set_alpha", "mo_set_gamma", "mo_set_time"):
+        for name in ("mo_set_Ms_uniform", "mo_set_A", "mo_set_Ku", "mo_set_Kc", "mo_set_alpha", "mo_set_gamma", "mo_set_time"):
             getattr(L, name).argtypes = [C.c_void_p, C.c_double]
         L.mo_set_D.argtypes = [C.c_void_p, C.c_double, C.c_int]
         L.mo_set_axis.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double]
@@ -34,6 +34,9 @@ def lib():
         L.mo_set_integrator.argtypes = [C.c_void_p, C.c_int]
         L.mo_set_demag.argtypes = [C.c_void_p, C.c_int]
         L.mo_set_Ms.argtypes = [C.c_void_p, _dp]
+        L.mo_set_A_cell.argtypes = [C.c_void_p, _dp]
+        L.mo_set_D_cell.argtypes = [C.c_void_p, _dp, C.c_int]
+        L.mo_set_H_ext_cell.argtypes = [C.c_void_p, _dp]
         L.mo_init_demag.argtypes = [C.c_void_p]
         L.mo_destroy.argtypes = [C.c_void_p]
         L.mo_time.argtypes = [C.c_void_p]
@@ -109,6 +112,18 @@ class Oracle:
     def set_A(self, A): _chk(self.L.mo_set_A(self.h, A), "set_A")
     def set_D(self, D, kind): _chk(self.L.mo_set_D(self.h, D, kind), "set_D")
     def set_Ku(self, Ku): _chk(self.L.mo_set_Ku(self.h, Ku), "set_Ku")
+    def set_Kc(self, Kc): _chk(self.L.mo_set_Kc(self.h, Kc), "set_Kc")
+
+    def _cell(self, a, n):
+        if a is None:
+            return None
+        a = np.ascontiguousarray(a, dtype=np.float64).reshape(-1)
+        assert a.size == n
+        return _p(a)
+
+    def set_A_cell(self, A): _chk(self.L.mo_set_A_cell(self.h, self._cell(A, self.N)), "set_A_cell")
+    def set_D_cell(self, D, kind): _chk(self.L.mo_set_D_cell(self.h, self._cell(D, self.N), kind), "set_D_cell")
+    def set_H_ext_cell(self, H): _chk(self.L.mo_set_H_ext_cell(self.h, self._cell(H, 3 * self.N)), "set_H_ext_cell")
     def set_axis(self, ux, uy, uz): _chk(self.L.mo_set_axis(self.h, ux, uy, uz), "set_axis")
     def set_H_ext(self, hx, hy, hz): _chk(self.L.mo_set_H_ext(self.h, hx, hy, hz), "set_H_ext")
     def set_alpha(self, a): _chk(self.L.mo_set_alpha(self.h, a), "set_alpha")

@@ -17,7 +17,8 @@
  *   mo_demag_fft      the same sum as a zero-padded FFT convolution, 3 forward + 3
  *                     inverse transforms
  *   exchange          Eq. 5  PAPER.md:122       DMI  Eq. 15
- *   anisotropy        Eq. 32 PAPER.md:269 in its continuum reading (R6)
+ *   anisotropy        Eq. 32 PAPER.md:269 in its continuum reading (R6); cubic Eq. 33
+ *   cell-based A, D   A_ij = 2 A_i A_j/(A_i + A_j) PAPER.md:120; D_ij likewise, D2d e_ij table
  *   Zeeman            Eq. 35
  *   LL right-hand side Eq. 37
  *   RK4 + projection  PAPER.md:425; Dormand-Prince + projection PAPER.md:298, ref [37]
@@ -48,7 +49,10 @@ typedef struct mo_sim {
     long N;
     double *Ms;                 /* N */
     double A, D, Ku, ux, uy, uz, hx, hy, hz, alpha, gamma;
-    int dmi_kind;               /* 0 none, 1 bulk, 2 interfacial */
+    double Kc;                  /* cubic anisotropy constant (Eq. 33), crystal axes = mesh axes */
+    double *Acell, *Dcell;      /* optional per-cell A_i, D_i (N each) or NULL: PAPER.md:120, 175 */
+    double *Hcell;              /* optional per-cell external field (3N, SoA) or NULL: Eq. 35 with H_z,i */
+    int dmi_kind;               /* 0 none, 1 bulk, 2 interfacial, 3 D2d */
     int integrator;             /* 0 RK4, 1 DOPRI5 */
     int demag;                  /* 0 off, 1 FFT path, 2 direct O(N^2) sum */
     double *Nten;               /* 6 * N: xx,yy,zz,xy,xz,yz at offsets i>=0,j>=0,k>=0 */
@@ -370,7 +374,7 @@ static void demag_fft(mo_sim *s, const double *m, double *H)
 }
 
 /* ------------------------------------------------------------------------------------
- * Local terms.  which: bit0 exchange, bit1 DMI, bit2 anisotropy, bit3 Zeeman.  Adds to H.
+ * Local terms.  which: bit0 exchange, bit1 DMI, bit2 uniaxial anisotropy, bit3 Zeeman, bit5 cubic anisotropy.  Adds to H.
  * ---------------------------------------------------------------------------------- */
 static void local_field_add(const mo_sim *s, const double *m, double *H, int which)
 {
@@ -380,9 +384,10 @@ static void local_field_add(const mo_sim *s, const double *m, double *H, int whi
     const double ux = un > 0 ? s->ux / un : 0, uy = un > 0 ? s->uy / un : 0, uz = un > 0 ? s->uz / un : 0;
     /* neighbour order: -x, +x, -y, +y, -z, +z */
     static const int off[6][3] = { { -1, 0, 0 }, { 1, 0, 0 }, { 0, -1, 0 }, { 0, 1, 0 }, { 0, 0, -1 }, { 0, 0, 1 } };
-    /* DMI vectors e_ij: bulk r^_ij; interfacial e_z x r^_ij */
+    /* DMI vectors e_ij: bulk r^_ij; interfacial e_z x r^_ij; D2d {e_x,-e_x,-e_y,e_y,0,0} */
     static const double e_bulk[6][3] = { { -1, 0, 0 }, { 1, 0, 0 }, { 0, -1, 0 }, { 0, 1, 0 }, { 0, 0, -1 }, { 0, 0, 1 } };
     static const double e_int[6][3] = { { 0, -1, 0 }, { 0, 1, 0 }, { 1, 0, 0 }, { -1, 0, 0 }, { 0, 0, 0 }, { 0, 0, 0 } };
+    static const double e_d2d[6][3] = { { 1, 0, 0 }, { -1, 0, 0 }, { 0, -1, 0 }, { 0, 1, 0 }, { 0, 0, 0 }, { 0, 0, 0 } };
     const double delta[6] = { s->dx, s->dx, s->dy, s->dy, s->dz, s->dz };
 #pragma omp parallel for collapse(2) schedule(static)
     for (int k = 0; k < nz; k++)
@@ -399,13 +404,23 @@ static void local_field_add(const mo_sim *s, const double *m, double *H, int whi
                     long p = a + (long)nx * (b + (long)ny * c);
                     if (s->Ms[p] == 0.0) continue;
                     double nxm = m[p], nym = m[N + p], nzm = m[2 * N + p];
-                    if (which & 1) {           /* Eq. 5 with A_ij = A */
-                        double f = 2.0 * s->A / (MO_MU0 * Msi) / (delta[nb] * delta[nb]);
+                    if (which & 1) {           /* Eq. 5; A_ij = A, or 2 A_i A_j / (A_i + A_j) for cell-based A */
+                        double Aij = s->A;
+                        if (s->Acell) {
+                            const double Ai = s->Acell[q], Aj = s->Acell[p];
+                            Aij = (Ai + Aj) != 0.0 ? 2.0 * Ai * Aj / (Ai + Aj) : 0.0;
+                        }
+                        double f = 2.0 * Aij / (MO_MU0 * Msi) / (delta[nb] * delta[nb]);
                         hx += f * (nxm - mx); hy += f * (nym - my); hz += f * (nzm - mz);
                     }
-                    if ((which & 2) && s->dmi_kind != 0) {   /* Eq. 15 with D_ij = D */
-                        const double *e = s->dmi_kind == 1 ? e_bulk[nb] : e_int[nb];
-                        double f = -s->D / (MO_MU0 * Msi) / delta[nb];
+                    if ((which & 2) && s->dmi_kind != 0) {   /* Eq. 15; D_ij = D, or 2 D_i D_j / (D_i + D_j) */
+                        const double *e = s->dmi_kind == 1 ? e_bulk[nb] : (s->dmi_kind == 2 ? e_int[nb] : e_d2d[nb]);
+                        double Dij = s->D;
+                        if (s->Dcell) {
+                            const double Di = s->Dcell[q], Dj = s->Dcell[p];
+                            Dij = (Di + Dj) != 0.0 ? 2.0 * Di * Dj / (Di + Dj) : 0.0;
+                        }
+                        double f = -Dij / (MO_MU0 * Msi) / delta[nb];
                         hx += f * (e[1] * nzm - e[2] * nym);
                         hy += f * (e[2] * nxm - e[0] * nzm);
                         hz += f * (e[0] * nym - e[1] * nxm);
@@ -415,12 +430,20 @@ static void local_field_add(const mo_sim *s, const double *m, double *H, int whi
                     double f = 2.0 * s->Ku / (MO_MU0 * Msi) * (mx * ux + my * uy + mz * uz);
                     hx += f * ux; hy += f * uy; hz += f * uz;
                 }
-                if (which & 8) { hx += s->hx; hy += s->hy; hz += s->hz; }
+                if (which & 32) {              /* cubic anisotropy, Eq. 33 w = Kc (mx^4 + my^4 + mz^4) in its continuum
+                                                * reading (R6): H = -(1/(mu0 Ms)) dw/dm = -(4 Kc/(mu0 Ms)) (mx^3, my^3, mz^3) */
+                    double f = -4.0 * s->Kc / (MO_MU0 * Msi);
+                    hx += f * mx * mx * mx; hy += f * my * my * my; hz += f * mz * mz * mz;
+                }
+                if (which & 8) {               /* Eq. 35: the external field itself, uniform or per cell */
+                    if (s->Hcell) { hx += s->Hcell[q]; hy += s->Hcell[N + q]; hz += s->Hcell[2 * N + q]; }
+                    else { hx += s->hx; hy += s->hy; hz += s->hz; }
+                }
                 H[q] += hx; H[N + q] += hy; H[2 * N + q] += hz;
             }
 }
 
-/* which: bits 0..3 as above, bit4 demag */
+/* which: bits 0..3 and 5 as above, bit4 demag */
 int mo_field_terms(mo_sim *s, const double *m, double *H, int which)
 {
     const long N = s->N;
@@ -431,11 +454,11 @@ int mo_field_terms(mo_sim *s, const double *m, double *H, int which)
         for (long q = 0; q < N; q++)
             if (s->Ms[q] == 0.0) H[q] = H[N + q] = H[2 * N + q] = 0.0;
     }
-    local_field_add(s, m, H, which & 15);
+    local_field_add(s, m, H, which & (15 | 32));
     return 0;
 }
 
-int mo_effective_field(mo_sim *s, const double *m, double *H) { return mo_field_terms(s, m, H, 31); }
+int mo_effective_field(mo_sim *s, const double *m, double *H) { return mo_field_terms(s, m, H, 63); }
 
 /* Eq. 37 */
 int mo_llg_rhs(mo_sim *s, const double *m, double *dmdt)
@@ -667,18 +690,23 @@ int mo_energy(mo_sim *s, const double *m, double *E_total, double E_terms[5])
 {
     const long N = s->N;
     double *H = (double *)malloc(sizeof(double) * 3 * N);
-    const int bits[5] = { 16, 1, 2, 4, 8 };
-    const double w[5] = { 0.5, 0.5, 0.5, 0.5, 1.0 };
+    /* quadratic terms carry 1/2, the quartic cubic-anisotropy term 1/4 (Euler), the linear Zeeman term 1;
+     * cubic anisotropy is reported inside the anisotropy slot */
+    const int bits[6] = { 16, 1, 2, 4, 8, 32 };
+    const double w[6] = { 0.5, 0.5, 0.5, 0.5, 1.0, 0.25 };
+    const int slot[6] = { 0, 1, 2, 3, 4, 3 };
     const double V = s->dx * s->dy * s->dz;
     double tot = 0;
-    for (int t = 0; t < 5; t++) {
+    if (E_terms) for (int t = 0; t < 5; t++) E_terms[t] = 0.0;
+    for (int t = 0; t < 6; t++) {
+        if (t == 5 && s->Kc == 0.0) continue;
         int rc = mo_field_terms(s, m, H, bits[t]);
         if (rc) { free(H); return rc; }
         double e = 0;
         for (long q = 0; q < N; q++)
             e += s->Ms[q] * (m[q] * H[q] + m[N + q] * H[N + q] + m[2 * N + q] * H[2 * N + q]);
         e *= -MO_MU0 * V * w[t];
-        if (E_terms) E_terms[t] = e;
+        if (E_terms) E_terms[slot[t]] += e;
         tot += e;
     }
     if (E_total) *E_total = tot;
@@ -717,15 +745,26 @@ int mo_create(mo_sim **out, int nx, int ny, int nz, double dx, double dy, double
 int mo_destroy(mo_sim *s)
 {
     if (!s) return 0;
-    free(s->Ms); free(s->Nten); free(s->Khat); free(s);
+    free(s->Ms); free(s->Nten); free(s->Khat); free(s->Acell); free(s->Dcell); free(s->Hcell); free(s);
     return 0;
 }
 
 int mo_set_Ms_uniform(mo_sim *s, double Ms) { for (long q = 0; q < s->N; q++) s->Ms[q] = Ms; return 0; }
 int mo_set_Ms(mo_sim *s, const double *Ms) { memcpy(s->Ms, Ms, sizeof(double) * s->N); return 0; }
 int mo_set_A(mo_sim *s, double A) { s->A = A; return 0; }
-int mo_set_D(mo_sim *s, double D, int kind) { if (kind < 0 || kind > 2) return -1; s->D = D; s->dmi_kind = kind; return 0; }
+int mo_set_D(mo_sim *s, double D, int kind) { if (kind < 0 || kind > 3) return -1; s->D = D; s->dmi_kind = kind; return 0; }
 int mo_set_Ku(mo_sim *s, double Ku) { s->Ku = Ku; return 0; }
+int mo_set_Kc(mo_sim *s, double Kc) { s->Kc = Kc; return 0; }
+static int set_cell_array(double **dst, const double *src, long n)
+{
+    free(*dst); *dst = NULL;
+    if (src) { *dst = (double *)malloc(sizeof(double) * n); memcpy(*dst, src, sizeof(double) * n); }
+    return 0;
+}
+/* cell-based constants (NULL: back to the uniform value) */
+int mo_set_A_cell(mo_sim *s, const double *A) { return set_cell_array(&s->Acell, A, s->N); }
+int mo_set_D_cell(mo_sim *s, const double *D, int kind) { if (kind < 0 || kind > 3) return -1; s->dmi_kind = kind; return set_cell_array(&s->Dcell, D, s->N); }
+int mo_set_H_ext_cell(mo_sim *s, const double *H) { return set_cell_array(&s->Hcell, H, 3 * s->N); }
 int mo_set_axis(mo_sim *s, double ux, double uy, double uz)
 {
     if (ux == 0 && uy == 0 && uz == 0) return -1;
