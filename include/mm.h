@@ -51,7 +51,9 @@ typedef enum {
     MM_ERR_NAN = -6,          /* non-finite error norm met in mm_step / mm_relax                */
     MM_ERR_INTERNAL = -7      /* a self-check of the library failed (e.g. K^ not real at setup)   */
 } mm_status;
-typedef enum { MM_DMI_NONE = 0, MM_DMI_BULK = 1, MM_DMI_INTERFACIAL = 2 } mm_dmi_kind;
+/* DMI vectors e_ij for the neighbours {-x,+x,-y,+y,-z,+z}: bulk r^_ij; interfacial z^ x r^_ij =
+ * {-y^,+y^,+x^,-x^,0,0}; D2d {+x^,-x^,-y^,+y^,0,0} (Eq. 14). */
+typedef enum { MM_DMI_NONE = 0, MM_DMI_BULK = 1, MM_DMI_INTERFACIAL = 2, MM_DMI_D2D = 3 } mm_dmi_kind;
 typedef enum { MM_RK4 = 0, MM_DOPRI5 = 1 } mm_integrator;
 
 /* Create a problem on `device`, all later work on `cuda_stream` (a cudaStream_t; NULL = default
@@ -80,6 +82,20 @@ int mm_set_D(mm_sim* sim, double D, mm_dmi_kind kind);
 int mm_set_Ku(mm_sim* sim, double Ku);
 int mm_set_axis(mm_sim* sim, double ux, double uy, double uz);    /* normalised inside; 0 => ARG */
 int mm_set_H_ext(mm_sim* sim, double hx, double hy, double hz);
+/* Cell-based material constants (PAPER.md:66 "cell-based", :120, :175): dev_A / dev_D hold N reals in the handle's
+ * precision, copied into the workspace.  The bond values are the harmonic means A_ij = 2 A_i A_j / (A_i + A_j)
+ * and D_ij = 2 D_i D_j / (D_i + D_j), 0 when both vanish.  While set they replace the
+ * uniform mm_set_A / mm_set_D value; NULL (or a later mm_set_A / mm_set_D) switches back.  Call after
+ * mm_set_workspace. */
+int mm_set_A_cell(mm_sim* sim, const void* dev_A);
+int mm_set_D_cell(mm_sim* sim, const void* dev_D, mm_dmi_kind kind);
+/* Cubic anisotropy, Eq. 33 in its continuum reading (R6): energy density
+ * Kc (mx^4 + my^4 + mz^4), crystal axes = mesh axes, H = -(4 Kc / (mu0 Ms)) (mx^3, my^3, mz^3).  mm_energy reports it
+ * inside the anisotropy term. */
+int mm_set_Kc(mm_sim* sim, double Kc);
+/* Per-cell external field (Eq. 35 with H_i): dev_H holds 3N reals (SoA, A/m), copied; NULL
+ * switches back to the uniform mm_set_H_ext value. */
+int mm_set_H_ext_cell(mm_sim* sim, const void* dev_H);
 int mm_set_alpha(mm_sim* sim, double alpha);
 int mm_set_gamma(mm_sim* sim, double gamma);
 int mm_set_integrator(mm_sim* sim, mm_integrator integ);

@@ -7,7 +7,7 @@ import os
 
 F32, F64 = 0, 1
 RK4, DOPRI5 = 0, 1
-DMI_NONE, DMI_BULK, DMI_INTERFACIAL = 0, 1, 2
+DMI_NONE, DMI_BULK, DMI_INTERFACIAL, DMI_D2D = 0, 1, 2, 3
 _STATUS = {0: "MM_OK", -1: "MM_ERR_ARG", -2: "MM_ERR_UNSUPPORTED", -3: "MM_ERR_STATE", -4: "MM_ERR_CUDA",
            -5: "MM_ERR_NOMEM", -6: "MM_ERR_NAN", -7: "MM_ERR_INTERNAL"}
 HERE = os.path.dirname(os.path.abspath(__file__))
@@ -27,6 +27,10 @@ SIGNATURES = {
     "mm_set_A": (_i, [_vp, _d]),
     "mm_set_D": (_i, [_vp, _d, _i]),
     "mm_set_Ku": (_i, [_vp, _d]),
+    "mm_set_Kc": (_i, [_vp, _d]),
+    "mm_set_A_cell": (_i, [_vp, _vp]),
+    "mm_set_D_cell": (_i, [_vp, _vp, _i]),
+    "mm_set_H_ext_cell": (_i, [_vp, _vp]),
     "mm_set_axis": (_i, [_vp, _d, _d, _d]),
     "mm_set_H_ext": (_i, [_vp, _d, _d, _d]),
     "mm_set_alpha": (_i, [_vp, _d]),
@@ -132,6 +136,29 @@ class Sim:
     def set_A(self, A): self._chk(self.L.mm_set_A(self.h, A), "mm_set_A")
     def set_D(self, D, kind): self._chk(self.L.mm_set_D(self.h, D, kind), "mm_set_D")
     def set_Ku(self, Ku): self._chk(self.L.mm_set_Ku(self.h, Ku), "mm_set_Ku")
+    def set_Kc(self, Kc): self._chk(self.L.mm_set_Kc(self.h, Kc), "mm_set_Kc")
+
+    def _cell(self, a, n):
+        """Device pointer of a per-cell array (numpy or tensor, copied by the library), or NULL for None."""
+        if a is None:
+            return None, None
+        t = a if self.torch.is_tensor(a) else self.to_device(a)
+        return t, self._dev(t, n)
+
+    def set_A_cell(self, A):
+        t, p = self._cell(A, self.N)
+        self._chk(self.L.mm_set_A_cell(self.h, p), "mm_set_A_cell")
+        self.torch.cuda.current_stream(self.device).synchronize()
+
+    def set_D_cell(self, D, kind):
+        t, p = self._cell(D, self.N)
+        self._chk(self.L.mm_set_D_cell(self.h, p, kind), "mm_set_D_cell")
+        self.torch.cuda.current_stream(self.device).synchronize()
+
+    def set_H_ext_cell(self, H):
+        t, p = self._cell(H, 3 * self.N)
+        self._chk(self.L.mm_set_H_ext_cell(self.h, p), "mm_set_H_ext_cell")
+        self.torch.cuda.current_stream(self.device).synchronize()
     def set_axis(self, ux, uy, uz): self._chk(self.L.mm_set_axis(self.h, ux, uy, uz), "mm_set_axis")
     def set_H_ext(self, hx, hy, hz): self._chk(self.L.mm_set_H_ext(self.h, hx, hy, hz), "mm_set_H_ext")
     def set_alpha(self, a): self._chk(self.L.mm_set_alpha(self.h, a), "mm_set_alpha")

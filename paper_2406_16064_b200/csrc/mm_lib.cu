@@ -34,6 +34,7 @@ extern "C" void mm_newell_near_box(int bx, int by, int bz, double dx, double dy,
 namespace mm {
 
 static const double MU0 = 4.0e-7 * 3.14159265358979323846264338327950288;
+static const int ALL_TERMS = 63;      // LocalP::terms: exchange | DMI | uniaxial | Zeeman | demag | cubic
 
 // Device-resident step controller state.
 struct DevState {
@@ -241,8 +242,10 @@ template <typename T, int CPT> __device__ __forceinline__ void stc(T* p, const c
 #ifndef MM_STAGEV_CPT
 #define MM_STAGEV_CPT 2      // cells per thread (8-byte loads in fp32, 16-byte in fp64): measured best on B200
 #endif
-template <typename T, int CPT, int MODE, int S, bool NEXT, bool ERR, bool MAXK>
-__global__ void __launch_bounds__(MM_STAGEV_THREADS, sizeof(T) == 8 ? 1 : 4) llg_stagev_kernel(Geom g, LocalP<T> lp, const T* __restrict__ y, const T* __restrict__ Ms,
+// GEN: cell-based A and / or D: the A_i, D_i of the six neighbours are loaded like the neighbour
+// values of m and turned into the harmonic-mean bond values.
+template <typename T, int CPT, int MODE, int S, bool NEXT, bool ERR, bool MAXK, bool GEN>
+__global__ void __launch_bounds__(MM_STAGEV_THREADS, sizeof(T) == 8 ? 1 : (GEN ? 3 : 4)) llg_stagev_kernel(Geom g, LocalP<T> lp, const T* __restrict__ y, const T* __restrict__ Ms,
                                                          const unsigned char* __restrict__ nbm, const T* __restrict__ Hd, T* __restrict__ out, StageArgs<T> sa, DevState* st)
 {
     if (st->done) return;
@@ -276,6 +279,16 @@ __global__ void __launch_bounds__(MM_STAGEV_THREADS, sizeof(T) == 8 ? 1 : 4) llg
 #pragma unroll
             for (int c = 0; c < 3; c++) m0[c] = ldc<T, CPT>(sa.m0 + c * N + q);
         }
+        CV hx[3];      // external field of the thread's cells: per cell (Eq. 35 with H_i) or uniform
+        if (lp.Hcell != nullptr && (lp.terms & 8)) {
+#pragma unroll
+            for (int c = 0; c < 3; c++) hx[c] = ldc<T, CPT>(lp.Hcell + c * N + q);
+        } else {
+#pragma unroll
+            for (int c = 0; c < 3; c++)
+#pragma unroll
+                for (int e = 0; e < CPT; e++) hx[c].e[e] = lp.hext[c];
+        }
         if ((lp.terms & 3) != 0) {
             // neighbour rows: index clamped to the own row when outside the mesh, then masked
             const long sy = g.nx, szz = (long)g.nx * g.ny;
@@ -289,6 +302,21 @@ __global__ void __launch_bounds__(MM_STAGEV_THREADS, sizeof(T) == 8 ? 1 : 4) llg
                 nym[c] = ldc<T, CPT>(y + c * N + qym); nyp[c] = ldc<T, CPT>(y + c * N + qyp);
                 nzm[c] = ldc<T, CPT>(y + c * N + qzm); nzp[c] = ldc<T, CPT>(y + c * N + qzp);
                 xl[c] = y[c * N + qxm]; xr[c] = y[c * N + qxp];
+            }
+            // cell-based constants of the thread's cells and of their neighbours (index 0 = A, 1 = D)
+            CV pc[2], pym[2], pyp[2], pzm[2], pzp[2];
+            T pxl[2], pxr[2];
+            if (GEN) {
+                const T* par[2] = { lp.Acell, lp.Dcell };
+#pragma unroll
+                for (int t = 0; t < 2; t++) {
+                    if (par[t] != nullptr) {
+                        pc[t] = ldc<T, CPT>(par[t] + q);
+                        pym[t] = ldc<T, CPT>(par[t] + qym); pyp[t] = ldc<T, CPT>(par[t] + qyp);
+                        pzm[t] = ldc<T, CPT>(par[t] + qzm); pzp[t] = ldc<T, CPT>(par[t] + qzp);
+                        pxl[t] = par[t][qxm]; pxr[t] = par[t][qxp];
+                    }
+                }
             }
             // neighbour-presence bits of the thread's cells (nbmask_kernel, written when Ms is set):
             // bit 0..5 = -x +x -y +y -z +z present (inside the mesh and Ms != 0)
@@ -311,14 +339,32 @@ __global__ void __launch_bounds__(MM_STAGEV_THREADS, sizeof(T) == 8 ? 1 : 4) llg
                 nb[4] = { nzm[0].e[e], nzm[1].e[e], nzm[2].e[e] };
                 nb[5] = { nzp[0].e[e], nzp[1].e[e], nzp[2].e[e] };
                 v3<T> h = { H[0].e[e], H[1].e[e], H[2].e[e] };
+                const v3<T> he = { hx[0].e[e], hx[1].e[e], hx[2].e[e] };
+                T w[2][6];
+                if (GEN) {
+                    const T* par[2] = { lp.Acell, lp.Dcell };
+#pragma unroll
+                    for (int t = 0; t < 2; t++) {
+                        if (par[t] != nullptr) {
+                            const T ci = pc[t].e[e];
+                            w[t][0] = harm<T>(ci, e > 0 ? pc[t].e[e > 0 ? e - 1 : 0] : pxl[t]);
+                            w[t][1] = harm<T>(ci, e < CPT - 1 ? pc[t].e[e < CPT - 1 ? e + 1 : 0] : pxr[t]);
+                            w[t][2] = harm<T>(ci, pym[t].e[e]); w[t][3] = harm<T>(ci, pyp[t].e[e]);
+                            w[t][4] = harm<T>(ci, pzm[t].e[e]); w[t][5] = harm<T>(ci, pzp[t].e[e]);
+                        } else {
+#pragma unroll
+                            for (int b = 0; b < 6; b++) w[t][b] = (T)1;
+                        }
+                    }
+                }
                 if (all_present) {      // interior of the magnetic region: no masking arithmetic at all
                     const bool ok[6] = { true, true, true, true, true, true };
-                    h = local_field_nb<T>(lp, inv, mi, nb, ok, h);
+                    h = local_field_nb<T, GEN>(lp, inv, mi, nb, ok, h, he, w[0], w[1]);
                 } else {
                     bool ok[6];
 #pragma unroll
                     for (int b = 0; b < 6; b++) ok[b] = (mk >> (8 * e + b)) & 1u;
-                    h = local_field_nb<T>(lp, inv, mi, nb, ok, h);
+                    h = local_field_nb<T, GEN>(lp, inv, mi, nb, ok, h, he, w[0], w[1]);
                 }
                 H[0].e[e] = h.x; H[1].e[e] = h.y; H[2].e[e] = h.z;
             }
@@ -329,7 +375,8 @@ __global__ void __launch_bounds__(MM_STAGEV_THREADS, sizeof(T) == 8 ? 1 : 4) llg
                 const T inv = (T)1 / (Msi != (T)0 ? Msi : (T)1);
                 const v3<T> mi = { m[0].e[e], m[1].e[e], m[2].e[e] };
                 v3<T> h = { H[0].e[e], H[1].e[e], H[2].e[e] };
-                h = local_field_rest<T>(lp, inv, mi, h);
+                const v3<T> he = { hx[0].e[e], hx[1].e[e], hx[2].e[e] };
+                h = local_field_rest<T>(lp, inv, mi, h, he);
                 H[0].e[e] = h.x; H[1].e[e] = h.y; H[2].e[e] = h.z;
             }
         }
@@ -698,12 +745,13 @@ struct mm_sim {
     int device;
     cudaStream_t stream;
     double dx, dy, dz;
-    double A, D, Ku, u[3], hext[3], alpha, gamma;
+    double A, D, Ku, Kc, u[3], hext[3], alpha, gamma;
     int dmi_kind, integ, demag_on, demag_ready, Ms_set;
+    int A_cell, D_cell, H_cell;      // cell-based A / D / external field set (arrays in the workspace)
     // workspace
     void* ws;
     size_t ws_bytes, ws_need;
-    size_t off_Ms, off_nbm, off_S, off_Kh, off_Kc, off_mh, off_Hd, off_k[7], off_y[2], off_tw, off_st, off_part, off_min;
+    size_t off_Ms, off_nbm, off_S, off_Kh, off_Kc, off_mh, off_Hd, off_k[7], off_y[2], off_tw, off_st, off_part, off_min, off_Ac, off_Dc, off_Hc;
     int twN;
     size_t smemA, smemA2, smemB;
     int thrA, thrB;
@@ -838,6 +886,9 @@ static void layout(mm_sim* s)
     s->off_tw = take((size_t)(s->twN / 2 + 1) * 2 * es);
     s->off_part = take(3 * (size_t)((N + 255) / 256) * sizeof(double) > 4 * 1024 * sizeof(double) ? 3 * (size_t)((N + 255) / 256) * sizeof(double) : 4 * 1024 * sizeof(double));
     s->off_min = take(sizeof(MinState));
+    s->off_Ac = take(N * es);          // cell-based A_i, D_i, H_ext,i (Eq. 35): 5N reals
+    s->off_Dc = take(N * es);
+    s->off_Hc = take(3 * N * es);
     s->ws_need = o;
 }
 
@@ -853,7 +904,7 @@ extern "C" int mm_create(mm_sim** out, int nx, int ny, int nz, double dx, double
     mm_sim* s = new mm_sim();
     s->prec = prec; s->device = device; s->stream = static_cast<cudaStream_t>(cuda_stream);
     s->dx = dx; s->dy = dy; s->dz = dz;
-    s->A = s->D = s->Ku = 0; s->u[0] = s->u[1] = 0; s->u[2] = 1; s->hext[0] = s->hext[1] = s->hext[2] = 0;
+    s->A = s->D = s->Ku = s->Kc = 0; s->A_cell = s->D_cell = s->H_cell = 0; s->u[0] = s->u[1] = 0; s->u[2] = 1; s->hext[0] = s->hext[1] = s->hext[2] = 0;
     s->alpha = 0.5; s->gamma = 2.211e5; s->dmi_kind = 0; s->integ = MM_DOPRI5; s->demag_on = 1; s->demag_ready = 0; s->Ms_set = 0;
     s->ws = nullptr; s->ws_bytes = 0; s->khat_imag_ratio = -1; s->t_host = 0; s->launches = 0; s->prof_on = 0; s->prof_open = 0; s->prof_used = 0; s->use_v2 = getenv("MM_FORCE_V1") ? 0 : 1; s->no_b7 = getenv("MM_NO_B7") ? 1 : 0; s->no_stagev = getenv("MM_NO_STAGEV") ? 1 : 0;
     Geom& g = s->g;
@@ -931,7 +982,7 @@ extern "C" int mm_set_workspace(mm_sim* s, void* dev_ptr, size_t bytes)
     s->ws = dev_ptr; s->ws_bytes = bytes;
     // zero state, Ms and the spectrum (pad columns of S are never written by pass A)
     MM_TRY(s, cudaMemsetAsync(dev_ptr, 0, s->off_Kh, s->stream));
-    s->demag_ready = 0; s->Ms_set = 0;
+    s->demag_ready = 0; s->Ms_set = 0; s->A_cell = s->D_cell = s->H_cell = 0;
     return s->prec == MM_F64 ? upload_twiddles<double>(s) : upload_twiddles<float>(s);
 }
 
@@ -971,13 +1022,31 @@ extern "C" int mm_set_Ms(mm_sim* s, const void* dev_Ms)
     s->Ms_set = 1;
     return MM_OK;
 }
-extern "C" int mm_set_A(mm_sim* s, double A) { if (!s) return MM_ERR_ARG; s->A = A; return MM_OK; }
+extern "C" int mm_set_A(mm_sim* s, double A) { if (!s) return MM_ERR_ARG; s->A = A; s->A_cell = 0; return MM_OK; }
 extern "C" int mm_set_D(mm_sim* s, double D, mm_dmi_kind kind)
 {
-    if (!s || kind < 0 || kind > 2) return MM_ERR_ARG;
-    s->D = D; s->dmi_kind = kind; return MM_OK;
+    if (!s || kind < 0 || kind > 3) return MM_ERR_ARG;
+    s->D = D; s->dmi_kind = kind; s->D_cell = 0; return MM_OK;
 }
+// cell-based constants: copied into the workspace; NULL switches back to the uniform value
+static int set_cell_array(mm_sim* s, size_t off, size_t count, const void* dev_src, int* flag)
+{
+    NEED_WS(s);
+    if (!dev_src) { *flag = 0; return MM_OK; }
+    MM_TRY(s, cudaMemcpyAsync(wsp<char>(s, off), dev_src, count * esize(s), cudaMemcpyDeviceToDevice, s->stream));
+    *flag = 1;
+    return MM_OK;
+}
+extern "C" int mm_set_A_cell(mm_sim* s, const void* dev_A) { if (!s) return MM_ERR_ARG; return set_cell_array(s, s->off_Ac, (size_t)s->g.N, dev_A, &s->A_cell); }
+extern "C" int mm_set_D_cell(mm_sim* s, const void* dev_D, mm_dmi_kind kind)
+{
+    if (!s || kind < 0 || kind > 3) return MM_ERR_ARG;
+    s->dmi_kind = kind;
+    return set_cell_array(s, s->off_Dc, (size_t)s->g.N, dev_D, &s->D_cell);
+}
+extern "C" int mm_set_H_ext_cell(mm_sim* s, const void* dev_H) { if (!s) return MM_ERR_ARG; return set_cell_array(s, s->off_Hc, 3 * (size_t)s->g.N, dev_H, &s->H_cell); }
 extern "C" int mm_set_Ku(mm_sim* s, double Ku) { if (!s) return MM_ERR_ARG; s->Ku = Ku; return MM_OK; }
+extern "C" int mm_set_Kc(mm_sim* s, double Kc) { if (!s) return MM_ERR_ARG; s->Kc = Kc; return MM_OK; }
 extern "C" int mm_set_axis(mm_sim* s, double ux, double uy, double uz)
 {
     if (!s) return MM_ERR_ARG;
@@ -1165,19 +1234,24 @@ template <typename T> static LocalP<T> make_local(const mm_sim* s, int terms)
     LocalP<T> lp;
     const double d[3] = { s->dx, s->dy, s->dz };
     for (int a = 0; a < 3; a++) {
-        lp.cex[a] = (T)(2.0 * s->A / (MU0 * d[a] * d[a]));
-        lp.cdm[a] = (T)(s->D / (MU0 * d[a]));
+        lp.cex[a] = (T)(2.0 * (s->A_cell ? 1.0 : s->A) / (MU0 * d[a] * d[a]));
+        lp.cdm[a] = (T)((s->D_cell ? 1.0 : s->D) / (MU0 * d[a]));
         lp.u[a] = (T)s->u[a];
         lp.hext[a] = (T)s->hext[a];
     }
+    lp.Acell = s->A_cell ? wsp<T>(s, s->off_Ac) : (const T*)nullptr;
+    lp.Dcell = s->D_cell ? wsp<T>(s, s->off_Dc) : (const T*)nullptr;
+    lp.Hcell = s->H_cell ? wsp<T>(s, s->off_Hc) : (const T*)nullptr;
     lp.cku = (T)(2.0 * s->Ku / MU0);
+    lp.ckc = (T)(4.0 * s->Kc / MU0);
     lp.gp = (T)(s->gamma / (1.0 + s->alpha * s->alpha));
     lp.agp = (T)(s->alpha * s->gamma / (1.0 + s->alpha * s->alpha));
     lp.dmi = s->dmi_kind;
     lp.terms = terms;
-    if (s->A == 0.0) lp.terms &= ~1;
-    if (s->D == 0.0 || s->dmi_kind == 0) lp.terms &= ~2;
+    if (s->A == 0.0 && !s->A_cell) lp.terms &= ~1;
+    if ((s->D == 0.0 && !s->D_cell) || s->dmi_kind == 0) lp.terms &= ~2;
     if (s->Ku == 0.0) lp.terms &= ~4;
+    if (s->Kc == 0.0) lp.terms &= ~32;
     return lp;
 }
 
@@ -1310,7 +1384,10 @@ static void launch_stage(mm_sim* s, const LocalP<T>& lp, const T* y, const T* Hd
     constexpr int CPT = MM_STAGEV_CPT;
     if (s->g.nx % CPT == 0 && !s->no_stagev) {
         const unsigned blocks = (unsigned)((s->g.N / CPT + MM_STAGEV_THREADS - 1) / MM_STAGEV_THREADS);
-        llg_stagev_kernel<T, CPT, MODE, S, NEXT, ERR, MAXK><<<blocks, MM_STAGEV_THREADS, 0, s->stream>>>(s->g, lp, y, wsp<T>(s, s->off_Ms), wsp<unsigned char>(s, s->off_nbm), Hd, out, sa, wsp<DevState>(s, s->off_st));
+        if (lp.Acell != nullptr || lp.Dcell != nullptr)
+            llg_stagev_kernel<T, CPT, MODE, S, NEXT, ERR, MAXK, true><<<blocks, MM_STAGEV_THREADS, 0, s->stream>>>(s->g, lp, y, wsp<T>(s, s->off_Ms), wsp<unsigned char>(s, s->off_nbm), Hd, out, sa, wsp<DevState>(s, s->off_st));
+        else
+            llg_stagev_kernel<T, CPT, MODE, S, NEXT, ERR, MAXK, false><<<blocks, MM_STAGEV_THREADS, 0, s->stream>>>(s->g, lp, y, wsp<T>(s, s->off_Ms), wsp<unsigned char>(s, s->off_nbm), Hd, out, sa, wsp<DevState>(s, s->off_st));
         return;
     }
     const unsigned blocks = (unsigned)((s->g.N + 255) / 256);
@@ -1368,8 +1445,8 @@ extern "C" int mm_effective_field(mm_sim* s, const void* dev_m, void* dev_H)
     if (!dev_m || !dev_H) return MM_ERR_ARG;
     int rc = set_state(s, 0, 0, 0, 0, 0, 1);
     if (rc) return rc;
-    if (s->prec == MM_F64) return eval<double, 0>(s, (const double*)dev_m, (double*)dev_H, no_stage<double>(), 31);
-    return eval<float, 0>(s, (const float*)dev_m, (float*)dev_H, no_stage<float>(), 31);
+    if (s->prec == MM_F64) return eval<double, 0>(s, (const double*)dev_m, (double*)dev_H, no_stage<double>(), ALL_TERMS);
+    return eval<float, 0>(s, (const float*)dev_m, (float*)dev_H, no_stage<float>(), ALL_TERMS);
 }
 
 extern "C" int mm_llg_rhs(mm_sim* s, const void* dev_m, void* dev_dmdt)
@@ -1378,8 +1455,8 @@ extern "C" int mm_llg_rhs(mm_sim* s, const void* dev_m, void* dev_dmdt)
     if (!dev_m || !dev_dmdt) return MM_ERR_ARG;
     int rc = set_state(s, 0, 0, 0, 0, 0, 1);
     if (rc) return rc;
-    if (s->prec == MM_F64) return eval<double, 1>(s, (const double*)dev_m, (double*)dev_dmdt, no_stage<double>(), 31);
-    return eval<float, 1>(s, (const float*)dev_m, (float*)dev_dmdt, no_stage<float>(), 31);
+    if (s->prec == MM_F64) return eval<double, 1>(s, (const double*)dev_m, (double*)dev_dmdt, no_stage<double>(), ALL_TERMS);
+    return eval<float, 1>(s, (const float*)dev_m, (float*)dev_dmdt, no_stage<float>(), ALL_TERMS);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -1417,7 +1494,7 @@ template <typename T> static int enqueue_step(mm_sim* s, T* m, int ctrl_mode)
             for (int j = 0; j <= st; j++) sa.coef[j] = (T)RK4_A[st][j];
         }
         const T* y = st == 0 ? m : yb[(st - 1) & 1];
-        int rc = eval<T, 1>(s, y, k[st], sa, 31);
+        int rc = eval<T, 1>(s, y, k[st], sa, ALL_TERMS);
         if (rc) return rc;
     }
     DevState* ds = wsp<DevState>(s, s->off_st);
@@ -1544,7 +1621,7 @@ template <typename T> static int minimize_t(mm_sim* s, T* m, double tau0, double
     double* part = wsp<double>(s, s->off_part);
     const bool demag = s->demag_on != 0;
     if (demag && !s->demag_ready) return fail(s, MM_ERR_STATE, "demag enabled but mm_init_demag not called");
-    const LocalP<T> lp = make_local<T>(s, 31);
+    const LocalP<T> lp = make_local<T>(s, ALL_TERMS);
     const unsigned nblk = (unsigned)((N + 255) / 256);
     long issued = 0;
     while (issued <= max_steps) {
@@ -1647,19 +1724,24 @@ extern "C" int mm_average_m(mm_sim* s, const void* dev_m, double out3[3])
 
 template <typename T> static int energy_t(mm_sim* s, const T* m, double* E_total, double E_terms[5])
 {
-    static const int bits[5] = { 16, 1, 2, 4, 8 };
-    static const double w[5] = { 0.5, 0.5, 0.5, 0.5, 1.0 };
+    // quadratic terms carry 1/2, the quartic cubic-anisotropy term 1/4 (Euler's theorem: m.H = -4 w / (mu0 Ms)), the
+    // linear Zeeman term 1; cubic anisotropy is reported inside the anisotropy slot
+    static const int bits[6] = { 16, 1, 2, 4, 8, 32 };
+    static const double w[6] = { 0.5, 0.5, 0.5, 0.5, 1.0, 0.25 };
+    static const int slot[6] = { 0, 1, 2, 3, 4, 3 };
     T* H = wsp<T>(s, s->off_k[6]);
     const double V = s->dx * s->dy * s->dz;
     double tot = 0;
     int rc = set_state(s, 0, 0, 0, 0, 0, 1);
     if (rc) return rc;
-    for (int t = 0; t < 5; t++) {
+    if (E_terms) for (int t = 0; t < 5; t++) E_terms[t] = 0.0;
+    for (int t = 0; t < 6; t++) {
+        if (t == 5 && s->Kc == 0.0) continue;
         if ((rc = eval<T, 0>(s, m, H, no_stage<T>(), bits[t]))) return rc;
         double r[4];
         if ((rc = reduce_dot<T>(s, m, H, 0, r))) return rc;
         const double e = -MU0 * V * w[t] * r[0];
-        if (E_terms) E_terms[t] = e;
+        if (E_terms) E_terms[slot[t]] += e;
         tot += e;
     }
     if (E_total) *E_total = tot;

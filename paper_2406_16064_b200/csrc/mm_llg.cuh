@@ -1,6 +1,9 @@
 // mm_llg.cuh — per-cell arithmetic of the fused local-field / LL-torque / RK-stage kernel.
 //   exchange  Eq. 5      DMI  Eq. 15
 //   anisotropy Eq. 32 continuum reading (R6)   Zeeman Eq. 35
+//   cell-based A and D: A_ij = 2 A_i A_j / (A_i + A_j), D_ij likewise; D2d DMI table
+//   (Eq. 14); cubic anisotropy Eq. 33-34 continuum reading (R6);
+//   per-cell external field (Eq. 35 with H_i)
 //   LL torque Eq. 37;  RK stage algebra: DESIGN.md R8
 // A neighbour is absent when outside the mesh or when its Ms is 0 (R4); Ms_i = 0 => H = 0, k = 0 (R5).
 #pragma once
@@ -10,32 +13,52 @@
 namespace mm {
 
 template <typename T> struct LocalP {
-    T cex[3];      // 2A/(mu0 d_a^2)
-    T cdm[3];      // D/(mu0 d_a)
+    T cex[3];      // 2A/(mu0 d_a^2)   (2/(mu0 d_a^2) when A is cell-based: the bond value A_ij multiplies it)
+    T cdm[3];      // D/(mu0 d_a)      (1/(mu0 d_a) when D is cell-based)
     T cku;         // 2Ku/mu0
+    T ckc;         // 4Kc/mu0 (cubic anisotropy, crystal axes = mesh axes)
     T u[3];        // unit axis
     T hext[3];
     T gp, agp;     // gamma/(1+alpha^2), alpha*gamma/(1+alpha^2)
-    int dmi;       // 0 none, 1 bulk, 2 interfacial
-    int terms;     // bit0 exchange, bit1 DMI, bit2 anisotropy, bit3 Zeeman, bit4 demag
+    int dmi;       // 0 none, 1 bulk, 2 interfacial, 3 D2d
+    int terms;     // bit0 exchange, bit1 DMI, bit2 uniaxial anisotropy, bit3 Zeeman, bit4 demag, bit5 cubic anisotropy
+    const T* Acell;   // N per-cell exchange constants or nullptr (uniform A)
+    const T* Dcell;   // N per-cell DMI constants or nullptr (uniform D)
+    const T* Hcell;   // 3N per-cell external field (SoA) or nullptr (uniform hext)
 };
+
+// bond value of a cell-based constant: harmonic mean, 0 when both vanish
+template <typename T> MM_HD T harm(T a, T b) { const T s = a + b; return s != (T)0 ? (T)2 * a * b / s : (T)0; }
 
 template <typename T> struct v3 { T x, y, z; };
 template <typename T> MM_HD v3<T> ld3(const T* p, long N, long q) { v3<T> r; r.x = p[q]; r.y = p[N + q]; r.z = p[2 * N + q]; return r; }
 
-// anisotropy + Zeeman part of H_eff (inv = 1/Ms_i)
-template <typename T> MM_HD v3<T> local_field_rest(const LocalP<T>& lp, T inv, v3<T> mi, v3<T> H)
+// anisotropy + Zeeman part of H_eff (inv = 1/Ms_i); hext = the external field of this cell
+template <typename T> MM_HD v3<T> local_field_rest(const LocalP<T>& lp, T inv, v3<T> mi, v3<T> H, v3<T> hext)
 {
     if (lp.terms & 4) {
         const T f = inv * lp.cku * (mi.x * lp.u[0] + mi.y * lp.u[1] + mi.z * lp.u[2]);
         H.x += f * lp.u[0]; H.y += f * lp.u[1]; H.z += f * lp.u[2];
     }
-    if (lp.terms & 8) { H.x += lp.hext[0]; H.y += lp.hext[1]; H.z += lp.hext[2]; }
+    if (lp.terms & 32) {     // Eq. 33: w = Kc (mx^4 + my^4 + mz^4)  =>  H = -(4Kc/(mu0 Ms)) (mx^3, my^3, mz^3)
+        const T f = -inv * lp.ckc;
+        H.x += f * mi.x * mi.x * mi.x; H.y += f * mi.y * mi.y * mi.y; H.z += f * mi.z * mi.z * mi.z;
+    }
+    if (lp.terms & 8) { H.x += hext.x; H.y += hext.y; H.z += hext.z; }
     return H;
+}
+template <typename T> MM_HD v3<T> local_field_rest(const LocalP<T>& lp, T inv, v3<T> mi, v3<T> H)
+{
+    const v3<T> h = { lp.hext[0], lp.hext[1], lp.hext[2] };
+    return local_field_rest<T>(lp, inv, mi, H, h);
 }
 
 // H_eff from the six neighbour values nb[-x,+x,-y,+y,-z,+z] (ok[] = neighbour present) added to H
-template <typename T> MM_HD v3<T> local_field_nb(const LocalP<T>& lp, T inv, v3<T> mi, const v3<T>* nb, const bool* ok, v3<T> H)
+// GEN: cell-based A and / or D — wA[b], wD[b] are the bond values A_ij, D_ij towards neighbour b (1 for a constant
+// that is uniform: it is then inside cex / cdm).
+template <typename T, bool GEN = false>
+MM_HD v3<T> local_field_nb(const LocalP<T>& lp, T inv, v3<T> mi, const v3<T>* nb, const bool* ok, v3<T> H, v3<T> hext,
+                           const T* wA = nullptr, const T* wD = nullptr)
 {
     v3<T> ex = { 0, 0, 0 };           // sum_a cex_a sum_{+-} (m_j - m_i)
     v3<T> S[3];                        // S_a = m_{+a} - m_{-a} over present neighbours
@@ -43,12 +66,21 @@ template <typename T> MM_HD v3<T> local_field_nb(const LocalP<T>& lp, T inv, v3<
     for (int a = 0; a < 3; a++) {
         const v3<T> mm_ = nb[2 * a], mp = nb[2 * a + 1];
         const bool bm = ok[2 * a], bp = ok[2 * a + 1];
-        const T dmx = bm ? mm_.x - mi.x : (T)0, dmy = bm ? mm_.y - mi.y : (T)0, dmz = bm ? mm_.z - mi.z : (T)0;
-        const T dpx = bp ? mp.x - mi.x : (T)0, dpy = bp ? mp.y - mi.y : (T)0, dpz = bp ? mp.z - mi.z : (T)0;
+        T dmx = bm ? mm_.x - mi.x : (T)0, dmy = bm ? mm_.y - mi.y : (T)0, dmz = bm ? mm_.z - mi.z : (T)0;
+        T dpx = bp ? mp.x - mi.x : (T)0, dpy = bp ? mp.y - mi.y : (T)0, dpz = bp ? mp.z - mi.z : (T)0;
+        if (GEN) {
+            const T am = wA[2 * a], ap = wA[2 * a + 1];
+            dmx *= am; dmy *= am; dmz *= am; dpx *= ap; dpy *= ap; dpz *= ap;
+        }
         ex.x += lp.cex[a] * (dmx + dpx); ex.y += lp.cex[a] * (dmy + dpy); ex.z += lp.cex[a] * (dmz + dpz);
-        S[a].x = (bp ? mp.x : (T)0) - (bm ? mm_.x : (T)0);
-        S[a].y = (bp ? mp.y : (T)0) - (bm ? mm_.y : (T)0);
-        S[a].z = (bp ? mp.z : (T)0) - (bm ? mm_.z : (T)0);
+        if (GEN) {
+            const T bm_ = bm ? wD[2 * a] : (T)0, bp_ = bp ? wD[2 * a + 1] : (T)0;
+            S[a].x = bp_ * mp.x - bm_ * mm_.x; S[a].y = bp_ * mp.y - bm_ * mm_.y; S[a].z = bp_ * mp.z - bm_ * mm_.z;
+        } else {
+            S[a].x = (bp ? mp.x : (T)0) - (bm ? mm_.x : (T)0);
+            S[a].y = (bp ? mp.y : (T)0) - (bm ? mm_.y : (T)0);
+            S[a].z = (bp ? mp.z : (T)0) - (bm ? mm_.z : (T)0);
+        }
     }
     if (lp.terms & 1) { H.x += inv * ex.x; H.y += inv * ex.y; H.z += inv * ex.z; }
     if ((lp.terms & 2) && lp.dmi != 0) {
@@ -57,14 +89,18 @@ template <typename T> MM_HD v3<T> local_field_nb(const LocalP<T>& lp, T inv, v3<
             d.x = lp.cdm[1] * S[1].z - lp.cdm[2] * S[2].y;
             d.y = -lp.cdm[0] * S[0].z + lp.cdm[2] * S[2].x;
             d.z = lp.cdm[0] * S[0].y - lp.cdm[1] * S[1].x;
-        } else {                // interfacial: e_ij = z^ x r^_ij : (y^ x S_x) - (x^ x S_y)
+        } else if (lp.dmi == 2) {   // interfacial: e_ij = z^ x r^_ij : (y^ x S_x) - (x^ x S_y)
             d.x = lp.cdm[0] * S[0].z;
             d.y = lp.cdm[1] * S[1].z;
             d.z = -lp.cdm[0] * S[0].x - lp.cdm[1] * S[1].y;
+        } else {                // D2d: e_ij = {+x^, -x^, -y^, +y^, 0, 0} : -(x^ x S_x) + (y^ x S_y)
+            d.x = lp.cdm[1] * S[1].z;
+            d.y = lp.cdm[0] * S[0].z;
+            d.z = -lp.cdm[0] * S[0].y - lp.cdm[1] * S[1].x;
         }
         H.x -= inv * d.x; H.y -= inv * d.y; H.z -= inv * d.z;
     }
-    return local_field_rest<T>(lp, inv, mi, H);
+    return local_field_rest<T>(lp, inv, mi, H, hext);
 }
 
 // H_eff at cell (i,j,k) given H_d (or 0).  y = stage magnetisation.  Branch-free in the data: every
@@ -76,11 +112,15 @@ MM_HD v3<T> local_field(const Geom& g, const LocalP<T>& lp, const T* __restrict_
 {
     const long N = g.N;
     const T inv = (T)1 / Msi;
-    if ((lp.terms & 3) == 0) return local_field_rest<T>(lp, inv, mi, H);
+    v3<T> hext = { lp.hext[0], lp.hext[1], lp.hext[2] };
+    if (lp.Hcell != nullptr && (lp.terms & 8)) hext = ld3(lp.Hcell, N, q);
+    if ((lp.terms & 3) == 0) return local_field_rest<T>(lp, inv, mi, H, hext);
     const long str[3] = { 1, g.nx, (long)g.nx * g.ny };
     const int pos[3] = { i, j, k }, lim[3] = { g.nx, g.ny, g.nz };
     v3<T> nb[6];
     bool ok[6];
+    const bool gen = lp.Acell != nullptr || lp.Dcell != nullptr;
+    T wA[6], wD[6];
 #pragma unroll
     for (int a = 0; a < 3; a++) {
         const bool im = pos[a] > 0, ip = pos[a] < lim[a] - 1;
@@ -89,8 +129,15 @@ MM_HD v3<T> local_field(const Geom& g, const LocalP<T>& lp, const T* __restrict_
         ok[2 * a + 1] = ip && (Ms[pp] != (T)0);
         nb[2 * a] = ld3(y, N, pm);
         nb[2 * a + 1] = ld3(y, N, pp);
+        if (gen) {
+            wA[2 * a] = lp.Acell ? harm<T>(lp.Acell[q], lp.Acell[pm]) : (T)1;
+            wA[2 * a + 1] = lp.Acell ? harm<T>(lp.Acell[q], lp.Acell[pp]) : (T)1;
+            wD[2 * a] = lp.Dcell ? harm<T>(lp.Dcell[q], lp.Dcell[pm]) : (T)1;
+            wD[2 * a + 1] = lp.Dcell ? harm<T>(lp.Dcell[q], lp.Dcell[pp]) : (T)1;
+        }
     }
-    return local_field_nb<T>(lp, inv, mi, nb, ok, H);
+    if (gen) return local_field_nb<T, true>(lp, inv, mi, nb, ok, H, hext, wA, wD);
+    return local_field_nb<T, false>(lp, inv, mi, nb, ok, H, hext);
 }
 
 template <typename T> MM_HD v3<T> ll_torque(const LocalP<T>& lp, v3<T> m, v3<T> H)

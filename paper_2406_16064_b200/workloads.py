@@ -11,7 +11,7 @@ from dataclasses import dataclass, field
 import numpy as np
 
 MU0 = 4e-7 * np.pi
-DMI_NONE, DMI_BULK, DMI_INTERFACIAL = 0, 1, 2
+DMI_NONE, DMI_BULK, DMI_INTERFACIAL, DMI_D2D = 0, 1, 2, 3
 RK4, DOPRI5 = 0, 1
 
 
@@ -38,6 +38,10 @@ class Workload:
     dt: float = 1e-14
     m0: np.ndarray = field(default=None, repr=False)
     seed: int = 0
+    Kc: float = 0.0                 # cubic anisotropy constant (Eq. 33)
+    A_cell: object = field(default=None, repr=False)       # ndarray [nz, ny, nx] or None: cell-based A
+    D_cell: object = field(default=None, repr=False)       # ndarray [nz, ny, nx] or None: cell-based D
+    H_ext_cell: object = field(default=None, repr=False)   # ndarray [3, nz, ny, nx] or None: per-cell external field
 
     @property
     def N(self):
@@ -66,6 +70,32 @@ def random_mask(seed, nx, ny, nz, fill=0.8):
     return (rng.random((nz, ny, nx)) < fill).astype(np.float64)
 
 
+def cell_params(w, seed, kind=None, Kc=0.0, zero_fraction=0.1):
+    """Cell-based material constants in the structure of a granular / multilayer sample ("cell-based",
+    :120, :175): A_i and D_i = the workload's uniform values x a seeded factor in [0.5, 1.5], piecewise constant on
+    4 x 4 x 2 grains with a sharp interface at mid-x (factor x 0.5 on the right half); D_i = 0 in a seeded fraction
+    of the cells (bond value 0 towards them); a per-cell external field = uniform value + a seeded smooth gradient +
+    noise.  Draws random numbers only; the bond arithmetic lives in the oracle and in the library."""
+    rng = np.random.default_rng(seed)
+    gx, gy, gz = -(-w.nx // 4), -(-w.ny // 4), -(-w.nz // 2)
+    grain = rng.uniform(0.5, 1.5, (2, gz, gy, gx))
+    up = [np.repeat(np.repeat(np.repeat(g, 2, axis=0), 4, axis=1), 4, axis=2)[:w.nz, :w.ny, :w.nx] for g in grain]
+    half = np.where(np.arange(w.nx) >= w.nx // 2, 0.5, 1.0)[None, None, :]
+    A0 = w.A if w.A != 0.0 else 1.3e-11
+    D0 = w.D if w.D != 0.0 else 1.5e-3
+    w.A_cell = A0 * up[0] * half
+    w.D_cell = D0 * up[1] * (rng.random((w.nz, w.ny, w.nx)) >= zero_fraction)
+    if kind is not None:
+        w.dmi_kind = kind
+    x = (np.arange(w.nx) + 0.5) / w.nx
+    H = np.empty((3, w.nz, w.ny, w.nx))
+    for c in range(3):
+        H[c] = w.H_ext[c] + 2e4 * (x[None, None, :] - 0.5) * (c + 1) + 1e3 * rng.standard_normal((w.nz, w.ny, w.nx))
+    w.H_ext_cell = H
+    w.Kc = Kc
+    return w
+
+
 def apply(sim, w, with_demag=None):
     """Push a Workload's parameters into any object with the mm_*/mo_* setter names."""
     sim.set_Ms(w.Ms if np.isscalar(w.Ms) else w.Ms_array())
@@ -74,6 +104,14 @@ def apply(sim, w, with_demag=None):
     sim.set_Ku(w.Ku)
     sim.set_axis(*w.axis)
     sim.set_H_ext(*w.H_ext)
+    if w.Kc != 0.0:
+        sim.set_Kc(w.Kc)
+    if w.A_cell is not None:
+        sim.set_A_cell(np.ascontiguousarray(w.A_cell, dtype=np.float64))
+    if w.D_cell is not None:
+        sim.set_D_cell(np.ascontiguousarray(w.D_cell, dtype=np.float64), w.dmi_kind)
+    if w.H_ext_cell is not None:
+        sim.set_H_ext_cell(np.ascontiguousarray(w.H_ext_cell, dtype=np.float64))
     sim.set_alpha(w.alpha)
     sim.set_gamma(w.gamma)
     sim.set_integrator(w.integrator)

@@ -117,6 +117,7 @@ extern "C" void emul_local(int nx, int ny, int nz, const double* par /* cex3,cdm
     LocalP<double> lp;
     for (int a = 0; a < 3; a++) { lp.cex[a] = par[a]; lp.cdm[a] = par[3 + a]; lp.u[a] = par[7 + a]; lp.hext[a] = par[10 + a]; }
     lp.cku = par[6]; lp.gp = par[13]; lp.agp = par[14]; lp.dmi = dmi; lp.terms = terms;
+    lp.ckc = 0; lp.Acell = nullptr; lp.Dcell = nullptr; lp.Hcell = nullptr;
     const long N = g.N;
     for (long q = 0; q < N; q++) {
         v3<double> res = { 0, 0, 0 };
@@ -124,6 +125,28 @@ extern "C" void emul_local(int nx, int ny, int nz, const double* par /* cex3,cdm
             int i = (int)(q % nx), j = (int)((q / nx) % ny), k = (int)(q / ((long)nx * ny));
             v3<double> mi = ld3(m, N, q), H = { 0, 0, 0 };
             if (Hd) H = ld3(Hd, N, q);
+            H = local_field<double>(g, lp, m, Ms, i, j, k, q, Ms[q], mi, H);
+            res = torque ? ll_torque<double>(lp, mi, H) : H;
+        }
+        out[q] = res.x; out[N + q] = res.y; out[2 * N + q] = res.z;
+    }
+}
+
+// the same with the (f)2 parameters: cell-based A / D (nullptr = uniform), cubic constant ckc = 4Kc/mu0, per-cell H_ext
+extern "C" void emul_local2(int nx, int ny, int nz, const double* par /* cex3,cdm3,cku,u3,h3,gp,agp,ckc */, int dmi, int terms,
+                            const double* Ms, const double* m, const double* Acell, const double* Dcell, const double* Hcell, int torque, double* out)
+{
+    Geom g = make_geom(nx, ny, nz, 1, 8, 1);
+    LocalP<double> lp;
+    for (int a = 0; a < 3; a++) { lp.cex[a] = par[a]; lp.cdm[a] = par[3 + a]; lp.u[a] = par[7 + a]; lp.hext[a] = par[10 + a]; }
+    lp.cku = par[6]; lp.gp = par[13]; lp.agp = par[14]; lp.ckc = par[15]; lp.dmi = dmi; lp.terms = terms;
+    lp.Acell = Acell; lp.Dcell = Dcell; lp.Hcell = Hcell;
+    const long N = g.N;
+    for (long q = 0; q < N; q++) {
+        v3<double> res = { 0, 0, 0 };
+        if (Ms[q] != 0.0) {
+            int i = (int)(q % nx), j = (int)((q / nx) % ny), k = (int)(q / ((long)nx * ny));
+            v3<double> mi = ld3(m, N, q), H = { 0, 0, 0 };
             H = local_field<double>(g, lp, m, Ms, i, j, k, q, Ms[q], mi, H);
             res = torque ? ll_torque<double>(lp, mi, H) : H;
         }

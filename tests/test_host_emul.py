@@ -26,6 +26,7 @@ def emul():
     L = C.CDLL(LIB)
     L.emul_demag.argtypes = [C.c_int] * 8 + [_dp] * 4
     L.emul_local.argtypes = [C.c_int] * 3 + [_dp, C.c_int, C.c_int, _dp, _dp, _dp, C.c_int, _dp]
+    L.emul_local2.argtypes = [C.c_int] * 3 + [_dp, C.c_int, C.c_int, _dp, _dp, _dp, _dp, _dp, C.c_int, _dp]
     return L
 
 
@@ -96,6 +97,42 @@ def test_local_field_and_torque_match_oracle(emul, kind):
     for torque, ref in ((0, o.effective_field(m)), (1, o.llg_rhs(m))):
         emul.emul_local(nx, ny, nz, par.ctypes.data_as(_dp), kind, 15, Msf.ctypes.data_as(_dp), m.ctypes.data_as(_dp),
                         None, torque, out.ctypes.data_as(_dp))
+        assert np.abs(out.reshape(ref.shape) - ref).max() <= 1e-12 * np.abs(ref).max()
+
+
+@pytest.mark.parametrize("use", ["A", "D", "AD", "H", "Kc", "all"])
+@pytest.mark.parametrize("kind", [wl.DMI_BULK, wl.DMI_INTERFACIAL, wl.DMI_D2D])
+def test_cell_based_local_field_matches_oracle(emul, kind, use):
+    """the library's per-cell arithmetic with cell-based A / D (harmonic-mean bonds),
+    the D2d table, cubic anisotropy (Eq. 33) and a per-cell external field, compiled for the host, against the oracle."""
+    nx, ny, nz = 8, 6, 4
+    w = wl.cfg4(nx, ny, nz)
+    w.Ms = 8.6e5 * wl.random_mask(33, nx, ny, nz, 0.8)
+    wl.cell_params(w, 77, kind=kind, Kc=-3e4)
+    if use in ("D", "H", "Kc"):
+        w.A_cell = None
+    if use in ("A", "H", "Kc"):
+        w.D_cell = None
+    if use not in ("H", "all"):
+        w.H_ext_cell = None
+    if use not in ("Kc", "all"):
+        w.Kc = 0.0
+    o = oracle.Oracle(nx, ny, nz, w.dx, w.dy, w.dz)
+    wl.apply(o, w, with_demag=False)
+    m = np.ascontiguousarray(w.m0 * (w.Ms > 0))
+    d = (w.dx, w.dy, w.dz)
+    u = np.array(w.axis) / np.linalg.norm(w.axis)
+    gp = w.gamma / (1 + w.alpha**2)
+    par = np.array([2 * (1.0 if w.A_cell is not None else w.A) / (MU0 * x * x) for x in d]
+                   + [(1.0 if w.D_cell is not None else w.D) / (MU0 * x) for x in d] + [2 * w.Ku / MU0] + list(u)
+                   + list(w.H_ext) + [gp, w.alpha * gp, 4 * w.Kc / MU0])
+    out = np.zeros(3 * w.N)
+    Msf = np.ascontiguousarray(w.Ms.reshape(-1))
+    ptr = lambda a: None if a is None else np.ascontiguousarray(a).ctypes.data_as(_dp)
+    arrs = [None if a is None else np.ascontiguousarray(a, dtype=np.float64) for a in (w.A_cell, w.D_cell, w.H_ext_cell)]
+    for torque, ref in ((0, o.effective_field(m)), (1, o.llg_rhs(m))):
+        emul.emul_local2(nx, ny, nz, par.ctypes.data_as(_dp), kind, 15 | 32, Msf.ctypes.data_as(_dp), m.ctypes.data_as(_dp),
+                         ptr(arrs[0]), ptr(arrs[1]), ptr(arrs[2]), torque, out.ctypes.data_as(_dp))
         assert np.abs(out.reshape(ref.shape) - ref).max() <= 1e-12 * np.abs(ref).max()
 
 
