@@ -12,7 +12,7 @@ from .build import build as _build
 _lib = None
 
 DMI_NONE, DMI_BULK, DMI_INTERFACIAL, DMI_D2D = 0, 1, 2, 3
-RK4, DOPRI5 = 0, 1
+RK4, DOPRI5, CAYLEY_RK4 = 0, 1, 2
 DEMAG_OFF, DEMAG_FFT, DEMAG_DIRECT = 0, 1, 2
 TERM_EXCHANGE, TERM_DMI, TERM_ANIS, TERM_ZEEMAN, TERM_DEMAG, TERM_CUBIC = 1, 2, 4, 8, 16, 32
 
@@ -58,6 +58,18 @@ def lib():
         L.mo_newell_point.argtypes = [C.c_double] * 6 + [_dp]
         L.mo_newell_tensor.argtypes = [C.c_int] * 3 + [C.c_double] * 3 + [_dp]
         L.mo_dopri5_tableau.argtypes = [_dp, _dp]
+        _up = C.POINTER(C.c_uint)
+        L.mo_philox4x32_10.argtypes = [_up, _up, _up]
+        L.mo_philox4x32_10.restype = None
+        L.mo_normals3.argtypes = [C.c_ulonglong, C.c_ulonglong, C.c_ulonglong, _dp]
+        L.mo_normals3.restype = None
+        L.mo_thermal_field.argtypes = [C.c_void_p, C.c_double, C.c_ulonglong, _dp]
+        L.mo_stt_tau.argtypes = [C.c_void_p, _dp, _dp]
+        L.mo_cayley_apply.argtypes = [_dp, _dp, _dp]
+        L.mo_cayley_apply.restype = None
+        L.mo_set_zhang_li.argtypes = [C.c_void_p] + [C.c_double] * 4
+        L.mo_set_slonczewski.argtypes = [C.c_void_p] + [C.c_double] * 5
+        L.mo_set_temperature.argtypes = [C.c_void_p, C.c_double, C.c_ulonglong]
         _lib = L
     return _lib
 
@@ -75,6 +87,26 @@ def _chk(rc, what):
 def newell_point(X, Y, Z, dx, dy, dz):
     out = np.zeros(6)
     lib().mo_newell_point(X, Y, Z, dx, dy, dz, _p(out))
+    return out
+
+
+def philox4x32_10(ctr, key):
+    c = (C.c_uint * 4)(*ctr)
+    k = (C.c_uint * 2)(*key)
+    o = (C.c_uint * 4)()
+    lib().mo_philox4x32_10(c, k, o)
+    return [int(v) for v in o]
+
+
+def normals3(seed, step, cell):
+    out = np.zeros(3)
+    lib().mo_normals3(seed, step, cell, _p(out))
+    return out
+
+
+def cayley_apply(w, m0):
+    out = np.zeros(3)
+    lib().mo_cayley_apply(_p(np.ascontiguousarray(w, dtype=np.float64)), _p(np.ascontiguousarray(m0, dtype=np.float64)), _p(out))
     return out
 
 
@@ -124,6 +156,9 @@ class Oracle:
     def set_A_cell(self, A): _chk(self.L.mo_set_A_cell(self.h, self._cell(A, self.N)), "set_A_cell")
     def set_D_cell(self, D, kind): _chk(self.L.mo_set_D_cell(self.h, self._cell(D, self.N), kind), "set_D_cell")
     def set_H_ext_cell(self, H): _chk(self.L.mo_set_H_ext_cell(self.h, self._cell(H, 3 * self.N)), "set_H_ext_cell")
+    def set_zhang_li(self, ux, uy, uz, beta): _chk(self.L.mo_set_zhang_li(self.h, ux, uy, uz, beta), "set_zhang_li")
+    def set_slonczewski(self, aJ, bJ, px, py, pz): _chk(self.L.mo_set_slonczewski(self.h, aJ, bJ, px, py, pz), "set_slonczewski")
+    def set_temperature(self, T, seed): _chk(self.L.mo_set_temperature(self.h, T, seed), "set_temperature")
     def set_axis(self, ux, uy, uz): _chk(self.L.mo_set_axis(self.h, ux, uy, uz), "set_axis")
     def set_H_ext(self, hx, hy, hz): _chk(self.L.mo_set_H_ext(self.h, hx, hy, hz), "set_H_ext")
     def set_alpha(self, a): _chk(self.L.mo_set_alpha(self.h, a), "set_alpha")
@@ -151,6 +186,17 @@ class Oracle:
         H = np.zeros_like(a)
         _chk(self.L.mo_field_terms(self.h, _p(a), _p(H), which), "field_terms")
         return H.reshape(3, self.nz, self.ny, self.nx)
+
+    def thermal_field(self, dt, step):
+        xi = np.zeros(3 * self.N)
+        _chk(self.L.mo_thermal_field(self.h, dt, step, _p(xi)), "thermal_field")
+        return xi.reshape(3, self.nz, self.ny, self.nx)
+
+    def stt_tau(self, m):
+        a = self._m(m)
+        t = np.zeros_like(a)
+        _chk(self.L.mo_stt_tau(self.h, _p(a), _p(t)), "stt_tau")
+        return t.reshape(3, self.nz, self.ny, self.nx)
 
     def llg_rhs(self, m):
         a = self._m(m)

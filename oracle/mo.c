@@ -24,6 +24,12 @@
  *   RK4 + projection  PAPER.md:425; Dormand-Prince + projection PAPER.md:298, ref [37]
  *   energy            Eq. 1, 2, 6/7, 10, 12 summed per cell
  *   mo_minimize       steepest descent with Barzilai-Borwein steps, Eq. 50-52
+ *   Zhang-Li torque   f_stt of Eq. 44's text with tau = (u.grad) m, PAPER.md:306-308 (Eq. 38), :345; sign of u as in
+ *                     Eq. 44 / Eq. 54 — Eq. 38 prints the opposite sign, R17
+ *   Slonczewski / SOT Eq. 40, solved for dm/dt (LL form)
+ *   thermal field     Eq. 41-42: one Gaussian vector per cell and step, held over the step's stages;
+ *                     normals from Philox4x32-10 + Box-Muller keyed by (seed, step, cell) (R18)
+ *   Cayley integrator Eq. 43-49: classical RK4 on omega (Eq. 49), restart (omega = 0) every step
  *
  * Layout: x fastest, idx = i + nx*(j + ny*k); vector fields are SoA, v[c*N + idx].
  * A neighbour is absent when outside the mesh or when its Ms is 0 (R4);
@@ -53,7 +59,14 @@ typedef struct mo_sim {
     double *Acell, *Dcell;      /* optional per-cell A_i, D_i (N each) or NULL: PAPER.md:120, 175 */
     double *Hcell;              /* optional per-cell external field (3N, SoA) or NULL: Eq. 35 with H_z,i */
     int dmi_kind;               /* 0 none, 1 bulk, 2 interfacial, 3 D2d */
-    int integrator;             /* 0 RK4, 1 DOPRI5 */
+    int integrator;             /* 0 RK4, 1 DOPRI5, 2 Cayley-transform RK4 (Eq. 49) */
+    double stt_u[3], stt_beta;  /* Zhang-Li: u in m/s (Eq. 39), beta */
+    int stt_on;
+    double sl_aJ, sl_bJ, sl_p[3]; /* Slonczewski / SOT (Eq. 40): a_J, b_J in 1/s, unit vector p */
+    int sl_on;
+    double temperature;         /* K; 0 = no thermal field */
+    unsigned long long th_seed, th_step;   /* Philox key / number of step attempts so far */
+    const double *Hth;          /* thermal field of the step in progress (3N) or NULL */
     int demag;                  /* 0 off, 1 FFT path, 2 direct O(N^2) sum */
     double *Nten;               /* 6 * N: xx,yy,zz,xy,xz,yz at offsets i>=0,j>=0,k>=0 */
     double *Khat;               /* 6 * P complex (interleaved) on the padded grid, or NULL */
@@ -460,13 +473,102 @@ int mo_field_terms(mo_sim *s, const double *m, double *H, int which)
 
 int mo_effective_field(mo_sim *s, const double *m, double *H) { return mo_field_terms(s, m, H, 63); }
 
-/* Eq. 37 */
+/* ------------------------------------------------------------------------------------
+ * Counter-based normals for the thermal field (R18): Philox4x32-10 (Salmon et al., SC'11: 10 rounds of
+ * two 32x32->64 multiplies with the constants below, key bumped by the Weyl constants between rounds) on
+ * counter = (cell lo, cell hi, step lo, step hi), key = (seed lo, seed hi); four 32-bit words x -> u = (x + 1/2) 2^-32
+ * in (0, 1); Box-Muller: (u0, u1) -> sqrt(-2 ln u0) (cos, sin)(2 pi u1) = (eta_x, eta_y), (u2, u3) -> eta_z (the sine
+ * of the second pair is not used).
+ * ---------------------------------------------------------------------------------- */
+void mo_philox4x32_10(const unsigned int ctr[4], const unsigned int key[2], unsigned int out[4])
+{
+    unsigned int c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3], k0 = key[0], k1 = key[1];
+    for (int r = 0; r < 10; r++) {
+        unsigned long long p0 = (unsigned long long)0xD2511F53u * c0, p1 = (unsigned long long)0xCD9E8D57u * c2;
+        unsigned int n0 = (unsigned int)(p1 >> 32) ^ c1 ^ k0, n1 = (unsigned int)p1;
+        unsigned int n2 = (unsigned int)(p0 >> 32) ^ c3 ^ k1, n3 = (unsigned int)p0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+void mo_normals3(unsigned long long seed, unsigned long long step, unsigned long long cell, double eta[3])
+{
+    const unsigned int ctr[4] = { (unsigned int)cell, (unsigned int)(cell >> 32), (unsigned int)step, (unsigned int)(step >> 32) };
+    const unsigned int key[2] = { (unsigned int)seed, (unsigned int)(seed >> 32) };
+    unsigned int x[4];
+    mo_philox4x32_10(ctr, key, x);
+    const double two_pi = 6.283185307179586476925286766559;
+    double u[4];
+    for (int i = 0; i < 4; i++) u[i] = ((double)x[i] + 0.5) * (1.0 / 4294967296.0);
+    const double r0 = sqrt(-2.0 * log(u[0])), r1 = sqrt(-2.0 * log(u[2]));
+    eta[0] = r0 * cos(two_pi * u[1]);
+    eta[1] = r0 * sin(two_pi * u[1]);
+    eta[2] = r1 * cos(two_pi * u[3]);
+}
+
+#define MO_KB 1.380649e-23
+
+/* Eq. 42: xi_i^u = eta sqrt(2 alpha kB T / (mu0 Ms_i gamma V dt)), V = cell volume; 0 where Ms = 0 */
+int mo_thermal_field(const mo_sim *s, double dt, unsigned long long step, double *xi)
+{
+    const long N = s->N;
+    const double V = s->dx * s->dy * s->dz;
+    for (long q = 0; q < N; q++) {
+        if (s->Ms[q] == 0.0 || !(s->temperature > 0.0)) { xi[q] = xi[N + q] = xi[2 * N + q] = 0.0; continue; }
+        double eta[3];
+        mo_normals3(s->th_seed, step, (unsigned long long)q, eta);
+        const double amp = sqrt(2.0 * s->alpha * MO_KB * s->temperature / (MO_MU0 * s->Ms[q] * s->gamma * V * dt));
+        for (int c = 0; c < 3; c++) xi[c * N + q] = eta[c] * amp;
+    }
+    return 0;
+}
+
+/* tau = (u . grad) m by central differences, tau_i = sum_a u_a (m_{i+a} - m_{i-a}) / (2 Delta_a); an absent
+ * neighbour (outside the mesh or Ms = 0) is replaced by the cell's own m (zero normal derivative, the free boundary
+ * of R4; the paper prints no discretisation: DESIGN.md R17) */
+int mo_stt_tau(const mo_sim *s, const double *m, double *tau)
+{
+    const int nx = s->nx, ny = s->ny, nz = s->nz;
+    const long N = s->N;
+    const double delta[3] = { s->dx, s->dy, s->dz };
+    for (int k = 0; k < nz; k++)
+        for (int j = 0; j < ny; j++)
+            for (int i = 0; i < nx; i++) {
+                long q = i + (long)nx * (j + (long)ny * k);
+                tau[q] = tau[N + q] = tau[2 * N + q] = 0.0;
+                if (s->Ms[q] == 0.0) continue;
+                const int pos[3] = { i, j, k }, lim[3] = { nx, ny, nz };
+                const long str[3] = { 1, nx, (long)nx * ny };
+                for (int a = 0; a < 3; a++) {
+                    long pm = q, pp = q;
+                    if (pos[a] > 0 && s->Ms[q - str[a]] != 0.0) pm = q - str[a];
+                    if (pos[a] < lim[a] - 1 && s->Ms[q + str[a]] != 0.0) pp = q + str[a];
+                    for (int c = 0; c < 3; c++) tau[c * N + q] += s->stt_u[a] * (m[c * N + pp] - m[c * N + pm]) / (2.0 * delta[a]);
+                }
+            }
+    return 0;
+}
+
+static void cross3(const double a[3], const double b[3], double c[3])
+{
+    c[0] = a[1] * b[2] - a[2] * b[1]; c[1] = a[2] * b[0] - a[0] * b[2]; c[2] = a[0] * b[1] - a[1] * b[0];
+}
+
+/* Eq. 37 with the thermal field of the step in progress added to H_eff, plus
+ *  - Zhang-Li: dm/dt += f_stt x m, f_stt = [(beta - alpha) tau + (1 + alpha beta) m x tau]/(1 + alpha^2)
+ *  - Slonczewski / SOT, Eq. 40: with T = -a_J m x (m x p) - b_J m x p the implicit equation
+ *    dm/dt = ... + alpha m x dm/dt + T solves to dm/dt += (T + alpha m x T)/(1 + alpha^2). */
 int mo_llg_rhs(mo_sim *s, const double *m, double *dmdt)
 {
     const long N = s->N;
     double *H = (double *)malloc(sizeof(double) * 3 * N);
     int rc = mo_effective_field(s, m, H);
     if (rc) { free(H); return rc; }
+    if (s->Hth) for (long q = 0; q < 3 * N; q++) H[q] += s->Hth[q];
+    double *tau = NULL;
+    if (s->stt_on) { tau = (double *)malloc(sizeof(double) * 3 * N); mo_stt_tau(s, m, tau); }
     const double gp = s->gamma / (1.0 + s->alpha * s->alpha), al = s->alpha;
     for (long q = 0; q < N; q++) {
         if (s->Ms[q] == 0.0) { dmdt[q] = dmdt[N + q] = dmdt[2 * N + q] = 0.0; continue; }
@@ -477,9 +579,146 @@ int mo_llg_rhs(mo_sim *s, const double *m, double *dmdt)
         dmdt[q] = -gp * ax - al * gp * bx;
         dmdt[N + q] = -gp * ay - al * gp * by;
         dmdt[2 * N + q] = -gp * az - al * gp * bz;
+        const double mv[3] = { mx, my, mz };
+        if (s->stt_on) {
+            const double t[3] = { tau[q], tau[N + q], tau[2 * N + q] };
+            double mt[3], f[3], fm[3];
+            cross3(mv, t, mt);
+            for (int c = 0; c < 3; c++) f[c] = ((s->stt_beta - al) * t[c] + (1.0 + al * s->stt_beta) * mt[c]) / (1.0 + al * al);
+            cross3(f, mv, fm);
+            for (int c = 0; c < 3; c++) dmdt[c * N + q] += fm[c];
+        }
+        if (s->sl_on) {
+            double mp[3], mmp[3], T[3], mT[3];
+            cross3(mv, s->sl_p, mp);
+            cross3(mv, mp, mmp);
+            for (int c = 0; c < 3; c++) T[c] = -s->sl_aJ * mmp[c] - s->sl_bJ * mp[c];
+            cross3(mv, T, mT);
+            for (int c = 0; c < 3; c++) dmdt[c * N + q] += (T[c] + al * mT[c]) / (1.0 + al * al);
+        }
     }
-    free(H);
+    free(H); free(tau);
     return 0;
+}
+
+/* ------------------------------------------------------------------------------------
+ * Cayley transform.  Eq. 47: Q = (I - Omega/2)^-1 (I + Omega/2), Omega = skew[omega] (Eq. 45);
+ * m = Q m0 (Eq. 43) by solving (I - Omega/2) x = (I + Omega/2) m0 with Cramer's rule.
+ * ---------------------------------------------------------------------------------- */
+void mo_cayley_apply(const double w[3], const double m0[3], double out[3])
+{
+    /* skew[w] = [[0,-w3,w2],[w3,0,-w1],[-w2,w1,0]] */
+    const double h[3] = { 0.5 * w[0], 0.5 * w[1], 0.5 * w[2] };
+    const double B[3][3] = { { 1, h[2], -h[1] }, { -h[2], 1, h[0] }, { h[1], -h[0], 1 } };      /* I - Omega/2 */
+    const double C[3][3] = { { 1, -h[2], h[1] }, { h[2], 1, -h[0] }, { -h[1], h[0], 1 } };      /* I + Omega/2 */
+    double r[3];
+    for (int i = 0; i < 3; i++) r[i] = C[i][0] * m0[0] + C[i][1] * m0[1] + C[i][2] * m0[2];
+    const double det = B[0][0] * (B[1][1] * B[2][2] - B[1][2] * B[2][1]) - B[0][1] * (B[1][0] * B[2][2] - B[1][2] * B[2][0])
+                     + B[0][2] * (B[1][0] * B[2][1] - B[1][1] * B[2][0]);
+    for (int c = 0; c < 3; c++) {
+        double M[3][3];
+        for (int i = 0; i < 3; i++) for (int j = 0; j < 3; j++) M[i][j] = j == c ? r[i] : B[i][j];
+        out[c] = (M[0][0] * (M[1][1] * M[2][2] - M[1][2] * M[2][1]) - M[0][1] * (M[1][0] * M[2][2] - M[1][2] * M[2][0])
+                  + M[0][2] * (M[1][0] * M[2][1] - M[1][1] * M[2][0])) / det;
+    }
+}
+
+/* f of Eq. 44 at the magnetisation mm: gamma (H + alpha m x H)/(1 + alpha^2) with H = H_eff (+ thermal field of the
+ * step) (+ the Slonczewski terms written as a field, (a_J/gamma) m x p + (b_J/gamma) p: "can be
+ * incorporated into the effective fields"), plus f_stt. */
+static int cayley_f(mo_sim *s, const double *mm, double *f)
+{
+    const long N = s->N;
+    double *H = (double *)malloc(sizeof(double) * 3 * N);
+    int rc = mo_effective_field(s, mm, H);
+    if (rc) { free(H); return rc; }
+    if (s->Hth) for (long q = 0; q < 3 * N; q++) H[q] += s->Hth[q];
+    double *tau = NULL;
+    if (s->stt_on) { tau = (double *)malloc(sizeof(double) * 3 * N); mo_stt_tau(s, mm, tau); }
+    const double al = s->alpha, den = 1.0 + al * al;
+    for (long q = 0; q < N; q++) {
+        if (s->Ms[q] == 0.0) { f[q] = f[N + q] = f[2 * N + q] = 0.0; continue; }
+        const double mv[3] = { mm[q], mm[N + q], mm[2 * N + q] };
+        double Hv[3] = { H[q], H[N + q], H[2 * N + q] }, mH[3];
+        if (s->sl_on) {
+            double mp[3];
+            cross3(mv, s->sl_p, mp);
+            for (int c = 0; c < 3; c++) Hv[c] += (s->sl_aJ * mp[c] + s->sl_bJ * s->sl_p[c]) / s->gamma;
+        }
+        cross3(mv, Hv, mH);
+        for (int c = 0; c < 3; c++) f[c * N + q] = s->gamma * (Hv[c] + al * mH[c]) / den;
+        if (s->stt_on) {
+            const double t[3] = { tau[q], tau[N + q], tau[2 * N + q] };
+            double mt[3];
+            cross3(mv, t, mt);
+            for (int c = 0; c < 3; c++) f[c * N + q] += ((s->stt_beta - al) * t[c] + (1.0 + al * s->stt_beta) * mt[c]) / den;
+        }
+    }
+    free(H); free(tau);
+    return 0;
+}
+
+/* d omega/dt of Eq. 49 at omega, for the step that started at m0: m = Q(omega) m0 (Eq. 43, 47), f = f(m) */
+static int cayley_rhs(mo_sim *s, const double *m0, const double *w, double *mm, double *f, double *dw)
+{
+    const long N = s->N;
+    for (long q = 0; q < N; q++) {
+        const double wv[3] = { w[q], w[N + q], w[2 * N + q] }, m0v[3] = { m0[q], m0[N + q], m0[2 * N + q] };
+        double o[3];
+        mo_cayley_apply(wv, m0v, o);
+        for (int c = 0; c < 3; c++) mm[c * N + q] = s->Ms[q] == 0.0 ? m0v[c] : o[c];
+    }
+    int rc = cayley_f(s, mm, f);
+    if (rc) return rc;
+    for (long q = 0; q < N; q++) {
+        const double wv[3] = { w[q], w[N + q], w[2 * N + q] }, fv[3] = { f[q], f[N + q], f[2 * N + q] };
+        double wf[3];
+        cross3(wv, fv, wf);
+        const double d = wv[0] * fv[0] + wv[1] * fv[1] + wv[2] * fv[2];
+        for (int c = 0; c < 3; c++) dw[c * N + q] = fv[c] - 0.5 * wf[c] + 0.25 * d * wv[c];
+    }
+    return 0;
+}
+
+/* One step of the Cayley-transform integrator: omega(0) = 0 (restart every step), classical RK4 on
+ * Eq. 49 over dt, m <- Q(omega(dt)) m.  No projection is applied: Q is a rotation.  max|dm/dt| = max_i |f_1 x m|. */
+static int cayley_step(mo_sim *s, double *m, double dt, double *max_dmdt)
+{
+    const long N = s->N, n3 = 3 * N;
+    double *k = (double *)malloc(sizeof(double) * n3 * 4), *w = (double *)calloc(n3, sizeof(double));
+    double *mm = (double *)malloc(sizeof(double) * n3), *f = (double *)malloc(sizeof(double) * n3);
+    int rc;
+    if ((rc = cayley_rhs(s, m, w, mm, f, k))) goto done;
+    if (max_dmdt) {
+        double mx = 0;
+        for (long q = 0; q < N; q++) {
+            if (s->Ms[q] == 0.0) continue;
+            const double fv[3] = { f[q], f[N + q], f[2 * N + q] }, mv[3] = { m[q], m[N + q], m[2 * N + q] };
+            double c[3];
+            cross3(fv, mv, c);
+            const double n = sqrt(c[0] * c[0] + c[1] * c[1] + c[2] * c[2]);
+            if (n > mx || n != n) mx = n;
+        }
+        *max_dmdt = mx;
+    }
+    for (long q = 0; q < n3; q++) w[q] = 0.5 * dt * k[q];
+    if ((rc = cayley_rhs(s, m, w, mm, f, k + n3))) goto done;
+    for (long q = 0; q < n3; q++) w[q] = 0.5 * dt * k[n3 + q];
+    if ((rc = cayley_rhs(s, m, w, mm, f, k + 2 * n3))) goto done;
+    for (long q = 0; q < n3; q++) w[q] = dt * k[2 * n3 + q];
+    if ((rc = cayley_rhs(s, m, w, mm, f, k + 3 * n3))) goto done;
+    for (long q = 0; q < n3; q++) w[q] = dt / 6.0 * (k[q] + 2 * k[n3 + q] + 2 * k[2 * n3 + q] + k[3 * n3 + q]);
+    for (long q = 0; q < N; q++) {
+        if (s->Ms[q] == 0.0) continue;
+        const double wv[3] = { w[q], w[N + q], w[2 * N + q] }, m0v[3] = { m[q], m[N + q], m[2 * N + q] };
+        double o[3];
+        mo_cayley_apply(wv, m0v, o);
+        for (int c = 0; c < 3; c++) m[c * N + q] = o[c];
+    }
+    s->t += dt;
+done:
+    free(k); free(w); free(mm); free(f);
+    return rc;
 }
 
 static void project(const mo_sim *s, double *m)
@@ -525,10 +764,17 @@ void mo_dopri5_tableau(double a[42], double e[7])
  * k1..k6, y5 = m + dt sum b5_j k_j, k7 = f(y5), E = dt sum e_j k_j, err = max_i |E_i|,
  * accept iff tol<=0 or err<=tol; on accept m <- y5/|y5|, t += dt;
  * dt_next = dt*clamp(0.9 (tol/err)^(1/5), 0.2, 5) (5 if err = 0); tol<=0: dt_next = dt. */
-int mo_step(mo_sim *s, double *m, double dt, double tol, int *accepted, double *err_out, double *dt_next, double *max_dmdt)
+static int step_inner(mo_sim *s, double *m, double dt, double tol, int *accepted, double *err_out, double *dt_next, double *max_dmdt)
 {
     const long N = s->N, n3 = 3 * N;
     int rc = 0;
+    if (s->integrator == 2) {
+        rc = cayley_step(s, m, dt, max_dmdt);
+        if (accepted) *accepted = 1;
+        if (err_out) *err_out = 0;
+        if (dt_next) *dt_next = dt;
+        return rc;
+    }
     if (s->integrator == 0) {
         double *k = (double *)malloc(sizeof(double) * n3 * 4), *y = (double *)malloc(sizeof(double) * n3);
         if ((rc = mo_llg_rhs(s, m, k))) goto done4;
@@ -585,6 +831,22 @@ int mo_step(mo_sim *s, double *m, double dt, double tol, int *accepted, double *
     }
 done5:
     free(k); free(y);
+    return rc;
+}
+
+/* The thermal field (Eq. 42) is drawn once per step attempt with that attempt's dt and held over its stages
+ * ("an effective field can be incorporated into existing integrators"). */
+int mo_step(mo_sim *s, double *m, double dt, double tol, int *accepted, double *err_out, double *dt_next, double *max_dmdt)
+{
+    double *xi = NULL;
+    if (s->temperature > 0.0) {
+        xi = (double *)malloc(sizeof(double) * 3 * s->N);
+        mo_thermal_field(s, dt, s->th_step, xi);
+        s->Hth = xi;
+    }
+    int rc = step_inner(s, m, dt, tol, accepted, err_out, dt_next, max_dmdt);
+    s->Hth = NULL;
+    if (xi) { s->th_step++; free(xi); }
     return rc;
 }
 
@@ -773,7 +1035,28 @@ int mo_set_axis(mo_sim *s, double ux, double uy, double uz)
 int mo_set_H_ext(mo_sim *s, double hx, double hy, double hz) { s->hx = hx; s->hy = hy; s->hz = hz; return 0; }
 int mo_set_alpha(mo_sim *s, double a) { s->alpha = a; return 0; }
 int mo_set_gamma(mo_sim *s, double g) { s->gamma = g; return 0; }
-int mo_set_integrator(mo_sim *s, int i) { if (i < 0 || i > 1) return -1; s->integrator = i; return 0; }
+int mo_set_integrator(mo_sim *s, int i) { if (i < 0 || i > 2) return -1; s->integrator = i; return 0; }
+int mo_set_zhang_li(mo_sim *s, double ux, double uy, double uz, double beta)
+{
+    s->stt_u[0] = ux; s->stt_u[1] = uy; s->stt_u[2] = uz; s->stt_beta = beta;
+    s->stt_on = (ux != 0.0 || uy != 0.0 || uz != 0.0);
+    return 0;
+}
+int mo_set_slonczewski(mo_sim *s, double aJ, double bJ, double px, double py, double pz)
+{
+    const double n = sqrt(px * px + py * py + pz * pz);
+    s->sl_on = (aJ != 0.0 || bJ != 0.0);
+    if (s->sl_on && !(n > 0)) return -1;
+    s->sl_aJ = aJ; s->sl_bJ = bJ;
+    s->sl_p[0] = n > 0 ? px / n : 0; s->sl_p[1] = n > 0 ? py / n : 0; s->sl_p[2] = n > 0 ? pz / n : 0;
+    return 0;
+}
+int mo_set_temperature(mo_sim *s, double T, unsigned long long seed)
+{
+    if (!(T >= 0.0)) return -1;
+    s->temperature = T; s->th_seed = seed; s->th_step = 0;
+    return 0;
+}
 /* 0 off, 1 FFT path, 2 direct O(N^2) */
 int mo_set_demag(mo_sim *s, int mode) { if (mode < 0 || mode > 2) return -1; s->demag = mode; return 0; }
 double mo_time(const mo_sim *s) { return s->t; }

@@ -24,3 +24,24 @@ def load_golden(name):
             k, v = line.split("=", 1)
             out[k.strip()] = [float(x) for x in v.split()]
     return out
+
+
+import contextlib
+import ctypes
+
+
+@contextlib.contextmanager
+def omp_threads(n):
+    """Run the oracle's OpenMP loops with n threads inside the block (tiny meshes stepped thousands of times spend
+    their time in thread wake-ups otherwise); restores the default afterwards."""
+    try:
+        gomp = ctypes.CDLL("libgomp.so.1")
+        old = gomp.omp_get_max_threads()
+        gomp.omp_set_num_threads(int(n))
+    except OSError:
+        gomp = None
+    try:
+        yield
+    finally:
+        if gomp is not None:
+            gomp.omp_set_num_threads(old)
