@@ -54,7 +54,9 @@ typedef enum {
 /* DMI vectors e_ij for the neighbours {-x,+x,-y,+y,-z,+z}: bulk r^_ij; interfacial z^ x r^_ij =
  * {-y^,+y^,+x^,-x^,0,0}; D2d {+x^,-x^,-y^,+y^,0,0} (Eq. 14). */
 typedef enum { MM_DMI_NONE = 0, MM_DMI_BULK = 1, MM_DMI_INTERFACIAL = 2, MM_DMI_D2D = 3 } mm_dmi_kind;
-typedef enum { MM_RK4 = 0, MM_DOPRI5 = 1 } mm_integrator;
+/* MM_CAYLEY_RK4: classical RK4 on omega of the Cayley transform (Eq. 43-49), omega restarted at 0
+ * every step, m <- Q(omega) m; fixed step, no projection (Q is a rotation). */
+typedef enum { MM_RK4 = 0, MM_DOPRI5 = 1, MM_CAYLEY_RK4 = 2 } mm_integrator;
 
 /* Create a problem on `device`, all later work on `cuda_stream` (a cudaStream_t; NULL = default
  * stream).  dx, dy, dz: cell edges in metres.  Defaults: Ms = 0 everywhere, A = D = Ku = 0, axis =
@@ -96,6 +98,21 @@ int mm_set_Kc(mm_sim* sim, double Kc);
 /* Per-cell external field (Eq. 35 with H_i): dev_H holds 3N reals (SoA, A/m), copied; NULL
  * switches back to the uniform mm_set_H_ext value. */
 int mm_set_H_ext_cell(mm_sim* sim, const void* dev_H);
+/* Zhang-Li spin-transfer torque: dm/dt += f_stt x m, f_stt = [(beta - alpha) tau + (1 + alpha beta)
+ * m x tau] / (1 + alpha^2), tau = (u . grad) m by central differences (a missing neighbour is replaced
+ * by the cell itself).  u in m/s (Eq. 39), uniform; (0,0,0) switches the term off.  Sign convention of Eq. 44 / Eq. 54
+ * (a head-to-head wall moves with -(1 + alpha beta) u / (1 + alpha^2)); Eq. 38 as printed has u -> -u (R17). */
+int mm_set_zhang_li(mm_sim* sim, double ux, double uy, double uz, double beta);
+/* Slonczewski / spin-orbit torque, Eq. 40: -a_J m x (m x p) - b_J m x p added to the Gilbert
+ * equation; a_J, b_J in 1/s, p normalised inside (zero p with non-zero a_J or b_J => MM_ERR_ARG). */
+int mm_set_slonczewski(mm_sim* sim, double a_J, double b_J, double px, double py, double pz);
+/* Thermal field, Eq. 41-42: xi = eta sqrt(2 alpha kB T / (mu0 Ms gamma V dt)) added to H_eff during
+ * mm_step / mm_relax / mm_run_until / mm_run_host, one Gaussian vector per cell and step attempt (held over the stages),
+ * eta from Philox4x32-10 + Box-Muller keyed by (seed, attempt counter, cell index) (R18).  Resets the
+ * attempt counter.  T = 0 switches it off.  mm_effective_field / mm_llg_rhs never include it.  Needs the workspace. */
+int mm_set_temperature(mm_sim* sim, double T_kelvin, unsigned long long seed);
+/* The thermal field a step of size dt with attempt counter `step` would use: 3N reals to dev_out (parity tests). */
+int mm_thermal_field(mm_sim* sim, double dt, unsigned long long step, void* dev_out);
 int mm_set_alpha(mm_sim* sim, double alpha);
 int mm_set_gamma(mm_sim* sim, double gamma);
 int mm_set_integrator(mm_sim* sim, mm_integrator integ);

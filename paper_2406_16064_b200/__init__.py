@@ -3,4 +3,4 @@
 `from paper_2406_16064_b200 import Sim` needs the CUDA library and a GPU and fails loudly without
 them; `paper_2406_16064_b200.workloads` (seeded inputs) is importable anywhere.
 """
-from .binding import Sim, MMError, load_library, F32, F64, RK4, DOPRI5, DMI_NONE, DMI_BULK, DMI_INTERFACIAL, DMI_D2D  # noqa: F401
+from .binding import Sim, MMError, load_library, F32, F64, RK4, DOPRI5, CAYLEY_RK4, DMI_NONE, DMI_BULK, DMI_INTERFACIAL, DMI_D2D  # noqa: F401

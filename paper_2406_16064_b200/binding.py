@@ -6,7 +6,7 @@ import ctypes as C
 import os
 
 F32, F64 = 0, 1
-RK4, DOPRI5 = 0, 1
+RK4, DOPRI5, CAYLEY_RK4 = 0, 1, 2
 DMI_NONE, DMI_BULK, DMI_INTERFACIAL, DMI_D2D = 0, 1, 2, 3
 _STATUS = {0: "MM_OK", -1: "MM_ERR_ARG", -2: "MM_ERR_UNSUPPORTED", -3: "MM_ERR_STATE", -4: "MM_ERR_CUDA",
            -5: "MM_ERR_NOMEM", -6: "MM_ERR_NAN", -7: "MM_ERR_INTERNAL"}
@@ -28,6 +28,10 @@ SIGNATURES = {
     "mm_set_D": (_i, [_vp, _d, _i]),
     "mm_set_Ku": (_i, [_vp, _d]),
     "mm_set_Kc": (_i, [_vp, _d]),
+    "mm_set_zhang_li": (_i, [_vp, _d, _d, _d, _d]),
+    "mm_set_slonczewski": (_i, [_vp, _d, _d, _d, _d, _d]),
+    "mm_set_temperature": (_i, [_vp, _d, C.c_ulonglong]),
+    "mm_thermal_field": (_i, [_vp, _d, C.c_ulonglong, _vp]),
     "mm_set_A_cell": (_i, [_vp, _vp]),
     "mm_set_D_cell": (_i, [_vp, _vp, _i]),
     "mm_set_H_ext_cell": (_i, [_vp, _vp]),
@@ -137,6 +141,14 @@ class Sim:
     def set_D(self, D, kind): self._chk(self.L.mm_set_D(self.h, D, kind), "mm_set_D")
     def set_Ku(self, Ku): self._chk(self.L.mm_set_Ku(self.h, Ku), "mm_set_Ku")
     def set_Kc(self, Kc): self._chk(self.L.mm_set_Kc(self.h, Kc), "mm_set_Kc")
+    def set_zhang_li(self, ux, uy, uz, beta): self._chk(self.L.mm_set_zhang_li(self.h, ux, uy, uz, beta), "mm_set_zhang_li")
+    def set_slonczewski(self, aJ, bJ, px, py, pz): self._chk(self.L.mm_set_slonczewski(self.h, aJ, bJ, px, py, pz), "mm_set_slonczewski")
+    def set_temperature(self, T, seed): self._chk(self.L.mm_set_temperature(self.h, T, seed), "mm_set_temperature")
+
+    def thermal_field(self, dt, step):
+        out = self.empty_field()
+        self._chk(self.L.mm_thermal_field(self.h, dt, step, self._dev(out, 3 * self.N)), "mm_thermal_field")
+        return out
 
     def _cell(self, a, n):
         """Device pointer of a per-cell array (numpy or tensor, copied by the library), or NULL for None."""

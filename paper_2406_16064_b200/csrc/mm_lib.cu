@@ -42,6 +42,7 @@ struct DevState {
     unsigned long long err_bits, maxk_bits;
     int accepted, done, nan, mode;     // mode: 0 single step, 1 relax, 2 run_until
     long long nacc, nrej, nsteps;
+    unsigned long long th_step;        // thermal field: step attempts since mm_set_temperature (Philox counter word)
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -115,6 +116,7 @@ template <typename T> struct StageArgs {
     T* ynext;             // next stage input (or the RK4 solution); may be NULL
     T coef[7];            // ynext = m0 + dt * sum_{j<=s} coef[j] k_j
     T ecoef[7];           // E = dt * sum_{j<=s} ecoef[j] k_j   (do_err)
+    T wcoef[7];           // Cayley (MODE 2): omega of THIS stage = dt * sum_{j<s} wcoef[j] k_j, k_j = d omega/dt of stage j
     int s;                // index of this stage
     int do_err, do_maxk;
 };
@@ -160,8 +162,29 @@ __device__ __forceinline__ void warp_max_bits(unsigned long long v, unsigned lon
     if ((threadIdx.x & 31) == 0 && v != 0ull && v > *reinterpret_cast<volatile unsigned long long*>(dst)) atomicMax(dst, v);
 }
 
-// MODE 0: out = H_eff ; MODE 1: out = k = LL torque, then the RK stage algebra selected at compile
-// time: S earlier stages, NEXT (write the next stage input), ERR (embedded error norm), MAXK (max |k|).
+// From the total field h of a cell (every H_eff term, plus the thermal field during a step) to the stage's output:
+// MODE 0 the field itself; MODE 1 dm/dt = Eq. 37 with the Slonczewski terms folded into the field (Eq. 40,
+// PAPER.md:319) plus f_stt x m; MODE 2 d omega/dt of Eq. 49 at omega = w with f of Eq. 44.
+// *kn = |dm/dt| when want_kn (MODE 2; MODE 1 takes it from the result).
+template <typename T, int MODE>
+__device__ __forceinline__ v3<T> stage_result(const LocalP<T>& lp, v3<T> mi, v3<T> h, v3<T> tau, v3<T> w, bool want_kn, T* kn)
+{
+    if (MODE == 0) return h;
+    if (lp.sl_on) h = add_slonczewski<T>(lp, mi, h);
+    if (MODE == 1) {
+        v3<T> r = ll_torque<T>(lp, mi, h);
+        if (lp.stt_on) { const v3<T> c = cross<T>(stt_f<T>(lp, mi, tau), mi); r.x += c.x; r.y += c.y; r.z += c.z; }
+        return r;
+    }
+    v3<T> f = llg_f<T>(lp, mi, h);
+    if (lp.stt_on) { const v3<T> fs = stt_f<T>(lp, mi, tau); f.x += fs.x; f.y += fs.y; f.z += fs.z; }
+    if (want_kn) { const v3<T> c = cross<T>(f, mi); *kn = sqrt(c.x * c.x + c.y * c.y + c.z * c.z); }
+    return cayley_domega<T>(w, f);
+}
+
+// MODE 0: out = H_eff ; MODE 1: out = k = LL torque ; MODE 2: out = d omega/dt (Cayley form, Eq. 49); then the RK
+// stage algebra selected at compile time: S earlier stages, NEXT (write the next stage input: m0 + dt sum a k, or
+// Q(dt sum a k) m0 in MODE 2), ERR (embedded error norm), MAXK (max |dm/dt|).
 // One thread per cell; indices by shifts (all mesh sizes are powers of two).
 template <typename T, int MODE, int S, bool NEXT, bool ERR, bool MAXK>
 __global__ void __launch_bounds__(256) llg_stage_kernel(Geom g, LocalP<T> lp, const T* __restrict__ y, const T* __restrict__ Ms,
@@ -183,17 +206,32 @@ __global__ void __launch_bounds__(256) llg_stage_kernel(Geom g, LocalP<T> lp, co
         for (int jj = 0; jj < S; jj++) kj[jj] = ld3(sa.kprev[jj], N, q);
         v3<T> m0 = { 0, 0, 0 };
         if (NEXT) m0 = ld3(sa.m0, N, q);
-        H = local_field<T>(g, lp, y, Ms, i, j, k, q, live ? Msi : (T)1, mi, H);
-        v3<T> res = MODE == 0 ? H : ll_torque<T>(lp, mi, H);
+        v3<T> tau = { 0, 0, 0 };
+        H = local_field<T>(g, lp, y, Ms, i, j, k, q, live ? Msi : (T)1, mi, H, MODE == 0 ? nullptr : &tau);
+        v3<T> w = { 0, 0, 0 };
+        if (MODE == 2) {
+            const T dtw = (T)st->dt;
+#pragma unroll
+            for (int jj = 0; jj < S; jj++) { w.x += sa.wcoef[jj] * kj[jj].x; w.y += sa.wcoef[jj] * kj[jj].y; w.z += sa.wcoef[jj] * kj[jj].z; }
+            w.x *= dtw; w.y *= dtw; w.z *= dtw;
+        }
+        T kn2 = 0;
+        v3<T> res = stage_result<T, MODE>(lp, mi, H, tau, w, MAXK, &kn2);
         if (!live) { res.x = 0; res.y = 0; res.z = 0; }
         out[q] = res.x; out[N + q] = res.y; out[2 * N + q] = res.z;
-        if (MODE == 1 && (NEXT || ERR)) {
+        if (MODE >= 1 && (NEXT || ERR)) {
             const T dt = (T)st->dt;
             if (NEXT) {
                 v3<T> acc = { sa.coef[S] * res.x, sa.coef[S] * res.y, sa.coef[S] * res.z };
 #pragma unroll
                 for (int jj = 0; jj < S; jj++) { acc.x += sa.coef[jj] * kj[jj].x; acc.y += sa.coef[jj] * kj[jj].y; acc.z += sa.coef[jj] * kj[jj].z; }
-                sa.ynext[q] = m0.x + dt * acc.x; sa.ynext[N + q] = m0.y + dt * acc.y; sa.ynext[2 * N + q] = m0.z + dt * acc.z;
+                if (MODE == 2) {
+                    const v3<T> wn = { dt * acc.x, dt * acc.y, dt * acc.z };
+                    const v3<T> yn = cayley_apply<T>(wn, m0);
+                    sa.ynext[q] = yn.x; sa.ynext[N + q] = yn.y; sa.ynext[2 * N + q] = yn.z;
+                } else {
+                    sa.ynext[q] = m0.x + dt * acc.x; sa.ynext[N + q] = m0.y + dt * acc.y; sa.ynext[2 * N + q] = m0.z + dt * acc.z;
+                }
             }
             if (ERR) {
                 v3<T> ea = { sa.ecoef[S] * res.x, sa.ecoef[S] * res.y, sa.ecoef[S] * res.z };
@@ -203,9 +241,10 @@ __global__ void __launch_bounds__(256) llg_stage_kernel(Geom g, LocalP<T> lp, co
             }
         }
         if (MODE == 1 && MAXK && live) kn = sqrt(res.x * res.x + res.y * res.y + res.z * res.z);
+        if (MODE == 2 && MAXK && live) kn = kn2;
     }
     if (MODE == 1 && ERR) block_max_bits(norm_bits(errn), &st->err_bits);
-    if (MODE == 1 && MAXK) block_max_bits(norm_bits(kn), &st->maxk_bits);
+    if (MODE >= 1 && MAXK) block_max_bits(norm_bits(kn), &st->maxk_bits);
 }
 
 // Neighbour-presence mask, one byte per cell: bit 0..5 = the -x +x -y +y -z +z neighbour is inside the mesh
@@ -289,7 +328,18 @@ __global__ void __launch_bounds__(MM_STAGEV_THREADS, sizeof(T) == 8 ? 1 : (GEN ?
 #pragma unroll
                 for (int e = 0; e < CPT; e++) hx[c].e[e] = lp.hext[c];
         }
-        if ((lp.terms & 3) != 0) {
+        if (GEN && lp.Hth != nullptr) {      // thermal field of the step in progress (Eq. 42)
+#pragma unroll
+            for (int c = 0; c < 3; c++) {
+                const CV t = ldc<T, CPT>(lp.Hth + c * N + q);
+#pragma unroll
+                for (int e = 0; e < CPT; e++) H[c].e[e] += t.e[e];
+            }
+        }
+        v3<T> tau[CPT];
+#pragma unroll
+        for (int e = 0; e < CPT; e++) tau[e] = { 0, 0, 0 };
+        if ((lp.terms & 3) != 0 || (GEN && MODE >= 1 && lp.stt_on)) {
             // neighbour rows: index clamped to the own row when outside the mesh, then masked
             const long sy = g.nx, szz = (long)g.nx * g.ny;
             const bool oym = j > 0, oyp = j < g.ny - 1, ozm = k > 0, ozp = k < g.nz - 1, oxm = i0 > 0, oxp = i0 + CPT < g.nx;
@@ -360,11 +410,13 @@ __global__ void __launch_bounds__(MM_STAGEV_THREADS, sizeof(T) == 8 ? 1 : (GEN ?
                 if (all_present) {      // interior of the magnetic region: no masking arithmetic at all
                     const bool ok[6] = { true, true, true, true, true, true };
                     h = local_field_nb<T, GEN>(lp, inv, mi, nb, ok, h, he, w[0], w[1]);
+                    if (GEN && MODE >= 1 && lp.stt_on) tau[e] = stt_tau<T>(lp, mi, nb, ok);
                 } else {
                     bool ok[6];
 #pragma unroll
                     for (int b = 0; b < 6; b++) ok[b] = (mk >> (8 * e + b)) & 1u;
                     h = local_field_nb<T, GEN>(lp, inv, mi, nb, ok, h, he, w[0], w[1]);
+                    if (GEN && MODE >= 1 && lp.stt_on) tau[e] = stt_tau<T>(lp, mi, nb, ok);
                 }
                 H[0].e[e] = h.x; H[1].e[e] = h.y; H[2].e[e] = h.z;
             }
@@ -386,28 +438,51 @@ __global__ void __launch_bounds__(MM_STAGEV_THREADS, sizeof(T) == 8 ? 1 : (GEN ?
             const bool live = Msv.e[e] != (T)0;
             const v3<T> mi = { m[0].e[e], m[1].e[e], m[2].e[e] };
             const v3<T> h = { H[0].e[e], H[1].e[e], H[2].e[e] };
-            v3<T> r = MODE == 0 ? h : ll_torque<T>(lp, mi, h);
+            v3<T> r;
+            T kn2 = 0;
+            if (GEN) {
+                v3<T> w = { 0, 0, 0 };
+                if (MODE == 2) {
+                    const T dtw = (T)st->dt;
+#pragma unroll
+                    for (int jj = 0; jj < S; jj++) { w.x += sa.wcoef[jj] * kj[jj][0].e[e]; w.y += sa.wcoef[jj] * kj[jj][1].e[e]; w.z += sa.wcoef[jj] * kj[jj][2].e[e]; }
+                    w.x *= dtw; w.y *= dtw; w.z *= dtw;
+                }
+                r = stage_result<T, MODE>(lp, mi, h, tau[e], w, MAXK, &kn2);
+            } else {
+                r = MODE == 0 ? h : ll_torque<T>(lp, mi, h);
+            }
             if (!live) { r.x = 0; r.y = 0; r.z = 0; }
             res[0].e[e] = r.x; res[1].e[e] = r.y; res[2].e[e] = r.z;
             if (MODE == 1 && MAXK && live) { const unsigned long long b = norm_bits(sqrt(r.x * r.x + r.y * r.y + r.z * r.z)); kb = b > kb ? b : kb; }
+            if (MODE == 2 && MAXK && live) { const unsigned long long b = norm_bits(kn2); kb = b > kb ? b : kb; }
         }
 #pragma unroll
         for (int c = 0; c < 3; c++) stc<T, CPT>(out + c * N + q, res[c]);
-        if (MODE == 1 && (NEXT || ERR)) {
+        if (MODE >= 1 && (NEXT || ERR)) {
             const T dt = (T)st->dt;
             if (NEXT) {
+                CV yn[3];
 #pragma unroll
                 for (int c = 0; c < 3; c++) {
-                    CV yn;
 #pragma unroll
                     for (int e = 0; e < CPT; e++) {
                         T acc = sa.coef[S] * res[c].e[e];
 #pragma unroll
                         for (int jj = 0; jj < S; jj++) acc += sa.coef[jj] * kj[jj][c].e[e];
-                        yn.e[e] = m0[c].e[e] + dt * acc;
+                        yn[c].e[e] = MODE == 2 ? dt * acc : m0[c].e[e] + dt * acc;
                     }
-                    stc<T, CPT>(sa.ynext + c * N + q, yn);
                 }
+                if (MODE == 2) {      // next stage input Q(omega) m0 (Eq. 43, 47)
+#pragma unroll
+                    for (int e = 0; e < CPT; e++) {
+                        const v3<T> wn = { yn[0].e[e], yn[1].e[e], yn[2].e[e] }, mm0 = { m0[0].e[e], m0[1].e[e], m0[2].e[e] };
+                        const v3<T> o = cayley_apply<T>(wn, mm0);
+                        yn[0].e[e] = o.x; yn[1].e[e] = o.y; yn[2].e[e] = o.z;
+                    }
+                }
+#pragma unroll
+                for (int c = 0; c < 3; c++) stc<T, CPT>(sa.ynext + c * N + q, yn[c]);
             }
             if (ERR) {
 #pragma unroll
@@ -428,13 +503,14 @@ __global__ void __launch_bounds__(MM_STAGEV_THREADS, sizeof(T) == 8 ? 1 : (GEN ?
         }
     }
     if (MODE == 1 && ERR) warp_max_bits(eb, &st->err_bits);
-    if (MODE == 1 && MAXK) warp_max_bits(kb, &st->maxk_bits);
+    if (MODE >= 1 && MAXK) warp_max_bits(kb, &st->maxk_bits);
 }
 
 // Step controller: one thread.  DESIGN.md R8.
-__global__ void ctrl_kernel(DevState* st, int is_f64, int adaptive_mode)
+__global__ void ctrl_kernel(DevState* st, int is_f64, int adaptive_mode, int thermal)
 {
     if (st->done) return;
+    if (thermal) st->th_step++;
     double err, maxk;
     if (is_f64) { err = __longlong_as_double((long long)st->err_bits); maxk = __longlong_as_double((long long)st->maxk_bits); }
     else { err = (double)__uint_as_float((unsigned)st->err_bits); maxk = (double)__uint_as_float((unsigned)st->maxk_bits); }
@@ -466,13 +542,13 @@ __global__ void ctrl_kernel(DevState* st, int is_f64, int adaptive_mode)
 
 // On acceptance: m <- y / |y| on cells with Ms > 0 (projection)
 template <typename T>
-__global__ void __launch_bounds__(256) accept_kernel(long N, const DevState* st, const T* __restrict__ ysol, const T* __restrict__ Ms, T* __restrict__ m)
+__global__ void __launch_bounds__(256) accept_kernel(long N, const DevState* st, const T* __restrict__ ysol, const T* __restrict__ Ms, T* __restrict__ m, int project)
 {
     if (!st->accepted) return;
     const long q = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (q >= N || Ms[q] == (T)0) return;
     const T x = ysol[q], y = ysol[N + q], z = ysol[2 * N + q];
-    const T n = sqrt(x * x + y * y + z * z);
+    const T n = project ? sqrt(x * x + y * y + z * z) : (T)1;      // Cayley steps are rotations: no projection
     m[q] = x / n; m[N + q] = y / n; m[2 * N + q] = z / n;
 }
 
@@ -613,6 +689,50 @@ __global__ void __launch_bounds__(256) sd_update_kernel(long N, T* __restrict__ 
 // separate launch: every block of sd_update_kernel must have read ms->iter-independent state before it moves on
 __global__ void sd_count_kernel(MinState* ms) { if (!ms->done) ms->iter++; }
 
+// ------------------------------------------------------------------------------------------------
+// Thermal field, Eq. 41-42: xi = eta sqrt(2 alpha kB T / (mu0 Ms gamma V dt)), one Gaussian vector
+// per cell and step attempt.  eta: Philox4x32-10 on counter (cell lo, cell hi, step lo, step hi), key (seed lo, seed hi);
+// the four words x -> u = (x + 1/2) 2^-32; Box-Muller (R18).  Generated in fp64 for both precisions (once
+// per step, 3N values), rounded once to the handle's precision.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void philox4x32_10(unsigned c0, unsigned c1, unsigned c2, unsigned c3, unsigned k0, unsigned k1, unsigned out[4])
+{
+#pragma unroll
+    for (int r = 0; r < 10; r++) {
+        const unsigned lo0 = 0xD2511F53u * c0, hi0 = __umulhi(0xD2511F53u, c0);
+        const unsigned lo1 = 0xCD9E8D57u * c2, hi1 = __umulhi(0xCD9E8D57u, c2);
+        c0 = hi1 ^ c1 ^ k0; c1 = lo1; c2 = hi0 ^ c3 ^ k1; c3 = lo0;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// amp2 = 2 alpha kB T / (mu0 gamma V); dt and step < 0: taken from the device controller (the step in progress)
+template <typename T>
+__global__ void __launch_bounds__(256) thermal_kernel(long N, const T* __restrict__ Ms, double amp2, unsigned long long seed, double dt_arg, long long step_arg,
+                                                      const DevState* st, T* __restrict__ xi)
+{
+    if (step_arg < 0 && st->done) return;
+    const long q = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= N) return;
+    const double Msi = (double)Ms[q];
+    double e0 = 0, e1 = 0, e2 = 0;
+    if (Msi != 0.0 && amp2 > 0.0) {
+        const double dt = step_arg < 0 ? st->dt : dt_arg;
+        const unsigned long long step = step_arg < 0 ? st->th_step : (unsigned long long)step_arg;
+        unsigned x[4];
+        philox4x32_10((unsigned)q, (unsigned)((unsigned long long)q >> 32), (unsigned)step, (unsigned)(step >> 32), (unsigned)seed, (unsigned)(seed >> 32), x);
+        const double two_pi = 6.283185307179586476925286766559, sc = 1.0 / 4294967296.0;
+        const double u0 = ((double)x[0] + 0.5) * sc, u1 = ((double)x[1] + 0.5) * sc, u2 = ((double)x[2] + 0.5) * sc, u3 = ((double)x[3] + 0.5) * sc;
+        const double r0 = sqrt(-2.0 * log(u0)), r1 = sqrt(-2.0 * log(u2));
+        double sn, cs;
+        sincos(two_pi * u1, &sn, &cs);
+        const double amp = sqrt(amp2 / (Msi * dt));
+        e0 = r0 * cs * amp; e1 = r0 * sn * amp; e2 = r1 * cos(two_pi * u3) * amp;
+    }
+    xi[q] = (T)e0; xi[N + q] = (T)e1; xi[2 * N + q] = (T)e2;
+}
+
 template <typename T> __global__ void fill_kernel(long n, T* p, T v)
 {
     const long q = (long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -748,10 +868,12 @@ struct mm_sim {
     double A, D, Ku, Kc, u[3], hext[3], alpha, gamma;
     int dmi_kind, integ, demag_on, demag_ready, Ms_set;
     int A_cell, D_cell, H_cell;      // cell-based A / D / external field set (arrays in the workspace)
+    double stt_u[3], stt_beta, sl_aJ, sl_bJ, sl_p[3], temperature;      // Zhang-Li, Slonczewski / SOT, thermal field
+    unsigned long long th_seed;
     // workspace
     void* ws;
     size_t ws_bytes, ws_need;
-    size_t off_Ms, off_nbm, off_S, off_Kh, off_Kc, off_mh, off_Hd, off_k[7], off_y[2], off_tw, off_st, off_part, off_min, off_Ac, off_Dc, off_Hc;
+    size_t off_Ms, off_nbm, off_S, off_Kh, off_Kc, off_mh, off_Hd, off_k[7], off_y[2], off_tw, off_st, off_part, off_min, off_Ac, off_Dc, off_Hc, off_Hth;
     int twN;
     size_t smemA, smemA2, smemB;
     int thrA, thrB;
@@ -889,6 +1011,7 @@ static void layout(mm_sim* s)
     s->off_Ac = take(N * es);          // cell-based A_i, D_i, H_ext,i (Eq. 35): 5N reals
     s->off_Dc = take(N * es);
     s->off_Hc = take(3 * N * es);
+    s->off_Hth = take(3 * N * es);     // thermal field of the step in progress (Eq. 42)
     s->ws_need = o;
 }
 
@@ -904,7 +1027,8 @@ extern "C" int mm_create(mm_sim** out, int nx, int ny, int nz, double dx, double
     mm_sim* s = new mm_sim();
     s->prec = prec; s->device = device; s->stream = static_cast<cudaStream_t>(cuda_stream);
     s->dx = dx; s->dy = dy; s->dz = dz;
-    s->A = s->D = s->Ku = s->Kc = 0; s->A_cell = s->D_cell = s->H_cell = 0; s->u[0] = s->u[1] = 0; s->u[2] = 1; s->hext[0] = s->hext[1] = s->hext[2] = 0;
+    s->A = s->D = s->Ku = s->Kc = 0; s->A_cell = s->D_cell = s->H_cell = 0;
+    s->stt_u[0] = s->stt_u[1] = s->stt_u[2] = s->stt_beta = 0; s->sl_aJ = s->sl_bJ = 0; s->sl_p[0] = s->sl_p[1] = 0; s->sl_p[2] = 1; s->temperature = 0; s->th_seed = 0; s->u[0] = s->u[1] = 0; s->u[2] = 1; s->hext[0] = s->hext[1] = s->hext[2] = 0;
     s->alpha = 0.5; s->gamma = 2.211e5; s->dmi_kind = 0; s->integ = MM_DOPRI5; s->demag_on = 1; s->demag_ready = 0; s->Ms_set = 0;
     s->ws = nullptr; s->ws_bytes = 0; s->khat_imag_ratio = -1; s->t_host = 0; s->launches = 0; s->prof_on = 0; s->prof_open = 0; s->prof_used = 0; s->use_v2 = getenv("MM_FORCE_V1") ? 0 : 1; s->no_b7 = getenv("MM_NO_B7") ? 1 : 0; s->no_stagev = getenv("MM_NO_STAGEV") ? 1 : 0;
     Geom& g = s->g;
@@ -1057,7 +1181,32 @@ extern "C" int mm_set_axis(mm_sim* s, double ux, double uy, double uz)
 extern "C" int mm_set_H_ext(mm_sim* s, double hx, double hy, double hz) { if (!s) return MM_ERR_ARG; s->hext[0] = hx; s->hext[1] = hy; s->hext[2] = hz; return MM_OK; }
 extern "C" int mm_set_alpha(mm_sim* s, double a) { if (!s || !(a >= 0)) return MM_ERR_ARG; s->alpha = a; return MM_OK; }
 extern "C" int mm_set_gamma(mm_sim* s, double g) { if (!s) return MM_ERR_ARG; s->gamma = g; return MM_OK; }
-extern "C" int mm_set_integrator(mm_sim* s, mm_integrator i) { if (!s || (i != MM_RK4 && i != MM_DOPRI5)) return MM_ERR_ARG; s->integ = i; return MM_OK; }
+extern "C" int mm_set_integrator(mm_sim* s, mm_integrator i) { if (!s || (i != MM_RK4 && i != MM_DOPRI5 && i != MM_CAYLEY_RK4)) return MM_ERR_ARG; s->integ = i; return MM_OK; }
+extern "C" int mm_set_zhang_li(mm_sim* s, double ux, double uy, double uz, double beta)
+{
+    if (!s) return MM_ERR_ARG;
+    s->stt_u[0] = ux; s->stt_u[1] = uy; s->stt_u[2] = uz; s->stt_beta = beta;
+    return MM_OK;
+}
+extern "C" int mm_set_slonczewski(mm_sim* s, double aJ, double bJ, double px, double py, double pz)
+{
+    if (!s) return MM_ERR_ARG;
+    const double n = sqrt(px * px + py * py + pz * pz);
+    if ((aJ != 0.0 || bJ != 0.0) && !(n > 0)) return fail(s, MM_ERR_ARG, "zero polarisation vector");
+    s->sl_aJ = aJ; s->sl_bJ = bJ;
+    if (n > 0) { s->sl_p[0] = px / n; s->sl_p[1] = py / n; s->sl_p[2] = pz / n; }
+    return MM_OK;
+}
+extern "C" int mm_set_temperature(mm_sim* s, double T, unsigned long long seed)
+{
+    NEED_WS(s);
+    if (!(T >= 0)) return MM_ERR_ARG;
+    s->temperature = T; s->th_seed = seed;
+    const unsigned long long zero = 0;
+    MM_TRY(s, cudaMemcpyAsync(reinterpret_cast<char*>(wsp<DevState>(s, s->off_st)) + offsetof(DevState, th_step), &zero, sizeof(zero), cudaMemcpyHostToDevice, s->stream));
+    MM_TRY(s, cudaStreamSynchronize(s->stream));
+    return MM_OK;
+}
 extern "C" int mm_set_demag(mm_sim* s, int on) { if (!s) return MM_ERR_ARG; s->demag_on = on ? 1 : 0; return MM_OK; }
 
 // ------------------------------------------------------------------------------------------------
@@ -1229,7 +1378,11 @@ extern "C" int mm_get_demag_kernel(mm_sim* s, int comp, void* dev_out)
 // ------------------------------------------------------------------------------------------------
 // Field / RHS evaluation
 // ------------------------------------------------------------------------------------------------
-template <typename T> static LocalP<T> make_local(const mm_sim* s, int terms)
+static const double KB = 1.380649e-23;      // J/K (exact, SI 2019)
+static bool thermal_on(const mm_sim* s) { return s->temperature > 0.0 && s->alpha > 0.0; }
+
+// in_step: the evaluation belongs to a time step (the thermal field of that step is part of the field)
+template <typename T> static LocalP<T> make_local(const mm_sim* s, int terms, bool in_step = false)
 {
     LocalP<T> lp;
     const double d[3] = { s->dx, s->dy, s->dz };
@@ -1244,6 +1397,13 @@ template <typename T> static LocalP<T> make_local(const mm_sim* s, int terms)
     lp.Hcell = s->H_cell ? wsp<T>(s, s->off_Hc) : (const T*)nullptr;
     lp.cku = (T)(2.0 * s->Ku / MU0);
     lp.ckc = (T)(4.0 * s->Kc / MU0);
+    lp.Hth = in_step && thermal_on(s) ? wsp<T>(s, s->off_Hth) : (const T*)nullptr;
+    for (int a = 0; a < 3; a++) { lp.stt[a] = (T)(s->stt_u[a] / (2.0 * d[a])); lp.p[a] = (T)s->sl_p[a]; }
+    lp.beta = (T)s->stt_beta;
+    lp.sl_a = (T)(s->sl_aJ / s->gamma); lp.sl_b = (T)(s->sl_bJ / s->gamma);
+    lp.gam = (T)s->gamma; lp.al = (T)s->alpha;
+    lp.stt_on = (s->stt_u[0] != 0.0 || s->stt_u[1] != 0.0 || s->stt_u[2] != 0.0) ? 1 : 0;
+    lp.sl_on = (s->sl_aJ != 0.0 || s->sl_bJ != 0.0) ? 1 : 0;
     lp.gp = (T)(s->gamma / (1.0 + s->alpha * s->alpha));
     lp.agp = (T)(s->alpha * s->gamma / (1.0 + s->alpha * s->alpha));
     lp.dmi = s->dmi_kind;
@@ -1384,17 +1544,18 @@ static void launch_stage(mm_sim* s, const LocalP<T>& lp, const T* y, const T* Hd
     constexpr int CPT = MM_STAGEV_CPT;
     if (s->g.nx % CPT == 0 && !s->no_stagev) {
         const unsigned blocks = (unsigned)((s->g.N / CPT + MM_STAGEV_THREADS - 1) / MM_STAGEV_THREADS);
-        if (lp.Acell != nullptr || lp.Dcell != nullptr)
+        // general form: cell-based A / D, thermal field, Zhang-Li / Slonczewski torques, Cayley stages
+        if (MODE == 2 || lp.Acell != nullptr || lp.Dcell != nullptr || lp.Hth != nullptr || lp.stt_on || lp.sl_on)
             llg_stagev_kernel<T, CPT, MODE, S, NEXT, ERR, MAXK, true><<<blocks, MM_STAGEV_THREADS, 0, s->stream>>>(s->g, lp, y, wsp<T>(s, s->off_Ms), wsp<unsigned char>(s, s->off_nbm), Hd, out, sa, wsp<DevState>(s, s->off_st));
-        else
-            llg_stagev_kernel<T, CPT, MODE, S, NEXT, ERR, MAXK, false><<<blocks, MM_STAGEV_THREADS, 0, s->stream>>>(s->g, lp, y, wsp<T>(s, s->off_Ms), wsp<unsigned char>(s, s->off_nbm), Hd, out, sa, wsp<DevState>(s, s->off_st));
+        else if (MODE != 2)
+            llg_stagev_kernel<T, CPT, MODE == 2 ? 1 : MODE, S, NEXT, ERR, MAXK, false><<<blocks, MM_STAGEV_THREADS, 0, s->stream>>>(s->g, lp, y, wsp<T>(s, s->off_Ms), wsp<unsigned char>(s, s->off_nbm), Hd, out, sa, wsp<DevState>(s, s->off_st));
         return;
     }
     const unsigned blocks = (unsigned)((s->g.N + 255) / 256);
     llg_stage_kernel<T, MODE, S, NEXT, ERR, MAXK><<<blocks, 256, 0, s->stream>>>(s->g, lp, y, wsp<T>(s, s->off_Ms), Hd, out, sa, wsp<DevState>(s, s->off_st));
 }
 
-template <typename T, int MODE> static int eval(mm_sim* s, const T* y, T* out, const StageArgs<T>& sa, int terms)
+template <typename T, int MODE> static int eval(mm_sim* s, const T* y, T* out, const StageArgs<T>& sa, int terms, bool in_step = false)
 {
     const bool demag = s->demag_on && (terms & 16);
     if (demag) {
@@ -1402,10 +1563,16 @@ template <typename T, int MODE> static int eval(mm_sim* s, const T* y, T* out, c
         int rc = demag_passes<T>(s, y);
         if (rc) return rc;
     }
-    const LocalP<T> lp = make_local<T>(s, terms);
+    const LocalP<T> lp = make_local<T>(s, terms, in_step);
     const T* Hd = demag ? wsp<T>(s, s->off_Hd) : (const T*)nullptr;
     prof_begin(s, 3);
-    if (MODE == 0) launch_stage<T, 0, 0, false, false, false>(s, lp, y, Hd, out, sa);
+    if (MODE == 2) switch (sa.s) {      // Cayley-transform RK4: d omega/dt stages (Eq. 49)
+        case 0: launch_stage<T, 2, 0, true, false, true>(s, lp, y, Hd, out, sa); break;
+        case 1: launch_stage<T, 2, 1, true, false, false>(s, lp, y, Hd, out, sa); break;
+        case 2: launch_stage<T, 2, 2, true, false, false>(s, lp, y, Hd, out, sa); break;
+        default: launch_stage<T, 2, 3, true, false, false>(s, lp, y, Hd, out, sa); break;
+    }
+    else if (MODE == 0) launch_stage<T, 0, 0, false, false, false>(s, lp, y, Hd, out, sa);
     else if (sa.do_err) launch_stage<T, 1, 6, false, true, false>(s, lp, y, Hd, out, sa);          // DOPRI5 stage 7
     else if (sa.ynext == nullptr) launch_stage<T, 1, 0, false, false, false>(s, lp, y, Hd, out, sa);
     else switch (sa.s) {
@@ -1459,6 +1626,21 @@ extern "C" int mm_llg_rhs(mm_sim* s, const void* dev_m, void* dev_dmdt)
     return eval<float, 1>(s, (const float*)dev_m, (float*)dev_dmdt, no_stage<float>(), ALL_TERMS);
 }
 
+extern "C" int mm_thermal_field(mm_sim* s, double dt, unsigned long long step, void* dev_out)
+{
+    NEED_READY(s);
+    if (!dev_out || !(dt > 0)) return MM_ERR_ARG;
+    const long N = s->g.N;
+    const double V = s->dx * s->dy * s->dz;
+    const double amp2 = thermal_on(s) ? 2.0 * s->alpha * KB * s->temperature / (MU0 * s->gamma * V) : 0.0;
+    const unsigned blocks = (unsigned)((N + 255) / 256);
+    if (s->prec == MM_F64) thermal_kernel<double><<<blocks, 256, 0, s->stream>>>(N, wsp<double>(s, s->off_Ms), amp2, s->th_seed, dt, (long long)step, wsp<DevState>(s, s->off_st), (double*)dev_out);
+    else thermal_kernel<float><<<blocks, 256, 0, s->stream>>>(N, wsp<float>(s, s->off_Ms), amp2, s->th_seed, dt, (long long)step, wsp<DevState>(s, s->off_st), (float*)dev_out);
+    s->launches++;
+    MM_TRY(s, cudaGetLastError());
+    return MM_OK;
+}
+
 // ------------------------------------------------------------------------------------------------
 // Time stepping (R8).  All kernels of a step are enqueued back to back; the accept /
 // reject decision and the next dt are taken on the device by ctrl_kernel.
@@ -1481,6 +1663,13 @@ template <typename T> static int enqueue_step(mm_sim* s, T* m, int ctrl_mode)
     for (int i = 0; i < 7; i++) k[i] = wsp<T>(s, s->off_k[i]);
     T* yb[2] = { wsp<T>(s, s->off_y[0]), wsp<T>(s, s->off_y[1]) };
     const int nst = s->integ == MM_DOPRI5 ? 7 : 4;
+    const bool thermal = thermal_on(s);
+    if (thermal) {      // Eq. 42: one field per step attempt, drawn with this attempt's dt, held over its stages
+        const double V = s->dx * s->dy * s->dz;
+        thermal_kernel<T><<<(unsigned)((N + 255) / 256), 256, 0, s->stream>>>(N, wsp<T>(s, s->off_Ms), 2.0 * s->alpha * KB * s->temperature / (MU0 * s->gamma * V),
+                                                                              s->th_seed, 0.0, -1, wsp<DevState>(s, s->off_st), wsp<T>(s, s->off_Hth));
+        s->launches++;
+    }
     for (int st = 0; st < nst; st++) {
         StageArgs<T> sa = no_stage<T>();
         sa.m0 = m; sa.s = st;
@@ -1490,17 +1679,19 @@ template <typename T> static int enqueue_step(mm_sim* s, T* m, int ctrl_mode)
             if (st < 6) { sa.ynext = yb[st & 1]; for (int j = 0; j <= st; j++) sa.coef[j] = (T)DP_A[st + 1][j]; }
             else { sa.ynext = nullptr; sa.do_err = 1; for (int j = 0; j < 7; j++) sa.ecoef[j] = (T)DP_E[j]; }
         } else {
+            // RK4 and Cayley-RK4 (k_j = d omega/dt there; omega of stage st = dt * RK4_A[st - 1] . k)
             sa.ynext = yb[st & 1];
             for (int j = 0; j <= st; j++) sa.coef[j] = (T)RK4_A[st][j];
+            if (st > 0) for (int j = 0; j < st; j++) sa.wcoef[j] = (T)RK4_A[st - 1][j];
         }
         const T* y = st == 0 ? m : yb[(st - 1) & 1];
-        int rc = eval<T, 1>(s, y, k[st], sa, ALL_TERMS);
+        int rc = s->integ == MM_CAYLEY_RK4 ? eval<T, 2>(s, y, k[st], sa, ALL_TERMS, true) : eval<T, 1>(s, y, k[st], sa, ALL_TERMS, true);
         if (rc) return rc;
     }
     DevState* ds = wsp<DevState>(s, s->off_st);
-    ctrl_kernel<<<1, 1, 0, s->stream>>>(ds, s->prec == MM_F64, ctrl_mode);
-    const T* ysol = yb[1];     // DOPRI5: y_6 written at stage 5 ; RK4: solution written at stage 3
-    accept_kernel<T><<<(unsigned)((N + 255) / 256), 256, 0, s->stream>>>(N, ds, ysol, wsp<T>(s, s->off_Ms), m);
+    ctrl_kernel<<<1, 1, 0, s->stream>>>(ds, s->prec == MM_F64, ctrl_mode, thermal ? 1 : 0);
+    const T* ysol = yb[1];     // DOPRI5: y_6 written at stage 5 ; RK4 / Cayley: solution written at stage 3
+    accept_kernel<T><<<(unsigned)((N + 255) / 256), 256, 0, s->stream>>>(N, ds, ysol, wsp<T>(s, s->off_Ms), m, s->integ == MM_CAYLEY_RK4 ? 0 : 1);
     s->launches += 2;
     MM_TRY(s, cudaGetLastError());
     return MM_OK;
@@ -1523,7 +1714,7 @@ extern "C" int mm_step(mm_sim* s, void* dev_m, double dt, double tol, int* accep
 {
     NEED_READY(s);
     if (!dev_m || !(dt > 0)) return MM_ERR_ARG;
-    int rc = set_state(s, dt, s->integ == MM_RK4 ? 0.0 : tol, 0, 0, 0, 1);
+    int rc = set_state(s, dt, s->integ == MM_DOPRI5 ? tol : 0.0, 0, 0, 0, 1);
     if (rc) return rc;
     if ((rc = enqueue_step_any(s, dev_m, 0))) return rc;
     if (accepted || err || dt_next || max_dmdt) {
@@ -1667,7 +1858,7 @@ extern "C" int mm_run_host(mm_sim* s, void* host_m, int nsteps, double dt, doubl
     // m lives in the workspace's own staging slot for the duration of the call
     void* dm = wsp<char>(s, s->off_mh);
     MM_TRY(s, cudaMemcpyAsync(dm, host_m, bytes, cudaMemcpyHostToDevice, s->stream));
-    int rc = set_state(s, dt, s->integ == MM_RK4 ? 0.0 : tol, 0, 0, 0, 1);
+    int rc = set_state(s, dt, s->integ == MM_DOPRI5 ? tol : 0.0, 0, 0, 0, 1);
     for (int i = 0; i < nsteps && !rc; i++) rc = enqueue_step_any(s, dm, 0);
     if (!rc) {
         cudaError_t e = cudaMemcpyAsync(host_m, dm, bytes, cudaMemcpyDeviceToHost, s->stream);

@@ -25,6 +25,14 @@ template <typename T> struct LocalP {
     const T* Acell;   // N per-cell exchange constants or nullptr (uniform A)
     const T* Dcell;   // N per-cell DMI constants or nullptr (uniform D)
     const T* Hcell;   // 3N per-cell external field (SoA) or nullptr (uniform hext)
+    // torque extensions and thermal field (general kernels only)
+    const T* Hth;     // 3N thermal field of the step in progress (Eq. 42) or nullptr
+    T stt[3];         // Zhang-Li: u_a / (2 Delta_a)  (central differences of (u.grad) m)
+    T beta;           // Zhang-Li non-adiabaticity
+    T sl_a, sl_b;     // Slonczewski / SOT written as a field: a_J / gamma, b_J / gamma
+    T p[3];           // unit polarisation vector
+    T gam, al;        // gamma, alpha (f of Eq. 44 and f_stt need them separately)
+    int stt_on, sl_on;
 };
 
 // bond value of a cell-based constant: harmonic mean, 0 when both vanish
@@ -56,6 +64,68 @@ template <typename T> MM_HD v3<T> local_field_rest(const LocalP<T>& lp, T inv, v
 // H_eff from the six neighbour values nb[-x,+x,-y,+y,-z,+z] (ok[] = neighbour present) added to H
 // GEN: cell-based A and / or D — wA[b], wD[b] are the bond values A_ij, D_ij towards neighbour b (1 for a constant
 // that is uniform: it is then inside cex / cdm).
+template <typename T> MM_HD v3<T> cross(v3<T> a, v3<T> b)
+{
+    v3<T> c = { a.y * b.z - a.z * b.y, a.z * b.x - a.x * b.z, a.x * b.y - a.y * b.x };
+    return c;
+}
+
+// tau = (u.grad) m by central differences; an absent neighbour is replaced by the cell itself (R17)
+template <typename T> MM_HD v3<T> stt_tau(const LocalP<T>& lp, v3<T> mi, const v3<T>* nb, const bool* ok)
+{
+    v3<T> t = { 0, 0, 0 };
+#pragma unroll
+    for (int a = 0; a < 3; a++) {
+        const v3<T> lo = ok[2 * a] ? nb[2 * a] : mi, hi = ok[2 * a + 1] ? nb[2 * a + 1] : mi;
+        t.x += lp.stt[a] * (hi.x - lo.x); t.y += lp.stt[a] * (hi.y - lo.y); t.z += lp.stt[a] * (hi.z - lo.z);
+    }
+    return t;
+}
+
+// f_stt = [(beta - alpha) tau + (1 + alpha beta) m x tau] / (1 + alpha^2)
+template <typename T> MM_HD v3<T> stt_f(const LocalP<T>& lp, v3<T> m, v3<T> tau)
+{
+    const v3<T> mt = cross<T>(m, tau);
+    const T den = (T)1 / ((T)1 + lp.al * lp.al), c1 = (lp.beta - lp.al) * den, c2 = ((T)1 + lp.al * lp.beta) * den;
+    v3<T> f = { c1 * tau.x + c2 * mt.x, c1 * tau.y + c2 * mt.y, c1 * tau.z + c2 * mt.z };
+    return f;
+}
+
+// Eq. 40 folded into the field: H + (a_J / gamma) m x p + (b_J / gamma) p
+template <typename T> MM_HD v3<T> add_slonczewski(const LocalP<T>& lp, v3<T> m, v3<T> H)
+{
+    const v3<T> p = { lp.p[0], lp.p[1], lp.p[2] };
+    const v3<T> mp = cross<T>(m, p);
+    H.x += lp.sl_a * mp.x + lp.sl_b * p.x; H.y += lp.sl_a * mp.y + lp.sl_b * p.y; H.z += lp.sl_a * mp.z + lp.sl_b * p.z;
+    return H;
+}
+
+// f of Eq. 44: gamma (H + alpha m x H) / (1 + alpha^2)
+template <typename T> MM_HD v3<T> llg_f(const LocalP<T>& lp, v3<T> m, v3<T> H)
+{
+    const v3<T> mH = cross<T>(m, H);
+    v3<T> f = { lp.gp * (H.x + lp.al * mH.x), lp.gp * (H.y + lp.al * mH.y), lp.gp * (H.z + lp.al * mH.z) };
+    return f;
+}
+
+// Eq. 49: d omega / dt = f - (omega x f) / 2 + (omega . f) omega / 4
+template <typename T> MM_HD v3<T> cayley_domega(v3<T> w, v3<T> f)
+{
+    const v3<T> wf = cross<T>(w, f);
+    const T d = (T)0.25 * (w.x * f.x + w.y * f.y + w.z * f.z);
+    v3<T> r = { f.x - (T)0.5 * wf.x + d * w.x, f.y - (T)0.5 * wf.y + d * w.y, f.z - (T)0.5 * wf.z + d * w.z };
+    return r;
+}
+
+// Eq. 43, 47 in closed vector form: Q(omega) m = m + (omega x m + omega x (omega x m) / 2) / (1 + |omega|^2 / 4)
+template <typename T> MM_HD v3<T> cayley_apply(v3<T> w, v3<T> m)
+{
+    const v3<T> wm = cross<T>(w, m), wwm = cross<T>(w, wm);
+    const T s = (T)1 / ((T)1 + (T)0.25 * (w.x * w.x + w.y * w.y + w.z * w.z));
+    v3<T> r = { m.x + s * (wm.x + (T)0.5 * wwm.x), m.y + s * (wm.y + (T)0.5 * wwm.y), m.z + s * (wm.z + (T)0.5 * wwm.z) };
+    return r;
+}
+
 template <typename T, bool GEN = false>
 MM_HD v3<T> local_field_nb(const LocalP<T>& lp, T inv, v3<T> mi, const v3<T>* nb, const bool* ok, v3<T> H, v3<T> hext,
                            const T* wA = nullptr, const T* wD = nullptr)
@@ -108,13 +178,18 @@ MM_HD v3<T> local_field_nb(const LocalP<T>& lp, T inv, v3<T> mi, const v3<T>* nb
 // so all loads of a thread are in flight together.
 template <typename T>
 MM_HD v3<T> local_field(const Geom& g, const LocalP<T>& lp, const T* __restrict__ y, const T* __restrict__ Ms,
-                        int i, int j, int k, long q, T Msi, v3<T> mi, v3<T> H)
+                        int i, int j, int k, long q, T Msi, v3<T> mi, v3<T> H, v3<T>* tau = nullptr)
 {
     const long N = g.N;
     const T inv = (T)1 / Msi;
     v3<T> hext = { lp.hext[0], lp.hext[1], lp.hext[2] };
     if (lp.Hcell != nullptr && (lp.terms & 8)) hext = ld3(lp.Hcell, N, q);
-    if ((lp.terms & 3) == 0) return local_field_rest<T>(lp, inv, mi, H, hext);
+    if (lp.Hth != nullptr) {      // thermal field of the step in progress: added whatever the term mask says
+        const v3<T> ht = ld3(lp.Hth, N, q);
+        H.x += ht.x; H.y += ht.y; H.z += ht.z;
+    }
+    if (tau != nullptr) { tau->x = 0; tau->y = 0; tau->z = 0; }
+    if ((lp.terms & 3) == 0 && !(lp.stt_on && tau != nullptr)) return local_field_rest<T>(lp, inv, mi, H, hext);
     const long str[3] = { 1, g.nx, (long)g.nx * g.ny };
     const int pos[3] = { i, j, k }, lim[3] = { g.nx, g.ny, g.nz };
     v3<T> nb[6];
@@ -136,6 +211,7 @@ MM_HD v3<T> local_field(const Geom& g, const LocalP<T>& lp, const T* __restrict_
             wD[2 * a + 1] = lp.Dcell ? harm<T>(lp.Dcell[q], lp.Dcell[pp]) : (T)1;
         }
     }
+    if (lp.stt_on && tau != nullptr) *tau = stt_tau<T>(lp, mi, nb, ok);
     if (gen) return local_field_nb<T, true>(lp, inv, mi, nb, ok, H, hext, wA, wD);
     return local_field_nb<T, false>(lp, inv, mi, nb, ok, H, hext);
 }

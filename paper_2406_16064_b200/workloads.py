@@ -12,7 +12,7 @@ import numpy as np
 
 MU0 = 4e-7 * np.pi
 DMI_NONE, DMI_BULK, DMI_INTERFACIAL, DMI_D2D = 0, 1, 2, 3
-RK4, DOPRI5 = 0, 1
+RK4, DOPRI5, CAYLEY_RK4 = 0, 1, 2
 
 
 @dataclass
