@@ -24,9 +24,11 @@
  *  - All work is enqueued on the CUDA stream given to mm_create and is asynchronous with respect
  *    to the host unless a non-NULL host out-parameter (or a host_* buffer) forces a
  *    synchronisation of that stream.
- *  - Supported meshes: nx, ny, nz powers of two (nz = 1 allowed: thin film); with demag enabled
- *    additionally nx >= 4, ny >= 2 and the per-CTA shared-memory tiles must fit (see
- *    DESIGN.md "Limits"); otherwise mm_init_demag returns MM_ERR_UNSUPPORTED.
+ *  - Meshes: any nx, ny, nz >= 1 (nz = 1: thin film).  The FFT passes are radix-2: a size that is not a power of two
+ *    is embedded in the next power of two with vacuum cells (the caller's arrays keep their own nx*ny*nz layout; the
+ *    library packs / unpacks at every call, two small kernels); powers of two take the direct path.  With demag
+ *    enabled the padded mesh needs nx >= 4, ny >= 2 and the per-CTA shared-memory tiles must fit (see DESIGN.md
+ *    "Limits"); otherwise mm_init_demag returns MM_ERR_UNSUPPORTED.
  */
 #ifndef MM_H
 #define MM_H

@@ -463,7 +463,9 @@ int mo_field_terms(mo_sim *s, const double *m, double *H, int which)
     memset(H, 0, sizeof(double) * 3 * N);
     if ((which & 16) && s->demag) {
         if (!s->Nten) return -3;
-        if (s->demag == 2) demag_direct(s, m, H); else demag_fft(s, m, H);
+        /* the own FFT is radix-2: meshes whose padded sizes are not powers of two take the defining direct sum */
+        const int pow2 = !(s->px & (s->px - 1)) && !(s->py & (s->py - 1)) && !(s->pz & (s->pz - 1));
+        if (s->demag == 2 || !pow2) demag_direct(s, m, H); else demag_fft(s, m, H);
         for (long q = 0; q < N; q++)
             if (s->Ms[q] == 0.0) H[q] = H[N + q] = H[2 * N + q] = 0.0;
     }

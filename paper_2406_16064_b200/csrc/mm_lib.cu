@@ -709,19 +709,22 @@ __device__ __forceinline__ void philox4x32_10(unsigned c0, unsigned c1, unsigned
 
 // amp2 = 2 alpha kB T / (mu0 gamma V); dt and step < 0: taken from the device controller (the step in progress)
 template <typename T>
-__global__ void __launch_bounds__(256) thermal_kernel(long N, const T* __restrict__ Ms, double amp2, unsigned long long seed, double dt_arg, long long step_arg,
+__global__ void __launch_bounds__(256) thermal_kernel(Geom g, int unx, int uny, const T* __restrict__ Ms, double amp2, unsigned long long seed, double dt_arg, long long step_arg,
                                                       const DevState* st, T* __restrict__ xi)
 {
     if (step_arg < 0 && st->done) return;
+    const long N = g.N;
     const long q = (long)blockIdx.x * blockDim.x + threadIdx.x;
     if (q >= N) return;
+    // Philox counter word = the cell's index in the CALLER's mesh (differs from q when the mesh is embedded)
+    const unsigned long long cell = (unsigned long long)((q & (g.nx - 1)) + (long)unx * (((q >> g.lognx) & (g.ny - 1)) + (long)uny * (q >> (g.lognx + g.logny))));
     const double Msi = (double)Ms[q];
     double e0 = 0, e1 = 0, e2 = 0;
     if (Msi != 0.0 && amp2 > 0.0) {
         const double dt = step_arg < 0 ? st->dt : dt_arg;
         const unsigned long long step = step_arg < 0 ? st->th_step : (unsigned long long)step_arg;
         unsigned x[4];
-        philox4x32_10((unsigned)q, (unsigned)((unsigned long long)q >> 32), (unsigned)step, (unsigned)(step >> 32), (unsigned)seed, (unsigned)(seed >> 32), x);
+        philox4x32_10((unsigned)cell, (unsigned)(cell >> 32), (unsigned)step, (unsigned)(step >> 32), (unsigned)seed, (unsigned)(seed >> 32), x);
         const double two_pi = 6.283185307179586476925286766559, sc = 1.0 / 4294967296.0;
         const double u0 = ((double)x[0] + 0.5) * sc, u1 = ((double)x[1] + 0.5) * sc, u2 = ((double)x[2] + 0.5) * sc, u3 = ((double)x[3] + 0.5) * sc;
         const double r0 = sqrt(-2.0 * log(u0)), r1 = sqrt(-2.0 * log(u2));
@@ -868,6 +871,9 @@ struct mm_sim {
     double A, D, Ku, Kc, u[3], hext[3], alpha, gamma;
     int dmi_kind, integ, demag_on, demag_ready, Ms_set;
     int A_cell, D_cell, H_cell;      // cell-based A / D / external field set (arrays in the workspace)
+    int unx, uny, unz, embed;        // the caller's mesh; embed: it is not 2^k per axis and lives inside the padded mesh g
+    long uN;
+    size_t off_ei, off_eo;           // embedding: inner-layout copies of the caller's input / output fields
     double stt_u[3], stt_beta, sl_aJ, sl_bJ, sl_p[3], temperature;      // Zhang-Li, Slonczewski / SOT, thermal field
     unsigned long long th_seed;
     // workspace
@@ -942,7 +948,7 @@ static bool raise_smem_limit(mm_sim* s, const void* func)
 static int fail(mm_sim* s, int code, const char* msg) { if (s) s->err = msg; return code; }
 static size_t esize(const mm_sim* s) { return s->prec == MM_F64 ? sizeof(double) : sizeof(float); }
 static size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
-static bool is_pow2(int v) { return v >= 1 && (v & (v - 1)) == 0; }
+static int next_pow2(int v) { int p = 1; while (p < v) p <<= 1; return p; }
 template <typename T> static T* wsp(const mm_sim* s, size_t off) { return reinterpret_cast<T*>(static_cast<char*>(s->ws) + off); }
 static const size_t SMEM_CAP = 200 * 1024;
 
@@ -1012,6 +1018,8 @@ static void layout(mm_sim* s)
     s->off_Dc = take(N * es);
     s->off_Hc = take(3 * N * es);
     s->off_Hth = take(3 * N * es);     // thermal field of the step in progress (Eq. 42)
+    s->off_ei = take(s->embed ? 3 * N * es : 0);
+    s->off_eo = take(s->embed ? 3 * N * es : 0);
     s->ws_need = o;
 }
 
@@ -1022,9 +1030,16 @@ extern "C" int mm_create(mm_sim** out, int nx, int ny, int nz, double dx, double
     if (!out) return MM_ERR_ARG;
     *out = nullptr;
     if (nx < 1 || ny < 1 || nz < 1 || !(dx > 0) || !(dy > 0) || !(dz > 0) || (prec != MM_F32 && prec != MM_F64)) return MM_ERR_ARG;
-    if (!is_pow2(nx) || !is_pow2(ny) || !is_pow2(nz)) return MM_ERR_UNSUPPORTED;
+    // Any mesh size: a size that is not a power of two is embedded in the next power of two with vacuum (Ms = 0) cells
+    // — the FFT passes are radix-2 and zero padding beyond 2n - 1 does not change the convolution (R3); the
+    // caller keeps its own nx x ny x nz layout, the library packs / unpacks at the ABI.
+    const int unx = nx, uny = ny, unz = nz;
+    if (nx > (1 << 20) || ny > (1 << 20) || nz > (1 << 20)) return MM_ERR_UNSUPPORTED;
+    nx = next_pow2(nx); ny = next_pow2(ny); nz = next_pow2(nz);
     if ((long)nx * ny * nz > (1L << 30)) return MM_ERR_UNSUPPORTED;
     mm_sim* s = new mm_sim();
+    s->unx = unx; s->uny = uny; s->unz = unz; s->uN = (long)unx * uny * unz;
+    s->embed = (unx != nx || uny != ny || unz != nz) ? 1 : 0;
     s->prec = prec; s->device = device; s->stream = static_cast<cudaStream_t>(cuda_stream);
     s->dx = dx; s->dy = dy; s->dz = dz;
     s->A = s->D = s->Ku = s->Kc = 0; s->A_cell = s->D_cell = s->H_cell = 0;
@@ -1123,7 +1138,7 @@ static int build_nbmask(mm_sim* s)
     return MM_OK;
 }
 
-extern "C" int mm_set_Ms_uniform(mm_sim* s, double Ms)
+static int in_set_Ms_uniform(mm_sim* s, double Ms)
 {
     NEED_WS(s);
     if (!(Ms >= 0)) return fail(s, MM_ERR_ARG, "Ms must be >= 0");
@@ -1137,7 +1152,7 @@ extern "C" int mm_set_Ms_uniform(mm_sim* s, double Ms)
     s->Ms_set = 1;
     return MM_OK;
 }
-extern "C" int mm_set_Ms(mm_sim* s, const void* dev_Ms)
+static int in_set_Ms(mm_sim* s, const void* dev_Ms)
 {
     NEED_WS(s);
     if (!dev_Ms) return MM_ERR_ARG;
@@ -1161,14 +1176,14 @@ static int set_cell_array(mm_sim* s, size_t off, size_t count, const void* dev_s
     *flag = 1;
     return MM_OK;
 }
-extern "C" int mm_set_A_cell(mm_sim* s, const void* dev_A) { if (!s) return MM_ERR_ARG; return set_cell_array(s, s->off_Ac, (size_t)s->g.N, dev_A, &s->A_cell); }
-extern "C" int mm_set_D_cell(mm_sim* s, const void* dev_D, mm_dmi_kind kind)
+static int in_set_A_cell(mm_sim* s, const void* dev_A) { if (!s) return MM_ERR_ARG; return set_cell_array(s, s->off_Ac, (size_t)s->g.N, dev_A, &s->A_cell); }
+static int in_set_D_cell(mm_sim* s, const void* dev_D, mm_dmi_kind kind)
 {
     if (!s || kind < 0 || kind > 3) return MM_ERR_ARG;
     s->dmi_kind = kind;
     return set_cell_array(s, s->off_Dc, (size_t)s->g.N, dev_D, &s->D_cell);
 }
-extern "C" int mm_set_H_ext_cell(mm_sim* s, const void* dev_H) { if (!s) return MM_ERR_ARG; return set_cell_array(s, s->off_Hc, 3 * (size_t)s->g.N, dev_H, &s->H_cell); }
+static int in_set_H_ext_cell(mm_sim* s, const void* dev_H) { if (!s) return MM_ERR_ARG; return set_cell_array(s, s->off_Hc, 3 * (size_t)s->g.N, dev_H, &s->H_cell); }
 extern "C" int mm_set_Ku(mm_sim* s, double Ku) { if (!s) return MM_ERR_ARG; s->Ku = Ku; return MM_OK; }
 extern "C" int mm_set_Kc(mm_sim* s, double Kc) { if (!s) return MM_ERR_ARG; s->Kc = Kc; return MM_OK; }
 extern "C" int mm_set_axis(mm_sim* s, double ux, double uy, double uz)
@@ -1359,7 +1374,7 @@ extern "C" int mm_init_demag(mm_sim* s)
     return MM_OK;
 }
 
-extern "C" int mm_get_demag_kernel(mm_sim* s, int comp, void* dev_out)
+static int in_get_demag_kernel(mm_sim* s, int comp, void* dev_out)
 {
     NEED_WS(s);
     if (!s->demag_ready) return fail(s, MM_ERR_STATE, "mm_init_demag not called");
@@ -1606,7 +1621,7 @@ static int set_state(mm_sim* s, double dt, double tol, double t_end, double stop
 
 #define NEED_READY(s) do { NEED_WS(s); if (!(s)->Ms_set) return fail((s), MM_ERR_STATE, "Ms not set"); MM_TRY((s), cudaSetDevice((s)->device)); } while (0)
 
-extern "C" int mm_effective_field(mm_sim* s, const void* dev_m, void* dev_H)
+static int in_effective_field(mm_sim* s, const void* dev_m, void* dev_H)
 {
     NEED_READY(s);
     if (!dev_m || !dev_H) return MM_ERR_ARG;
@@ -1616,7 +1631,7 @@ extern "C" int mm_effective_field(mm_sim* s, const void* dev_m, void* dev_H)
     return eval<float, 0>(s, (const float*)dev_m, (float*)dev_H, no_stage<float>(), ALL_TERMS);
 }
 
-extern "C" int mm_llg_rhs(mm_sim* s, const void* dev_m, void* dev_dmdt)
+static int in_llg_rhs(mm_sim* s, const void* dev_m, void* dev_dmdt)
 {
     NEED_READY(s);
     if (!dev_m || !dev_dmdt) return MM_ERR_ARG;
@@ -1626,7 +1641,7 @@ extern "C" int mm_llg_rhs(mm_sim* s, const void* dev_m, void* dev_dmdt)
     return eval<float, 1>(s, (const float*)dev_m, (float*)dev_dmdt, no_stage<float>(), ALL_TERMS);
 }
 
-extern "C" int mm_thermal_field(mm_sim* s, double dt, unsigned long long step, void* dev_out)
+static int in_thermal_field(mm_sim* s, double dt, unsigned long long step, void* dev_out)
 {
     NEED_READY(s);
     if (!dev_out || !(dt > 0)) return MM_ERR_ARG;
@@ -1634,8 +1649,8 @@ extern "C" int mm_thermal_field(mm_sim* s, double dt, unsigned long long step, v
     const double V = s->dx * s->dy * s->dz;
     const double amp2 = thermal_on(s) ? 2.0 * s->alpha * KB * s->temperature / (MU0 * s->gamma * V) : 0.0;
     const unsigned blocks = (unsigned)((N + 255) / 256);
-    if (s->prec == MM_F64) thermal_kernel<double><<<blocks, 256, 0, s->stream>>>(N, wsp<double>(s, s->off_Ms), amp2, s->th_seed, dt, (long long)step, wsp<DevState>(s, s->off_st), (double*)dev_out);
-    else thermal_kernel<float><<<blocks, 256, 0, s->stream>>>(N, wsp<float>(s, s->off_Ms), amp2, s->th_seed, dt, (long long)step, wsp<DevState>(s, s->off_st), (float*)dev_out);
+    if (s->prec == MM_F64) thermal_kernel<double><<<blocks, 256, 0, s->stream>>>(s->g, s->unx, s->uny, wsp<double>(s, s->off_Ms), amp2, s->th_seed, dt, (long long)step, wsp<DevState>(s, s->off_st), (double*)dev_out);
+    else thermal_kernel<float><<<blocks, 256, 0, s->stream>>>(s->g, s->unx, s->uny, wsp<float>(s, s->off_Ms), amp2, s->th_seed, dt, (long long)step, wsp<DevState>(s, s->off_st), (float*)dev_out);
     s->launches++;
     MM_TRY(s, cudaGetLastError());
     return MM_OK;
@@ -1666,7 +1681,7 @@ template <typename T> static int enqueue_step(mm_sim* s, T* m, int ctrl_mode)
     const bool thermal = thermal_on(s);
     if (thermal) {      // Eq. 42: one field per step attempt, drawn with this attempt's dt, held over its stages
         const double V = s->dx * s->dy * s->dz;
-        thermal_kernel<T><<<(unsigned)((N + 255) / 256), 256, 0, s->stream>>>(N, wsp<T>(s, s->off_Ms), 2.0 * s->alpha * KB * s->temperature / (MU0 * s->gamma * V),
+        thermal_kernel<T><<<(unsigned)((N + 255) / 256), 256, 0, s->stream>>>(s->g, s->unx, s->uny, wsp<T>(s, s->off_Ms), 2.0 * s->alpha * KB * s->temperature / (MU0 * s->gamma * V),
                                                                               s->th_seed, 0.0, -1, wsp<DevState>(s, s->off_st), wsp<T>(s, s->off_Hth));
         s->launches++;
     }
@@ -1710,7 +1725,7 @@ static int read_state(mm_sim* s, DevState* h)
     return MM_OK;
 }
 
-extern "C" int mm_step(mm_sim* s, void* dev_m, double dt, double tol, int* accepted, double* err, double* dt_next, double* max_dmdt)
+static int in_step(mm_sim* s, void* dev_m, double dt, double tol, int* accepted, double* err, double* dt_next, double* max_dmdt)
 {
     NEED_READY(s);
     if (!dev_m || !(dt > 0)) return MM_ERR_ARG;
@@ -1754,13 +1769,13 @@ static int adaptive_loop(mm_sim* s, void* dev_m, double tol, double dt0, double 
     return MM_OK;
 }
 
-extern "C" int mm_relax(mm_sim* s, void* dev_m, double tol, double stop_dmdt, long max_steps, double dt0, long* steps_done, double* max_dmdt)
+static int in_relax(mm_sim* s, void* dev_m, double tol, double stop_dmdt, long max_steps, double dt0, long* steps_done, double* max_dmdt)
 {
     NEED_READY(s);
     return adaptive_loop(s, dev_m, tol, dt0, 0.0, stop_dmdt, 1, max_steps, steps_done, max_dmdt);
 }
 
-extern "C" int mm_run_until(mm_sim* s, void* dev_m, double t_end, double tol, double dt0, long max_steps, long* steps_done)
+static int in_run_until(mm_sim* s, void* dev_m, double t_end, double tol, double dt0, long max_steps, long* steps_done)
 {
     NEED_READY(s);
     {   // steps enqueued without a host read-back (mm_step with NULL out-pointers) have advanced the device clock
@@ -1838,7 +1853,7 @@ template <typename T> static int minimize_t(mm_sim* s, T* m, double tau0, double
     return MM_OK;
 }
 
-extern "C" int mm_minimize(mm_sim* s, void* dev_m, double tau0, double tau_min, double tau_max, double stop_torque, long max_steps,
+static int in_minimize(mm_sim* s, void* dev_m, double tau0, double tau_min, double tau_max, double stop_torque, long max_steps,
                            long* steps_done, double* max_torque, double* tau_last)
 {
     NEED_READY(s);
@@ -1850,7 +1865,7 @@ extern "C" int mm_minimize(mm_sim* s, void* dev_m, double tau0, double tau_min, 
 // ------------------------------------------------------------------------------------------------
 // Host-buffer entry points (end-to-end path: H2D, compute, D2H inside the call)
 // ------------------------------------------------------------------------------------------------
-extern "C" int mm_run_host(mm_sim* s, void* host_m, int nsteps, double dt, double tol)
+static int in_run_host(mm_sim* s, void* host_m, int nsteps, double dt, double tol)
 {
     NEED_READY(s);
     if (!host_m || nsteps < 0 || !(dt > 0)) return MM_ERR_ARG;
@@ -1869,7 +1884,7 @@ extern "C" int mm_run_host(mm_sim* s, void* host_m, int nsteps, double dt, doubl
     return rc ? rc : rc2;
 }
 
-extern "C" int mm_llg_rhs_host(mm_sim* s, const void* host_m, void* host_dmdt)
+static int in_llg_rhs_host(mm_sim* s, const void* host_m, void* host_dmdt)
 {
     NEED_READY(s);
     if (!host_m || !host_dmdt) return MM_ERR_ARG;
@@ -1877,7 +1892,7 @@ extern "C" int mm_llg_rhs_host(mm_sim* s, const void* host_m, void* host_dmdt)
     void* dm = wsp<char>(s, s->off_y[0]);
     void* dk = wsp<char>(s, s->off_k[0]);
     MM_TRY(s, cudaMemcpyAsync(dm, host_m, bytes, cudaMemcpyHostToDevice, s->stream));
-    int rc = mm_llg_rhs(s, dm, dk);
+    int rc = in_llg_rhs(s, dm, dk);
     if (rc) return rc;
     MM_TRY(s, cudaMemcpyAsync(host_dmdt, dk, bytes, cudaMemcpyDeviceToHost, s->stream));
     MM_TRY(s, cudaStreamSynchronize(s->stream));
@@ -1901,7 +1916,7 @@ template <typename T> static int reduce_dot(mm_sim* s, const T* a, const T* b, i
     return MM_OK;
 }
 
-extern "C" int mm_average_m(mm_sim* s, const void* dev_m, double out3[3])
+static int in_average_m(mm_sim* s, const void* dev_m, double out3[3])
 {
     NEED_READY(s);
     if (!dev_m || !out3) return MM_ERR_ARG;
@@ -1939,9 +1954,221 @@ template <typename T> static int energy_t(mm_sim* s, const T* m, double* E_total
     return MM_OK;
 }
 
-extern "C" int mm_energy(mm_sim* s, const void* dev_m, double* E_total, double E_terms[5])
+static int in_energy(mm_sim* s, const void* dev_m, double* E_total, double E_terms[5])
 {
     NEED_READY(s);
     if (!dev_m) return MM_ERR_ARG;
     return s->prec == MM_F64 ? energy_t<double>(s, (const double*)dev_m, E_total, E_terms) : energy_t<float>(s, (const float*)dev_m, E_total, E_terms);
+}
+
+// ------------------------------------------------------------------------------------------------
+// The ABI entry points that take cell arrays.  A mesh whose sizes are powers of two goes straight to the inner
+// functions above.  Any other mesh is EMBEDDED (SURVEY 8(f)4 "non-power-of-two meshes"): the caller's nx x ny x nz
+// arrays are packed into / unpacked from the padded 2^k mesh whose extra cells are vacuum (Ms = 0: no field, no
+// torque, absent as neighbours — exactly the free boundary of R4), and the demag tensor depends on offsets only, so
+// every result at the caller's cells is the one of the caller's mesh.
+// ------------------------------------------------------------------------------------------------
+namespace mm {
+// dir 0: user -> inner (zero outside the caller's mesh); dir 1: inner -> user.  One thread per inner cell.
+template <typename T>
+__global__ void __launch_bounds__(256) embed_kernel(Geom g, int unx, int uny, int unz, int ncomp, const T* __restrict__ src, T* __restrict__ dst, int dir)
+{
+    const long q = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= g.N) return;
+    const int i = (int)(q & (g.nx - 1)), j = (int)((q >> g.lognx) & (g.ny - 1)), k = (int)(q >> (g.lognx + g.logny));
+    const bool inside = i < unx && j < uny && k < unz;
+    const long uN = (long)unx * uny * unz, uq = i + (long)unx * (j + (long)uny * k);
+    for (int c = 0; c < ncomp; c++) {
+        if (dir == 0) dst[c * g.N + q] = inside ? src[c * uN + uq] : (T)0;
+        else if (inside) dst[c * uN + uq] = src[c * g.N + q];
+    }
+}
+}  // namespace mm
+
+template <typename T> static int embed_t(mm_sim* s, const void* src, void* dst, int ncomp, int dir)
+{
+    embed_kernel<T><<<(unsigned)((s->g.N + 255) / 256), 256, 0, s->stream>>>(s->g, s->unx, s->uny, s->unz, ncomp, (const T*)src, (T*)dst, dir);
+    s->launches++;
+    MM_TRY(s, cudaGetLastError());
+    return MM_OK;
+}
+static int embed_in(mm_sim* s, const void* user, void* inner, int ncomp) { return s->prec == MM_F64 ? embed_t<double>(s, user, inner, ncomp, 0) : embed_t<float>(s, user, inner, ncomp, 0); }
+static int embed_out(mm_sim* s, const void* inner, void* user, int ncomp) { return s->prec == MM_F64 ? embed_t<double>(s, inner, user, ncomp, 1) : embed_t<float>(s, inner, user, ncomp, 1); }
+static void* slot_in(mm_sim* s) { return wsp<char>(s, s->off_ei); }
+static void* slot_out(mm_sim* s) { return wsp<char>(s, s->off_eo); }
+#define MM_EMB_CHECK(s, p) do { NEED_WS(s); if (!(p)) return MM_ERR_ARG; MM_TRY((s), cudaSetDevice((s)->device)); } while (0)
+
+extern "C" int mm_set_Ms_uniform(mm_sim* s, double Ms)
+{
+    if (!s || !s->embed) return in_set_Ms_uniform(s, Ms);
+    // uniform inside the caller's mesh, vacuum in the padding: fill a caller-shaped array and pack it
+    NEED_WS(s);
+    if (!(Ms >= 0)) return fail(s, MM_ERR_ARG, "Ms must be >= 0");
+    MM_TRY(s, cudaSetDevice(s->device));
+    const int blocks = (int)((s->uN + 255) / 256);
+    if (s->prec == MM_F64) fill_kernel<double><<<blocks, 256, 0, s->stream>>>(s->uN, (double*)slot_out(s), Ms);
+    else fill_kernel<float><<<blocks, 256, 0, s->stream>>>(s->uN, (float*)slot_out(s), (float)Ms);
+    s->launches++;
+    int rc = embed_in(s, slot_out(s), slot_in(s), 1);
+    return rc ? rc : in_set_Ms(s, slot_in(s));
+}
+extern "C" int mm_set_Ms(mm_sim* s, const void* dev_Ms)
+{
+    if (!s || !s->embed) return in_set_Ms(s, dev_Ms);
+    MM_EMB_CHECK(s, dev_Ms);
+    int rc = embed_in(s, dev_Ms, slot_in(s), 1);
+    return rc ? rc : in_set_Ms(s, slot_in(s));
+}
+extern "C" int mm_set_A_cell(mm_sim* s, const void* dev_A)
+{
+    if (!s || !s->embed || !dev_A) return in_set_A_cell(s, dev_A);
+    MM_EMB_CHECK(s, dev_A);
+    int rc = embed_in(s, dev_A, slot_in(s), 1);
+    return rc ? rc : in_set_A_cell(s, slot_in(s));
+}
+extern "C" int mm_set_D_cell(mm_sim* s, const void* dev_D, mm_dmi_kind kind)
+{
+    if (!s || !s->embed || !dev_D) return in_set_D_cell(s, dev_D, kind);
+    MM_EMB_CHECK(s, dev_D);
+    int rc = embed_in(s, dev_D, slot_in(s), 1);
+    return rc ? rc : in_set_D_cell(s, slot_in(s), kind);
+}
+extern "C" int mm_set_H_ext_cell(mm_sim* s, const void* dev_H)
+{
+    if (!s || !s->embed || !dev_H) return in_set_H_ext_cell(s, dev_H);
+    MM_EMB_CHECK(s, dev_H);
+    int rc = embed_in(s, dev_H, slot_in(s), 3);
+    return rc ? rc : in_set_H_ext_cell(s, slot_in(s));
+}
+extern "C" int mm_get_demag_kernel(mm_sim* s, int comp, void* dev_out)
+{
+    if (!s || !s->embed) return in_get_demag_kernel(s, comp, dev_out);
+    MM_EMB_CHECK(s, dev_out);
+    // N doubles of the inner mesh fit the 3N-real slot in either precision (8 N <= 12 N bytes)
+    int rc = in_get_demag_kernel(s, comp, slot_in(s));
+    if (rc) return rc;
+    rc = embed_t<double>(s, slot_in(s), dev_out, 1, 1);
+    if (rc) return rc;
+    MM_TRY(s, cudaStreamSynchronize(s->stream));
+    return MM_OK;
+}
+extern "C" int mm_effective_field(mm_sim* s, const void* dev_m, void* dev_H)
+{
+    if (!s || !s->embed) return in_effective_field(s, dev_m, dev_H);
+    MM_EMB_CHECK(s, dev_m && dev_H);
+    int rc = embed_in(s, dev_m, slot_in(s), 3);
+    if (!rc) rc = in_effective_field(s, slot_in(s), slot_out(s));
+    return rc ? rc : embed_out(s, slot_out(s), dev_H, 3);
+}
+extern "C" int mm_llg_rhs(mm_sim* s, const void* dev_m, void* dev_dmdt)
+{
+    if (!s || !s->embed) return in_llg_rhs(s, dev_m, dev_dmdt);
+    MM_EMB_CHECK(s, dev_m && dev_dmdt);
+    int rc = embed_in(s, dev_m, slot_in(s), 3);
+    if (!rc) rc = in_llg_rhs(s, slot_in(s), slot_out(s));
+    return rc ? rc : embed_out(s, slot_out(s), dev_dmdt, 3);
+}
+extern "C" int mm_thermal_field(mm_sim* s, double dt, unsigned long long step, void* dev_out)
+{
+    if (!s || !s->embed) return in_thermal_field(s, dt, step, dev_out);
+    MM_EMB_CHECK(s, dev_out);
+    int rc = in_thermal_field(s, dt, step, slot_out(s));
+    return rc ? rc : embed_out(s, slot_out(s), dev_out, 3);
+}
+// in-place integrators: pack m, run on the inner copy, unpack (stream-ordered; the inner call decides about syncing,
+// so the unpack is enqueued BEFORE a call that may read back would return — hence pack / unpack around an async core)
+extern "C" int mm_step(mm_sim* s, void* dev_m, double dt, double tol, int* accepted, double* err, double* dt_next, double* max_dmdt)
+{
+    if (!s || !s->embed) return in_step(s, dev_m, dt, tol, accepted, err, dt_next, max_dmdt);
+    MM_EMB_CHECK(s, dev_m);
+    int rc = embed_in(s, dev_m, slot_in(s), 3);
+    if (!rc) rc = in_step(s, slot_in(s), dt, tol, nullptr, nullptr, nullptr, nullptr);
+    if (!rc) rc = embed_out(s, slot_in(s), dev_m, 3);
+    if (rc) return rc;
+    if (accepted || err || dt_next || max_dmdt) {
+        DevState h;
+        if ((rc = read_state(s, &h))) return rc;
+        if (accepted) *accepted = h.accepted;
+        if (err) *err = h.err;
+        if (dt_next) *dt_next = h.dt;
+        if (max_dmdt) *max_dmdt = h.maxk;
+        if (h.nan) return fail(s, MM_ERR_NAN, "non-finite error norm or torque");
+    }
+    return MM_OK;
+}
+extern "C" int mm_relax(mm_sim* s, void* dev_m, double tol, double stop_dmdt, long max_steps, double dt0, long* steps_done, double* max_dmdt)
+{
+    if (!s || !s->embed) return in_relax(s, dev_m, tol, stop_dmdt, max_steps, dt0, steps_done, max_dmdt);
+    MM_EMB_CHECK(s, dev_m);
+    int rc = embed_in(s, dev_m, slot_in(s), 3);
+    if (!rc) rc = in_relax(s, slot_in(s), tol, stop_dmdt, max_steps, dt0, steps_done, max_dmdt);
+    const int rc2 = embed_out(s, slot_in(s), dev_m, 3);
+    return rc ? rc : rc2;
+}
+extern "C" int mm_run_until(mm_sim* s, void* dev_m, double t_end, double tol, double dt0, long max_steps, long* steps_done)
+{
+    if (!s || !s->embed) return in_run_until(s, dev_m, t_end, tol, dt0, max_steps, steps_done);
+    MM_EMB_CHECK(s, dev_m);
+    int rc = embed_in(s, dev_m, slot_in(s), 3);
+    if (!rc) rc = in_run_until(s, slot_in(s), t_end, tol, dt0, max_steps, steps_done);
+    const int rc2 = embed_out(s, slot_in(s), dev_m, 3);
+    return rc ? rc : rc2;
+}
+extern "C" int mm_minimize(mm_sim* s, void* dev_m, double tau0, double tau_min, double tau_max, double stop_torque, long max_steps,
+                           long* steps_done, double* max_torque, double* tau_last)
+{
+    if (!s || !s->embed) return in_minimize(s, dev_m, tau0, tau_min, tau_max, stop_torque, max_steps, steps_done, max_torque, tau_last);
+    MM_EMB_CHECK(s, dev_m);
+    int rc = embed_in(s, dev_m, slot_in(s), 3);
+    if (!rc) rc = in_minimize(s, slot_in(s), tau0, tau_min, tau_max, stop_torque, max_steps, steps_done, max_torque, tau_last);
+    const int rc2 = embed_out(s, slot_in(s), dev_m, 3);
+    return rc ? rc : rc2;
+}
+extern "C" int mm_run_host(mm_sim* s, void* host_m, int nsteps, double dt, double tol)
+{
+    if (!s || !s->embed) return in_run_host(s, host_m, nsteps, dt, tol);
+    MM_EMB_CHECK(s, host_m);
+    if (!s->Ms_set) return fail(s, MM_ERR_STATE, "Ms not set");
+    if (nsteps < 0 || !(dt > 0)) return MM_ERR_ARG;
+    const size_t bytes = 3 * (size_t)s->uN * esize(s);
+    MM_TRY(s, cudaMemcpyAsync(slot_out(s), host_m, bytes, cudaMemcpyHostToDevice, s->stream));
+    int rc = embed_in(s, slot_out(s), slot_in(s), 3);
+    if (!rc) rc = set_state(s, dt, s->integ == MM_DOPRI5 ? tol : 0.0, 0, 0, 0, 1);
+    for (int i = 0; i < nsteps && !rc; i++) rc = enqueue_step_any(s, slot_in(s), 0);
+    if (!rc) rc = embed_out(s, slot_in(s), slot_out(s), 3);
+    if (!rc) {
+        cudaError_t e = cudaMemcpyAsync(host_m, slot_out(s), bytes, cudaMemcpyDeviceToHost, s->stream);
+        if (e != cudaSuccess) { s->err = cudaGetErrorString(e); rc = MM_ERR_CUDA; }
+    }
+    DevState h;
+    const int rc2 = read_state(s, &h);
+    return rc ? rc : rc2;
+}
+extern "C" int mm_llg_rhs_host(mm_sim* s, const void* host_m, void* host_dmdt)
+{
+    if (!s || !s->embed) return in_llg_rhs_host(s, host_m, host_dmdt);
+    MM_EMB_CHECK(s, host_m && host_dmdt);
+    const size_t bytes = 3 * (size_t)s->uN * esize(s);
+    MM_TRY(s, cudaMemcpyAsync(slot_out(s), host_m, bytes, cudaMemcpyHostToDevice, s->stream));
+    int rc = embed_in(s, slot_out(s), slot_in(s), 3);
+    if (!rc) rc = in_llg_rhs(s, slot_in(s), slot_out(s));
+    if (!rc) rc = embed_out(s, slot_out(s), slot_in(s), 3);      // caller layout, staged in the input slot
+    if (rc) return rc;
+    MM_TRY(s, cudaMemcpyAsync(host_dmdt, slot_in(s), bytes, cudaMemcpyDeviceToHost, s->stream));
+    MM_TRY(s, cudaStreamSynchronize(s->stream));
+    return MM_OK;
+}
+extern "C" int mm_average_m(mm_sim* s, const void* dev_m, double out3[3])
+{
+    if (!s || !s->embed) return in_average_m(s, dev_m, out3);
+    MM_EMB_CHECK(s, dev_m);
+    int rc = embed_in(s, dev_m, slot_in(s), 3);
+    return rc ? rc : in_average_m(s, slot_in(s), out3);
+}
+extern "C" int mm_energy(mm_sim* s, const void* dev_m, double* E_total, double E_terms[5])
+{
+    if (!s || !s->embed) return in_energy(s, dev_m, E_total, E_terms);
+    MM_EMB_CHECK(s, dev_m);
+    int rc = embed_in(s, dev_m, slot_in(s), 3);
+    return rc ? rc : in_energy(s, slot_in(s), E_total, E_terms);
 }

@@ -34,7 +34,16 @@ def test_argument_errors_without_gpu():
     f.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_int, C.c_int, C.c_void_p]
     assert f(C.byref(h), 0, 4, 4, 1e-9, 1e-9, 1e-9, 0, 0, None) == -1          # MM_ERR_ARG
     assert f(C.byref(h), 4, 4, 4, -1e-9, 1e-9, 1e-9, 0, 0, None) == -1
-    assert f(C.byref(h), 12, 4, 4, 1e-9, 1e-9, 1e-9, 0, 0, None) == -2         # MM_ERR_UNSUPPORTED (not 2^k)
+    assert f(C.byref(h), 1 << 21, 4, 4, 1e-9, 1e-9, 1e-9, 0, 0, None) == -2    # MM_ERR_UNSUPPORTED (too large)
+    assert f(C.byref(h), 12, 5, 3, 1e-9, 1e-9, 1e-9, 0, 0, None) == 0           # not 2^k: embedded in 16 x 8 x 4
+    lib.mm_workspace_bytes.restype = C.c_size_t
+    lib.mm_workspace_bytes.argtypes = [C.c_void_p]
+    lib.mm_destroy.argtypes = [C.c_void_p]
+    emb = lib.mm_workspace_bytes(h)
+    assert lib.mm_destroy(h) == 0
+    assert f(C.byref(h), 16, 8, 4, 1e-9, 1e-9, 1e-9, 0, 0, None) == 0
+    assert emb > lib.mm_workspace_bytes(h)                                       # two extra inner-layout slots
+    assert lib.mm_destroy(h) == 0
     assert f(C.byref(h), 16, 16, 1, 1e-9, 1e-9, 1e-9, 1, 0, None) == 0
     lib.mm_workspace_bytes.restype = C.c_size_t
     lib.mm_workspace_bytes.argtypes = [C.c_void_p]

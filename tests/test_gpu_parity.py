@@ -253,8 +253,9 @@ def test_edge_cases_and_errors():
     assert float(s.llg_rhs(m).abs().max()) == 0.0
     with pytest.raises(MMError):
         Sim(2, 16, 1, 1e-9, 1e-9, 1e-9).init_demag()   # nx < 4
+    Sim(24, 16, 1, 1e-9, 1e-9, 1e-9).init_demag()     # not a power of two: embedded (tests/test_gpu_anysize.py)
     with pytest.raises(MMError):
-        Sim(24, 16, 1, 1e-9, 1e-9, 1e-9)              # not a power of two
+        Sim(0, 16, 1, 1e-9, 1e-9, 1e-9)               # empty mesh
     # NaN in m is reported, not silently propagated
     s2 = Sim(16, 16, 1, 2e-9, 2e-9, 2e-9, prec=F32)
     s2.set_Ms(8e5); s2.set_A(1.3e-11); s2.init_demag()
