@@ -16,6 +16,7 @@
 #include "mm_kernels2.cuh"
 #include "mm_passAC.cuh"
 #include "mm_passB7.cuh"
+#include "mm_passB3.cuh"
 #include "mm_llg.cuh"
 
 #ifndef MM_OCC_A
@@ -89,6 +90,13 @@ __global__ void __launch_bounds__(MM_B5_THR, MM_B5_OCC) y_conv5_kernel(Geom g, c
 {
     __shared__ __align__(8) unsigned long long bar[3];
     y_conv_body5<T, V>(g, S, Kh, tw, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x, &tmS, bar, &st->done);
+}
+// half-tile form (mm_passB3.cuh): the long-line path; reads S, writes the second spectrum buffer S2
+template <typename T, int V>
+__global__ void __launch_bounds__(512) y_conv3_kernel(Geom g, const cx<T>* S, cx<T>* S2, const T* Kh, twiddles<T> tw, const DevState* st)
+{
+    if (st->done) return;
+    y_conv_body3<T, V>(g, S, S2, Kh, tw, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x);
 }
 // compile-time specialised form of the TMA pass B (mm_passB7.cuh): ny = 2^LOGM; fp32: TC = 4, 256 threads; fp64: TC = 2,
 // 128 threads (rows of 32 bytes and tiles of py * 96 bytes in both; two CTAs per SM)
@@ -873,6 +881,8 @@ struct mm_sim {
     int A_cell, D_cell, H_cell;      // cell-based A / D / external field set (arrays in the workspace)
     int unx, uny, unz, embed;        // the caller's mesh; embed: it is not 2^k per axis and lives inside the padded mesh g
     long uN;
+    int use_b3;                      // pass B runs the half-tile form (a full py-row tile does not fit one CTA)
+    size_t off_S2;                   // its output spectrum
     size_t off_ei, off_eo;           // embedding: inner-layout copies of the caller's input / output fields
     double stt_u[3], stt_beta, sl_aJ, sl_bJ, sl_p[3], temperature;      // Zhang-Li, Slonczewski / SOT, thermal field
     unsigned long long th_seed;
@@ -973,12 +983,20 @@ static void configure(mm_sim* s)
     if (getenv("MM_TC")) TC = atoi(getenv("MM_TC"));       // tuning knob (power of two)
     g.TC = TC;
     while (g.TC > 1 && (size_t)smemB_elems(g) * cs > SMEM_CAP) g.TC /= 2;
+    // a line that does not fit even one column wide (or MM_B3=1, for measurements): half-tile form, ny rows per tile
+    s->use_b3 = 0;
+    if (s->use_v2 && g.ny >= 16 && ((size_t)smemB_elems(g) * cs > SMEM_CAP || getenv("MM_B3"))) {
+        s->use_b3 = 1;
+        g.TC = s->prec == MM_F64 ? 4 : 8;
+        if (getenv("MM_TC")) g.TC = atoi(getenv("MM_TC"));
+        while (g.TC > 1 && (size_t)g.ny * 3 * g.TC * cs > SMEM_CAP) g.TC /= 2;
+    }
     // fp32: two resident CTAs per SM (tile <= 98 KB) beat one CTA with a tile twice as wide — one CTA's
     // shared-memory-bound stages overlap the other's FP32-bound ones (measured, profiles/r01_experiments.md)
     if (s->prec == MM_F32 && !getenv("MM_TC") && g.TC >= 4 && (size_t)smemB_elems(g) * cs > 98 * 1024) g.TC /= 2;
-    while (g.TC > 2 && ((g.nx + g.TC) / g.TC) * g.pz < target) g.TC /= 2;
+    while (g.TC > 2 && ((g.nx + g.TC) / g.TC) * g.pz < target && !s->use_b3) g.TC /= 2;
     // fp64: the specialised pass B (mm_passB7.cuh) wants rows of 32 bytes = two columns, tiles of py * 96 bytes
-    const bool b7_f64 = s->prec == MM_F64 && !getenv("MM_TC") && !s->no_b7 && s->use_v2 && g.logny >= 4 && g.logny <= 9 && g.TC >= 2;
+    const bool b7_f64 = s->prec == MM_F64 && !getenv("MM_TC") && !s->no_b7 && !s->use_b3 && s->use_v2 && g.logny >= 4 && g.logny <= 9 && g.TC >= 2;
     if (b7_f64) g.TC = 2;
     g.Lx = ((g.nx + 1 + g.TC - 1) / g.TC) * g.TC;
     g.plane = (long)g.ny * g.Lx;
@@ -988,10 +1006,11 @@ static void configure(mm_sim* s)
     s->smemA = (size_t)smemA_elems(g) * cs;
     // the v2 bodies of passes A / C do the z transform in registers: no scratch tile
     s->smemA2 = (size_t)(g.nx + 1) * odd_pitch(g.G * g.nz) * cs;
-    s->smemB = (size_t)smemB_elems(g) * cs;
+    s->smemB = s->use_b3 ? (size_t)smemB3_elems(g) * cs : (size_t)smemB_elems(g) * cs;
     s->thrA = 256;
     s->thrB = (s->prec == MM_F32 && s->smemB > 98 * 1024) ? 512 : 256;
     if (b7_f64) s->thrB = 128;
+    if (s->use_b3) s->thrB = (g.ny / 8) * (g.TC / (s->prec == MM_F32 && g.TC % 2 == 0 ? 2 : 1)) >= 512 ? 512 : 256;
     if (getenv("MM_THRB")) s->thrB = atoi(getenv("MM_THRB"));
 }
 
@@ -1005,8 +1024,9 @@ static void layout(mm_sim* s)
     s->off_Ms = take(N * es);
     s->off_nbm = take(N);
     s->off_S = take((size_t)3 * g.comp * 2 * es);
+    s->off_S2 = take(s->use_b3 ? (size_t)3 * g.comp * 2 * es : 0);
     s->off_Kh = take((size_t)6 * g.kcomp * es);
-    s->off_Kc = take((s->use_v2 && g.ny >= 16 ? (size_t)kc_elems(g) : 0) * es);      // pass B v2: K^ in consumption order
+    s->off_Kc = take((s->use_v2 && g.ny >= 16 && !s->use_b3 ? (size_t)kc_elems(g) : 0) * es);      // pass B v2: K^ in consumption order
     s->off_Hd = take(3 * N * es);
     for (int i = 0; i < 7; i++) s->off_k[i] = take(3 * N * es);
     for (int i = 0; i < 2; i++) s->off_y[i] = take(3 * N * es);
@@ -1331,7 +1351,7 @@ template <typename T> static int init_demag_t(mm_sim* s)
         s->launches++;
         MM_TRY(s, cudaGetLastError());
     }
-    if (s->use_v2 && g.ny >= 16) {
+    if (s->use_v2 && g.ny >= 16 && !s->use_b3) {
         const long total = kc_elems(g);
         kc_fill_kernel<T><<<(unsigned)((total + 255) / 256), 256, 0, st>>>(g, Kh, wsp<T>(s, s->off_Kc), total);
         s->launches++;
@@ -1436,6 +1456,11 @@ template <typename T, int NZ> static void launch_A2(mm_sim* s, unsigned grid, co
     if (!raise_smem_limit(s, (const void*)fwd_xz2_kernel<T, NZ>)) return;
     fwd_xz2_kernel<T, NZ><<<grid, s->thrA, s->smemA2, s->stream>>>(s->g, y, wsp<T>(s, s->off_Ms), S, tw, st);
 }
+template <typename T, int V> static void launch_B3(mm_sim* s, unsigned grid, cx<T>* S, twiddles<T> tw, const DevState* st)
+{
+    if (!raise_smem_limit(s, (const void*)y_conv3_kernel<T, V>)) return;
+    y_conv3_kernel<T, V><<<grid, s->thrB, s->smemB, s->stream>>>(s->g, S, wsp<cx<T>>(s, s->off_S2), wsp<T>(s, s->off_Kh), tw, st);
+}
 template <typename T, int NZ> static void launch_C2(mm_sim* s, unsigned grid, cx<T>* S, twiddles<T> tw, T sc, const DevState* st)
 {
     if (!raise_smem_limit(s, (const void*)inv_zx2_kernel<T, NZ>)) return;
@@ -1456,7 +1481,7 @@ template <typename T, int V> static void launch_B5(mm_sim* s, unsigned grid, cx<
 template <typename T> static bool b7_applies(const mm_sim* s)
 {
     const Geom& g = s->g;
-    return s->use_v2 && !s->no_b7 && g.logny >= 4 && g.logny <= 9 && g.TC == (sizeof(T) == 8 ? 2 : 4) && s->thrB == (sizeof(T) == 8 ? 128 : 256);
+    return s->use_v2 && !s->no_b7 && !s->use_b3 && g.logny >= 4 && g.logny <= 9 && g.TC == (sizeof(T) == 8 ? 2 : 4) && s->thrB == (sizeof(T) == 8 ? 128 : 256);
 }
 template <typename T, int LOGM, bool IS3D> static void launch_B7(mm_sim* s, unsigned grid, cx<T>* S, twiddles<T> tw, const DevState* st)
 {
@@ -1528,7 +1553,11 @@ template <typename T> static int demag_passes(mm_sim* s, const T* y)
     }
     prof_end(s);
     prof_begin(s, 1);
-    if (b2 && try_launch_B7<T>(s, gridB, S, tw, st)) {
+    if (b2 && s->use_b3) {
+        if (sizeof(T) == 4 && g.TC % 2 == 0) launch_B3<T, (sizeof(T) == 4 ? 2 : 1)>(s, gridB, S, tw, st);
+        else launch_B3<T, 1>(s, gridB, S, tw, st);
+        S = wsp<cx<T>>(s, s->off_S2);      // pass C reads the half-tile form's output buffer
+    } else if (b2 && try_launch_B7<T>(s, gridB, S, tw, st)) {
     } else if (b2 && s->use_tma) {
         if (sizeof(T) == 4 && g.TC % 2 == 0) launch_B5<T, (sizeof(T) == 4 ? 2 : 1)>(s, gridB, S, tw, st);
         else launch_B5<T, 1>(s, gridB, S, tw, st);

@@ -9,6 +9,7 @@
 #include "../../paper_2406_16064_b200/csrc/mm_kernels2.cuh"
 #include "../../paper_2406_16064_b200/csrc/mm_passAC.cuh"
 #include "../../paper_2406_16064_b200/csrc/mm_passB7.cuh"
+#include "../../paper_2406_16064_b200/csrc/mm_passB3.cuh"
 #include "../../paper_2406_16064_b200/csrc/mm_llg.cuh"
 
 using namespace mm;
@@ -78,8 +79,13 @@ static void run(int ver, int nx, int ny, int nz, int G, int CH, int TC, const do
     const bool b7 = ver == 7 && TC == (sizeof(T) == 8 ? 2 : 4) && ny >= 16 && ny <= 512;
     unsigned long long* nobar = nullptr;
     constexpr int LOGTC7 = sizeof(T) == 8 ? 1 : 2;
+    const bool b3 = ver == 3 && ny >= 16;
+    std::vector<cx<T>> S2(b3 ? S.size() : 0);      // half-tile pass B writes a second spectrum buffer
     for (int b = 0; b < gridB; b++) {
-        if (b7) {
+        if (b3) {
+            if (sizeof(T) == 4 && TC % 2 == 0) y_conv_body3<T, (sizeof(T) == 4 ? 2 : 1)>(g, S.data(), S2.data(), Kh.data(), tw, smem.data(), b, 0, 1);
+            else y_conv_body3<T, 1>(g, S.data(), S2.data(), Kh.data(), tw, smem.data(), b, 0, 1);
+        } else if (b7) {
             switch (g.logny * 2 + (nz > 1)) {
 #define CASE_B7(L) case 2 * L: y_conv_body7<L, LOGTC7, false, 1, T>(g, S.data(), Kc.data(), tw, ilog2(twN), smem.data(), b, 0, 1, nullptr, nobar, nullptr); break; \
                    case 2 * L + 1: y_conv_body7<L, LOGTC7, true, 1, T>(g, S.data(), Kc.data(), tw, ilog2(twN), smem.data(), b, 0, 1, nullptr, nobar, nullptr); break;
@@ -92,6 +98,7 @@ static void run(int ver, int nx, int ny, int nz, int G, int CH, int TC, const do
         else if (sizeof(T) == 4 && TC % 2 == 0) y_conv_body2<T, (sizeof(T) == 4 ? 2 : 1)>(g, S.data(), Kc.data(), tw, smem.data(), b, 0, 1);
         else y_conv_body2<T, 1>(g, S.data(), Kc.data(), tw, smem.data(), b, 0, 1);
     }
+    if (b3) S.swap(S2);
     for (int b = 0; b < gridA; b++) {
         if (!a2) inv_zx_body<T>(g, S.data(), Hdt.data(), tw, (T)(1.0 / P), smem.data(), b, 0, 1);
         else switch (nz) {

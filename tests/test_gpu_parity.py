@@ -290,7 +290,7 @@ def test_cfg4_full_size_sampled_direct_sum():
         del s
 
 
-@pytest.mark.parametrize("case", ["cfg4", "film4096_f32", "film2048_f64", "film1024_f64"])
+@pytest.mark.parametrize("case", ["cfg4", "film4096_f32", "film4096_f64", "film2048_f64", "film1024_f64"])
 def test_full_size_block_aggregation_identity(case):
     """Uniformly magnetised full mesh: the MEAN demag field is -Ms N_self(block) m exactly, with N_self the
     Newell self term of the whole block as one cell (SURVEY.md §8c pins; holds at any size)."""
@@ -311,6 +311,59 @@ def test_full_size_block_aggregation_identity(case):
         ref = -w.Ms_max * np.array(nself) * u
         assert np.abs(H - ref).max() / w.Ms_max <= (1e-10 if prec == F64 else 2e-5), (case, prec, H, ref)
         del s
+
+
+@pytest.mark.parametrize("prec", [F64, F32])
+def test_film4096_point_source_is_the_newell_tensor(prec):
+    """configs[4] at N = 4096 (fp64 runs the half-tile pass B: a full 8192-row tile does not fit one CTA): the field
+    of ONE magnetised cell is -Ms N(r - r0) m at every cell; sampled cells against the oracle's quad-precision
+    tensor, including the far corners of the film and the source's neighbours."""
+    from paper_2406_16064_b200 import Sim
+    import torch
+    w = wl.cfg5(4096, with_m=False)
+    s = Sim(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, prec=prec)
+    wl.apply(s, w)
+    s.set_A(0.0); s.set_H_ext(0, 0, 0)
+    i0, j0 = 1234, 3071
+    mvec = np.array([0.6, -0.64, 0.48])
+    dm = torch.zeros((3, 1, 4096, 4096), dtype=s.dtype, device=s.device)
+    dm[:, 0, j0, i0] = torch.tensor(mvec, dtype=s.dtype)
+    H = s.effective_field(dm)
+    rng = np.random.default_rng(7)
+    cells = [(i0, j0), (i0 + 1, j0), (i0, j0 - 1), (i0 - 1, j0 + 1), (0, 0), (4095, 4095), (0, 4095), (4095, 0), (i0, 0), (2048, 2048)]
+    cells += [(int(a), int(b)) for a, b in rng.integers(0, 4096, (30, 2))]
+    cells += [(i0 + int(a), j0 + int(b)) for a, b in rng.integers(-12, 13, (30, 2))]
+    worst = 0.0
+    for (i, j) in cells:
+        n = oracle.newell_point((i - i0) * w.dx, (j - j0) * w.dy, 0.0, w.dx, w.dy, w.dz)      # xx yy zz xy xz yz
+        N = np.array([[n[0], n[3], n[4]], [n[3], n[1], n[5]], [n[4], n[5], n[2]]])
+        ref = -w.Ms_max * N @ mvec
+        got = H[:, 0, j, i].double().cpu().numpy()
+        worst = max(worst, np.abs(got - ref).max() / w.Ms_max)
+    assert worst <= (1e-12 if prec == F64 else 2e-7), worst
+    del s
+
+
+@pytest.mark.parametrize("prec", [F64, F32])
+def test_pass_b_half_tile_form(monkeypatch, prec):
+    """The half-tile form of pass B (mm_passB3.cuh, the long-line path) forced on small meshes (MM_B3): 3-D and film,
+    both precisions, against the oracle."""
+    monkeypatch.setenv("MM_B3", "1")
+    w = small3d(64, 64, 16)
+    o, s = make_pair(w, prec)
+    m = masked_m(w)
+    assert np.abs(to_np(s.effective_field(s.to_device(m))) - o.effective_field(m)).max() / w.Ms_max <= HTOL[prec]
+    wf = film(512)
+    o, s = make_pair(wf, prec)
+    H = to_np(s.effective_field(s.to_device(wf.m0)))
+    assert np.abs(H - o.effective_field(np.ascontiguousarray(wf.m0))).max() / wf.Ms_max <= HTOL[prec]
+    wn = small3d(32, 16, 2)
+    o, s = make_pair(wn, prec)
+    m = masked_m(wn)
+    dm = s.to_device(m)
+    for _ in range(3):
+        o.step(m, wn.dt); s.step(dm, wn.dt, sync=False)
+    assert np.abs(to_np(dm) - m).max() <= (1e-9 if prec == F64 else 2e-3)
 
 
 def test_cfg4_full_size_step_invariants():
