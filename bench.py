@@ -308,8 +308,9 @@ def measure(args, w, prec_name, rank, world, local, barrier, dev, sample_clocks)
     barrier()
     warm_ms, warm_cnt = s.get_profile()
     dom = max(range(4), key=lambda i: warm_ms[i])
-    # timed region: only the dominant class keeps its events (2 stream operations per bracketed kernel)
-    s.set_profiling(2 << dom)
+    # timed region: only the dominant class keeps its events (2 stream operations per bracketed kernel);
+    # --no-kernel-events: none at all (the library then replays each step as one CUDA graph: small meshes)
+    s.set_profiling(0 if args.no_kernel_events else (2 << dom))
     sampler = ClockSampler(local) if sample_clocks else None
     if sampler:
         sampler.start()
@@ -327,8 +328,24 @@ def measure(args, w, prec_name, rank, world, local, barrier, dev, sample_clocks)
     sec = e0.elapsed_time(e1) * 1e-3
     launches = s.launch_count() - l0
     dom_ms, dom_cnt = s.get_profile()
+    if args.no_kernel_events:
+        dom_ms, dom_cnt = warm_ms, warm_cnt
     clocks = sampler.stop(t_host0, t_host1) if sampler else None
     assert bool(torch.isfinite(dm).all()), "non-finite magnetisation after the timed region"
+
+    # the same K steps once more with no events at all: the library replays each step as one captured CUDA graph
+    # (reported beside `value`, which keeps the dominant kernel's events inside its timed region)
+    s.set_profiling(0)
+    for _ in range(2):
+        s.step(dm, w.dt, sync=False)
+    g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    g0.record()
+    for _ in range(args.steps):
+        s.step(dm, w.dt, sync=False)
+    g1.record()
+    barrier()
+    graph_sec = g0.elapsed_time(g1) * 1e-3
 
     # per-kernel times of every class: a separate profiled pass over the same number of steps (not part of `value`)
     s.set_profiling(True)
@@ -349,6 +366,7 @@ def measure(args, w, prec_name, rank, world, local, barrier, dev, sample_clocks)
     e2e_sec = time.perf_counter() - t0
 
     units = w.N * RHS_PER_STEP * args.steps
+    graph_max, _ = aggregate_over_ranks(graph_sec, units, dev)
     sec_max, units_all = aggregate_over_ranks(sec, units, dev)
     e2e_max, e2e_units = aggregate_over_ranks(e2e_sec, w.N * RHS_PER_STEP * e2e_steps, dev)
     version = load_library().mm_version().decode()
@@ -371,13 +389,16 @@ def measure(args, w, prec_name, rank, world, local, barrier, dev, sample_clocks)
         "e2e": {"value": e2e_units / e2e_max, "unit": UNIT, "h2d_bytes_per_step": 3 * w.N * esize, "d2h_bytes_per_step": 3 * w.N * esize,
                 "api": "mm_run_host (pinned host m in, one DOPRI5 step, m out)"},
         "gpu_launches": launches, "clocks": clocks,
+        "graph_replay": {"value": units_all / graph_max, "ms_per_step": 1e3 * graph_max / args.steps, "unit": UNIT,
+                         "note": "same K steps, no CUDA events in the region: each step is one captured CUDA graph launch"},
         "roofline": {"bound": "hbm", "kernel": dom_name, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "peak_kind": peak_kind, "traffic": ncu_traffic(version, w.name, prec_name, dom_name),
                      "traffic_source": "profiles/ncu_traffic.csv row of this mm_version / workload / precision, else null",
                      "algorithmic_bytes_per_launch": dom_bytes, "avg_launch_ms": dom_avg, "kernel_ms": per,
                      "kernel_frac": {n: (ab["class"][n] / (per[n] * 1e-3) / 1e9 / peak if per[n] else None) for n in CLASSES},
                      "kernel_share": {n: prof_ms[i] / tot for i, n in enumerate(CLASSES)},
-                     "kernel_ms_source": f"{dom_name}: CUDA events inside the timed region; the other classes and kernel_share: a profiled "
+                     "kernel_ms_source": (f"{dom_name}: CUDA events over the warm-up steps (no events in the timed region: --no-kernel-events)" if args.no_kernel_events else
+                                          f"{dom_name}: CUDA events inside the timed region") + "; the other classes and kernel_share: a profiled "
                                          "pass of the same steps after it (all classes bracketed, ~3 % slower)",
                      "step_algorithmic_gbs": step_gbs, "step_frac": step_gbs / peak, "step_frac_nominal_8TBs": step_gbs / 8000.0,
                      "mm_version": version},
@@ -419,11 +440,12 @@ def run_mm(args):
                        "rhs_per_step": RHS_PER_STEP, "parallelism": f"replicas x{world}",
                        "l2": "working set (spectra + stage vectors > 1 GB) exceeds the 126 MB L2; no explicit flush"},
             "e2e": top["e2e"], "gpu_launches": top["gpu_launches"], "clocks": top["clocks"], "roofline": top["roofline"],
+            "graph_replay": top["graph_replay"],
             "cpu_baseline": cpu,
         }
         if len(precs) > 1:
             o = res["f64"]
-            line["fp64"] = {k: o[k] for k in ("value", "ms_per_step", "dtype", "e2e", "gpu_launches", "clocks", "roofline")}
+            line["fp64"] = {k: o[k] for k in ("value", "ms_per_step", "dtype", "e2e", "gpu_launches", "clocks", "roofline", "graph_replay")}
             line["fp64"]["unit"] = UNIT
         print(json.dumps(line), flush=True)
     if world > 1:
@@ -445,6 +467,7 @@ def main():
     ap.add_argument("--prec", default="both", choices=["f32", "f64", "both"])
     ap.add_argument("--workload", default="cfg4")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-kernel-events", action="store_true", help="no CUDA events inside the timed region (whole-step CUDA graphs stay on)")
     args = ap.parse_args()
     world_env = os.environ.get("WORLD_SIZE")
     if world_env is None and args.gpus > 1:

@@ -881,6 +881,11 @@ struct mm_sim {
     int A_cell, D_cell, H_cell;      // cell-based A / D / external field set (arrays in the workspace)
     int unx, uny, unz, embed;        // the caller's mesh; embed: it is not 2^k per axis and lives inside the padded mesh g
     long uN;
+    // whole-step CUDA graphs (one launch per step instead of ~30): captured on the second step with the same key
+    struct StepGraph { unsigned char key[256]; size_t key_len; cudaGraphExec_t exec; long launches; };
+    std::vector<StepGraph> graphs;
+    cudaStream_t cap_stream;         // capture happens on a private stream (the caller's may be the legacy default stream)
+    int use_graph;
     int use_b3;                      // pass B runs the half-tile form (a full py-row tile does not fit one CTA)
     size_t off_S2;                   // its output spectrum
     size_t off_ei, off_eo;           // embedding: inner-layout copies of the caller's input / output fields
@@ -1058,6 +1063,7 @@ extern "C" int mm_create(mm_sim** out, int nx, int ny, int nz, double dx, double
     nx = next_pow2(nx); ny = next_pow2(ny); nz = next_pow2(nz);
     if ((long)nx * ny * nz > (1L << 30)) return MM_ERR_UNSUPPORTED;
     mm_sim* s = new mm_sim();
+    s->cap_stream = nullptr; s->use_graph = getenv("MM_NO_GRAPH") ? 0 : 1;
     s->unx = unx; s->uny = uny; s->unz = unz; s->uN = (long)unx * uny * unz;
     s->embed = (unx != nx || uny != ny || unz != nz) ? 1 : 0;
     s->prec = prec; s->device = device; s->stream = static_cast<cudaStream_t>(cuda_stream);
@@ -1084,7 +1090,11 @@ extern "C" int mm_create(mm_sim** out, int nx, int ny, int nz, double dx, double
 
 extern "C" int mm_destroy(mm_sim* s)
 {
-    if (s) for (cudaEvent_t e : s->prof_ev) cudaEventDestroy(e);
+    if (s) {
+        for (cudaEvent_t e : s->prof_ev) cudaEventDestroy(e);
+        for (auto& g : s->graphs) if (g.exec) cudaGraphExecDestroy(g.exec);
+        if (s->cap_stream) cudaStreamDestroy(s->cap_stream);
+    }
     delete s;
     return MM_OK;
 }
@@ -1741,9 +1751,66 @@ template <typename T> static int enqueue_step(mm_sim* s, T* m, int ctrl_mode)
     return MM_OK;
 }
 
-static int enqueue_step_any(mm_sim* s, void* m, int ctrl_mode)
+static int enqueue_step_eager(mm_sim* s, void* m, int ctrl_mode)
 {
     return s->prec == MM_F64 ? enqueue_step<double>(s, (double*)m, ctrl_mode) : enqueue_step<float>(s, (float*)m, ctrl_mode);
+}
+
+// Everything a captured step bakes into its kernel arguments: a graph is replayed only while all of it is unchanged.
+// (dt, tol, the clock, the thermal attempt counter and m itself live in device memory and are read at run time.)
+static size_t step_key(const mm_sim* s, const void* m, int ctrl_mode, unsigned char* out)
+{
+    size_t n = 0;
+    auto put = [&](const void* p, size_t b) { memcpy(out + n, p, b); n += b; };
+    put(&m, sizeof(m)); put(&ctrl_mode, sizeof(int)); put(&s->ws, sizeof(void*));
+    put(&s->A, sizeof(double)); put(&s->D, sizeof(double)); put(&s->Ku, sizeof(double)); put(&s->Kc, sizeof(double));
+    put(s->u, sizeof(s->u)); put(s->hext, sizeof(s->hext)); put(&s->alpha, sizeof(double)); put(&s->gamma, sizeof(double));
+    put(&s->dmi_kind, sizeof(int)); put(&s->integ, sizeof(int)); put(&s->demag_on, sizeof(int)); put(&s->demag_ready, sizeof(int));
+    put(&s->A_cell, sizeof(int)); put(&s->D_cell, sizeof(int)); put(&s->H_cell, sizeof(int));
+    put(s->stt_u, sizeof(s->stt_u)); put(&s->stt_beta, sizeof(double)); put(&s->sl_aJ, sizeof(double)); put(&s->sl_bJ, sizeof(double));
+    put(s->sl_p, sizeof(s->sl_p)); put(&s->temperature, sizeof(double)); put(&s->th_seed, sizeof(s->th_seed));
+    return n;
+}
+
+// One step: replayed from a captured CUDA graph when possible (SURVEY 7 hard part 5: small meshes are launch bound —
+// ~30 kernels of a few microseconds each per DOPRI5 step), enqueued kernel by kernel otherwise.
+static int enqueue_step_any(mm_sim* s, void* m, int ctrl_mode)
+{
+    if (!s->use_graph || s->prof_on) return enqueue_step_eager(s, m, ctrl_mode);
+    unsigned char key[256];
+    const size_t klen = step_key(s, m, ctrl_mode, key);
+    mm_sim::StepGraph* e = nullptr;
+    for (auto& g : s->graphs) if (g.key_len == klen && memcmp(g.key, key, klen) == 0) { e = &g; break; }
+    if (!e) {      // first step with this key: run it eagerly (this also sets the kernels' shared-memory attributes)
+        if (s->graphs.size() >= 8) { if (s->graphs[0].exec) cudaGraphExecDestroy(s->graphs[0].exec); s->graphs.erase(s->graphs.begin()); }
+        mm_sim::StepGraph g;
+        memcpy(g.key, key, klen); g.key_len = klen; g.exec = nullptr; g.launches = 0;
+        s->graphs.push_back(g);
+        return enqueue_step_eager(s, m, ctrl_mode);
+    }
+    if (!e->exec) {      // second step: capture
+        if (!s->cap_stream && cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); s->use_graph = 0; return enqueue_step_eager(s, m, ctrl_mode); }
+        cudaStream_t user = s->stream;
+        const long l0 = s->launches;
+        cudaGraph_t graph = nullptr;
+        if (cudaStreamBeginCapture(s->cap_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); s->use_graph = 0; return enqueue_step_eager(s, m, ctrl_mode); }
+        s->stream = s->cap_stream;
+        const int rc = enqueue_step_eager(s, m, ctrl_mode);
+        s->stream = user;
+        const cudaError_t ce = cudaStreamEndCapture(s->cap_stream, &graph);
+        e->launches = s->launches - l0;
+        s->launches = l0;
+        if (rc != MM_OK || ce != cudaSuccess || !graph || cudaGraphInstantiate(&e->exec, graph, 0) != cudaSuccess) {
+            cudaGetLastError();
+            if (graph) cudaGraphDestroy(graph);
+            e->exec = nullptr; s->use_graph = 0;
+            return enqueue_step_eager(s, m, ctrl_mode);
+        }
+        cudaGraphDestroy(graph);
+    }
+    MM_TRY(s, cudaGraphLaunch(e->exec, s->stream));
+    s->launches += e->launches;
+    return MM_OK;
 }
 
 static int read_state(mm_sim* s, DevState* h)
