@@ -100,12 +100,13 @@ __global__ void __launch_bounds__(512) y_conv3_kernel(Geom g, const cx<T>* S, cx
 }
 // compile-time specialised form of the TMA pass B (mm_passB7.cuh): ny = 2^LOGM; fp32: TC = 4, 256 threads; fp64: TC = 2,
 // 128 threads (rows of 32 bytes and tiles of py * 96 bytes in both; two CTAs per SM)
+// ny = 1024: one CTA per SM with twice the threads (tile py * 96 bytes = 196 KB)
 template <typename T, int LOGM, bool IS3D>
-__global__ void __launch_bounds__(sizeof(T) == 8 ? 128 : 256, 2) y_conv7_kernel(Geom g, cx<T>* S, const T* Kc, twiddles<T> tw, int logtw, const DevState* st,
+__global__ void __launch_bounds__((sizeof(T) == 8 ? 128 : 256) * (LOGM >= 10 ? 2 : 1), LOGM >= 10 ? 1 : 2) y_conv7_kernel(Geom g, cx<T>* S, const T* Kc, twiddles<T> tw, int logtw, const DevState* st,
                                                                                 const __grid_constant__ CUtensorMap tmS)
 {
     __shared__ __align__(8) unsigned long long bar[3];
-    constexpr int LOGTC = sizeof(T) == 8 ? 1 : 2, NTHR = sizeof(T) == 8 ? 128 : 256;
+    constexpr int LOGTC = sizeof(T) == 8 ? 1 : 2, NTHR = (sizeof(T) == 8 ? 128 : 256) * (LOGM >= 10 ? 2 : 1);
     y_conv_body7<LOGM, LOGTC, IS3D, NTHR, T>(g, S, Kc, tw, logtw, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, NTHR, &tmS, bar, &st->done);
 }
 template <typename T, int NZ>
@@ -1001,8 +1002,11 @@ static void configure(mm_sim* s)
     if (s->prec == MM_F32 && !getenv("MM_TC") && g.TC >= 4 && (size_t)smemB_elems(g) * cs > 98 * 1024) g.TC /= 2;
     while (g.TC > 2 && ((g.nx + g.TC) / g.TC) * g.pz < target && !s->use_b3) g.TC /= 2;
     // fp64: the specialised pass B (mm_passB7.cuh) wants rows of 32 bytes = two columns, tiles of py * 96 bytes
-    const bool b7_f64 = s->prec == MM_F64 && !getenv("MM_TC") && !s->no_b7 && !s->use_b3 && s->use_v2 && g.logny >= 4 && g.logny <= 9 && g.TC >= 2;
+    const bool b7_f64 = s->prec == MM_F64 && !getenv("MM_TC") && !s->no_b7 && !s->use_b3 && s->use_v2 && g.logny >= 4 && g.logny <= 10 && g.TC >= 2;
     if (b7_f64) g.TC = 2;
+    // ny = 1024: the specialised pass B with one 196 KB tile per SM (rows of 32 bytes in both precisions)
+    const bool b7_10 = g.logny == 10 && !getenv("MM_TC") && !s->no_b7 && !s->use_b3 && s->use_v2 && !getenv("MM_NO_B7_10");
+    if (b7_10 && s->prec == MM_F32) g.TC = 4;
     g.Lx = ((g.nx + 1 + g.TC - 1) / g.TC) * g.TC;
     g.plane = (long)g.ny * g.Lx;
     g.comp = (long)g.pz * g.plane;
@@ -1015,6 +1019,7 @@ static void configure(mm_sim* s)
     s->thrA = 256;
     s->thrB = (s->prec == MM_F32 && s->smemB > 98 * 1024) ? 512 : 256;
     if (b7_f64) s->thrB = 128;
+    if (b7_10) s->thrB = s->prec == MM_F64 ? 256 : 512;
     if (s->use_b3) s->thrB = (g.ny / 8) * (g.TC / (s->prec == MM_F32 && g.TC % 2 == 0 ? 2 : 1)) >= 512 ? 512 : 256;
     if (getenv("MM_THRB")) s->thrB = atoi(getenv("MM_THRB"));
 }
@@ -1491,7 +1496,8 @@ template <typename T, int V> static void launch_B5(mm_sim* s, unsigned grid, cx<
 template <typename T> static bool b7_applies(const mm_sim* s)
 {
     const Geom& g = s->g;
-    return s->use_v2 && !s->no_b7 && !s->use_b3 && g.logny >= 4 && g.logny <= 9 && g.TC == (sizeof(T) == 8 ? 2 : 4) && s->thrB == (sizeof(T) == 8 ? 128 : 256);
+    return s->use_v2 && !s->no_b7 && !s->use_b3 && g.logny >= 4 && g.logny <= 10 && g.TC == (sizeof(T) == 8 ? 2 : 4) &&
+           s->thrB == (sizeof(T) == 8 ? 128 : 256) * (g.logny >= 10 ? 2 : 1);
 }
 template <typename T, int LOGM, bool IS3D> static void launch_B7(mm_sim* s, unsigned grid, cx<T>* S, twiddles<T> tw, const DevState* st)
 {
@@ -1506,7 +1512,7 @@ template <typename T> static bool try_launch_B7(mm_sim* s, unsigned grid, cx<T>*
     const bool d3 = g.nz > 1;
     switch (g.logny) {
 #define MM_B7_CASE(L) case L: if (d3) launch_B7<T, L, true>(s, grid, S, tw, st); else launch_B7<T, L, false>(s, grid, S, tw, st); return true;
-        MM_B7_CASE(4) MM_B7_CASE(5) MM_B7_CASE(6) MM_B7_CASE(7) MM_B7_CASE(8) MM_B7_CASE(9)
+        MM_B7_CASE(4) MM_B7_CASE(5) MM_B7_CASE(6) MM_B7_CASE(7) MM_B7_CASE(8) MM_B7_CASE(9) MM_B7_CASE(10)
 #undef MM_B7_CASE
         default: return false;
     }

@@ -76,7 +76,7 @@ static void run(int ver, int nx, int ny, int nz, int G, int CH, int TC, const do
             CASE_A(1) CASE_A(2) CASE_A(4) CASE_A(8) CASE_A(16) CASE_A(32)
         }
     }
-    const bool b7 = ver == 7 && TC == (sizeof(T) == 8 ? 2 : 4) && ny >= 16 && ny <= 512;
+    const bool b7 = ver == 7 && TC == (sizeof(T) == 8 ? 2 : 4) && ny >= 16 && ny <= 1024;
     unsigned long long* nobar = nullptr;
     constexpr int LOGTC7 = sizeof(T) == 8 ? 1 : 2;
     const bool b3 = ver == 3 && ny >= 16;
@@ -89,7 +89,7 @@ static void run(int ver, int nx, int ny, int nz, int G, int CH, int TC, const do
             switch (g.logny * 2 + (nz > 1)) {
 #define CASE_B7(L) case 2 * L: y_conv_body7<L, LOGTC7, false, 1, T>(g, S.data(), Kc.data(), tw, ilog2(twN), smem.data(), b, 0, 1, nullptr, nobar, nullptr); break; \
                    case 2 * L + 1: y_conv_body7<L, LOGTC7, true, 1, T>(g, S.data(), Kc.data(), tw, ilog2(twN), smem.data(), b, 0, 1, nullptr, nobar, nullptr); break;
-                CASE_B7(4) CASE_B7(5) CASE_B7(6) CASE_B7(7) CASE_B7(8) CASE_B7(9)
+                CASE_B7(4) CASE_B7(5) CASE_B7(6) CASE_B7(7) CASE_B7(8) CASE_B7(9) CASE_B7(10)
             }
         } else if (b5) {
             if (sizeof(T) == 4 && TC % 2 == 0) y_conv_body5<T, (sizeof(T) == 4 ? 2 : 1)>(g, S.data(), Kc.data(), tw, smem.data(), b, 0, 1, nullptr, nullptr);

@@ -64,6 +64,8 @@ CASES = {
     "slab_128x32x4": lambda: small3d(128, 32, 4),
     "film_128_masked": lambda: film(128, mask=True),
     "film_512": lambda: film(512),
+    "slab_32x1024x2_b7_ny1024": lambda: small3d(32, 1024, 2),
+    "film_64x1024_b7_ny1024": lambda: small3d(64, 1024, 1, kind=wl.DMI_INTERFACIAL),
     "film_4x2": lambda: wl.cfg5(4).__class__("tiny", 4, 2, 1, 4e-9, 4e-9, 4e-9, Ms=8e5, A=1.3e-11, m0=wl.random_unit(3, 4, 2, 1)),
 }
 

@@ -137,7 +137,7 @@ def test_cell_based_local_field_matches_oracle(emul, kind, use):
 
 
 @pytest.mark.parametrize("prec64", [0, 1])
-@pytest.mark.parametrize("shape", [(16, 16, 1), (8, 32, 2), (32, 64, 1), (8, 128, 2), (4, 256, 1), (4, 512, 1), (4, 512, 2), (16, 64, 4)])
+@pytest.mark.parametrize("shape", [(16, 16, 1), (8, 32, 2), (32, 64, 1), (8, 128, 2), (4, 256, 1), (4, 512, 1), (4, 512, 2), (16, 64, 4), (4, 1024, 1), (4, 1024, 2)])
 def test_specialised_pass_B_matches_oracle(emul, shape, prec64):
     """mm_passB7.cuh (compile-time ny; fp32 with TC = 4, fp64 with TC = 2): every instantiated ny, films and 3-D."""
     nx, ny, nz = shape
