@@ -32,9 +32,17 @@ struct Geom {
     long kplane;           // (ny+1) * Lx    (one kz' plane of K^)
     long kcomp;            // (nz>1 ? nz+1 : 1) * kplane
     int flags;             // tuning bits (MM_FLAGS), 0 = defaults
+    int xpad;              // passes A / C (v3 bodies): x tile with one pad point per 8 points and pitch = L (few lines)
 };
 
 MM_HD int odd_pitch(int n) { return n | 1; }
+// x tile of the v3 passes A / C.  Many lines (L >= 16): pitch L|1, a half-warp covers 16 lines of one point.  Few
+// lines (long film lines, L <= 4): the late radix-8 stages would step through the tile with a stride that is a multiple of the
+// 32 banks, so point p lives at padded position p + p/8 and the pitch is L itself: a half-warp's 16 (line, butterfly)
+// pairs then fall on 32 distinct words at every stage.  ppos is additive over multiples of 8 (all stage strides are).
+MM_HD int ppos(int p, int pad) { return pad ? p + (p >> 3) : p; }
+MM_HD int x_pitch(const Geom& g) { return g.xpad ? g.G * g.nz : odd_pitch(g.G * g.nz); }
+MM_HD long smemA2_elems(const Geom& g) { return (long)(ppos(g.nx, g.xpad) + 1) * x_pitch(g); }
 
 // K^ in the order pass B (v2) consumes it, "Kc": one contiguous tile per (kz', x tile).  The multiply stage
 // works on radix-8 blocks b8 of the bit-reversed y spectrum: slot r of block b8 holds ky = brev3(r)*nbk + beta,

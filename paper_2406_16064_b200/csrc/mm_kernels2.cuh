@@ -410,9 +410,10 @@ MM_HD void xA_first(const Geom& g, const T* mc, const T* Ms, cx<T>* s, int pitch
 #pragma unroll
                 for (int r = 1; r < R; r++) { a[r] = cmul(a[r], pw[r]); u[r] = cmul(u[r], pw[r]); }
             }
-            cx<T>* dst = s + i * pitch + l;
+            cx<T>* dst = s + ppos(i, g.xpad) * pitch + l;
+            const int sp = ppos(sub, g.xpad) * pitch, mp = ppos(m, g.xpad) * pitch;
 #pragma unroll
-            for (int r = 0; r < R; r++) { dst[r * sub * pitch] = a[r]; dst[(m + r * sub) * pitch] = u[r]; }
+            for (int r = 0; r < R; r++) { dst[r * sp] = a[r]; dst[mp + r * sp] = u[r]; }
         }
     }
 }
@@ -432,10 +433,11 @@ MM_HD void xC_last(const Geom& g, T* Hc, const cx<T>* s, int pitch, int j0, T in
         for (int l = tid >> logisub; l < L; l += lstep) {
             const int gg = l >> lognz, z = l & (g.nz - 1);
             T* hrow = Hc + ((long)z * g.ny + (j0 + gg)) * g.nx + 2 * i;
-            const cx<T>* src = s + i * pitch + l;
+            const cx<T>* src = s + ppos(i, g.xpad) * pitch + l;
+            const int sp = ppos(sub, g.xpad) * pitch, mp = ppos(m, g.xpad) * pitch;
             cx<T> a[R], u[R];
 #pragma unroll
-            for (int r = 0; r < R; r++) { a[r] = src[r * sub * pitch]; u[r] = src[(m + r * sub) * pitch]; }
+            for (int r = 0; r < R; r++) { a[r] = src[r * sp]; u[r] = src[mp + r * sp]; }
             if (R > 1 && i != 0) {
 #pragma unroll
                 for (int r = 1; r < R; r++) { a[r] = cmulc(a[r], pw[r]); u[r] = cmulc(u[r], pw[r]); }
@@ -449,42 +451,6 @@ MM_HD void xC_last(const Geom& g, T* Hc, const cx<T>* s, int pitch, int j0, T in
     }
 }
 
-// split (DIR 0: Z -> X half spectrum) / merge (DIR 1: X -> 2Z) of the packed real transform
-template <typename T, int DIR>
-MM_HD void x_split_merge(const Geom& g, cx<T>* s, int pitch, twiddles<T> tw, int tid, int nthr)
-{
-    const int n = g.nx, h = n / 2, L = g.G * g.nz, logL = ilog2(L);
-    for (int f = tid; f < L * (h + 1); f += nthr) {
-        const int l = f & (L - 1), k = f >> logL;
-        if (k == 0) {
-            if (DIR == 0) {
-                const cx<T> z0 = s[l];
-                s[l] = mk<T>(z0.x + z0.y, (T)0);
-                s[n * pitch + l] = mk<T>(z0.x - z0.y, (T)0);
-            } else {
-                const cx<T> A = s[l], B = conj(s[n * pitch + l]);
-                s[l] = (A + B) + mul_pi(A - B);
-            }
-        } else if (k == h) {
-            const int p = (int)brev(k, g.lognx) * pitch + l;
-            s[p] = DIR == 0 ? conj(s[p]) : scale(conj(s[p]), (T)2);
-        } else {
-            const int pa = (int)brev(k, g.lognx) * pitch + l, pb = (int)brev(n - k, g.lognx) * pitch + l;
-            const cx<T> A = s[pa], B = conj(s[pb]);
-            if (DIR == 0) {
-                const cx<T> E = scale(A + B, (T)0.5), D = scale(A - B, (T)0.5);
-                const cx<T> t = cmul(tw.get(k, 2 * n), D);
-                s[pa] = E + mul_mi(t);
-                s[pb] = conj(E) + mul_mi(conj(t));
-            } else {
-                const cx<T> E = A + B, O = cmulc(A - B, tw.get(k, 2 * n));
-                s[pa] = E + mul_pi(O);
-                s[pb] = conj(E) + mul_pi(conj(O));
-            }
-        }
-    }
-}
-
 // z transform in registers, inverse + crop: S -> tile
 template <typename T, int NZ>
 MM_HD void zC_regs(const Geom& g, const cx<T>* Sc, cx<T>* s, int pitch, int j0, twiddles<T> tw, int tid, int nthr)
@@ -492,7 +458,7 @@ MM_HD void zC_regs(const Geom& g, const cx<T>* Sc, cx<T>* s, int pitch, int j0, 
     const int np = g.nx + 1;
     for (int f = tid; f < np * g.G; f += nthr) {
         const int xp = f % np, gg = f / np;
-        cx<T>* dst = s + xp * pitch + gg * NZ;
+        cx<T>* dst = s + ppos(xp, g.xpad) * pitch + gg * NZ;
         const cx<T>* src = Sc + (long)(j0 + gg) * g.Lx + xp;
         cx<T> a[NZ], u[NZ];
 #pragma unroll

@@ -983,6 +983,8 @@ static void configure(mm_sim* s)
     g.G = G;
     g.CH = 64;
     if (g.nz > 1) while (g.CH > 8 && (size_t)g.pz * g.G * g.CH * cs > 32 * 1024) g.CH /= 2;
+    // at most 4 lines per CTA (long film lines): padded x tile, see ppos() in mm_kernels.cuh (measured: 4096^2 pass A 673 -> 568 us, 2048^2 168 -> 158; with 8 lines it is slower, 1024^2 41 -> 53 us)
+    g.xpad = g.G * g.nz <= 4 ? 1 : 0;
     // <= 100 KB: two CTAs per SM (one 200 KB tile per SM measured 15-30 % slower on films of 2048^2 and 4096^2)
     while (g.G > 1 && (size_t)smemA_elems(g) * cs > 100 * 1024) g.G /= 2;
     // pass B: TC columns per CTA
@@ -1015,7 +1017,8 @@ static void configure(mm_sim* s)
     g.kcomp = (long)(g.nz > 1 ? g.nz + 1 : 1) * g.kplane;
     s->smemA = (size_t)smemA_elems(g) * cs;
     // the v2 bodies of passes A / C do the z transform in registers: no scratch tile
-    s->smemA2 = (size_t)(g.nx + 1) * odd_pitch(g.G * g.nz) * cs;
+    g.xpad = g.G * g.nz <= 4 ? 1 : 0;      // G may have shrunk above
+    s->smemA2 = (size_t)smemA2_elems(g) * cs;
     s->smemB = s->use_b3 ? (size_t)smemB3_elems(g) * cs : (size_t)smemB_elems(g) * cs;
     s->thrA = 256;
     s->thrB = (s->prec == MM_F32 && s->smemB > 98 * 1024) ? 512 : 256;

@@ -18,17 +18,17 @@ namespace mm {
 
 // radix-8 stage on blocks of length Lc of n-point lines; lanes run over lines, TB blocks per thread
 template <typename T, int DIR, int TB>
-MM_HD void xs_mid8b(cx<T>* s, int pitch, int L, int n, int Lc, twiddles<T> tw, int tid, int nthr)
+MM_HD void xs_mid8b(cx<T>* s, int pitch, int pad, int L, int n, int Lc, twiddles<T> tw, int tid, int nthr)
 {
     const int logL = ilog2(L), sub = Lc >> 3, logsub = ilog2(sub);
-    const int stride = sub * pitch, bstride = Lc * pitch;
+    const int stride = ppos(sub, pad) * pitch, bstride = ppos(Lc, pad) * pitch;
     const int nitem = L * sub * ((n / Lc) / TB);
     for (int f = tid; f < nitem; f += nthr) {
         const int l = f & (L - 1), rest = f >> logL;
         const int i = rest & (sub - 1), bg = rest >> logsub;
         cx<T> pw[8];
         if (i != 0) twiddle_powers<T, 8>(tw.get(i, Lc), pw);
-        cx<T>* p = s + (bg * TB * Lc + i) * pitch + l;
+        cx<T>* p = s + (bg * TB * ppos(Lc, pad) + ppos(i, pad)) * pitch + l;
 #pragma unroll
         for (int t = 0; t < TB; t++, p += bstride) {
             cx<T> v[8];
@@ -54,12 +54,12 @@ MM_HD void xs_mid8b(cx<T>* s, int pitch, int L, int n, int Lc, twiddles<T> tw, i
 }
 
 template <typename T, int DIR>
-MM_HD void xs_mid8_any(cx<T>* s, int pitch, int L, int n, int Lc, twiddles<T> tw, int tid, int nthr)
+MM_HD void xs_mid8_any(cx<T>* s, int pitch, int pad, int L, int n, int Lc, twiddles<T> tw, int tid, int nthr)
 {
     const int nblk = n / Lc;
-    if (nblk % 4 == 0) xs_mid8b<T, DIR, 4>(s, pitch, L, n, Lc, tw, tid, nthr);
-    else if (nblk % 2 == 0) xs_mid8b<T, DIR, 2>(s, pitch, L, n, Lc, tw, tid, nthr);
-    else xs_mid8b<T, DIR, 1>(s, pitch, L, n, Lc, tw, tid, nthr);
+    if (nblk % 4 == 0) xs_mid8b<T, DIR, 4>(s, pitch, pad, L, n, Lc, tw, tid, nthr);
+    else if (nblk % 2 == 0) xs_mid8b<T, DIR, 2>(s, pitch, pad, L, n, Lc, tw, tid, nthr);
+    else xs_mid8b<T, DIR, 1>(s, pitch, pad, L, n, Lc, tw, tid, nthr);
 }
 
 // padded z transform of the NZ values a[] of one (row, x position) and store to S (NZ = 1: plain store)
@@ -94,13 +94,13 @@ MM_HD void zA_split_regs(const Geom& g, cx<T>* Sc, const cx<T>* s, int pitch, in
     for (int f = tid; f < n * g.G; f += nthr) {
         const int xp = f & (n - 1), gg = f >> lognx;
         const int k = (int)brev((unsigned)xp, lognx);
-        const cx<T>* pa = s + xp * pitch + gg * NZ;
+        const cx<T>* pa = s + ppos(xp, g.xpad) * pitch + gg * NZ;
         cx<T> a[NZ];
         if (k == 0) {
 #pragma unroll
             for (int z = 0; z < NZ; z++) { const cx<T> z0 = pa[z]; a[z] = mk<T>(z0.x + z0.y, (T)0); }
         } else {
-            const cx<T>* pb = s + (int)brev((unsigned)(n - k), lognx) * pitch + gg * NZ;
+            const cx<T>* pb = s + ppos((int)brev((unsigned)(n - k), lognx), g.xpad) * pitch + gg * NZ;
             const cx<T> w = tw.get(k, 2 * n);
             const cx<T> w2 = mk<T>((T)0.5 * w.y, (T)-0.5 * w.x);      // -i w / 2
 #pragma unroll
@@ -127,14 +127,14 @@ MM_HD void fwd_xz_body3(const Geom g, const T* __restrict__ mvec, const T* __res
                         twiddles<T> tw, cx<T>* s, int bid, int tid, int nthr)
 {
     const int c = bid % 3, j0 = (bid / 3) * g.G;
-    const int n = g.nx, m = n / 2, L = g.G * g.nz, pitch = odd_pitch(L);
+    const int n = g.nx, m = n / 2, L = g.G * g.nz, pitch = x_pitch(g);
     const T* mc = mvec + (long)c * g.N;
     const int R1 = first_radix(m);
     if (R1 == 8) xA_first<T, 8>(g, mc, Ms, s, pitch, j0, tw, tid, nthr);
     else if (R1 == 4) xA_first<T, 4>(g, mc, Ms, s, pitch, j0, tw, tid, nthr);
     else xA_first<T, 2>(g, mc, Ms, s, pitch, j0, tw, tid, nthr);
     MM_SYNC();
-    for (int Lc = m / R1; Lc > 1; Lc >>= 3) { xs_mid8_any<T, 0>(s, pitch, L, n, Lc, tw, tid, nthr); MM_SYNC(); }
+    for (int Lc = m / R1; Lc > 1; Lc >>= 3) { xs_mid8_any<T, 0>(s, pitch, g.xpad, L, n, Lc, tw, tid, nthr); MM_SYNC(); }
     zA_split_regs<T, NZ>(g, S + (long)c * g.comp, s, pitch, j0, tw, tid, nthr);
 }
 
@@ -150,7 +150,7 @@ MM_HD void xC_merge8(const Geom& g, cx<T>* s, int pitch, int L, twiddles<T> tw, 
     const int n = g.nx, nb = n >> 3, logb = g.lognx - 3, logL = ilog2(L);
     for (int f = tid; f < (nb / 2 + 1) * L; f += nthr) {
         const int l = f & (L - 1), beta = f >> logL;
-        cx<T>* pA = s + (int)brev((unsigned)beta, logb) * 8 * pitch + l;
+        cx<T>* pA = s + ppos((int)brev((unsigned)beta, logb) * 8, g.xpad) * pitch + l;
         cx<T> w[8];
 #pragma unroll
         for (int r = 0; r < 8; r++) w[r] = tw.get((int)brev((unsigned)r, 3) * nb + beta, 2 * n);
@@ -158,7 +158,7 @@ MM_HD void xC_merge8(const Geom& g, cx<T>* s, int pitch, int L, twiddles<T> tw, 
 #pragma unroll
         for (int r = 0; r < 8; r++) ZA[r] = pA[r * pitch];
         if (beta != 0 && beta != nb / 2) {
-            cx<T>* pB = s + (int)brev((unsigned)(nb - beta), logb) * 8 * pitch + l;
+            cx<T>* pB = s + ppos((int)brev((unsigned)(nb - beta), logb) * 8, g.xpad) * pitch + l;
             cx<T> ZB[8];
 #pragma unroll
             for (int r = 0; r < 8; r++) ZB[r] = pB[r * pitch];
@@ -182,7 +182,7 @@ MM_HD void xC_merge8(const Geom& g, cx<T>* s, int pitch, int L, twiddles<T> tw, 
             }
         } else {                     // block 0: k = rho*nb; r=0 <-> Nyquist slot, r=1 is k = n/2, pairs (4,7) (2,3) (6,5)
             {
-                const cx<T> A = ZA[0], B = conj(s[n * pitch + l]);
+                const cx<T> A = ZA[0], B = conj(s[ppos(n, g.xpad) * pitch + l]);
                 ZA[0] = (A + B) + mul_pi(A - B);
             }
             ZA[1] = scale(conj(ZA[1]), (T)2);
@@ -206,12 +206,12 @@ MM_HD void inv_zx_body3(const Geom g, const cx<T>* __restrict__ S, T* __restrict
                         cx<T>* s, int bid, int tid, int nthr)
 {
     const int c = bid % 3, j0 = (bid / 3) * g.G;
-    const int n = g.nx, m = n / 2, L = g.G * g.nz, pitch = odd_pitch(L);
+    const int n = g.nx, m = n / 2, L = g.G * g.nz, pitch = x_pitch(g);
     const cx<T>* Sc = S + (long)c * g.comp;
     if (NZ == 1) {
         for (int f = tid; f < L * (n + 1); f += nthr) {
             const int xp = f % (n + 1), l = f / (n + 1);
-            s[xp * pitch + l] = Sc[(long)(j0 + l) * g.Lx + xp];
+            s[ppos(xp, g.xpad) * pitch + l] = Sc[(long)(j0 + l) * g.Lx + xp];
         }
     } else {
         zC_regs<T, NZ>(g, Sc, s, pitch, j0, tw, tid, nthr);
@@ -220,7 +220,7 @@ MM_HD void inv_zx_body3(const Geom g, const cx<T>* __restrict__ S, T* __restrict
     xC_merge8<T>(g, s, pitch, L, tw, tid, nthr);
     MM_SYNC();
     const int R1 = first_radix(m);
-    for (int Lc = 64; Lc <= m / R1; Lc <<= 3) { xs_mid8_any<T, 1>(s, pitch, L, n, Lc, tw, tid, nthr); MM_SYNC(); }
+    for (int Lc = 64; Lc <= m / R1; Lc <<= 3) { xs_mid8_any<T, 1>(s, pitch, g.xpad, L, n, Lc, tw, tid, nthr); MM_SYNC(); }
     T* Hc = Hd + (long)c * g.N;
     if (R1 == 8) xC_last<T, 8>(g, Hc, s, pitch, j0, inv_scale, tw, tid, nthr);
     else if (R1 == 4) xC_last<T, 4>(g, Hc, s, pitch, j0, inv_scale, tw, tid, nthr);

@@ -2,6 +2,7 @@
 // paper_2406_16064_b200/csrc with g++ and runs every CTA sequentially with one "thread"
 // (tid = 0, nthr = 1).  TEST HARNESS ONLY — checks the index arithmetic of the kernels on a box
 // without a GPU; it is not a product path and nothing in the package loads it.
+#include <algorithm>
 #include <cmath>
 #include <cstring>
 #include <vector>
@@ -33,6 +34,7 @@ static Geom make_geom(int nx, int ny, int nz, int G, int CH, int TC)
     g.lognx = ilog2(nx); g.logny = ilog2(ny); g.logpy = ilog2(g.py); g.logpz = ilog2(g.pz);
     g.N = (long)nx * ny * nz;
     g.G = G; g.CH = CH; g.TC = TC;
+    g.xpad = G * nz <= 4 ? 1 : 0;      // the library's rule (configure() in mm_lib.cu)
     g.Lx = ((nx + 1 + TC - 1) / TC) * TC;
     g.plane = (long)ny * g.Lx; g.comp = (long)g.pz * g.plane;
     g.kplane = (long)(ny + 1) * g.Lx; g.kcomp = (long)(nz > 1 ? nz + 1 : 1) * g.kplane;
@@ -65,7 +67,7 @@ static void run(int ver, int nx, int ny, int nz, int G, int CH, int TC, const do
     for (long i = 0; i < g.N; i++) Mst[i] = (T)Ms[i];
     std::vector<cx<T>> S((size_t)3 * g.comp);
     memset(S.data(), 0, S.size() * sizeof(cx<T>));
-    std::vector<cx<T>> smem((size_t)(smemA_elems(g) > smemB_elems(g) ? smemA_elems(g) : smemB_elems(g)) + 16);
+    std::vector<cx<T>> smem((size_t)std::max(std::max(smemA_elems(g), smemA2_elems(g)), smemB_elems(g)) + 16);
     const int gridA = 3 * (ny / G), gridB = (g.Lx / TC) * g.pz;
     const double P = (double)g.px * g.py * g.pz;
     const bool a2 = ver >= 2 && nx >= 32 && nz <= 32, b2 = ver >= 2 && ny >= 16, b5 = (ver == 5 || ver == 7) && ny >= 16;
