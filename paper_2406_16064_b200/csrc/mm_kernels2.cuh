@@ -381,7 +381,7 @@ MM_HD void y_conv_body5(const Geom g, cx<T>* __restrict__ S, const T* __restrict
 // first x stage: load Ms*m pairs from global (i fastest: coalesced), pad twiddle, radix R, both blocks.
 // A thread keeps one i (butterfly index) and walks the lines: the pad twiddles w_n^(i + r sub) and the
 // stage twiddles are loaded / formed once per thread, not once per line.
-template <typename T, int R>
+template <typename T, int R, bool PAD>
 MM_HD void xA_first(const Geom& g, const T* mc, const T* Ms, cx<T>* s, int pitch, int j0, twiddles<T> tw, int tid, int nthr)
 {
     const int n = g.nx, m = n / 2, sub = m / R, L = g.G * g.nz, lognz = ilog2(g.nz);
@@ -410,8 +410,8 @@ MM_HD void xA_first(const Geom& g, const T* mc, const T* Ms, cx<T>* s, int pitch
 #pragma unroll
                 for (int r = 1; r < R; r++) { a[r] = cmul(a[r], pw[r]); u[r] = cmul(u[r], pw[r]); }
             }
-            cx<T>* dst = s + ppos(i, g.xpad) * pitch + l;
-            const int sp = ppos(sub, g.xpad) * pitch, mp = ppos(m, g.xpad) * pitch;
+            cx<T>* dst = s + ppos(i, PAD) * pitch + l;
+            const int sp = ppos(sub, PAD) * pitch, mp = ppos(m, PAD) * pitch;
 #pragma unroll
             for (int r = 0; r < R; r++) { dst[r * sp] = a[r]; dst[mp + r * sp] = u[r]; }
         }
@@ -420,7 +420,7 @@ MM_HD void xA_first(const Geom& g, const T* mc, const T* Ms, cx<T>* s, int pitch
 
 // last x stage of pass C: inverse radix R on both blocks, crop combine, scale, store H_d pairs (same
 // thread -> (i, lines) mapping as xA_first)
-template <typename T, int R>
+template <typename T, int R, bool PAD>
 MM_HD void xC_last(const Geom& g, T* Hc, const cx<T>* s, int pitch, int j0, T inv_scale, twiddles<T> tw, int tid, int nthr)
 {
     const int n = g.nx, m = n / 2, sub = m / R, L = g.G * g.nz, lognz = ilog2(g.nz);
@@ -433,8 +433,8 @@ MM_HD void xC_last(const Geom& g, T* Hc, const cx<T>* s, int pitch, int j0, T in
         for (int l = tid >> logisub; l < L; l += lstep) {
             const int gg = l >> lognz, z = l & (g.nz - 1);
             T* hrow = Hc + ((long)z * g.ny + (j0 + gg)) * g.nx + 2 * i;
-            const cx<T>* src = s + ppos(i, g.xpad) * pitch + l;
-            const int sp = ppos(sub, g.xpad) * pitch, mp = ppos(m, g.xpad) * pitch;
+            const cx<T>* src = s + ppos(i, PAD) * pitch + l;
+            const int sp = ppos(sub, PAD) * pitch, mp = ppos(m, PAD) * pitch;
             cx<T> a[R], u[R];
 #pragma unroll
             for (int r = 0; r < R; r++) { a[r] = src[r * sp]; u[r] = src[mp + r * sp]; }
@@ -452,13 +452,13 @@ MM_HD void xC_last(const Geom& g, T* Hc, const cx<T>* s, int pitch, int j0, T in
 }
 
 // z transform in registers, inverse + crop: S -> tile
-template <typename T, int NZ>
+template <typename T, int NZ, bool PAD>
 MM_HD void zC_regs(const Geom& g, const cx<T>* Sc, cx<T>* s, int pitch, int j0, twiddles<T> tw, int tid, int nthr)
 {
     const int np = g.nx + 1;
     for (int f = tid; f < np * g.G; f += nthr) {
         const int xp = f % np, gg = f / np;
-        cx<T>* dst = s + ppos(xp, g.xpad) * pitch + gg * NZ;
+        cx<T>* dst = s + ppos(xp, PAD) * pitch + gg * NZ;
         const cx<T>* src = Sc + (long)(j0 + gg) * g.Lx + xp;
         cx<T> a[NZ], u[NZ];
 #pragma unroll

@@ -71,11 +71,11 @@ __global__ void __launch_bounds__(256) inv_zx_kernel(Geom g, const cx<T>* S, T* 
 }
 
 // v2 wrappers (mm_kernels2.cuh)
-template <typename T, int NZ>
+template <typename T, int NZ, bool PAD>
 __global__ void __launch_bounds__(256, sizeof(T) == 8 ? 1 : MM_OCC_A) fwd_xz2_kernel(Geom g, const T* m, const T* Ms, cx<T>* S, twiddles<T> tw, const DevState* st)
 {
     if (st->done) return;
-    fwd_xz_body3<T, NZ>(g, m, Ms, S, tw, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x);
+    fwd_xz_body3<T, NZ, PAD>(g, m, Ms, S, tw, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x);
 }
 template <typename T, int V>
 __global__ void __launch_bounds__(sizeof(T) == 8 ? 256 : 512) y_conv2_kernel(Geom g, cx<T>* S, const T* Kh, twiddles<T> tw, const DevState* st)
@@ -109,11 +109,11 @@ __global__ void __launch_bounds__((sizeof(T) == 8 ? 128 : 256) * (LOGM >= 10 ? 2
     constexpr int LOGTC = sizeof(T) == 8 ? 1 : 2, NTHR = (sizeof(T) == 8 ? 128 : 256) * (LOGM >= 10 ? 2 : 1);
     y_conv_body7<LOGM, LOGTC, IS3D, NTHR, T>(g, S, Kc, tw, logtw, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, NTHR, &tmS, bar, &st->done);
 }
-template <typename T, int NZ>
+template <typename T, int NZ, bool PAD>
 __global__ void __launch_bounds__(256, sizeof(T) == 8 ? 1 : MM_OCC_C) inv_zx2_kernel(Geom g, const cx<T>* S, T* Hd, twiddles<T> tw, T inv_scale, const DevState* st)
 {
     if (st->done) return;
-    inv_zx_body3<T, NZ>(g, S, Hd, tw, inv_scale, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x);
+    inv_zx_body3<T, NZ, PAD>(g, S, Hd, tw, inv_scale, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -1472,8 +1472,14 @@ template <typename T> static LocalP<T> make_local(const mm_sim* s, int terms, bo
 // demag passes A, B, C: y -> Hd.  v2 kernels where the mesh allows, v1 otherwise (tiny meshes).
 template <typename T, int NZ> static void launch_A2(mm_sim* s, unsigned grid, const T* y, cx<T>* S, twiddles<T> tw, const DevState* st)
 {
-    if (!raise_smem_limit(s, (const void*)fwd_xz2_kernel<T, NZ>)) return;
-    fwd_xz2_kernel<T, NZ><<<grid, s->thrA, s->smemA2, s->stream>>>(s->g, y, wsp<T>(s, s->off_Ms), S, tw, st);
+    // the padded x tile exists only for nz <= 4 (at most 4 lines per CTA)
+    if (NZ <= 4 && s->g.xpad) {
+        if (!raise_smem_limit(s, (const void*)fwd_xz2_kernel<T, NZ, (NZ <= 4)>)) return;
+        fwd_xz2_kernel<T, NZ, (NZ <= 4)><<<grid, s->thrA, s->smemA2, s->stream>>>(s->g, y, wsp<T>(s, s->off_Ms), S, tw, st);
+        return;
+    }
+    if (!raise_smem_limit(s, (const void*)fwd_xz2_kernel<T, NZ, false>)) return;
+    fwd_xz2_kernel<T, NZ, false><<<grid, s->thrA, s->smemA2, s->stream>>>(s->g, y, wsp<T>(s, s->off_Ms), S, tw, st);
 }
 template <typename T, int V> static void launch_B3(mm_sim* s, unsigned grid, cx<T>* S, twiddles<T> tw, const DevState* st)
 {
@@ -1482,8 +1488,13 @@ template <typename T, int V> static void launch_B3(mm_sim* s, unsigned grid, cx<
 }
 template <typename T, int NZ> static void launch_C2(mm_sim* s, unsigned grid, cx<T>* S, twiddles<T> tw, T sc, const DevState* st)
 {
-    if (!raise_smem_limit(s, (const void*)inv_zx2_kernel<T, NZ>)) return;
-    inv_zx2_kernel<T, NZ><<<grid, s->thrA, s->smemA2, s->stream>>>(s->g, S, wsp<T>(s, s->off_Hd), tw, sc, st);
+    if (NZ <= 4 && s->g.xpad) {
+        if (!raise_smem_limit(s, (const void*)inv_zx2_kernel<T, NZ, (NZ <= 4)>)) return;
+        inv_zx2_kernel<T, NZ, (NZ <= 4)><<<grid, s->thrA, s->smemA2, s->stream>>>(s->g, S, wsp<T>(s, s->off_Hd), tw, sc, st);
+        return;
+    }
+    if (!raise_smem_limit(s, (const void*)inv_zx2_kernel<T, NZ, false>)) return;
+    inv_zx2_kernel<T, NZ, false><<<grid, s->thrA, s->smemA2, s->stream>>>(s->g, S, wsp<T>(s, s->off_Hd), tw, sc, st);
 }
 template <typename T, int V> static void launch_B2(mm_sim* s, unsigned grid, cx<T>* S, twiddles<T> tw, const DevState* st)
 {

@@ -148,19 +148,34 @@ MM_HD void b7_mid8(cx<T>* s, const tw8<T>& pre, twiddles<T> tw, int logtw, int t
 template <int LOGTC, typename T> MM_HD int b7_mid_i(int f, int logLc) { return (f >> (LOGTC - b7_v<T>::LOGV)) & ((1 << (logLc - 3)) - 1); }
 
 template <typename T, int NJ> struct kset { T k[NJ]; };
-template <typename T, bool IS3D, int TC> MM_HD kset<T, IS3D ? 48 : 32> b7_kload(const T* Kt, int set, int col)
+// 16-byte loads jq in [JQ0, JQ1) of the K^ set `set` of column `col` into r (the whole set: JQ0 = 0, JQ1 = NJQ)
+template <typename T, bool IS3D, int TC, int JQ0, int JQ1> MM_HD void b7_kload_part(const T* Kt, int set, int col, kset<T, IS3D ? 48 : 32>& r)
 {
-    constexpr int NQ = IS3D ? 6 : 4, NJ = 8 * NQ, EPL = 16 / (int)sizeof(T), NJQ = NJ / EPL;
-    kset<T, NJ> r;
+    constexpr int NQ = IS3D ? 6 : 4, NJ = 8 * NQ, EPL = 16 / (int)sizeof(T);
     const T* Kp = Kt + (long)set * (NJ * TC) + col * EPL;
 #pragma unroll
-    for (int jq = 0; jq < NJQ; jq++) {
+    for (int jq = JQ0; jq < JQ1; jq++) {
         const kvec<T> v = *reinterpret_cast<const kvec<T>*>(Kp + jq * TC * EPL);
 #pragma unroll
         for (int e = 0; e < EPL; e++) r.k[jq * EPL + e] = v.e[e];
     }
+}
+template <typename T, bool IS3D, int TC> MM_HD kset<T, IS3D ? 48 : 32> b7_kload(const T* Kt, int set, int col)
+{
+    constexpr int NJQ = 8 * (IS3D ? 6 : 4) / (16 / (int)sizeof(T));
+    kset<T, IS3D ? 48 : 32> r;
+    b7_kload_part<T, IS3D, TC, 0, NJQ>(Kt, set, col, r);
     return r;
 }
+// how much of the first multiply item's K^ set is loaded BEFORE the barrier that precedes the multiply stage (its
+// latency hides under the barrier wait); the rest is loaded right after the barrier and hides under the three 8-point
+// transforms.  3-D: one third (MM_B7_PRE3 = 1).  Measured on cfg4 fp32 (profiles/r02_experiments.md): the whole set
+// (48 registers) across the barrier spilled 9 registers whose spill stores waited for the loads — 193.2 us; one third
+// 186.4 us; nothing before the barrier 191.3 us.
+#ifndef MM_B7_PRE3
+#define MM_B7_PRE3 1
+#endif
+template <typename T, bool IS3D> struct B7Pre { static constexpr int NJQ = 8 * (IS3D ? 6 : 4) / (16 / (int)sizeof(T)), PRE = IS3D ? (MM_B7_PRE3 * NJQ) / 3 : NJQ; };
 
 // multiply stage: item = (column, mirror pair of 8-row blocks), see yB_mul8 in mm_kernels2.cuh
 template <int LOGM, int LOGTC, bool IS3D, int NTHR, typename T>
@@ -171,7 +186,9 @@ MM_HD void b7_mul8(cx<T>* s, const kset<T, IS3D ? 48 : 32>& pre, const T* Kt, T 
     bool first = true;
     for (int f = tid; f < (NBK >> 1) * TC; f += NTHR, first = false) {
         const int col = f & (TC - 1), t = f >> LOGTC;
-        kset<T, NJ> K = first ? pre : b7_kload<T, IS3D, TC>(Kt, t, col);
+        kset<T, NJ> K;
+        if (first) { K = pre; b7_kload_part<T, IS3D, TC, B7Pre<T, IS3D>::PRE, B7Pre<T, IS3D>::NJQ>(Kt, t, col, K); }
+        else K = b7_kload<T, IS3D, TC>(Kt, t, col);
         int ro[8];
 #pragma unroll
         for (int r = 0; r < 8; r++) ro[r] = ((r + t) & 7) * TC;
@@ -225,7 +242,8 @@ MM_HD void b7_fwd_mids(cx<T>* s, twiddles<T> tw, int logtw, const T* Kt, int tid
         b7_mid8<LOGM, LOGTC, LOGLC, 0, NTHR, T>(s, t, tw, logtw, tid, nthr);
         b7_fwd_mids<LOGM, LOGTC, LOGLC - 3, IS3D, NTHR, T>(s, tw, logtw, Kt, tid, nthr, kpre);
     } else {
-        if (tid < (B7<LOGM, LOGTC>::NBK >> 1) * B7<LOGM, LOGTC>::TC) kpre = b7_kload<T, IS3D, B7<LOGM, LOGTC>::TC>(Kt, tid >> LOGTC, tid & (B7<LOGM, LOGTC>::TC - 1));      // K^ set of the thread's first multiply item
+        if (tid < (B7<LOGM, LOGTC>::NBK >> 1) * B7<LOGM, LOGTC>::TC)      // K^ set of the thread's first multiply item (the part that fits in registers)
+            b7_kload_part<T, IS3D, B7<LOGM, LOGTC>::TC, 0, B7Pre<T, IS3D>::PRE>(Kt, tid >> LOGTC, tid & (B7<LOGM, LOGTC>::TC - 1), kpre);
         MM_SYNC();
     }
 }

@@ -74,7 +74,7 @@ static void run(int ver, int nx, int ny, int nz, int G, int CH, int TC, const do
     for (int b = 0; b < gridA; b++) {
         if (!a2) fwd_xz_body<T>(g, mt.data(), Mst.data(), S.data(), tw, smem.data(), b, 0, 1);
         else switch (nz) {
-#define CASE_A(NZ) case NZ: fwd_xz_body3<T, NZ>(g, mt.data(), Mst.data(), S.data(), tw, smem.data(), b, 0, 1); break;
+#define CASE_A(NZ) case NZ: if (NZ <= 4 && g.xpad) fwd_xz_body3<T, NZ, (NZ <= 4)>(g, mt.data(), Mst.data(), S.data(), tw, smem.data(), b, 0, 1); else fwd_xz_body3<T, NZ, false>(g, mt.data(), Mst.data(), S.data(), tw, smem.data(), b, 0, 1); break;
             CASE_A(1) CASE_A(2) CASE_A(4) CASE_A(8) CASE_A(16) CASE_A(32)
         }
     }
@@ -104,7 +104,7 @@ static void run(int ver, int nx, int ny, int nz, int G, int CH, int TC, const do
     for (int b = 0; b < gridA; b++) {
         if (!a2) inv_zx_body<T>(g, S.data(), Hdt.data(), tw, (T)(1.0 / P), smem.data(), b, 0, 1);
         else switch (nz) {
-#define CASE_C(NZ) case NZ: inv_zx_body3<T, NZ>(g, S.data(), Hdt.data(), tw, (T)(1.0 / P), smem.data(), b, 0, 1); break;
+#define CASE_C(NZ) case NZ: if (NZ <= 4 && g.xpad) inv_zx_body3<T, NZ, (NZ <= 4)>(g, S.data(), Hdt.data(), tw, (T)(1.0 / P), smem.data(), b, 0, 1); else inv_zx_body3<T, NZ, false>(g, S.data(), Hdt.data(), tw, (T)(1.0 / P), smem.data(), b, 0, 1); break;
             CASE_C(1) CASE_C(2) CASE_C(4) CASE_C(8) CASE_C(16) CASE_C(32)
         }
     }
