@@ -93,7 +93,7 @@ __global__ void __launch_bounds__(MM_B5_THR, MM_B5_OCC) y_conv5_kernel(Geom g, c
 }
 // half-tile form (mm_passB3.cuh): the long-line path; reads S, writes the second spectrum buffer S2
 template <typename T, int V>
-__global__ void __launch_bounds__(512) y_conv3_kernel(Geom g, const cx<T>* S, cx<T>* S2, const T* Kh, twiddles<T> tw, const DevState* st)
+__global__ void __launch_bounds__(256) y_conv3_kernel(Geom g, const cx<T>* S, cx<T>* S2, const T* Kh, twiddles<T> tw, const DevState* st)
 {
     if (st->done) return;
     y_conv_body3<T, V>(g, S, S2, Kh, tw, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x);
@@ -1024,7 +1024,7 @@ static void configure(mm_sim* s)
     s->thrB = (s->prec == MM_F32 && s->smemB > 98 * 1024) ? 512 : 256;
     if (b7_f64) s->thrB = 128;
     if (b7_10) s->thrB = s->prec == MM_F64 ? 256 : 512;
-    if (s->use_b3) s->thrB = (g.ny / 8) * (g.TC / (s->prec == MM_F32 && g.TC % 2 == 0 ? 2 : 1)) >= 512 ? 512 : 256;
+    if (s->use_b3) s->thrB = 256;      // 255 registers per thread: the multiply stage holds 3 x 8 complex values + K^ (512 threads spilled kilobytes)
     if (getenv("MM_THRB")) s->thrB = atoi(getenv("MM_THRB"));
 }
 
