@@ -391,29 +391,47 @@ MM_HD void xA_first(const Geom& g, const T* mc, const T* Ms, cx<T>* s, int pitch
 #pragma unroll
         for (int r = 0; r < R; r++) wp[r] = tw.get(i + r * sub, n);
         if (R > 1 && i != 0) twiddle_powers<T, R>(tw.get(i, m), pw);
-        for (int l = tid >> logisub; l < L; l += lstep) {
-            const int gg = l >> lognz, z = l & (g.nz - 1);
-            const long row = ((long)z * g.ny + (j0 + gg)) * g.nx + 2 * i;
-            const T* mrow = mc + row;
-            const T* srow = Ms + row;
-            cx<T> a[R], u[R];
+        // fp64: two lines per trip, the global loads of both in flight before the first butterfly (the load latency is
+        // exposed once per trip: 29 % of the pass's stall samples; cfg4 pass A 188.8 -> 178.7 us).  fp32 keeps one line:
+        // two need more than the 85 registers of three CTAs per SM (measured 78.8 -> 87.0 us with two).
+        constexpr int NB = sizeof(T) == 8 ? 2 : 1;
+        for (int l0 = tid >> logisub; l0 < L; l0 += NB * lstep) {
+            cx<T> a[NB][R], u[NB][R];
+            cx<T> mm2[NB][R], ms2[NB][R];
 #pragma unroll
-            for (int r = 0; r < R; r++) {
-                const cx<T> mm2 = *reinterpret_cast<const cx<T>*>(mrow + 2 * r * sub);
-                const cx<T> ms2 = *reinterpret_cast<const cx<T>*>(srow + 2 * r * sub);
-                a[r] = mk<T>(ms2.x == (T)0 ? (T)0 : ms2.x * mm2.x, ms2.y == (T)0 ? (T)0 : ms2.y * mm2.y);
-                u[r] = cmul(a[r], wp[r]);
+            for (int b = 0; b < NB; b++) {
+                const int l = l0 + b * lstep;
+                if (l < L) {
+                    const int gg = l >> lognz, z = l & (g.nz - 1);
+                    const long row = ((long)z * g.ny + (j0 + gg)) * g.nx + 2 * i;
+#pragma unroll
+                    for (int r = 0; r < R; r++) {
+                        mm2[b][r] = *reinterpret_cast<const cx<T>*>(mc + row + 2 * r * sub);
+                        ms2[b][r] = *reinterpret_cast<const cx<T>*>(Ms + row + 2 * r * sub);
+                    }
+                }
             }
-            rad<cx<T>, R>::fwd(a);
-            rad<cx<T>, R>::fwd(u);
-            if (R > 1 && i != 0) {
 #pragma unroll
-                for (int r = 1; r < R; r++) { a[r] = cmul(a[r], pw[r]); u[r] = cmul(u[r], pw[r]); }
+            for (int b = 0; b < NB; b++) {
+                const int l = l0 + b * lstep;
+                if (l < L) {
+#pragma unroll
+                    for (int r = 0; r < R; r++) {
+                        a[b][r] = mk<T>(ms2[b][r].x == (T)0 ? (T)0 : ms2[b][r].x * mm2[b][r].x, ms2[b][r].y == (T)0 ? (T)0 : ms2[b][r].y * mm2[b][r].y);
+                        u[b][r] = cmul(a[b][r], wp[r]);
+                    }
+                    rad<cx<T>, R>::fwd(a[b]);
+                    rad<cx<T>, R>::fwd(u[b]);
+                    if (R > 1 && i != 0) {
+#pragma unroll
+                        for (int r = 1; r < R; r++) { a[b][r] = cmul(a[b][r], pw[r]); u[b][r] = cmul(u[b][r], pw[r]); }
+                    }
+                    cx<T>* dst = s + ppos(i, PAD) * pitch + l;
+                    const int sp = ppos(sub, PAD) * pitch, mp = ppos(m, PAD) * pitch;
+#pragma unroll
+                    for (int r = 0; r < R; r++) { dst[r * sp] = a[b][r]; dst[mp + r * sp] = u[b][r]; }
+                }
             }
-            cx<T>* dst = s + ppos(i, PAD) * pitch + l;
-            const int sp = ppos(sub, PAD) * pitch, mp = ppos(m, PAD) * pitch;
-#pragma unroll
-            for (int r = 0; r < R; r++) { dst[r * sp] = a[r]; dst[mp + r * sp] = u[r]; }
         }
     }
 }

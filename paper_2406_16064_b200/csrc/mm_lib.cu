@@ -288,7 +288,7 @@ template <typename T, int CPT> __device__ __forceinline__ void stc(T* p, const c
 #define MM_STAGEV_THREADS 128
 #endif
 #ifndef MM_STAGEV_CPT
-#define MM_STAGEV_CPT 2      // cells per thread (8-byte loads in fp32, 16-byte in fp64): measured best on B200
+#define MM_STAGEV_CPT 2      // fp32 cells per thread (8-byte loads): measured best on B200; fp64 takes 1 (see launch_stage)
 #endif
 // GEN: cell-based A and / or D: the A_i, D_i of the six neighbours are loaded like the neighbour
 // values of m and turned into the harmonic-mean bond values.
@@ -1616,7 +1616,8 @@ template <typename T> static int demag_passes(mm_sim* s, const T* y)
 template <typename T, int MODE, int S, bool NEXT, bool ERR, bool MAXK>
 static void launch_stage(mm_sim* s, const LocalP<T>& lp, const T* y, const T* Hd, T* out, const StageArgs<T>& sa)
 {
-    constexpr int CPT = MM_STAGEV_CPT;
+    // fp64: one cell per thread (148 instead of 228 registers; cfg4 stage kernel 154.3 -> 148.2 us)
+    constexpr int CPT = sizeof(T) == 8 ? 1 : MM_STAGEV_CPT;
     if (s->g.nx % CPT == 0 && !s->no_stagev) {
         const unsigned blocks = (unsigned)((s->g.N / CPT + MM_STAGEV_THREADS - 1) / MM_STAGEV_THREADS);
         // general form: cell-based A / D, thermal field, Zhang-Li / Slonczewski torques, Cayley stages
