@@ -68,6 +68,7 @@ def lib():
         L.mo_cayley_apply.argtypes = [_dp, _dp, _dp]
         L.mo_cayley_apply.restype = None
         L.mo_set_zhang_li.argtypes = [C.c_void_p] + [C.c_double] * 4
+        L.mo_set_zhang_li_pulse.argtypes = [C.c_void_p, C.c_double, C.c_double]
         L.mo_set_slonczewski.argtypes = [C.c_void_p] + [C.c_double] * 5
         L.mo_set_temperature.argtypes = [C.c_void_p, C.c_double, C.c_ulonglong]
         _lib = L
@@ -157,6 +158,7 @@ class Oracle:
     def set_D_cell(self, D, kind): _chk(self.L.mo_set_D_cell(self.h, self._cell(D, self.N), kind), "set_D_cell")
     def set_H_ext_cell(self, H): _chk(self.L.mo_set_H_ext_cell(self.h, self._cell(H, 3 * self.N)), "set_H_ext_cell")
     def set_zhang_li(self, ux, uy, uz, beta): _chk(self.L.mo_set_zhang_li(self.h, ux, uy, uz, beta), "set_zhang_li")
+    def set_zhang_li_pulse(self, b, w): _chk(self.L.mo_set_zhang_li_pulse(self.h, b, w), "set_zhang_li_pulse")
     def set_slonczewski(self, aJ, bJ, px, py, pz): _chk(self.L.mo_set_slonczewski(self.h, aJ, bJ, px, py, pz), "set_slonczewski")
     def set_temperature(self, T, seed): _chk(self.L.mo_set_temperature(self.h, T, seed), "set_temperature")
     def set_axis(self, ux, uy, uz): _chk(self.L.mo_set_axis(self.h, ux, uy, uz), "set_axis")

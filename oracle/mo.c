@@ -62,6 +62,9 @@ typedef struct mo_sim {
     int integrator;             /* 0 RK4, 1 DOPRI5, 2 Cayley-transform RK4 (Eq. 49) */
     double stt_u[3], stt_beta;  /* Zhang-Li: u in m/s (Eq. 39), beta */
     int stt_on;
+    double stt_b, stt_w;        /* time profile of the current: u(t) = u exp(-b t) cos(w t); 0, 0 = constant */
+    double t_eval;              /* time at which the right-hand side is being evaluated (stage time inside a step) */
+    int in_step;
     double sl_aJ, sl_bJ, sl_p[3]; /* Slonczewski / SOT (Eq. 40): a_J, b_J in 1/s, unit vector p */
     int sl_on;
     double temperature;         /* K; 0 = no thermal field */
@@ -530,8 +533,9 @@ int mo_thermal_field(const mo_sim *s, double dt, unsigned long long step, double
 /* tau = (u . grad) m by central differences, tau_i = sum_a u_a (m_{i+a} - m_{i-a}) / (2 Delta_a); an absent
  * neighbour (outside the mesh or Ms = 0) is replaced by the cell's own m (zero normal derivative, the free boundary
  * of R4; the paper prints no discretisation: DESIGN.md R17) */
-int mo_stt_tau(const mo_sim *s, const double *m, double *tau)
+int mo_stt_tau(mo_sim *s, const double *m, double *tau)
 {
+    if (!s->in_step) s->t_eval = s->t;
     const int nx = s->nx, ny = s->ny, nz = s->nz;
     const long N = s->N;
     const double delta[3] = { s->dx, s->dy, s->dz };
@@ -549,6 +553,11 @@ int mo_stt_tau(const mo_sim *s, const double *m, double *tau)
                     if (pos[a] < lim[a] - 1 && s->Ms[q + str[a]] != 0.0) pp = q + str[a];
                     for (int c = 0; c < 3; c++) tau[c * N + q] += s->stt_u[a] * (m[c * N + pp] - m[c * N + pm]) / (2.0 * delta[a]);
                 }
+                /* u(t) = u exp(-b t) cos(w t) at the evaluation time ("u(t) = u0 e^{-bt} cos(wt)") */
+                if (s->stt_b != 0.0 || s->stt_w != 0.0) {
+                    const double f = exp(-s->stt_b * s->t_eval) * cos(s->stt_w * s->t_eval);
+                    for (int c = 0; c < 3; c++) tau[c * N + q] *= f;
+                }
             }
     return 0;
 }
@@ -565,6 +574,7 @@ static void cross3(const double a[3], const double b[3], double c[3])
 int mo_llg_rhs(mo_sim *s, const double *m, double *dmdt)
 {
     const long N = s->N;
+    if (!s->in_step) s->t_eval = s->t;
     double *H = (double *)malloc(sizeof(double) * 3 * N);
     int rc = mo_effective_field(s, m, H);
     if (rc) { free(H); return rc; }
@@ -690,6 +700,7 @@ static int cayley_step(mo_sim *s, double *m, double dt, double *max_dmdt)
     double *k = (double *)malloc(sizeof(double) * n3 * 4), *w = (double *)calloc(n3, sizeof(double));
     double *mm = (double *)malloc(sizeof(double) * n3), *f = (double *)malloc(sizeof(double) * n3);
     int rc;
+    s->t_eval = s->t;
     if ((rc = cayley_rhs(s, m, w, mm, f, k))) goto done;
     if (max_dmdt) {
         double mx = 0;
@@ -704,10 +715,12 @@ static int cayley_step(mo_sim *s, double *m, double dt, double *max_dmdt)
         *max_dmdt = mx;
     }
     for (long q = 0; q < n3; q++) w[q] = 0.5 * dt * k[q];
+    s->t_eval = s->t + 0.5 * dt;
     if ((rc = cayley_rhs(s, m, w, mm, f, k + n3))) goto done;
     for (long q = 0; q < n3; q++) w[q] = 0.5 * dt * k[n3 + q];
     if ((rc = cayley_rhs(s, m, w, mm, f, k + 2 * n3))) goto done;
     for (long q = 0; q < n3; q++) w[q] = dt * k[2 * n3 + q];
+    s->t_eval = s->t + dt;
     if ((rc = cayley_rhs(s, m, w, mm, f, k + 3 * n3))) goto done;
     for (long q = 0; q < n3; q++) w[q] = dt / 6.0 * (k[q] + 2 * k[n3 + q] + 2 * k[2 * n3 + q] + k[3 * n3 + q]);
     for (long q = 0; q < N; q++) {
@@ -779,12 +792,15 @@ static int step_inner(mo_sim *s, double *m, double dt, double tol, int *accepted
     }
     if (s->integrator == 0) {
         double *k = (double *)malloc(sizeof(double) * n3 * 4), *y = (double *)malloc(sizeof(double) * n3);
+        s->t_eval = s->t;
         if ((rc = mo_llg_rhs(s, m, k))) goto done4;
         for (long q = 0; q < n3; q++) y[q] = m[q] + 0.5 * dt * k[q];
+        s->t_eval = s->t + 0.5 * dt;
         if ((rc = mo_llg_rhs(s, y, k + n3))) goto done4;
         for (long q = 0; q < n3; q++) y[q] = m[q] + 0.5 * dt * k[n3 + q];
         if ((rc = mo_llg_rhs(s, y, k + 2 * n3))) goto done4;
         for (long q = 0; q < n3; q++) y[q] = m[q] + dt * k[2 * n3 + q];
+        s->t_eval = s->t + dt;
         if ((rc = mo_llg_rhs(s, y, k + 3 * n3))) goto done4;
         if (max_dmdt) *max_dmdt = max_norm(s, k);
         for (long q = 0; q < n3; q++) m[q] += dt / 6.0 * (k[q] + 2 * k[n3 + q] + 2 * k[2 * n3 + q] + k[3 * n3 + q]);
@@ -803,6 +819,10 @@ static int step_inner(mo_sim *s, double *m, double dt, double tol, int *accepted
             double acc = 0;
             for (int j = 0; j < st; j++) acc += DP_A[st][j] * k[j * n3 + q];
             y[q] = m[q] + dt * acc;
+        }
+        {
+            static const double DP_C[7] = { 0.0, 1.0 / 5, 3.0 / 10, 4.0 / 5, 8.0 / 9, 1.0, 1.0 };      /* row sums of DP_A */
+            s->t_eval = s->t + DP_C[st] * dt;
         }
         if ((rc = mo_llg_rhs(s, y, k + st * n3))) goto done5;
     }
@@ -846,7 +866,9 @@ int mo_step(mo_sim *s, double *m, double dt, double tol, int *accepted, double *
         mo_thermal_field(s, dt, s->th_step, xi);
         s->Hth = xi;
     }
+    s->in_step = 1;
     int rc = step_inner(s, m, dt, tol, accepted, err_out, dt_next, max_dmdt);
+    s->in_step = 0;
     s->Hth = NULL;
     if (xi) { s->th_step++; free(xi); }
     return rc;
@@ -1044,6 +1066,7 @@ int mo_set_zhang_li(mo_sim *s, double ux, double uy, double uz, double beta)
     s->stt_on = (ux != 0.0 || uy != 0.0 || uz != 0.0);
     return 0;
 }
+int mo_set_zhang_li_pulse(mo_sim *s, double b, double w) { s->stt_b = b; s->stt_w = w; return 0; }
 int mo_set_slonczewski(mo_sim *s, double aJ, double bJ, double px, double py, double pz)
 {
     const double n = sqrt(px * px + py * py + pz * pz);

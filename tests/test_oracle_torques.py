@@ -300,3 +300,51 @@ def test_slonczewski_macrospin_closed_forms(which):
             t = i * dt
             ref = [np.cos(wp * t) / np.cosh(wd * t), np.sin(wp * t) / np.cosh(wd * t), np.tanh(wd * t)]
             assert np.abs(m.reshape(3) - ref).max() < 1e-9
+
+
+def pulse_integral(t, u0, b, w):
+    """int_0^t u0 exp(-b s) cos(w s) ds"""
+    return u0 * (np.exp(-b * t) * (w * np.sin(w * t) - b * np.cos(w * t)) + b) / (b * b + w * w)
+
+
+@pytest.mark.parametrize("integrator", [oracle.RK4, oracle.DOPRI5, oracle.CAYLEY_RK4])
+def test_domain_wall_under_the_papers_current_pulse(integrator):
+    """PAPER.md:436-448 (Eq. 54, Fig. 5): "u = u(t) ... an arbitrary time dependence"; the paper's run uses
+    u(t) = u0 exp(-b t) cos(w t), b = 5e8 1/s, w = 2e9 1/s, alpha = 0.1.  Wall position and tilt angle at several times
+    against z(t) - z(0) = -(1 + alpha beta) U(t) / (1 + alpha^2), phi(t) - phi(0) = (alpha - beta) U(t) / ((1 + alpha^2) Delta),
+    U = int u dt in closed form; the stage times of every integrator enter (a u frozen over the step would be first order)."""
+    nx, dx, alpha, beta, A, K, u0, b, w = 320, 1e-9, 0.1, 0.3, 1.3e-11, 1e5, 300.0, 5e8, 2e9
+    Delta = np.sqrt(A / K)
+    o = chain(nx, dx, alpha, A, K)
+    o.set_integrator(integrator)
+    x = (np.arange(nx) + 0.5) * dx
+    m = np.zeros((3, 1, 1, nx))
+    m[0, 0, 0] = -np.tanh((x - 160e-9) / Delta)
+    m[1, 0, 0] = 1 / np.cosh((x - 160e-9) / Delta)
+    m = np.ascontiguousarray(m)
+
+    def wall(m):
+        return 0.5 * nx * dx * (1 + m[0].mean()), np.arctan2(m[2].sum(), m[1].sum())
+
+    dt = 1e-13      # exchange stiffness of 1 nm cells: explicit RK stability needs gamma H_ex dt < 2.8
+    with omp_threads(1):
+        for _ in range(200):
+            o.step(m, dt)
+        o.set_time(0.0)
+        o.set_zhang_li(u0, 0, 0, beta)
+        o.set_zhang_li_pulse(b, w)
+        p0, f0 = wall(m)
+        for i in range(1, 6001):
+            o.step(m, dt)
+            if i % 1500 == 0:
+                t = i * dt
+                U = pulse_integral(t, u0, b, w)
+                p, f = wall(m)
+                assert abs((p - p0) + (1 + alpha * beta) * U / (1 + alpha**2)) <= 0.01 * abs(pulse_integral(7.85e-10, u0, b, w)) + 2e-11
+                assert abs((f - f0) - (alpha - beta) * U / ((1 + alpha**2) * Delta)) <= 0.02 * abs((alpha - beta) * pulse_integral(7.85e-10, u0, b, w) / Delta)
+    # the factor multiplies tau itself; b = w = 0 is the constant current
+    o.set_time(3e-10)
+    t1 = o.stt_tau(m)
+    o.set_zhang_li_pulse(0.0, 0.0)
+    t0 = o.stt_tau(m)
+    assert np.allclose(t1, t0 * np.exp(-b * 3e-10) * np.cos(w * 3e-10), rtol=1e-12, atol=1e-30)
