@@ -105,6 +105,9 @@ int mm_set_H_ext_cell(mm_sim* sim, const void* dev_H);
  * by the cell itself).  u in m/s (Eq. 39), uniform; (0,0,0) switches the term off.  Sign convention of Eq. 44 / Eq. 54
  * (a head-to-head wall moves with -(1 + alpha beta) u / (1 + alpha^2)); Eq. 38 as printed has u -> -u (R17). */
 int mm_set_zhang_li(mm_sim* sim, double ux, double uy, double uz, double beta);
+/* Time profile of that current: u(t) = u exp(-b t) cos(w t) (the pulse of PAPER.md:446; Eq. 54 holds for any u(t)),
+ * evaluated at every RK stage's own time t + c dt on the device.  b = w = 0 (the default): constant current. */
+int mm_set_zhang_li_pulse(mm_sim* sim, double b, double w);
 /* Slonczewski / spin-orbit torque, Eq. 40: -a_J m x (m x p) - b_J m x p added to the Gilbert
  * equation; a_J, b_J in 1/s, p normalised inside (zero p with non-zero a_J or b_J => MM_ERR_ARG). */
 int mm_set_slonczewski(mm_sim* sim, double a_J, double b_J, double px, double py, double pz);

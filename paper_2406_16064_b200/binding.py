@@ -29,6 +29,7 @@ SIGNATURES = {
     "mm_set_Ku": (_i, [_vp, _d]),
     "mm_set_Kc": (_i, [_vp, _d]),
     "mm_set_zhang_li": (_i, [_vp, _d, _d, _d, _d]),
+    "mm_set_zhang_li_pulse": (_i, [_vp, _d, _d]),
     "mm_set_slonczewski": (_i, [_vp, _d, _d, _d, _d, _d]),
     "mm_set_temperature": (_i, [_vp, _d, C.c_ulonglong]),
     "mm_thermal_field": (_i, [_vp, _d, C.c_ulonglong, _vp]),
@@ -142,6 +143,7 @@ class Sim:
     def set_Ku(self, Ku): self._chk(self.L.mm_set_Ku(self.h, Ku), "mm_set_Ku")
     def set_Kc(self, Kc): self._chk(self.L.mm_set_Kc(self.h, Kc), "mm_set_Kc")
     def set_zhang_li(self, ux, uy, uz, beta): self._chk(self.L.mm_set_zhang_li(self.h, ux, uy, uz, beta), "mm_set_zhang_li")
+    def set_zhang_li_pulse(self, b, w): self._chk(self.L.mm_set_zhang_li_pulse(self.h, b, w), "mm_set_zhang_li_pulse")
     def set_slonczewski(self, aJ, bJ, px, py, pz): self._chk(self.L.mm_set_slonczewski(self.h, aJ, bJ, px, py, pz), "mm_set_slonczewski")
     def set_temperature(self, T, seed): self._chk(self.L.mm_set_temperature(self.h, T, seed), "mm_set_temperature")
 

@@ -125,6 +125,7 @@ template <typename T> struct StageArgs {
     T* ynext;             // next stage input (or the RK4 solution); may be NULL
     T coef[7];            // ynext = m0 + dt * sum_{j<=s} coef[j] k_j
     T ecoef[7];           // E = dt * sum_{j<=s} ecoef[j] k_j   (do_err)
+    T cstage;             // stage time = t + cstage * dt (time-dependent current)
     T wcoef[7];           // Cayley (MODE 2): omega of THIS stage = dt * sum_{j<s} wcoef[j] k_j, k_j = d omega/dt of stage j
     int s;                // index of this stage
     int do_err, do_maxk;
@@ -191,6 +192,14 @@ __device__ __forceinline__ v3<T> stage_result(const LocalP<T>& lp, v3<T> mi, v3<
     return cayley_domega<T>(w, f);
 }
 
+// u(t) / u of the Zhang-Li current at this stage's time (1 when the current is constant)
+template <typename T> __device__ __forceinline__ T stt_pulse(const LocalP<T>& lp, const DevState* st, T cstage)
+{
+    if (!lp.stt_on || (lp.stt_b == 0.0 && lp.stt_w == 0.0)) return (T)1;
+    const double ts = st->t + (double)cstage * st->dt;
+    return (T)(exp(-lp.stt_b * ts) * cos(lp.stt_w * ts));
+}
+
 // MODE 0: out = H_eff ; MODE 1: out = k = LL torque ; MODE 2: out = d omega/dt (Cayley form, Eq. 49); then the RK
 // stage algebra selected at compile time: S earlier stages, NEXT (write the next stage input: m0 + dt sum a k, or
 // Q(dt sum a k) m0 in MODE 2), ERR (embedded error norm), MAXK (max |dm/dt|).
@@ -217,6 +226,7 @@ __global__ void __launch_bounds__(256) llg_stage_kernel(Geom g, LocalP<T> lp, co
         if (NEXT) m0 = ld3(sa.m0, N, q);
         v3<T> tau = { 0, 0, 0 };
         H = local_field<T>(g, lp, y, Ms, i, j, k, q, live ? Msi : (T)1, mi, H, MODE == 0 ? nullptr : &tau);
+        if (MODE >= 1) { const T fp = stt_pulse<T>(lp, st, sa.cstage); tau.x *= fp; tau.y *= fp; tau.z *= fp; }
         v3<T> w = { 0, 0, 0 };
         if (MODE == 2) {
             const T dtw = (T)st->dt;
@@ -457,7 +467,9 @@ __global__ void __launch_bounds__(MM_STAGEV_THREADS, sizeof(T) == 8 ? 1 : (GEN ?
                     for (int jj = 0; jj < S; jj++) { w.x += sa.wcoef[jj] * kj[jj][0].e[e]; w.y += sa.wcoef[jj] * kj[jj][1].e[e]; w.z += sa.wcoef[jj] * kj[jj][2].e[e]; }
                     w.x *= dtw; w.y *= dtw; w.z *= dtw;
                 }
-                r = stage_result<T, MODE>(lp, mi, h, tau[e], w, MAXK, &kn2);
+                v3<T> te = tau[e];
+                if (MODE >= 1) { const T fp = stt_pulse<T>(lp, st, sa.cstage); te.x *= fp; te.y *= fp; te.z *= fp; }
+                r = stage_result<T, MODE>(lp, mi, h, te, w, MAXK, &kn2);
             } else {
                 r = MODE == 0 ? h : ll_torque<T>(lp, mi, h);
             }
@@ -890,7 +902,7 @@ struct mm_sim {
     int use_b3;                      // pass B runs the half-tile form (a full py-row tile does not fit one CTA)
     size_t off_S2;                   // its output spectrum
     size_t off_ei, off_eo;           // embedding: inner-layout copies of the caller's input / output fields
-    double stt_u[3], stt_beta, sl_aJ, sl_bJ, sl_p[3], temperature;      // Zhang-Li, Slonczewski / SOT, thermal field
+    double stt_u[3], stt_beta, stt_b, stt_w, sl_aJ, sl_bJ, sl_p[3], temperature;      // Zhang-Li, Slonczewski / SOT, thermal field
     unsigned long long th_seed;
     // workspace
     void* ws;
@@ -1078,7 +1090,7 @@ extern "C" int mm_create(mm_sim** out, int nx, int ny, int nz, double dx, double
     s->prec = prec; s->device = device; s->stream = static_cast<cudaStream_t>(cuda_stream);
     s->dx = dx; s->dy = dy; s->dz = dz;
     s->A = s->D = s->Ku = s->Kc = 0; s->A_cell = s->D_cell = s->H_cell = 0;
-    s->stt_u[0] = s->stt_u[1] = s->stt_u[2] = s->stt_beta = 0; s->sl_aJ = s->sl_bJ = 0; s->sl_p[0] = s->sl_p[1] = 0; s->sl_p[2] = 1; s->temperature = 0; s->th_seed = 0; s->u[0] = s->u[1] = 0; s->u[2] = 1; s->hext[0] = s->hext[1] = s->hext[2] = 0;
+    s->stt_u[0] = s->stt_u[1] = s->stt_u[2] = s->stt_beta = 0; s->stt_b = s->stt_w = 0; s->sl_aJ = s->sl_bJ = 0; s->sl_p[0] = s->sl_p[1] = 0; s->sl_p[2] = 1; s->temperature = 0; s->th_seed = 0; s->u[0] = s->u[1] = 0; s->u[2] = 1; s->hext[0] = s->hext[1] = s->hext[2] = 0;
     s->alpha = 0.5; s->gamma = 2.211e5; s->dmi_kind = 0; s->integ = MM_DOPRI5; s->demag_on = 1; s->demag_ready = 0; s->Ms_set = 0;
     s->ws = nullptr; s->ws_bytes = 0; s->khat_imag_ratio = -1; s->t_host = 0; s->launches = 0; s->prof_on = 0; s->prof_open = 0; s->prof_used = 0; s->use_v2 = getenv("MM_FORCE_V1") ? 0 : 1; s->no_b7 = getenv("MM_NO_B7") ? 1 : 0; s->no_stagev = getenv("MM_NO_STAGEV") ? 1 : 0;
     Geom& g = s->g;
@@ -1240,6 +1252,12 @@ extern "C" int mm_set_zhang_li(mm_sim* s, double ux, double uy, double uz, doubl
 {
     if (!s) return MM_ERR_ARG;
     s->stt_u[0] = ux; s->stt_u[1] = uy; s->stt_u[2] = uz; s->stt_beta = beta;
+    return MM_OK;
+}
+extern "C" int mm_set_zhang_li_pulse(mm_sim* s, double b, double w)
+{
+    if (!s) return MM_ERR_ARG;
+    s->stt_b = b; s->stt_w = w;
     return MM_OK;
 }
 extern "C" int mm_set_slonczewski(mm_sim* s, double aJ, double bJ, double px, double py, double pz)
@@ -1456,6 +1474,7 @@ template <typename T> static LocalP<T> make_local(const mm_sim* s, int terms, bo
     lp.beta = (T)s->stt_beta;
     lp.sl_a = (T)(s->sl_aJ / s->gamma); lp.sl_b = (T)(s->sl_bJ / s->gamma);
     lp.gam = (T)s->gamma; lp.al = (T)s->alpha;
+    lp.stt_b = s->stt_b; lp.stt_w = s->stt_w;
     lp.stt_on = (s->stt_u[0] != 0.0 || s->stt_u[1] != 0.0 || s->stt_u[2] != 0.0) ? 1 : 0;
     lp.sl_on = (s->sl_aJ != 0.0 || s->sl_bJ != 0.0) ? 1 : 0;
     lp.gp = (T)(s->gamma / (1.0 + s->alpha * s->alpha));
@@ -1749,6 +1768,10 @@ template <typename T> static int enqueue_step(mm_sim* s, T* m, int ctrl_mode)
     for (int st = 0; st < nst; st++) {
         StageArgs<T> sa = no_stage<T>();
         sa.m0 = m; sa.s = st;
+        {   // stage time t + c dt: row sums of the tableau
+            static const double DP_C[7] = { 0.0, 1.0 / 5, 3.0 / 10, 4.0 / 5, 8.0 / 9, 1.0, 1.0 }, RK4_C[4] = { 0.0, 0.5, 0.5, 1.0 };
+            sa.cstage = (T)(s->integ == MM_DOPRI5 ? DP_C[st] : RK4_C[st]);
+        }
         for (int j = 0; j < st && j < 6; j++) sa.kprev[j] = k[j];
         sa.do_maxk = st == 0;
         if (s->integ == MM_DOPRI5) {
@@ -1789,7 +1812,7 @@ static size_t step_key(const mm_sim* s, const void* m, int ctrl_mode, unsigned c
     put(s->u, sizeof(s->u)); put(s->hext, sizeof(s->hext)); put(&s->alpha, sizeof(double)); put(&s->gamma, sizeof(double));
     put(&s->dmi_kind, sizeof(int)); put(&s->integ, sizeof(int)); put(&s->demag_on, sizeof(int)); put(&s->demag_ready, sizeof(int));
     put(&s->A_cell, sizeof(int)); put(&s->D_cell, sizeof(int)); put(&s->H_cell, sizeof(int));
-    put(s->stt_u, sizeof(s->stt_u)); put(&s->stt_beta, sizeof(double)); put(&s->sl_aJ, sizeof(double)); put(&s->sl_bJ, sizeof(double));
+    put(s->stt_u, sizeof(s->stt_u)); put(&s->stt_beta, sizeof(double)); put(&s->stt_b, sizeof(double)); put(&s->stt_w, sizeof(double)); put(&s->sl_aJ, sizeof(double)); put(&s->sl_bJ, sizeof(double));
     put(s->sl_p, sizeof(s->sl_p)); put(&s->temperature, sizeof(double)); put(&s->th_seed, sizeof(s->th_seed));
     return n;
 }

@@ -33,6 +33,7 @@ template <typename T> struct LocalP {
     T p[3];           // unit polarisation vector
     T gam, al;        // gamma, alpha (f of Eq. 44 and f_stt need them separately)
     int stt_on, sl_on;
+    double stt_b, stt_w;   // time profile of the Zhang-Li current: u(t) = u exp(-b t) cos(w t); 0, 0 = constant
 };
 
 // bond value of a cell-based constant: harmonic mean, 0 when both vanish

@@ -126,7 +126,7 @@ extern "C" void emul_local(int nx, int ny, int nz, const double* par /* cex3,cdm
     LocalP<double> lp;
     for (int a = 0; a < 3; a++) { lp.cex[a] = par[a]; lp.cdm[a] = par[3 + a]; lp.u[a] = par[7 + a]; lp.hext[a] = par[10 + a]; }
     lp.cku = par[6]; lp.gp = par[13]; lp.agp = par[14]; lp.dmi = dmi; lp.terms = terms;
-    lp.ckc = 0; lp.Acell = nullptr; lp.Dcell = nullptr; lp.Hcell = nullptr; lp.Hth = nullptr; lp.stt_on = 0; lp.sl_on = 0;
+    lp.ckc = 0; lp.Acell = nullptr; lp.Dcell = nullptr; lp.Hcell = nullptr; lp.Hth = nullptr; lp.stt_on = 0; lp.sl_on = 0; lp.stt_b = 0; lp.stt_w = 0;
     const long N = g.N;
     for (long q = 0; q < N; q++) {
         v3<double> res = { 0, 0, 0 };
@@ -149,7 +149,7 @@ extern "C" void emul_local2(int nx, int ny, int nz, const double* par /* cex3,cd
     LocalP<double> lp;
     for (int a = 0; a < 3; a++) { lp.cex[a] = par[a]; lp.cdm[a] = par[3 + a]; lp.u[a] = par[7 + a]; lp.hext[a] = par[10 + a]; }
     lp.cku = par[6]; lp.gp = par[13]; lp.agp = par[14]; lp.ckc = par[15]; lp.dmi = dmi; lp.terms = terms;
-    lp.Acell = Acell; lp.Dcell = Dcell; lp.Hcell = Hcell; lp.Hth = nullptr; lp.stt_on = 0; lp.sl_on = 0;
+    lp.Acell = Acell; lp.Dcell = Dcell; lp.Hcell = Hcell; lp.Hth = nullptr; lp.stt_on = 0; lp.sl_on = 0; lp.stt_b = 0; lp.stt_w = 0;
     const long N = g.N;
     for (long q = 0; q < N; q++) {
         v3<double> res = { 0, 0, 0 };

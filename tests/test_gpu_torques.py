@@ -175,3 +175,63 @@ def test_equilibrium_distribution_on_the_gpu(prec):
     ref2 = np.sum(wq * p * x * x) / np.sum(wq * p)
     assert abs(np.mean(mz2) - ref2) < 4 * 0.3 / np.sqrt(n * n * len(mz2)) + 0.01
     assert np.abs(np.sqrt((a * a).sum(axis=0)) - 1).max() < (1e-12 if prec == F64 else 1e-5)
+
+
+@pytest.mark.parametrize("prec", [F64, F32])
+@pytest.mark.parametrize("integ", [wl.RK4, wl.DOPRI5, wl.CAYLEY_RK4])
+def test_time_dependent_current_matches_oracle(integ, prec):
+    """u(t) = u exp(-b t) cos(w t) evaluated at every stage's own time on the device: ten fixed-dt steps
+    from a non-zero start time against the oracle, every integrator; and the right-hand side alone at that time."""
+    w = problem(32, 16, 2)
+    w.integrator = integ
+    o, s = make_pair(w, prec)
+    both(o, s, "set_zhang_li", 200.0, -50.0, 30.0, 0.25)
+    both(o, s, "set_zhang_li_pulse", 5e8, 2e9)
+    both(o, s, "set_time", 3.7e-10)
+    m = masked_m(w)
+    dm = s.to_device(m)
+    kref = o.llg_rhs(m)
+    k = to_np(s.llg_rhs(dm))
+    assert np.abs(k - kref).max() <= (1e-9 if prec == F64 else 2e-4) * np.abs(kref).max()
+    dt = 4e-13 if integ != wl.DOPRI5 else 1e-13       # large steps: a current frozen at the step start would show
+    for _ in range(10):
+        o.step(m, dt)
+        s.step(dm, dt, sync=False)
+    assert np.abs(to_np(dm) - m).max() <= (1e-9 if prec == F64 else 5e-3)
+    assert np.isclose(s.time(), o.time(), rtol=1e-12)
+
+
+def test_domain_wall_under_the_papers_pulse_on_the_gpu():
+    """PAPER.md:436-448, Fig. 5 on the GPU (fp64, DOPRI5): wall position and tilt under u0 exp(-b t) cos(w t) against
+    Eq. 54 integrated in closed form."""
+    nx, dx, alpha, beta, A, K, u0, b, om = 512, 1e-9, 0.1, 0.3, 1.3e-11, 1e5, 300.0, 5e8, 2e9
+    Delta = np.sqrt(A / K)
+    w = wl.Workload("wall", nx, 1, 1, dx, dx, dx, Ms=8e5, A=A, Ku=K, axis=(1.0, 0.0, 0.0), alpha=alpha, gamma=GAMMA, integrator=wl.DOPRI5, demag=False)
+    x = (np.arange(nx) + 0.5) * dx
+    m = np.zeros((3, 1, 1, nx))
+    m[0, 0, 0] = -np.tanh((x - 256e-9) / Delta)
+    m[1, 0, 0] = 1 / np.cosh((x - 256e-9) / Delta)
+    w.m0 = m
+    s = make_pair(w, F64)[1]
+    dm = s.to_device(m)
+
+    def wall():
+        a = to_np(dm)
+        return 0.5 * nx * dx * (1 + a[0].mean()), np.arctan2(a[2].sum(), a[1].sum())
+
+    dt = 1e-13
+    for _ in range(200):
+        s.step(dm, dt, sync=False)
+    s.set_time(0.0)
+    s.set_zhang_li(u0, 0, 0, beta)
+    s.set_zhang_li_pulse(b, om)
+    p0, f0 = wall()
+    U = lambda t: u0 * (np.exp(-b * t) * (om * np.sin(om * t) - b * np.cos(om * t)) + b) / (b * b + om * om)
+    Umax = abs(U(7.85e-10))
+    for i in range(1, 12001):
+        s.step(dm, dt, sync=False)
+        if i % 3000 == 0:
+            t = i * dt
+            p, f = wall()
+            assert abs((p - p0) + (1 + alpha * beta) * U(t) / (1 + alpha**2)) <= 0.01 * Umax + 2e-11
+            assert abs((f - f0) - (alpha - beta) * U(t) / ((1 + alpha**2) * Delta)) <= 0.02 * abs(alpha - beta) * Umax / Delta
