@@ -6,7 +6,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmm.so")
 SOURCES = ["mm_lib.cu", "mm_newell_host.cpp"]
-HEADERS = ["mm_fft.cuh", "mm_kernels.cuh", "mm_kernels2.cuh", "mm_passAC.cuh", "mm_passB7.cuh", "mm_passB3.cuh", "mm_llg.cuh", os.path.join("..", "..", "include", "mm.h")]
+HEADERS = ["mm_fft.cuh", "mm_kernels.cuh", "mm_kernels2.cuh", "mm_passAC.cuh", "mm_passB7.cuh", "mm_passB3.cuh", "mm_passB4.cuh", "mm_llg.cuh", os.path.join("..", "..", "include", "mm.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 
 

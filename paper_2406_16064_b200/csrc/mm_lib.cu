@@ -2,6 +2,7 @@
 // Hand-written CUDA for sm_100a; no cuFFT, no cuBLAS, no CPU fallback.
 #include <cuda.h>
 #include <cuda_runtime.h>
+#include <cooperative_groups.h>
 #include <math.h>
 #include <stdint.h>
 #include <stdio.h>
@@ -17,6 +18,7 @@
 #include "mm_passAC.cuh"
 #include "mm_passB7.cuh"
 #include "mm_passB3.cuh"
+#include "mm_passB4.cuh"
 #include "mm_llg.cuh"
 
 #ifndef MM_OCC_A
@@ -97,6 +99,24 @@ __global__ void __launch_bounds__(256) y_conv3_kernel(Geom g, const cx<T>* S, cx
 {
     if (st->done) return;
     y_conv_body3<T, V>(g, S, S2, Kh, tw, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, blockDim.x);
+}
+// cluster form (mm_passB4.cuh): the long-line path; Q CTAs of a thread-block cluster share one line through
+// distributed shared memory
+template <typename T, int V, int Q>
+__global__ void __launch_bounds__(256, sizeof(T) == 8 ? 1 : 2) y_conv4_kernel(Geom g, cx<T>* S, const T* Kh, twiddles<T> tw, const DevState* st)
+{
+    if (st->done) return;      // the same for every CTA of the cluster
+    namespace cg = cooperative_groups;
+    cg::cluster_group cl = cg::this_cluster();
+    const int q = (int)cl.block_rank(), tile = (int)(blockIdx.x / Q);
+    cx<T>* s = reinterpret_cast<cx<T>*>(mm_smem);
+    y_conv_body4_compute<T, V, Q>(g, S, Kh, tw, s, tile, q, threadIdx.x, blockDim.x);
+    cl.sync();      // every block's z_q is complete and visible across the cluster
+    cx<T>* tiles[Q];
+#pragma unroll
+    for (int qq = 0; qq < Q; qq++) tiles[qq] = cl.map_shared_rank(s, qq);
+    y_conv_body4_combine<T, V, Q>(g, S, tiles, tile, q, threadIdx.x, blockDim.x);
+    cl.sync();      // nobody leaves while a neighbour still reads its tile
 }
 // compile-time specialised form of the TMA pass B (mm_passB7.cuh): ny = 2^LOGM; fp32: TC = 4, 256 threads; fp64: TC = 2,
 // 128 threads (rows of 32 bytes and tiles of py * 96 bytes in both; two CTAs per SM)
@@ -899,6 +919,7 @@ struct mm_sim {
     std::vector<StepGraph> graphs;
     cudaStream_t cap_stream;         // capture happens on a private stream (the caller's may be the legacy default stream)
     int use_graph;
+    int use_b4, clQ;                 // pass B runs the cluster form with clusters of clQ CTAs (long lines)
     int use_b3;                      // pass B runs the half-tile form (a full py-row tile does not fit one CTA)
     size_t off_S2;                   // its output spectrum
     size_t off_ei, off_eo;           // embedding: inner-layout copies of the caller's input / output fields
@@ -1004,9 +1025,26 @@ static void configure(mm_sim* s)
     if (getenv("MM_TC")) TC = atoi(getenv("MM_TC"));       // tuning knob (power of two)
     g.TC = TC;
     while (g.TC > 1 && (size_t)smemB_elems(g) * cs > SMEM_CAP) g.TC /= 2;
+    // a line that does not fit one CTA even one column wide (fp64, ny = 4096) -> a cluster of Q CTAs shares the line,
+    // each with a tile of py/Q rows of 32 bytes (mm_passB4.cuh).  Measured (profiles/r02_experiments.md): 4096^2 fp64
+    // 4.2 ms against 5.2 ms of the half-tile form; where a full tile still fits (TC = 2 or 1) the single-CTA kernels
+    // stay faster (2048^2 fp32 184 us against 306 / 418 us with clusters of 2 / 4), so they keep those sizes.
+    s->use_b4 = 0; s->clQ = 0;
+    {
+        const int tcmin = s->prec == MM_F64 ? 2 : 4;
+        if (s->use_v2 && !getenv("MM_NO_B4") && !getenv("MM_B3") && ((size_t)g.py * 3 * cs > SMEM_CAP || getenv("MM_B4"))) {
+            // the smallest cluster whose tile fits, with the widest rows that fit it (measured at 4096^2 fp64: Q = 2 with
+            // 16-byte rows 2.9 ms, Q = 4 with 32-byte rows 4.2 ms — every CTA re-reads the whole input line)
+            for (int Q = 2; Q <= 4 && !s->use_b4; Q *= 2) {
+                if (getenv("MM_Q") && atoi(getenv("MM_Q")) != Q) continue;
+                for (int tc = getenv("MM_TC") ? atoi(getenv("MM_TC")) : tcmin; tc >= 1 && !s->use_b4; tc /= 2)
+                    if (g.py / Q >= 16 && (size_t)(g.py / Q) * 3 * tc * cs <= SMEM_CAP) { s->use_b4 = 1; s->clQ = Q; g.TC = tc; }
+            }
+        }
+    }
     // a line that does not fit even one column wide (or MM_B3=1, for measurements): half-tile form, ny rows per tile
     s->use_b3 = 0;
-    if (s->use_v2 && g.ny >= 16 && ((size_t)smemB_elems(g) * cs > SMEM_CAP || getenv("MM_B3"))) {
+    if (!s->use_b4 && s->use_v2 && g.ny >= 16 && ((size_t)smemB_elems(g) * cs > SMEM_CAP || getenv("MM_B3"))) {
         s->use_b3 = 1;
         g.TC = s->prec == MM_F64 ? 4 : 8;
         if (getenv("MM_TC")) g.TC = atoi(getenv("MM_TC"));
@@ -1015,12 +1053,12 @@ static void configure(mm_sim* s)
     // fp32: two resident CTAs per SM (tile <= 98 KB) beat one CTA with a tile twice as wide — one CTA's
     // shared-memory-bound stages overlap the other's FP32-bound ones (measured, profiles/r01_experiments.md)
     if (s->prec == MM_F32 && !getenv("MM_TC") && g.TC >= 4 && (size_t)smemB_elems(g) * cs > 98 * 1024) g.TC /= 2;
-    while (g.TC > 2 && ((g.nx + g.TC) / g.TC) * g.pz < target && !s->use_b3) g.TC /= 2;
+    while (g.TC > 2 && ((g.nx + g.TC) / g.TC) * g.pz < target && !s->use_b3 && !s->use_b4) g.TC /= 2;
     // fp64: the specialised pass B (mm_passB7.cuh) wants rows of 32 bytes = two columns, tiles of py * 96 bytes
-    const bool b7_f64 = s->prec == MM_F64 && !getenv("MM_TC") && !s->no_b7 && !s->use_b3 && s->use_v2 && g.logny >= 4 && g.logny <= 10 && g.TC >= 2;
+    const bool b7_f64 = s->prec == MM_F64 && !getenv("MM_TC") && !s->no_b7 && !s->use_b3 && !s->use_b4 && s->use_v2 && g.logny >= 4 && g.logny <= 10 && g.TC >= 2;
     if (b7_f64) g.TC = 2;
     // ny = 1024: the specialised pass B with one 196 KB tile per SM (rows of 32 bytes in both precisions)
-    const bool b7_10 = g.logny == 10 && !getenv("MM_TC") && !s->no_b7 && !s->use_b3 && s->use_v2;
+    const bool b7_10 = g.logny == 10 && !getenv("MM_TC") && !s->no_b7 && !s->use_b3 && !s->use_b4 && s->use_v2;
     if (b7_10 && s->prec == MM_F32) g.TC = 4;
     g.Lx = ((g.nx + 1 + g.TC - 1) / g.TC) * g.TC;
     g.plane = (long)g.ny * g.Lx;
@@ -1031,11 +1069,12 @@ static void configure(mm_sim* s)
     // the v2 bodies of passes A / C do the z transform in registers: no scratch tile
     g.xpad = g.G * g.nz <= 4 ? 1 : 0;      // G may have shrunk above
     s->smemA2 = (size_t)smemA2_elems(g) * cs;
-    s->smemB = s->use_b3 ? (size_t)smemB3_elems(g) * cs : (size_t)smemB_elems(g) * cs;
+    s->smemB = s->use_b4 ? (size_t)smemB4_elems(g, s->clQ) * cs : (s->use_b3 ? (size_t)smemB3_elems(g) * cs : (size_t)smemB_elems(g) * cs);
     s->thrA = 256;
     s->thrB = (s->prec == MM_F32 && s->smemB > 98 * 1024) ? 512 : 256;
     if (b7_f64) s->thrB = 128;
     if (b7_10) s->thrB = s->prec == MM_F64 ? 256 : 512;
+    if (s->use_b4) s->thrB = 256;
     if (s->use_b3) s->thrB = 256;      // 255 registers per thread: the multiply stage holds 3 x 8 complex values + K^ (512 threads spilled kilobytes)
     if (getenv("MM_THRB")) s->thrB = atoi(getenv("MM_THRB"));
 }
@@ -1052,7 +1091,7 @@ static void layout(mm_sim* s)
     s->off_S = take((size_t)3 * g.comp * 2 * es);
     s->off_S2 = take(s->use_b3 ? (size_t)3 * g.comp * 2 * es : 0);
     s->off_Kh = take((size_t)6 * g.kcomp * es);
-    s->off_Kc = take((s->use_v2 && g.ny >= 16 && !s->use_b3 ? (size_t)kc_elems(g) : 0) * es);      // pass B v2: K^ in consumption order
+    s->off_Kc = take((s->use_v2 && g.ny >= 16 && !s->use_b3 && !s->use_b4 ? (size_t)kc_elems(g) : 0) * es);      // pass B v2: K^ in consumption order
     s->off_Hd = take(3 * N * es);
     for (int i = 0; i < 7; i++) s->off_k[i] = take(3 * N * es);
     for (int i = 0; i < 2; i++) s->off_y[i] = take(3 * N * es);
@@ -1388,7 +1427,7 @@ template <typename T> static int init_demag_t(mm_sim* s)
         s->launches++;
         MM_TRY(s, cudaGetLastError());
     }
-    if (s->use_v2 && g.ny >= 16 && !s->use_b3) {
+    if (s->use_v2 && g.ny >= 16 && !s->use_b3 && !s->use_b4) {
         const long total = kc_elems(g);
         kc_fill_kernel<T><<<(unsigned)((total + 255) / 256), 256, 0, st>>>(g, Kh, wsp<T>(s, s->off_Kc), total);
         s->launches++;
@@ -1500,6 +1539,18 @@ template <typename T, int NZ> static void launch_A2(mm_sim* s, unsigned grid, co
     if (!raise_smem_limit(s, (const void*)fwd_xz2_kernel<T, NZ, false>)) return;
     fwd_xz2_kernel<T, NZ, false><<<grid, s->thrA, s->smemA2, s->stream>>>(s->g, y, wsp<T>(s, s->off_Ms), S, tw, st);
 }
+template <typename T, int V, int Q> static void launch_B4(mm_sim* s, unsigned ntile, cx<T>* S, twiddles<T> tw, const DevState* st)
+{
+    if (!raise_smem_limit(s, (const void*)y_conv4_kernel<T, V, Q>)) return;
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = dim3(ntile * Q); cfg.blockDim = dim3(s->thrB); cfg.dynamicSmemBytes = s->smemB; cfg.stream = s->stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = Q; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, y_conv4_kernel<T, V, Q>, s->g, S, (const T*)wsp<T>(s, s->off_Kh), tw, st);
+}
 template <typename T, int V> static void launch_B3(mm_sim* s, unsigned grid, cx<T>* S, twiddles<T> tw, const DevState* st)
 {
     if (!raise_smem_limit(s, (const void*)y_conv3_kernel<T, V>)) return;
@@ -1530,7 +1581,7 @@ template <typename T, int V> static void launch_B5(mm_sim* s, unsigned grid, cx<
 template <typename T> static bool b7_applies(const mm_sim* s)
 {
     const Geom& g = s->g;
-    return s->use_v2 && !s->no_b7 && !s->use_b3 && g.logny >= 4 && g.logny <= 10 && g.TC == (sizeof(T) == 8 ? 2 : 4) &&
+    return s->use_v2 && !s->no_b7 && !s->use_b3 && !s->use_b4 && g.logny >= 4 && g.logny <= 10 && g.TC == (sizeof(T) == 8 ? 2 : 4) &&
            s->thrB == (sizeof(T) == 8 ? 128 : 256) * (g.logny >= 10 ? 2 : 1);
 }
 template <typename T, int LOGM, bool IS3D> static void launch_B7(mm_sim* s, unsigned grid, cx<T>* S, twiddles<T> tw, const DevState* st)
@@ -1603,7 +1654,11 @@ template <typename T> static int demag_passes(mm_sim* s, const T* y)
     }
     prof_end(s);
     prof_begin(s, 1);
-    if (b2 && s->use_b3) {
+    if (b2 && s->use_b4) {
+        constexpr int V4 = sizeof(T) == 4 ? 2 : 1;
+        if (s->clQ == 4) { if (g.TC % V4 == 0) launch_B4<T, V4, 4>(s, gridB, S, tw, st); else launch_B4<T, 1, 4>(s, gridB, S, tw, st); }
+        else { if (g.TC % V4 == 0) launch_B4<T, V4, 2>(s, gridB, S, tw, st); else launch_B4<T, 1, 2>(s, gridB, S, tw, st); }
+    } else if (b2 && s->use_b3) {
         if (sizeof(T) == 4 && g.TC % 2 == 0) launch_B3<T, (sizeof(T) == 4 ? 2 : 1)>(s, gridB, S, tw, st);
         else launch_B3<T, 1>(s, gridB, S, tw, st);
         S = wsp<cx<T>>(s, s->off_S2);      // pass C reads the half-tile form's output buffer

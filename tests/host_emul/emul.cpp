@@ -11,6 +11,7 @@
 #include "../../paper_2406_16064_b200/csrc/mm_passAC.cuh"
 #include "../../paper_2406_16064_b200/csrc/mm_passB7.cuh"
 #include "../../paper_2406_16064_b200/csrc/mm_passB3.cuh"
+#include "../../paper_2406_16064_b200/csrc/mm_passB4.cuh"
 #include "../../paper_2406_16064_b200/csrc/mm_llg.cuh"
 
 using namespace mm;
@@ -70,7 +71,7 @@ static void run(int ver, int nx, int ny, int nz, int G, int CH, int TC, const do
     std::vector<cx<T>> smem((size_t)std::max(std::max(smemA_elems(g), smemA2_elems(g)), smemB_elems(g)) + 16);
     const int gridA = 3 * (ny / G), gridB = (g.Lx / TC) * g.pz;
     const double P = (double)g.px * g.py * g.pz;
-    const bool a2 = ver >= 2 && nx >= 32 && nz <= 32, b2 = ver >= 2 && ny >= 16, b5 = (ver == 5 || ver == 7) && ny >= 16;
+    const bool a2 = ver >= 2 && nx >= 32 && nz <= 32, b2 = ver >= 2 && ny >= 16, b5 = (ver == 5 || ver == 7) && ny >= 16;      // ver 42 / 44 without room for the cluster form fall to y_conv_body2
     for (int b = 0; b < gridA; b++) {
         if (!a2) fwd_xz_body<T>(g, mt.data(), Mst.data(), S.data(), tw, smem.data(), b, 0, 1);
         else switch (nz) {
@@ -83,7 +84,24 @@ static void run(int ver, int nx, int ny, int nz, int G, int CH, int TC, const do
     constexpr int LOGTC7 = sizeof(T) == 8 ? 1 : 2;
     const bool b3 = ver == 3 && ny >= 16;
     std::vector<cx<T>> S2(b3 ? S.size() : 0);      // half-tile pass B writes a second spectrum buffer
-    for (int b = 0; b < gridB; b++) {
+    const int Q4 = ver == 42 ? 2 : (ver == 44 ? 4 : 0);      // cluster pass B: the Q CTAs of a cluster run one after the other
+    const bool b4 = Q4 != 0 && g.py / Q4 >= 16;
+    if (b4) {
+        std::vector<std::vector<cx<T>>> tiles(Q4, std::vector<cx<T>>((size_t)smemB4_elems(g, Q4) + 16));
+        cx<T>* tp[4] = { nullptr, nullptr, nullptr, nullptr };
+        for (int qq = 0; qq < Q4; qq++) tp[qq] = tiles[qq].data();
+        for (int b = 0; b < gridB; b++) {
+            for (int qq = 0; qq < Q4; qq++) {
+                if (Q4 == 2) { if (sizeof(T) == 4 && TC % 2 == 0) y_conv_body4_compute<T, (sizeof(T) == 4 ? 2 : 1), 2>(g, S.data(), Kh.data(), tw, tp[qq], b, qq, 0, 1); else y_conv_body4_compute<T, 1, 2>(g, S.data(), Kh.data(), tw, tp[qq], b, qq, 0, 1); }
+                else { if (sizeof(T) == 4 && TC % 2 == 0) y_conv_body4_compute<T, (sizeof(T) == 4 ? 2 : 1), 4>(g, S.data(), Kh.data(), tw, tp[qq], b, qq, 0, 1); else y_conv_body4_compute<T, 1, 4>(g, S.data(), Kh.data(), tw, tp[qq], b, qq, 0, 1); }
+            }
+            for (int qq = 0; qq < Q4; qq++) {
+                if (Q4 == 2) { if (sizeof(T) == 4 && TC % 2 == 0) y_conv_body4_combine<T, (sizeof(T) == 4 ? 2 : 1), 2>(g, S.data(), tp, b, qq, 0, 1); else y_conv_body4_combine<T, 1, 2>(g, S.data(), tp, b, qq, 0, 1); }
+                else { if (sizeof(T) == 4 && TC % 2 == 0) y_conv_body4_combine<T, (sizeof(T) == 4 ? 2 : 1), 4>(g, S.data(), tp, b, qq, 0, 1); else y_conv_body4_combine<T, 1, 4>(g, S.data(), tp, b, qq, 0, 1); }
+            }
+        }
+    }
+    for (int b = 0; b < gridB && !b4; b++) {
         if (b3) {
             if (sizeof(T) == 4 && TC % 2 == 0) y_conv_body3<T, (sizeof(T) == 4 ? 2 : 1)>(g, S.data(), S2.data(), Kh.data(), tw, smem.data(), b, 0, 1);
             else y_conv_body3<T, 1>(g, S.data(), S2.data(), Kh.data(), tw, smem.data(), b, 0, 1);

@@ -368,6 +368,30 @@ def test_pass_b_half_tile_form(monkeypatch, prec):
     assert np.abs(to_np(dm) - m).max() <= (1e-9 if prec == F64 else 2e-3)
 
 
+@pytest.mark.parametrize("prec", [F64, F32])
+@pytest.mark.parametrize("Q", ["2", "4"])
+def test_pass_b_cluster_form(monkeypatch, prec, Q):
+    """The cluster form of pass B (mm_passB4.cuh: Q CTAs share one long y line through distributed shared memory) forced
+    on small meshes (MM_B4, MM_Q): 3-D and film, both precisions, against the oracle; then a few steps."""
+    monkeypatch.setenv("MM_B4", "1")
+    monkeypatch.setenv("MM_Q", Q)
+    w = small3d(64, 64, 16)
+    o, s = make_pair(w, prec)
+    m = masked_m(w)
+    assert np.abs(to_np(s.effective_field(s.to_device(m))) - o.effective_field(m)).max() / w.Ms_max <= HTOL[prec]
+    wf = film(512)
+    o, s = make_pair(wf, prec)
+    H = to_np(s.effective_field(s.to_device(wf.m0)))
+    assert np.abs(H - o.effective_field(np.ascontiguousarray(wf.m0))).max() / wf.Ms_max <= HTOL[prec]
+    wn = small3d(32, 32, 2)
+    o, s = make_pair(wn, prec)
+    m = masked_m(wn)
+    dm = s.to_device(m)
+    for _ in range(3):
+        o.step(m, wn.dt); s.step(dm, wn.dt, sync=False)
+    assert np.abs(to_np(dm) - m).max() <= (1e-9 if prec == F64 else 2e-3)
+
+
 def test_cfg4_full_size_step_invariants():
     """configs[3] in bench.py's configuration (fp32, fixed-dt DOPRI5): |m| = 1 after every step, finite,
     and the energy does not increase (alpha > 0, constant field)."""

@@ -20,7 +20,7 @@ _dp = C.POINTER(C.c_double)
 
 @pytest.fixture(scope="module")
 def emul():
-    deps = [SRC] + [os.path.join(ROOT, "paper_2406_16064_b200", "csrc", f) for f in ("mm_fft.cuh", "mm_kernels.cuh", "mm_kernels2.cuh", "mm_passAC.cuh", "mm_passB7.cuh", "mm_passB3.cuh", "mm_llg.cuh")]
+    deps = [SRC] + [os.path.join(ROOT, "paper_2406_16064_b200", "csrc", f) for f in ("mm_fft.cuh", "mm_kernels.cuh", "mm_kernels2.cuh", "mm_passAC.cuh", "mm_passB7.cuh", "mm_passB3.cuh", "mm_passB4.cuh", "mm_llg.cuh")]
     if not os.path.exists(LIB) or os.path.getmtime(LIB) < max(os.path.getmtime(d) for d in deps):
         subprocess.run(["g++", "-O1", "-std=c++17", "-fPIC", "-shared", "-o", LIB, SRC], check=True)
     L = C.CDLL(LIB)
@@ -57,7 +57,7 @@ def khat_full(o, nx, ny, nz):
                                        ((32, 16, 1), (4, 8, 8)), ((64, 32, 2), (2, 8, 4)), ((32, 64, 16), (1, 8, 8)),
                                        ((128, 128, 1), (2, 8, 2)), ((256, 16, 4), (1, 8, 1)), ((32, 32, 32), (1, 8, 4))])
 @pytest.mark.parametrize("prec64", [1, 0])
-@pytest.mark.parametrize("ver", [1, 2, 3, 5])
+@pytest.mark.parametrize("ver", [1, 2, 3, 5, 42, 44])
 def test_demag_passes_match_oracle(emul, shape, cfg, prec64, ver):
     nx, ny, nz = shape
     G, CH, TC = cfg
