@@ -1151,6 +1151,7 @@ extern "C" int mm_create(mm_sim** out, int nx, int ny, int nz, double dx, double
 extern "C" int mm_destroy(mm_sim* s)
 {
     if (s) {
+        if (s->ws && !s->graphs.empty()) { cudaSetDevice(s->device); cudaStreamSynchronize(s->stream); cudaGetLastError(); }      // no replay in flight
         for (cudaEvent_t e : s->prof_ev) cudaEventDestroy(e);
         for (auto& g : s->graphs) if (g.exec) cudaGraphExecDestroy(g.exec);
         if (s->cap_stream) cudaStreamDestroy(s->cap_stream);

@@ -392,6 +392,30 @@ def test_pass_b_cluster_form(monkeypatch, prec, Q):
     assert np.abs(to_np(dm) - m).max() <= (1e-9 if prec == F64 else 2e-3)
 
 
+@pytest.mark.parametrize("prec", [F64, F32])
+def test_step_graph_replay_is_bitwise_the_eager_path(monkeypatch, prec):
+    """Whole-step CUDA graphs (captured on the second step, replayed afterwards) must give exactly what kernel-by-kernel
+    launches give: fixed-dt steps, a parameter change in between (new key -> new capture), adaptive steps."""
+    w = small3d(32, 32, 4)
+    m0 = masked_m(w)
+    res = []
+    for no_graph in ("", "1"):
+        if no_graph:
+            monkeypatch.setenv("MM_NO_GRAPH", "1")
+        s = make_pair(w, prec)[1]
+        dm = s.to_device(m0)
+        for _ in range(5):
+            s.step(dm, w.dt, sync=False)
+        s.set_alpha(0.3)
+        for _ in range(4):
+            s.step(dm, w.dt, sync=False)
+        n, _ = s.relax(dm, 1e-5, 0.0, 12, 1e-14)
+        assert n == 12
+        res.append((to_np(dm), s.time(), s.launch_count()))
+    assert np.array_equal(res[0][0], res[1][0])
+    assert res[0][1] == res[1][1] and res[0][2] == res[1][2]
+
+
 def test_cfg4_full_size_step_invariants():
     """configs[3] in bench.py's configuration (fp32, fixed-dt DOPRI5): |m| = 1 after every step, finite,
     and the energy does not increase (alpha > 0, constant field)."""
