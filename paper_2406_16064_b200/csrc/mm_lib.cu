@@ -1115,7 +1115,7 @@ static void layout(mm_sim* s)
     s->ws_need = o;
 }
 
-extern "C" const char* mm_version(void) { return "mm-b200 0.3 (sm_100a)"; }
+extern "C" const char* mm_version(void) { return "mm-b200 0.4 (sm_100a)"; }
 
 extern "C" int mm_create(mm_sim** out, int nx, int ny, int nz, double dx, double dy, double dz, mm_prec prec, int device, void* cuda_stream)
 {
