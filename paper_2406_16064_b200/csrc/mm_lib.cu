@@ -121,14 +121,15 @@ __global__ void __launch_bounds__(256, sizeof(T) == 8 ? 1 : 2) y_conv4_kernel(Ge
 // compile-time specialised form of the TMA pass B (mm_passB7.cuh): ny = 2^LOGM; fp32: TC = 4, 256 threads; fp64: TC = 2,
 // 128 threads (rows of 32 bytes and tiles of py * 96 bytes in both; two CTAs per SM)
 // ny = 1024: one CTA per SM with twice the threads (tile py * 96 bytes = 196 KB)
-// NARROW (fp32, ny = 512): tiles of 2 columns (16-byte rows, 48 KB), 128 threads, four CTAs per SM — the phases of four
-// small CTAs interleave better than those of two (cfg4 pass B 186.5 -> 180.2 us, profiles/r02_experiments.md)
+// NARROW (fp32, ny = 512 / 1024): tiles of 2 columns (16-byte rows, 48 / 96 KB), 128 / 256 threads, four / two CTAs per
+// SM — the phases of more, smaller CTAs interleave better (cfg4 pass B 186.5 -> 182 us, film 1024^2 45.3 -> 43.0 us,
+// profiles/r02_experiments.md)
 template <typename T, int LOGM, bool IS3D, bool NARROW = false>
-__global__ void __launch_bounds__(NARROW ? 128 : (sizeof(T) == 8 ? 128 : 256) * (LOGM >= 10 ? 2 : 1), NARROW ? 4 : (LOGM >= 10 ? 1 : 2)) y_conv7_kernel(Geom g, cx<T>* S, const T* Kc, twiddles<T> tw, int logtw, const DevState* st,
+__global__ void __launch_bounds__((NARROW || sizeof(T) == 8 ? 128 : 256) * (LOGM >= 10 ? 2 : 1), (NARROW ? 4 : 2) / (LOGM >= 10 ? 2 : 1)) y_conv7_kernel(Geom g, cx<T>* S, const T* Kc, twiddles<T> tw, int logtw, const DevState* st,
                                                                                 const __grid_constant__ CUtensorMap tmS)
 {
     __shared__ __align__(8) unsigned long long bar[3];
-    constexpr int LOGTC = (NARROW || sizeof(T) == 8) ? 1 : 2, NTHR = NARROW ? 128 : (sizeof(T) == 8 ? 128 : 256) * (LOGM >= 10 ? 2 : 1);
+    constexpr int LOGTC = (NARROW || sizeof(T) == 8) ? 1 : 2, NTHR = (NARROW || sizeof(T) == 8 ? 128 : 256) * (LOGM >= 10 ? 2 : 1);
     y_conv_body7<LOGM, LOGTC, IS3D, NTHR, T>(g, S, Kc, tw, logtw, reinterpret_cast<cx<T>*>(mm_smem), blockIdx.x, threadIdx.x, NTHR, &tmS, bar, &st->done);
 }
 template <typename T, int NZ, bool PAD>
@@ -921,7 +922,7 @@ struct mm_sim {
     std::vector<StepGraph> graphs;
     cudaStream_t cap_stream;         // capture happens on a private stream (the caller's may be the legacy default stream)
     int use_graph;
-    int b7_narrow;                   // fp32, ny = 512: the specialised pass B runs tiles of 2 columns, four CTAs per SM
+    int b7_narrow;                   // fp32, ny = 512 / 1024: the specialised pass B runs tiles of 2 columns, four / two CTAs per SM
     int use_b4, clQ;                 // pass B runs the cluster form with clusters of clQ CTAs (long lines)
     int use_b3;                      // pass B runs the half-tile form (a full py-row tile does not fit one CTA)
     size_t off_S2;                   // its output spectrum
@@ -1063,7 +1064,7 @@ static void configure(mm_sim* s)
     // ny = 1024: the specialised pass B with one 196 KB tile per SM (rows of 32 bytes in both precisions)
     const bool b7_10 = g.logny == 10 && !getenv("MM_TC") && !s->no_b7 && !s->use_b3 && !s->use_b4 && s->use_v2;
     if (b7_10 && s->prec == MM_F32) g.TC = 4;
-    s->b7_narrow = (s->prec == MM_F32 && g.logny == 9 && g.TC == 4 && !getenv("MM_TC") && !s->no_b7 && !s->use_b3 && !s->use_b4 && s->use_v2 && !(getenv("MM_NO_NARROW") && getenv("MM_NO_NARROW")[0])) ? 1 : 0;
+    s->b7_narrow = (s->prec == MM_F32 && (g.logny == 9 || g.logny == 10) && g.TC == 4 && !getenv("MM_TC") && !s->no_b7 && !s->use_b3 && !s->use_b4 && s->use_v2 && !(getenv("MM_NO_NARROW") && getenv("MM_NO_NARROW")[0])) ? 1 : 0;
     if (s->b7_narrow) g.TC = 2;
     g.Lx = ((g.nx + 1 + g.TC - 1) / g.TC) * g.TC;
     if (s->b7_narrow) g.Lx = ((g.nx + 1 + 3) / 4) * 4;      // rows of S keep their 32-byte alignment for passes A / C
@@ -1080,7 +1081,7 @@ static void configure(mm_sim* s)
     s->thrB = (s->prec == MM_F32 && s->smemB > 98 * 1024) ? 512 : 256;
     if (b7_f64) s->thrB = 128;
     if (b7_10) s->thrB = s->prec == MM_F64 ? 256 : 512;
-    if (s->b7_narrow) s->thrB = 128;
+    if (s->b7_narrow) s->thrB = g.logny >= 10 ? 256 : 128;
     if (s->use_b4) s->thrB = 256;
     if (s->use_b3) s->thrB = 256;      // 255 registers per thread: the multiply stage holds 3 x 8 complex values + K^ (512 threads spilled kilobytes)
     if (getenv("MM_THRB")) s->thrB = atoi(getenv("MM_THRB"));
@@ -1589,7 +1590,7 @@ template <typename T, int V> static void launch_B5(mm_sim* s, unsigned grid, cx<
 template <typename T> static bool b7_applies(const mm_sim* s)
 {
     const Geom& g = s->g;
-    if (sizeof(T) == 4 && s->b7_narrow) return g.TC == 2 && s->thrB == 128;
+    if (sizeof(T) == 4 && s->b7_narrow) return g.TC == 2 && s->thrB == (g.logny >= 10 ? 256 : 128);
     return s->use_v2 && !s->no_b7 && !s->use_b3 && !s->use_b4 && g.logny >= 4 && g.logny <= 10 && g.TC == (sizeof(T) == 8 ? 2 : 4) &&
            s->thrB == (sizeof(T) == 8 ? 128 : 256) * (g.logny >= 10 ? 2 : 1);
 }
@@ -1604,6 +1605,11 @@ template <typename T> static bool try_launch_B7(mm_sim* s, unsigned grid, cx<T>*
     const Geom& g = s->g;
     if (!s->use_tma || !b7_applies<T>(s)) return false;
     const bool d3 = g.nz > 1;
+    if (sizeof(T) == 4 && s->b7_narrow && g.logny == 10) {
+        if (d3) { if (raise_smem_limit(s, (const void*)y_conv7_kernel<float, 10, true, true>)) y_conv7_kernel<float, 10, true, true><<<grid, 256, s->smemB, s->stream>>>(s->g, (cx<float>*)S, (const float*)wsp<float>(s, s->off_Kc), *reinterpret_cast<twiddles<float>*>(&tw), ilog2(s->twN), st, s->tmS); }
+        else { if (raise_smem_limit(s, (const void*)y_conv7_kernel<float, 10, false, true>)) y_conv7_kernel<float, 10, false, true><<<grid, 256, s->smemB, s->stream>>>(s->g, (cx<float>*)S, (const float*)wsp<float>(s, s->off_Kc), *reinterpret_cast<twiddles<float>*>(&tw), ilog2(s->twN), st, s->tmS); }
+        return true;
+    }
     if (sizeof(T) == 4 && s->b7_narrow) {
         if (d3) { if (raise_smem_limit(s, (const void*)y_conv7_kernel<float, 9, true, true>)) y_conv7_kernel<float, 9, true, true><<<grid, 128, s->smemB, s->stream>>>(s->g, (cx<float>*)S, (const float*)wsp<float>(s, s->off_Kc), *reinterpret_cast<twiddles<float>*>(&tw), ilog2(s->twN), st, s->tmS); }
         else { if (raise_smem_limit(s, (const void*)y_conv7_kernel<float, 9, false, true>)) y_conv7_kernel<float, 9, false, true><<<grid, 128, s->smemB, s->stream>>>(s->g, (cx<float>*)S, (const float*)wsp<float>(s, s->off_Kc), *reinterpret_cast<twiddles<float>*>(&tw), ilog2(s->twN), st, s->tmS); }

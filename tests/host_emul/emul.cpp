@@ -80,7 +80,7 @@ static void run(int ver, int nx, int ny, int nz, int G, int CH, int TC, const do
         }
     }
     const bool b7 = ver == 7 && TC == (sizeof(T) == 8 ? 2 : 4) && ny >= 16 && ny <= 1024;
-    const bool b7n = ver == 7 && sizeof(T) == 4 && TC == 2 && ny >= 16 && ny <= 512;      // fp32 with 2-column tiles (the library's ny = 512 form)
+    const bool b7n = ver == 7 && sizeof(T) == 4 && TC == 2 && ny >= 16 && ny <= 1024;      // fp32 with 2-column tiles (the library's ny = 512 form)
     unsigned long long* nobar = nullptr;
     constexpr int LOGTC7 = sizeof(T) == 8 ? 1 : 2;
     const bool b3 = ver == 3 && ny >= 16;
@@ -110,7 +110,7 @@ static void run(int ver, int nx, int ny, int nz, int G, int CH, int TC, const do
             switch (g.logny * 2 + (nz > 1)) {
 #define CASE_B7N(L) case 2 * L: y_conv_body7<L, 1, false, 1, T>(g, S.data(), Kc.data(), tw, ilog2(twN), smem.data(), b, 0, 1, nullptr, nobar, nullptr); break; \
                     case 2 * L + 1: y_conv_body7<L, 1, true, 1, T>(g, S.data(), Kc.data(), tw, ilog2(twN), smem.data(), b, 0, 1, nullptr, nobar, nullptr); break;
-                CASE_B7N(4) CASE_B7N(5) CASE_B7N(6) CASE_B7N(7) CASE_B7N(8) CASE_B7N(9)
+                CASE_B7N(4) CASE_B7N(5) CASE_B7N(6) CASE_B7N(7) CASE_B7N(8) CASE_B7N(9) CASE_B7N(10)
             }
         } else if (b7) {
             switch (g.logny * 2 + (nz > 1)) {

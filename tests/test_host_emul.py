@@ -151,7 +151,7 @@ def test_specialised_pass_B_matches_oracle(emul, shape, prec64):
     K = khat_full(o, nx, ny, nz)
     Hd = np.zeros(3 * nx * ny * nz)
     Msf = np.ascontiguousarray(Ms.reshape(-1))
-    for tc in ((2,) if prec64 else ((4, 2) if ny <= 512 else (4,))):      # fp32 also with 2-column tiles (the ny = 512 form)
+    for tc in ((2,) if prec64 else (4, 2)):      # fp32 also with 2-column tiles (the library's ny = 512 / 1024 form)
         emul.emul_demag(7, prec64, nx, ny, nz, 1, 8, tc, K.ctypes.data_as(_dp), Msf.ctypes.data_as(_dp), m.ctypes.data_as(_dp),
                         Hd.ctypes.data_as(_dp))
         H2 = Hd.reshape(3, nz, ny, nx) * (Ms > 0)
