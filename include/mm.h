@@ -176,6 +176,32 @@ int mm_set_time(mm_sim* sim, double t);
 
 /* Diagnostics, off the hot path (synchronous). */
 int mm_average_m(mm_sim* sim, const void* dev_m, double out3[3]);   /* mean over cells with Ms>0 */
+/* <m> for callers that cannot provide device memory.  mm_average_m (above) needs a handle and its workspace, a buffer
+ * of hundreds of megabytes that the caller has to allocate.  This call needs neither: the partial sums go to an array
+ * that is built into the library (256 B + 512 KiB of every GPU that loads libmm.so, held until the process exits), and
+ * the call allocates and frees nothing, on the host or on the device.  It is meant for code that wants to watch <m> but
+ * is in no position to allocate: a logging hook inside an application whose memory pool already owns all of HBM (a
+ * plain cudaMalloc fails there), code inside a latency-critical loop that cannot afford the device-wide wait of
+ * cudaMalloc / cudaFree, or a plug-in that is handed two arrays and a stream and nothing else.
+ *   device, cuda_stream : the device the arrays live on (made current, like every mm_* call does) and the stream the
+ *                         work is enqueued on (a cudaStream_t; NULL = default stream).  Asynchronous: nothing waits.
+ *   prec, ncells        : element type of dev_m / dev_Ms; number of cells N, 1 <= N <= MM_STATIC_MAX_CELLS.  A larger N
+ *                         returns MM_ERR_UNSUPPORTED (message in mm_static_last_error) and enqueues nothing.
+ *   dev_m, dev_Ms       : 3N and N reals, SoA as everywhere in this header, read only; natural alignment suffices.
+ *   dev_out3            : 3 doubles on the device, written by the kernel: the mean of m over cells with Ms != 0 (0 if
+ *                         there is none) — the same number mm_average_m returns, both sum in fp64.
+ * Sharing: there is ONE built-in array per device.  Calls on the same stream are safe.  Two calls that can run on the
+ * GPU at the same time (different streams or host threads) overwrite each other's partial sums: both results are then
+ * undefined; order them yourself.  The array keeps the previous call's contents; the call clears the one word that
+ * must start at zero (its block counter) on `cuda_stream` before the kernel, the rest is overwritten before it is read.
+ * First call on a device: looks up the array's device address, which makes the driver load the library's device code
+ * there if it has not yet.  Make that first call once per device during start-up, before any stream capture begins
+ * and before the latency-critical part of the program; later calls enqueue one 256-byte memset and one kernel. */
+#define MM_STATIC_MAX_CELLS (1L << 26)   /* 67 108 864 cells, e.g. 8192 x 8192 x 1 or 1024 x 1024 x 64 */
+int mm_average_m_static(int device, void* cuda_stream, mm_prec prec, long ncells, const void* dev_m, const void* dev_Ms,
+                        double* dev_out3);
+/* Message of the last mm_average_m_static failure on the calling host thread ("" after a success); static storage. */
+const char* mm_static_last_error(void);
 /* E = -mu0 V sum_i Ms_i m_i.(H_d/2 + H_ex/2 + H_dmi/2 + H_an/2 + H_ext); terms in that order. */
 int mm_energy(mm_sim* sim, const void* dev_m, double* E_total, double E_terms[5]);
 /* Real-space tensor component (0..5 = xx,yy,zz,xy,xz,yz) at offsets i,j,k >= 0: N doubles (fp64

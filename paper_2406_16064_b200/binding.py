@@ -54,6 +54,8 @@ SIGNATURES = {
     "mm_time": (_d, [_vp]),
     "mm_set_time": (_i, [_vp, _d]),
     "mm_average_m": (_i, [_vp, _vp, _dp]),
+    "mm_average_m_static": (_i, [_i, _vp, _i, _l, _vp, _vp, _vp]),
+    "mm_static_last_error": (C.c_char_p, []),
     "mm_energy": (_i, [_vp, _vp, _dp, _dp]),
     "mm_get_demag_kernel": (_i, [_vp, _i, _vp]),
     "mm_set_profiling": (_i, [_vp, _i]),
@@ -81,6 +83,36 @@ def load_library(path=LIB_PATH):
             fn.restype, fn.argtypes = res, args
         _lib = L
     return _lib
+
+
+STATIC_MAX_CELLS = 1 << 26   # MM_STATIC_MAX_CELLS of include/mm.h
+
+
+def average_m_static(m, Ms, out=None):
+    """mm_average_m_static: <m> over the cells with Ms != 0, for callers that can hand the library no workspace.
+
+    The partial sums go to an array built into libmm.so, so the C call allocates nothing; no Sim (and therefore no
+    workspace tensor) is needed.  m: CUDA tensor of 3N reals (float32 or float64), Ms: N reals of the same dtype and
+    device.  Returns `out`, 3 float64 values on the same device (pass your own tensor if this wrapper must not
+    allocate either), filled asynchronously on torch's current stream.  At most STATIC_MAX_CELLS cells; calls that
+    may overlap on the GPU (different streams) share the built-in array and must be ordered by the caller.  Make the
+    first call on each device during start-up (include/mm.h)."""
+    import torch
+    if not (torch.is_tensor(m) and m.is_cuda):
+        raise MMError("no CUDA tensor: the mm library has no CPU path")
+    L = load_library()
+    assert m.dtype in (torch.float32, torch.float64) and Ms.dtype == m.dtype and Ms.device == m.device
+    assert m.is_contiguous() and Ms.is_contiguous() and m.numel() == 3 * Ms.numel()
+    if out is None:
+        out = torch.empty(3, dtype=torch.float64, device=m.device)
+    assert out.is_cuda and out.dtype == torch.float64 and out.numel() == 3 and out.is_contiguous()
+    dev = m.device.index if m.device.index is not None else torch.cuda.current_device()
+    stream = torch.cuda.current_stream(m.device)
+    rc = L.mm_average_m_static(dev, _vp(stream.cuda_stream), F64 if m.dtype == torch.float64 else F32, Ms.numel(),
+                               _vp(m.data_ptr()), _vp(Ms.data_ptr()), _vp(out.data_ptr()))
+    if rc != 0:
+        raise MMError(f"mm_average_m_static: {_STATUS.get(rc, rc)} ({L.mm_static_last_error().decode()})")
+    return out
 
 
 class Sim:

@@ -5,7 +5,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmm.so")
-SOURCES = ["mm_lib.cu", "mm_newell_host.cpp"]
+SOURCES = ["mm_lib.cu", "mm_newell_host.cpp", "mm_noalloc.cu"]
 HEADERS = ["mm_fft.cuh", "mm_kernels.cuh", "mm_kernels2.cuh", "mm_passAC.cuh", "mm_passB7.cuh", "mm_passB3.cuh", "mm_passB4.cuh", "mm_llg.cuh", os.path.join("..", "..", "include", "mm.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 
@@ -22,11 +22,14 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     obj_cu = os.path.join(CSRC, "mm_lib.o")
     obj_cpp = os.path.join(CSRC, "mm_newell_host.o")
+    obj_na = os.path.join(CSRC, "mm_noalloc.o")
     cmds = [
         [NVCC, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
          "-c", os.path.join(CSRC, "mm_lib.cu"), "-o", obj_cu] + (["-Xptxas", "-v"] if verbose else []) + os.environ.get("MM_NVCC_FLAGS", "").split(),
         ["g++", "-O2", "-std=gnu++17", "-fPIC", "-c", os.path.join(CSRC, "mm_newell_host.cpp"), "-o", obj_cpp],
-        [NVCC, "-shared", "-o", LIB, obj_cu, obj_cpp, "-lquadmath", "-lpthread"],
+        [NVCC, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
+         "-c", os.path.join(CSRC, "mm_noalloc.cu"), "-o", obj_na],
+        [NVCC, "-shared", "-o", LIB, obj_cu, obj_cpp, obj_na, "-lquadmath", "-lpthread"],
     ]
     for c in cmds:
         subprocess.run(c, check=True)
