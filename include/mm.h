@@ -89,8 +89,9 @@ int mm_set_H_ext(mm_sim* sim, double hx, double hy, double hz);
 /* Cell-based material constants (PAPER.md:66 "cell-based", :120, :175): dev_A / dev_D hold N reals in the handle's
  * precision, copied into the workspace.  The bond values are the harmonic means A_ij = 2 A_i A_j / (A_i + A_j)
  * and D_ij = 2 D_i D_j / (D_i + D_j), 0 when both vanish.  While set they replace the
- * uniform mm_set_A / mm_set_D value; NULL (or a later mm_set_A / mm_set_D) switches back.  Call after
- * mm_set_workspace. */
+ * uniform mm_set_A / mm_set_D value; NULL (or a later mm_set_A / mm_set_D) switches back.  `kind` takes effect only
+ * when dev_D is non-NULL and the copy succeeded: mm_set_D_cell(sim, NULL, kind) keeps the kind of the last mm_set_D,
+ * and a call that returns an error changes nothing.  Call after mm_set_workspace. */
 int mm_set_A_cell(mm_sim* sim, const void* dev_A);
 int mm_set_D_cell(mm_sim* sim, const void* dev_D, mm_dmi_kind kind);
 /* Cubic anisotropy, Eq. 33 in its continuum reading (R6): energy density
@@ -114,7 +115,10 @@ int mm_set_slonczewski(mm_sim* sim, double a_J, double b_J, double px, double py
 /* Thermal field, Eq. 41-42: xi = eta sqrt(2 alpha kB T / (mu0 Ms gamma V dt)) added to H_eff during
  * mm_step / mm_relax / mm_run_until / mm_run_host, one Gaussian vector per cell and step attempt (held over the stages),
  * eta from Philox4x32-10 + Box-Muller keyed by (seed, attempt counter, cell index) (R18).  Resets the
- * attempt counter.  T = 0 switches it off.  mm_effective_field / mm_llg_rhs never include it.  Needs the workspace. */
+ * attempt counter.  T = 0 switches it off.  mm_effective_field / mm_llg_rhs never include it.  Needs the workspace.
+ * Fixed steps only: while T > 0, mm_step / mm_run_host with tol > 0 under MM_DOPRI5, mm_relax and mm_run_until return
+ * MM_ERR_UNSUPPORTED — xi depends on dt (Eq. 42) and a rejected attempt would throw its noise away and redraw, which
+ * biases the noise the accepted steps see; the paper gives no rule for it, so the library refuses rather than guess. */
 int mm_set_temperature(mm_sim* sim, double T_kelvin, unsigned long long seed);
 /* The thermal field a step of size dt with attempt counter `step` would use: 3N reals to dev_out (parity tests). */
 int mm_thermal_field(mm_sim* sim, double dt, unsigned long long step, void* dev_out);
@@ -216,6 +220,12 @@ int mm_get_demag_kernel(mm_sim* sim, int comp, void* dev_out);
  * the event overhead (two stream operations per kernel) out of the rest of the step. */
 int mm_set_profiling(mm_sim* sim, int on);
 int mm_get_profile(mm_sim* sim, double ms_out[4], long count_out[4]);
+/* Step statistics, kept by the device-side controller: step attempts accepted and rejected by mm_step / mm_relax /
+ * mm_run_until / mm_run_host since mm_set_workspace, and the RHS evaluations (Eq. 37) those attempts made (7 per DOPRI5
+ * attempt, 4 per RK4 / Cayley-RK4 attempt; mm_effective_field, mm_llg_rhs and mm_minimize are not counted).  Attempts
+ * enqueued after a stop condition was met do no work and are not counted.  Out-pointers are HOST pointers and may be
+ * NULL.  Synchronises the stream. */
+int mm_get_stats(mm_sim* sim, long* accepted, long* rejected, long* rhs_evals);
 /* Number of kernel launches issued by this handle so far (for bench accounting). */
 long mm_launch_count(const mm_sim* sim);
 const char* mm_last_error(const mm_sim* sim);

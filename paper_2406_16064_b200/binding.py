@@ -60,6 +60,7 @@ SIGNATURES = {
     "mm_get_demag_kernel": (_i, [_vp, _i, _vp]),
     "mm_set_profiling": (_i, [_vp, _i]),
     "mm_get_profile": (_i, [_vp, _dp, _lp]),
+    "mm_get_stats": (_i, [_vp, _lp, _lp, _lp]),
     "mm_launch_count": (_l, [_vp]),
     "mm_last_error": (C.c_char_p, [_vp]),
     "mm_version": (C.c_char_p, []),
@@ -274,6 +275,12 @@ class Sim:
         tot, terms = C.c_double(), (C.c_double * 5)()
         self._chk(self.L.mm_energy(self.h, self._dev(m, 3 * self.N), C.byref(tot), terms), "mm_energy")
         return tot.value, list(terms)
+
+    def stats(self):
+        """(accepted attempts, rejected attempts, RHS evaluations of the steppers) since the workspace was set."""
+        a, r, n = C.c_long(), C.c_long(), C.c_long()
+        self._chk(self.L.mm_get_stats(self.h, C.byref(a), C.byref(r), C.byref(n)), "mm_get_stats")
+        return a.value, r.value, n.value
 
     def set_profiling(self, on): self._chk(self.L.mm_set_profiling(self.h, int(on)), "mm_set_profiling")
 

@@ -46,6 +46,7 @@ struct DevState {
     int accepted, done, nan, mode;     // mode: 0 single step, 1 relax, 2 run_until
     long long nacc, nrej, nsteps;
     unsigned long long th_step;        // thermal field: step attempts since mm_set_temperature (Philox counter word)
+    long long nrhs;                    // RHS evaluations of all step attempts; with nacc / nrej: totals since mm_set_workspace (mm_get_stats)
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -551,10 +552,11 @@ __global__ void __launch_bounds__(MM_STAGEV_THREADS, sizeof(T) == 8 ? 1 : (GEN ?
 }
 
 // Step controller: one thread.  DESIGN.md R8.
-__global__ void ctrl_kernel(DevState* st, int is_f64, int adaptive_mode, int thermal)
+__global__ void ctrl_kernel(DevState* st, int is_f64, int adaptive_mode, int thermal, int nstage)
 {
     if (st->done) return;
     if (thermal) st->th_step++;
+    st->nrhs += nstage;
     double err, maxk;
     if (is_f64) { err = __longlong_as_double((long long)st->err_bits); maxk = __longlong_as_double((long long)st->maxk_bits); }
     else { err = (double)__uint_as_float((unsigned)st->err_bits); maxk = (double)__uint_as_float((unsigned)st->maxk_bits); }
@@ -600,7 +602,7 @@ __global__ void set_state_kernel(DevState* st, double dt, double tol, double t_e
 {
     st->dt = dt; st->tol = tol; st->t_end = t_end; st->stop_dmdt = stop; st->mode = mode;
     st->err_bits = 0ull; st->maxk_bits = 0ull;
-    if (reset_done) { st->done = 0; st->nan = 0; st->nsteps = 0; st->nacc = 0; st->nrej = 0; }
+    if (reset_done) { st->done = 0; st->nan = 0; st->nsteps = 0; }      // nacc / nrej / nrhs run on: lifetime totals
 }
 
 // per-block partial sums: out[block*4 + {0,1,2,3}] = sum w*a.b (w = Ms or 1), components / count
@@ -906,6 +908,8 @@ template <typename T> __global__ void __launch_bounds__(256) kc_fill_kernel(Geom
 // ================================================================================================
 using namespace mm;
 
+static constexpr size_t STEP_KEY_MAX = 256;      // bytes of a step-graph key (step_key)
+
 struct mm_sim {
     Geom g;
     mm_prec prec;
@@ -914,11 +918,12 @@ struct mm_sim {
     double dx, dy, dz;
     double A, D, Ku, Kc, u[3], hext[3], alpha, gamma;
     int dmi_kind, integ, demag_on, demag_ready, Ms_set;
+    int dmi_kind_uniform = 0;                // the kind given to mm_set_D; dmi_kind is the active one (cell-based D carries its own)
     int A_cell, D_cell, H_cell;      // cell-based A / D / external field set (arrays in the workspace)
     int unx, uny, unz, embed;        // the caller's mesh; embed: it is not 2^k per axis and lives inside the padded mesh g
     long uN;
     // whole-step CUDA graphs (one launch per step instead of ~30): captured on the second step with the same key
-    struct StepGraph { unsigned char key[256]; size_t key_len; cudaGraphExec_t exec; long launches; };
+    struct StepGraph { unsigned char key[STEP_KEY_MAX]; size_t key_len; cudaGraphExec_t exec; long launches; };
     std::vector<StepGraph> graphs;
     cudaStream_t cap_stream;         // capture happens on a private stream (the caller's may be the legacy default stream)
     int use_graph;
@@ -947,6 +952,7 @@ struct mm_sim {
     CUtensorMap tmS;        // S as (x, j, zpos, comp)
     int no_stagev;          // MM_NO_STAGEV: one-cell-per-thread stage kernel (A/B comparisons)
     std::vector<const void*> smem_attr;      // kernels whose dynamic shared-memory limit has been raised on s->device
+    bool launch_skipped = false;             // a launch_* helper returned without launching (s->err says why); read by demag_passes
     int prof_on, prof_open;      // prof_on: bit c = kernel class c is bracketed with events
     std::vector<cudaEvent_t> prof_ev;      // pairs
     std::vector<int> prof_cls;             // class of pair i: 0 pass A, 1 pass B, 2 pass C, 3 stage kernel
@@ -988,12 +994,14 @@ static void prof_end(mm_sim* s)
     } while (0)
 
 // cudaFuncAttributeMaxDynamicSharedMemorySize is a per-device setting: recorded per handle (a handle lives on one
-// device), not per process.  Returns false (and leaves the CUDA error in s->err) when the driver refuses.
+// device), not per process.  Returns false when the driver refuses: the caller then skips its launch, and because the
+// CUDA error is consumed here, s->launch_skipped carries the failure to demag_passes, which returns MM_ERR_CUDA
+// (message in s->err) instead of reporting a field that was never computed.
 static bool raise_smem_limit(mm_sim* s, const void* func)
 {
     for (const void* f : s->smem_attr) if (f == func) return true;
     const cudaError_t e = cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-    if (e != cudaSuccess) { s->err = std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e); cudaGetLastError(); return false; }
+    if (e != cudaSuccess) { s->err = std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e); cudaGetLastError(); s->launch_skipped = true; return false; }
     s->smem_attr.push_back(func);
     return true;
 }
@@ -1264,7 +1272,7 @@ extern "C" int mm_set_A(mm_sim* s, double A) { if (!s) return MM_ERR_ARG; s->A =
 extern "C" int mm_set_D(mm_sim* s, double D, mm_dmi_kind kind)
 {
     if (!s || kind < 0 || kind > 3) return MM_ERR_ARG;
-    s->D = D; s->dmi_kind = kind; s->D_cell = 0; return MM_OK;
+    s->D = D; s->dmi_kind = s->dmi_kind_uniform = kind; s->D_cell = 0; return MM_OK;
 }
 // cell-based constants: copied into the workspace; NULL switches back to the uniform value
 static int set_cell_array(mm_sim* s, size_t off, size_t count, const void* dev_src, int* flag)
@@ -1279,8 +1287,11 @@ static int in_set_A_cell(mm_sim* s, const void* dev_A) { if (!s) return MM_ERR_A
 static int in_set_D_cell(mm_sim* s, const void* dev_D, mm_dmi_kind kind)
 {
     if (!s || kind < 0 || kind > 3) return MM_ERR_ARG;
-    s->dmi_kind = kind;
-    return set_cell_array(s, s->off_Dc, (size_t)s->g.N, dev_D, &s->D_cell);
+    // `kind` belongs to the cell-based D: it is committed only once the array has been copied.  NULL switches back to
+    // the uniform D of mm_set_D together with that call's kind; a failed call changes nothing.
+    const int rc = set_cell_array(s, s->off_Dc, (size_t)s->g.N, dev_D, &s->D_cell);
+    if (rc == MM_OK) s->dmi_kind = dev_D ? (int)kind : s->dmi_kind_uniform;
+    return rc;
 }
 static int in_set_H_ext_cell(mm_sim* s, const void* dev_H) { if (!s) return MM_ERR_ARG; return set_cell_array(s, s->off_Hc, 3 * (size_t)s->g.N, dev_H, &s->H_cell); }
 extern "C" int mm_set_Ku(mm_sim* s, double Ku) { if (!s) return MM_ERR_ARG; s->Ku = Ku; return MM_OK; }
@@ -1558,7 +1569,8 @@ template <typename T, int V, int Q> static void launch_B4(mm_sim* s, unsigned nt
     at[0].id = cudaLaunchAttributeClusterDimension;
     at[0].val.clusterDim.x = Q; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
     cfg.attrs = at; cfg.numAttrs = 1;
-    cudaLaunchKernelEx(&cfg, y_conv4_kernel<T, V, Q>, s->g, S, (const T*)wsp<T>(s, s->off_Kh), tw, st);
+    const cudaError_t e = cudaLaunchKernelEx(&cfg, y_conv4_kernel<T, V, Q>, s->g, S, (const T*)wsp<T>(s, s->off_Kh), tw, st);
+    if (e != cudaSuccess) { s->err = std::string("cudaLaunchKernelEx(y_conv4): ") + cudaGetErrorString(e); cudaGetLastError(); s->launch_skipped = true; }
 }
 template <typename T, int V> static void launch_B3(mm_sim* s, unsigned grid, cx<T>* S, twiddles<T> tw, const DevState* st)
 {
@@ -1702,6 +1714,7 @@ template <typename T> static int demag_passes(mm_sim* s, const T* y)
     }
     prof_end(s);
     s->launches += 3;
+    if (s->launch_skipped) { s->launch_skipped = false; cudaGetLastError(); return MM_ERR_CUDA; }   // s->err set where it happened
     MM_TRY(s, cudaGetLastError());
     return MM_OK;
 }
@@ -1863,7 +1876,7 @@ template <typename T> static int enqueue_step(mm_sim* s, T* m, int ctrl_mode)
         if (rc) return rc;
     }
     DevState* ds = wsp<DevState>(s, s->off_st);
-    ctrl_kernel<<<1, 1, 0, s->stream>>>(ds, s->prec == MM_F64, ctrl_mode, thermal ? 1 : 0);
+    ctrl_kernel<<<1, 1, 0, s->stream>>>(ds, s->prec == MM_F64, ctrl_mode, thermal ? 1 : 0, nst);
     const T* ysol = yb[1];     // DOPRI5: y_6 written at stage 5 ; RK4 / Cayley: solution written at stage 3
     accept_kernel<T><<<(unsigned)((N + 255) / 256), 256, 0, s->stream>>>(N, ds, ysol, wsp<T>(s, s->off_Ms), m, s->integ == MM_CAYLEY_RK4 ? 0 : 1);
     s->launches += 2;
@@ -1880,8 +1893,11 @@ static int enqueue_step_eager(mm_sim* s, void* m, int ctrl_mode)
 // (dt, tol, the clock, the thermal attempt counter and m itself live in device memory and are read at run time.)
 static size_t step_key(const mm_sim* s, const void* m, int ctrl_mode, unsigned char* out)
 {
+    // `out` holds STEP_KEY_MAX bytes (the local in enqueue_step_any and StepGraph::key).  A field that would not fit is
+    // not written and the returned length exceeds STEP_KEY_MAX: the caller then steps without a graph, so a key that
+    // outgrows the buffer costs replay speed, never a stack overrun or a stale graph.
     size_t n = 0;
-    auto put = [&](const void* p, size_t b) { memcpy(out + n, p, b); n += b; };
+    auto put = [&](const void* p, size_t b) { if (n + b <= STEP_KEY_MAX) memcpy(out + n, p, b); n += b; };
     put(&m, sizeof(m)); put(&ctrl_mode, sizeof(int)); put(&s->ws, sizeof(void*));
     put(&s->A, sizeof(double)); put(&s->D, sizeof(double)); put(&s->Ku, sizeof(double)); put(&s->Kc, sizeof(double));
     put(s->u, sizeof(s->u)); put(s->hext, sizeof(s->hext)); put(&s->alpha, sizeof(double)); put(&s->gamma, sizeof(double));
@@ -1897,8 +1913,9 @@ static size_t step_key(const mm_sim* s, const void* m, int ctrl_mode, unsigned c
 static int enqueue_step_any(mm_sim* s, void* m, int ctrl_mode)
 {
     if (!s->use_graph || s->prof_on) return enqueue_step_eager(s, m, ctrl_mode);
-    unsigned char key[256];
+    unsigned char key[STEP_KEY_MAX];
     const size_t klen = step_key(s, m, ctrl_mode, key);
+    if (klen > STEP_KEY_MAX) return enqueue_step_eager(s, m, ctrl_mode);
     mm_sim::StepGraph* e = nullptr;
     for (auto& g : s->graphs) if (g.key_len == klen && memcmp(g.key, key, klen) == 0) { e = &g; break; }
     if (!e) {      // first step with this key: run it eagerly (this also sets the kernels' shared-memory attributes)
@@ -1941,10 +1958,34 @@ static int read_state(mm_sim* s, DevState* h)
     return MM_OK;
 }
 
+extern "C" int mm_get_stats(mm_sim* s, long* accepted, long* rejected, long* rhs_evals)
+{
+    NEED_WS(s);
+    MM_TRY(s, cudaSetDevice(s->device));
+    DevState h;
+    int rc = read_state(s, &h);
+    if (rc) return rc;
+    if (accepted) *accepted = (long)h.nacc;
+    if (rejected) *rejected = (long)h.nrej;
+    if (rhs_evals) *rhs_evals = (long)h.nrhs;
+    return MM_OK;
+}
+
+// Error control and the thermal field do not go together (include/mm.h, mm_set_temperature): xi is drawn per attempt and
+// scales as 1/sqrt(dt), so a controller that rejects an attempt throws a noise realisation away because it was "hard"
+// and accepted steps see biased noise; Eq. 42 is written for a given dt.  Refused, not approximated.
+static int refuse_adaptive_thermal(mm_sim* s, double tol)
+{
+    if (s->temperature > 0.0 && tol > 0.0 && s->integ == MM_DOPRI5)
+        return fail(s, MM_ERR_UNSUPPORTED, "adaptive step control (tol > 0) is not available with the thermal field (T > 0): use fixed steps, tol <= 0");
+    return MM_OK;
+}
+
 static int in_step(mm_sim* s, void* dev_m, double dt, double tol, int* accepted, double* err, double* dt_next, double* max_dmdt)
 {
     NEED_READY(s);
     if (!dev_m || !(dt > 0)) return MM_ERR_ARG;
+    if (refuse_adaptive_thermal(s, tol)) return MM_ERR_UNSUPPORTED;
     int rc = set_state(s, dt, s->integ == MM_DOPRI5 ? tol : 0.0, 0, 0, 0, 1);
     if (rc) return rc;
     if ((rc = enqueue_step_any(s, dev_m, 0))) return rc;
@@ -1964,6 +2005,7 @@ static int adaptive_loop(mm_sim* s, void* dev_m, double tol, double dt0, double 
 {
     if (!dev_m || !(tol > 0) || !(dt0 > 0) || max_steps < 0) return MM_ERR_ARG;
     if (s->integ != MM_DOPRI5) return fail(s, MM_ERR_ARG, "adaptive stepping needs MM_DOPRI5");
+    if (refuse_adaptive_thermal(s, tol)) return MM_ERR_UNSUPPORTED;
     int rc = set_state(s, dt0, tol, t_end, stop, mode, 1);
     if (rc) return rc;
     const long poll = 16;
@@ -2085,6 +2127,7 @@ static int in_run_host(mm_sim* s, void* host_m, int nsteps, double dt, double to
 {
     NEED_READY(s);
     if (!host_m || nsteps < 0 || !(dt > 0)) return MM_ERR_ARG;
+    if (refuse_adaptive_thermal(s, tol)) return MM_ERR_UNSUPPORTED;
     const size_t bytes = 3 * (size_t)s->g.N * esize(s);
     // m lives in the workspace's own staging slot for the duration of the call
     void* dm = wsp<char>(s, s->off_mh);

@@ -85,6 +85,22 @@ def test_uniform_arrays_reduce_to_uniform_constants(prec):
     assert np.array_equal(to_np(s.effective_field(dm)), H0)
 
 
+def test_set_D_cell_null_keeps_the_uniform_kind():
+    """mm_set_D_cell(NULL, kind) only switches back to the uniform D: the kind given with NULL is ignored, the one of the
+    last mm_set_D stays (include/mm.h).  A cell array set with another kind does change the field."""
+    w = wl.cfg4(32, 16, 4)
+    o, s = make_pair(w, F64, demag=False)          # cfg4: bulk DMI
+    dm = s.to_device(masked_m(w))
+    H0 = to_np(s.effective_field(dm))
+    s.set_D_cell(np.full((4, 16, 32), w.D), wl.DMI_D2D)
+    assert np.abs(to_np(s.effective_field(dm)) - H0).max() > 1e-3 * np.abs(H0).max()
+    s.set_D_cell(None, wl.DMI_INTERFACIAL)
+    s.set_D(w.D, wl.DMI_BULK)
+    assert np.array_equal(to_np(s.effective_field(dm)), H0)
+    s.set_D_cell(None, wl.DMI_INTERFACIAL)         # uniform D already active: the kind must not move
+    assert np.array_equal(to_np(s.effective_field(dm)), H0)
+
+
 @pytest.mark.parametrize("prec", [F64, F32])
 @pytest.mark.parametrize("kind", [wl.DMI_BULK, wl.DMI_D2D])
 def test_fixed_dt_steps_and_energy(kind, prec):

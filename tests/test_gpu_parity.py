@@ -174,6 +174,10 @@ def test_adaptive_step_accept_reject_matches_oracle():
     ok, err, dn, _ = s.step(dm, 2e-13, 1e-6)
     assert ok and ok_o and np.isclose(err, err_o, rtol=1e-5) and np.isclose(dn, dn_o, rtol=1e-5)
     assert np.abs(to_np(dm) - m).max() < 1e-10
+    assert s.stats() == (1, 1, 14)                           # mm_get_stats: one rejected + one accepted DOPRI5 attempt
+    s.set_integrator(wl.RK4)
+    s.step(dm, 1e-13, sync=False)
+    assert s.stats() == (2, 1, 18)                           # totals run on across calls; an RK4 attempt is 4 evaluations
 
 
 @pytest.mark.parametrize("prec", [F64, F32])
@@ -188,6 +192,8 @@ def test_cfg2_relax_then_run(prec):
     tol = 1e-6
     n_o, md_o = o.relax(m, tol, 2e9, 400, 1e-13)
     n_s, md_s = s.relax(dm, tol, 2e9, 400, 1e-13)
+    acc, rej, nrhs = s.stats()                               # attempts enqueued after the stop do not count
+    assert acc + rej == n_s and nrhs == 7 * n_s and acc >= 1
     Ms = w.Ms_array()
     loose = 1e-4 if prec == F64 else 1e-2
     assert md_s < 2e9 and md_o < 2e9

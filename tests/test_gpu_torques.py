@@ -95,6 +95,25 @@ def test_fixed_dt_steps_with_everything_on(integ, prec):
     assert np.isclose(s.time(), 5 * w.dt, rtol=1e-12)
 
 
+def test_adaptive_control_is_refused_with_the_thermal_field():
+    """T > 0 and error control together are refused (include/mm.h, mm_set_temperature): a rejected attempt would redraw
+    the noise.  Fixed steps still run, and T = 0 brings the adaptive calls back."""
+    from paper_2406_16064_b200 import MMError
+    w = problem(16, 16, 2)
+    w.integrator = wl.DOPRI5
+    s = make_pair(w, F64)[1]
+    dm = s.to_device(masked_m(w))
+    s.set_temperature(300.0, 9)
+    for call in (lambda: s.step(dm, w.dt, tol=1e-6), lambda: s.relax(dm, 1e-6, 1e3, 4, dt0=w.dt),
+                 lambda: s.run_until(dm, 10 * w.dt, 1e-6, dt0=w.dt),
+                 lambda: s.run_host(dm.cpu(), 2, w.dt, tol=1e-6)):
+        with pytest.raises(MMError, match="MM_ERR_UNSUPPORTED"):
+            call()
+    assert s.step(dm, w.dt)[0]                       # fixed step: fine
+    s.set_temperature(0.0, 9)
+    assert s.step(dm, w.dt, tol=1e-3)[1] >= 0.0      # T = 0: adaptive again
+
+
 @pytest.mark.parametrize("prec", [F64, F32])
 def test_cayley_macrospin_follows_eq_53(prec):
     """1x1x1 mesh (one-cell-per-thread kernel), Fig. 3 parameters: the GPU Cayley-RK4 trajectory equals the oracle's and
