@@ -102,11 +102,11 @@ int mm_set_Kc(mm_sim* sim, double Kc);
  * switches back to the uniform mm_set_H_ext value. */
 int mm_set_H_ext_cell(mm_sim* sim, const void* dev_H);
 /* Zhang-Li spin-transfer torque: dm/dt += f_stt x m, f_stt = [(beta - alpha) tau + (1 + alpha beta)
- * m x tau] / (1 + alpha^2) (PAPER.md:345), tau = (u . grad) m by central differences (a missing neighbour is replaced
+ * m x tau] / (1 + alpha^2) (PAPER.md:352), tau = (u . grad) m by central differences (a missing neighbour is replaced
  * by the cell itself).  u in m/s (Eq. 39), uniform; (0,0,0) switches the term off.  Sign convention of Eq. 44 / Eq. 54
  * (a head-to-head wall moves with -(1 + alpha beta) u / (1 + alpha^2)); Eq. 38 as printed has u -> -u (R17). */
 int mm_set_zhang_li(mm_sim* sim, double ux, double uy, double uz, double beta);
-/* Time profile of that current: u(t) = u exp(-b t) cos(w t) (the pulse of PAPER.md:446; Eq. 54 holds for any u(t)),
+/* Time profile of that current: u(t) = u exp(-b t) cos(w t) (the pulse of PAPER.md:444; Eq. 54 holds for any u(t)),
  * evaluated at every RK stage's own time t + c dt on the device.  b = w = 0 (the default): constant current. */
 int mm_set_zhang_li_pulse(mm_sim* sim, double b, double w);
 /* Slonczewski / spin-orbit torque, Eq. 40: -a_J m x (m x p) - b_J m x p added to the Gilbert

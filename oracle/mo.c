@@ -24,8 +24,8 @@
  *   RK4 + projection  PAPER.md:425; Dormand-Prince + projection PAPER.md:298, ref [37]
  *   energy            Eq. 1, 2, 6/7, 10, 12 summed per cell
  *   mo_minimize       steepest descent with Barzilai-Borwein steps, Eq. 50-52
- *   Zhang-Li torque   f_stt of Eq. 44's text with tau = (u.grad) m, PAPER.md:306-308 (Eq. 38), :345; sign of u as in
- *                     Eq. 44 / Eq. 54 (PAPER.md:345, 436) — Eq. 38 prints the opposite sign, DESIGN.md R17
+ *   Zhang-Li torque   f_stt of Eq. 44's text with tau = (u.grad) m, PAPER.md:306-308 (Eq. 38), :352; sign of u as in
+ *                     Eq. 44 / Eq. 54 (PAPER.md:352, 435-436) — Eq. 38 prints the opposite sign, DESIGN.md R17
  *   Slonczewski / SOT Eq. 40, solved for dm/dt (LL form)
  *   thermal field     Eq. 41-42: one Gaussian vector per cell and step, held over the step's stages;
  *                     normals from Philox4x32-10 + Box-Muller keyed by (seed, step, cell) (R18)
@@ -62,7 +62,7 @@ typedef struct mo_sim {
     int integrator;             /* 0 RK4, 1 DOPRI5, 2 Cayley-transform RK4 (Eq. 49) */
     double stt_u[3], stt_beta;  /* Zhang-Li: u in m/s (Eq. 39), beta */
     int stt_on;
-    double stt_b, stt_w;        /* time profile of the current: u(t) = u exp(-b t) cos(w t) (PAPER.md:446); 0, 0 = constant */
+    double stt_b, stt_w;        /* time profile of the current: u(t) = u exp(-b t) cos(w t) (PAPER.md:444); 0, 0 = constant */
     double t_eval;              /* time at which the right-hand side is being evaluated (stage time inside a step) */
     int in_step;
     double sl_aJ, sl_bJ, sl_p[3]; /* Slonczewski / SOT (Eq. 40): a_J, b_J in 1/s, unit vector p */
@@ -515,7 +515,7 @@ void mo_normals3(unsigned long long seed, unsigned long long step, unsigned long
 
 #define MO_KB 1.380649e-23
 
-/* Eq. 42 (PAPER.md:335): xi_i^u = eta sqrt(2 alpha kB T / (mu0 Ms_i gamma V dt)), V = cell volume; 0 where Ms = 0 */
+/* Eq. 42 (PAPER.md:337): xi_i^u = eta sqrt(2 alpha kB T / (mu0 Ms_i gamma V dt)), V = cell volume; 0 where Ms = 0 */
 int mo_thermal_field(const mo_sim *s, double dt, unsigned long long step, double *xi)
 {
     const long N = s->N;
@@ -553,7 +553,7 @@ int mo_stt_tau(mo_sim *s, const double *m, double *tau)
                     if (pos[a] < lim[a] - 1 && s->Ms[q + str[a]] != 0.0) pp = q + str[a];
                     for (int c = 0; c < 3; c++) tau[c * N + q] += s->stt_u[a] * (m[c * N + pp] - m[c * N + pm]) / (2.0 * delta[a]);
                 }
-                /* u(t) = u exp(-b t) cos(w t) at the evaluation time (PAPER.md:446 "u(t) = u0 e^{-bt} cos(wt)") */
+                /* u(t) = u exp(-b t) cos(w t) at the evaluation time (PAPER.md:444 "u(t) = u0 e^{-bt} cos(wt)") */
                 if (s->stt_b != 0.0 || s->stt_w != 0.0) {
                     const double f = exp(-s->stt_b * s->t_eval) * cos(s->stt_w * s->t_eval);
                     for (int c = 0; c < 3; c++) tau[c * N + q] *= f;
@@ -568,7 +568,7 @@ static void cross3(const double a[3], const double b[3], double c[3])
 }
 
 /* Eq. 37 with the thermal field of the step in progress added to H_eff, plus
- *  - Zhang-Li (PAPER.md:345): dm/dt += f_stt x m, f_stt = [(beta - alpha) tau + (1 + alpha beta) m x tau]/(1 + alpha^2)
+ *  - Zhang-Li (PAPER.md:352): dm/dt += f_stt x m, f_stt = [(beta - alpha) tau + (1 + alpha beta) m x tau]/(1 + alpha^2)
  *  - Slonczewski / SOT, Eq. 40: with T = -a_J m x (m x p) - b_J m x p the implicit equation
  *    dm/dt = ... + alpha m x dm/dt + T solves to dm/dt += (T + alpha m x T)/(1 + alpha^2). */
 int mo_llg_rhs(mo_sim *s, const double *m, double *dmdt)
@@ -637,7 +637,7 @@ void mo_cayley_apply(const double w[3], const double m0[3], double out[3])
 
 /* f of Eq. 44 at the magnetisation mm: gamma (H + alpha m x H)/(1 + alpha^2) with H = H_eff (+ thermal field of the
  * step) (+ the Slonczewski terms written as a field, (a_J/gamma) m x p + (b_J/gamma) p: "can be
- * incorporated into the effective fields"), plus f_stt (PAPER.md:345). */
+ * incorporated into the effective fields"), plus f_stt (PAPER.md:352). */
 static int cayley_f(mo_sim *s, const double *mm, double *f)
 {
     const long N = s->N;

@@ -198,7 +198,7 @@ __device__ __forceinline__ void warp_max_bits(unsigned long long v, unsigned lon
 
 // From the total field h of a cell (every H_eff term, plus the thermal field during a step) to the stage's output:
 // MODE 0 the field itself; MODE 1 dm/dt = Eq. 37 with the Slonczewski terms folded into the field (Eq. 40,
-// PAPER.md:319) plus f_stt x m (PAPER.md:345); MODE 2 d omega/dt of Eq. 49 at omega = w with f of Eq. 44.
+// PAPER.md:319) plus f_stt x m (PAPER.md:352); MODE 2 d omega/dt of Eq. 49 at omega = w with f of Eq. 44.
 // *kn = |dm/dt| when want_kn (MODE 2; MODE 1 takes it from the result).
 template <typename T, int MODE>
 __device__ __forceinline__ v3<T> stage_result(const LocalP<T>& lp, v3<T> mi, v3<T> h, v3<T> tau, v3<T> w, bool want_kn, T* kn)

@@ -33,7 +33,7 @@ template <typename T> struct LocalP {
     T p[3];           // unit polarisation vector
     T gam, al;        // gamma, alpha (f of Eq. 44 and f_stt need them separately)
     int stt_on, sl_on;
-    double stt_b, stt_w;   // time profile of the Zhang-Li current: u(t) = u exp(-b t) cos(w t) (PAPER.md:446); 0, 0 = constant
+    double stt_b, stt_w;   // time profile of the Zhang-Li current: u(t) = u exp(-b t) cos(w t) (PAPER.md:444); 0, 0 = constant
 };
 
 // bond value of a cell-based constant: harmonic mean, 0 when both vanish
@@ -83,7 +83,7 @@ template <typename T> MM_HD v3<T> stt_tau(const LocalP<T>& lp, v3<T> mi, const v
     return t;
 }
 
-// f_stt = [(beta - alpha) tau + (1 + alpha beta) m x tau] / (1 + alpha^2)   (PAPER.md:345)
+// f_stt = [(beta - alpha) tau + (1 + alpha beta) m x tau] / (1 + alpha^2)   (PAPER.md:352)
 template <typename T> MM_HD v3<T> stt_f(const LocalP<T>& lp, v3<T> m, v3<T> tau)
 {
     const v3<T> mt = cross<T>(m, tau);

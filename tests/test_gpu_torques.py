@@ -199,7 +199,7 @@ def test_equilibrium_distribution_on_the_gpu(prec):
 @pytest.mark.parametrize("prec", [F64, F32])
 @pytest.mark.parametrize("integ", [wl.RK4, wl.DOPRI5, wl.CAYLEY_RK4])
 def test_time_dependent_current_matches_oracle(integ, prec):
-    """u(t) = u exp(-b t) cos(w t) (PAPER.md:446) evaluated at every stage's own time on the device: ten fixed-dt steps
+    """u(t) = u exp(-b t) cos(w t) (PAPER.md:444) evaluated at every stage's own time on the device: ten fixed-dt steps
     from a non-zero start time against the oracle, every integrator; and the right-hand side alone at that time."""
     w = problem(32, 16, 2)
     w.integrator = integ
@@ -221,7 +221,7 @@ def test_time_dependent_current_matches_oracle(integ, prec):
 
 
 def test_domain_wall_under_the_papers_pulse_on_the_gpu():
-    """PAPER.md:436-448, Fig. 5 on the GPU (fp64, DOPRI5): wall position and tilt under u0 exp(-b t) cos(w t) against
+    """PAPER.md:433-446, Fig. 5 on the GPU (fp64, DOPRI5): wall position and tilt under u0 exp(-b t) cos(w t) against
     Eq. 54 integrated in closed form."""
     nx, dx, alpha, beta, A, K, u0, b, om = 512, 1e-9, 0.1, 0.3, 1.3e-11, 1e5, 300.0, 5e8, 2e9
     Delta = np.sqrt(A / K)

@@ -69,7 +69,9 @@ def test_thin_film_limit():
     H = o.field_terms(m, oracle.TERM_DEMAG)
     assert abs(H[2].mean() / 8e5 + G["block_256_256_4_zz"][0]) < 1e-13
     assert -1.0 < H[2, 0, 32, 32] / 8e5 < -0.97           # centre of the film close to -Ms
-    assert np.abs(H[:2]).mean() / 8e5 < 1e-12 or True
+    # in-plane components: odd under the film's mirror symmetries, so they cancel in the mean (not cell by cell: they are
+    # of order 1e-2 Ms at the edges)
+    assert np.abs(H[:2].mean(axis=(1, 2, 3))).max() / 8e5 < 1e-13
 
 
 def test_demag_energy_nonnegative_and_masked_cells_zero():

@@ -82,6 +82,45 @@ def test_eq52_on_a_hand_case():
     assert np.abs(m - (lambda mm: (o.sd_update(mm, o.effective_field(mm), taus[2]), mm)[1])(ms[2].copy())).max() < 1e-15
 
 
+def test_clamp_reading_on_the_hand_case():
+    """DESIGN.md R16 (the paper prints no bounds): |tau| is clamped to [tau_min, tau_max].  Same 2-cell system as above:
+    the Barzilai-Borwein value of the second update is computed by hand; with tau_max below it (tau_min above it) the
+    update must use exactly the bound, and the resulting m is Eq. 51 with that bound."""
+    o = oracle.Oracle(2, 1, 1, 2e-9, 2e-9, 2e-9)
+    o.set_Ms(8e5); o.set_A(1.3e-11); o.set_Ku(5e4); o.set_axis(0, 0, 1); o.set_H_ext(2e4, 0, 1e4); o.set_demag(0)
+    m0 = np.array([[0.6, 0.0], [0.0, 0.8], [0.8, 0.6]]).reshape(3, 1, 1, 2).copy()
+    tau0 = 1e-7
+
+    def gof(m):
+        a, h = m.reshape(3, -1).T, o.effective_field(m).reshape(3, -1).T
+        return np.cross(a, np.cross(a, h))
+
+    m1 = m0.copy()
+    o.sd_update(m1, o.effective_field(m1), tau0)
+    sv, yv = (m1 - m0).reshape(3, -1).T, gof(m1) - gof(m0)
+    bb = abs((sv * sv).sum() / (sv * yv).sum())
+    for lo, hi, expect in ((1e-14, bb / 3, bb / 3), (3 * bb, 1.0, 3 * bb), (bb / 2, 2 * bb, bb)):
+        m = m0.copy()
+        n, _, tau_last = o.minimize(m, tau0, lo, hi, 0.0, 2)
+        assert n == 2 and np.isclose(tau_last, expect, rtol=1e-12), (tau_last, expect)
+        ref = m1.copy()
+        o.sd_update(ref, o.effective_field(ref), expect)
+        assert np.abs(m - ref).max() < 1e-15
+
+
+def test_fallback_reading_when_the_quotient_is_undefined():
+    """DESIGN.md R16: a vanishing or non-finite Barzilai-Borwein quotient falls back to tau0.  At an exact equilibrium
+    (m parallel to H in every cell: g = 0) nothing moves, s = y = 0 and both quotients of Eq. 52 are 0/0; with the stop
+    criterion off the iteration must carry on with tau0 and leave m finite and untouched."""
+    o = oracle.Oracle(2, 1, 1, 2e-9, 2e-9, 2e-9)
+    o.set_Ms(8e5); o.set_A(1.3e-11); o.set_Ku(5e4); o.set_axis(0, 0, 1); o.set_H_ext(0, 0, 1e4); o.set_demag(0)
+    m = np.zeros((3, 1, 1, 2))
+    m[2] = 1.0
+    n, maxg, tau_last = o.minimize(m, 3e-8, 1e-14, 1.0, 0.0, 4)
+    assert n == 4 and maxg == 0.0 and tau_last == 3e-8
+    assert np.array_equal(m[2], np.ones((1, 1, 2))) and np.all(m[:2] == 0)
+
+
 @pytest.mark.parametrize("kind", [wl.DMI_BULK, wl.DMI_INTERFACIAL])
 def test_minimiser_and_llg_relaxation_reach_the_same_minimum(kind):
     w, o, m = small_problem(kind=kind, shape=(4, 4, 2))

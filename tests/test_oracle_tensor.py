@@ -114,7 +114,10 @@ def test_block_aggregation_identity_small():
     assert np.allclose(acc, blk, atol=1e-14)
 
 
-@pytest.mark.parametrize("shape,cell", [((5, 4, 3), (1.0, 0.8, 1.3)), ((12, 7, 1), (3.90625, 3.90625, 3.0)), ((6, 9, 4), (2.0, 1.0, 0.5))])
+@pytest.mark.parametrize("shape,cell", [((5, 4, 3), (1.0, 0.8, 1.3)), ((12, 7, 1), (3.90625, 3.90625, 3.0)), ((6, 9, 4), (2.0, 1.0, 0.5)),
+                                        # larger than the library's near box (8 cell edges per direction): offsets where the
+                                        # table's index arithmetic is furthest from the origin, with and without a z extent
+                                        ((40, 24, 3), (2.5, 2.5, 2.5)), ((40, 24, 1), (4.0, 4.0, 4.0))])
 def test_tabulated_tensor_equals_pointwise(shape, cell):
     """mo_newell_tensor (lattice tabulation of f / g + 27-point stencil + odd-axis signs) against the independent
     point evaluation mo_newell_point at EVERY offset of the mesh, all six components (one mesh has nz = 1)."""

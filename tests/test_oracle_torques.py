@@ -1,5 +1,5 @@
 """Pins of the oracle's SURVEY 8(f)3 parts: Zhang-Li and Slonczewski / SOT torques (Eq. 38-40,
-f_stt of PAPER.md:345) and the thermal field (Eq. 41-42) with its counter-based normals.  Each pin is
+f_stt of PAPER.md:352) and the thermal field (Eq. 41-42) with its counter-based normals.  Each pin is
 something the paper or the mathematics fixes: the Philox known-answer vectors, Gaussian moments, Eq. 42's variance,
 the equilibrium distribution of Eq. 56, the Gilbert-form residual of Eq. 38 / Eq. 40, the
 domain-wall solution Eq. 54 and closed forms that follow from Eq. 53."""
@@ -223,7 +223,7 @@ def test_zhang_li_rhs_solves_the_gilbert_form(beta):
 def test_domain_wall_motion_is_eq_54(beta):
     """PAPER.md:432-444 (Eq. 54): a 1-D head-to-head wall under a constant u moves rigidly with
     dz/dt = -(1 + alpha beta) u / (1 + alpha^2) and tilts with dphi/dt = (alpha - beta) u / ((1 + alpha^2) Delta),
-    Delta = sqrt(A/K); Permalloy parameters of PAPER.md:446-448, alpha = 0.1."""
+    Delta = sqrt(A/K); Permalloy parameters of PAPER.md:444-446, alpha = 0.1."""
     nx, dx, alpha, A, K, u = 400, 1e-9, 0.1, 1.3e-11, 1e5, 100.0
     Delta = np.sqrt(A / K)
     o = chain(nx, dx, alpha, A, K)
@@ -309,7 +309,7 @@ def pulse_integral(t, u0, b, w):
 
 @pytest.mark.parametrize("integrator", [oracle.RK4, oracle.DOPRI5, oracle.CAYLEY_RK4])
 def test_domain_wall_under_the_papers_current_pulse(integrator):
-    """PAPER.md:436-448 (Eq. 54, Fig. 5): "u = u(t) ... an arbitrary time dependence"; the paper's run uses
+    """PAPER.md:433-446 (Eq. 54, Fig. 5): "u = u(t) ... an arbitrary time dependence"; the paper's run uses
     u(t) = u0 exp(-b t) cos(w t), b = 5e8 1/s, w = 2e9 1/s, alpha = 0.1.  Wall position and tilt angle at several times
     against z(t) - z(0) = -(1 + alpha beta) U(t) / (1 + alpha^2), phi(t) - phi(0) = (alpha - beta) U(t) / ((1 + alpha^2) Delta),
     U = int u dt in closed form; the stage times of every integrator enter (a u frozen over the step would be first order)."""
