@@ -57,7 +57,9 @@ typedef enum {
  * {-y^,+y^,+x^,-x^,0,0}; D2d {+x^,-x^,-y^,+y^,0,0} (Eq. 14). */
 typedef enum { MM_DMI_NONE = 0, MM_DMI_BULK = 1, MM_DMI_INTERFACIAL = 2, MM_DMI_D2D = 3 } mm_dmi_kind;
 /* MM_CAYLEY_RK4: classical RK4 on omega of the Cayley transform (Eq. 43-49), omega restarted at 0
- * every step, m <- Q(omega) m; fixed step, no projection (Q is a rotation). */
+ * every step, m <- Q(omega) m; fixed step, no projection (Q is a rotation).  In fp32 the rounding of Q m lets |m| drift
+ * like a random walk, about 1e-7 sqrt(steps) (measured 2e4 steps: tests/test_gpu_torques.py); callers running millions
+ * of fp32 Cayley steps should renormalise m themselves now and then. */
 typedef enum { MM_RK4 = 0, MM_DOPRI5 = 1, MM_CAYLEY_RK4 = 2 } mm_integrator;
 
 /* Create a problem on `device`, all later work on `cuda_stream` (a cudaStream_t; NULL = default

@@ -43,6 +43,35 @@ def test_fixed_number_of_updates_matches_oracle(shape, kind, nsteps, prec):
 
 
 @pytest.mark.parametrize("prec", [F64, F32])
+def test_clamp_and_fallback_readings_match_the_oracle(prec):
+    """DESIGN.md R16 on the GPU: tau pinned to the bound when the Barzilai-Borwein value leaves [tau_min, tau_max]; tau0
+    when the quotient is 0/0 (exact equilibrium, stop criterion off)."""
+    w = problem(32, 16, 2)
+    # the free BB values of this problem alternate around 1e-6 (tau^1) and 2e-8 (tau^2): the first window caps every
+    # update from above, the second lifts the third update (a tau^2) to tau_min
+    for lo, hi, nsteps in ((1e-12, 3e-9, 6), (1e-7, 1e-4, 3)):
+        o, s = make_pair(w, prec)
+        m = masked_m(w)
+        dm = s.to_device(m)
+        _, _, tau_o = o.minimize(m, 1e-8, lo, hi, 0.0, nsteps)
+        _, _, tau_s = s.minimize(dm, 1e-8, lo, hi, 0.0, nsteps)
+        assert tau_o in (lo, hi) and tau_s == tau_o
+        assert np.abs(to_np(dm) - m).max() <= (1e-9 if prec == F64 else 2e-3)
+    w = problem(16, 16, 1, mask=False)
+    w.demag = False
+    w.D = 0.0
+    w.axis, w.H_ext = (0.0, 0.0, 1.0), (0.0, 0.0, 5e4)
+    o, s = make_pair(w, prec)
+    m = np.zeros((3, 1, 16, 16))
+    m[2] = 1.0
+    dm = s.to_device(m)
+    n_s, g_s, tau_s = s.minimize(dm, 3e-8, 1e-12, 1e-4, 0.0, 4)
+    n_o, g_o, tau_o = o.minimize(m, 3e-8, 1e-12, 1e-4, 0.0, 4)
+    assert (n_s, g_s, tau_s) == (n_o, g_o, tau_o) == (4, 0.0, 3e-8)
+    assert np.array_equal(to_np(dm), m)
+
+
+@pytest.mark.parametrize("prec", [F64, F32])
 def test_minimise_to_convergence_same_minimum_as_oracle(prec):
     w = problem(16, 16, 2)
     o, s = make_pair(w, prec)

@@ -133,7 +133,7 @@ def test_cfg1_200_rk4_steps(prec):
 
 
 @pytest.mark.parametrize("prec", [F64, F32])
-@pytest.mark.parametrize("case,nsteps", [("cfg2", 20), ("cfg3_64", 20), ("slab_32x16x8_bulk", 5), ("slab_64x64x16", 5)])
+@pytest.mark.parametrize("case,nsteps", [("cfg2", 20), ("cfg3_64", 20), ("cfg3_256", 20), ("slab_32x16x8_bulk", 5), ("slab_64x64x16", 5)])
 def test_fixed_dt_dopri5_steps(case, nsteps, prec):
     w = CASES[case]()
     o, s = make_pair(w, prec)
@@ -298,7 +298,7 @@ def test_cfg4_full_size_sampled_direct_sum():
         del s
 
 
-@pytest.mark.parametrize("case", ["cfg4", "film4096_f32", "film4096_f64", "film2048_f64", "film1024_f64"])
+@pytest.mark.parametrize("case", ["cfg4", "film4096_f32", "film4096_f64", "film2048_f64", "film1024_f64", "film2048_f32", "film1024_f32"])
 def test_full_size_block_aggregation_identity(case):
     """Uniformly magnetised full mesh: the MEAN demag field is -Ms N_self(block) m exactly, with N_self the
     Newell self term of the whole block as one cell (SURVEY.md §8c pins; holds at any size)."""
@@ -322,24 +322,26 @@ def test_full_size_block_aggregation_identity(case):
 
 
 @pytest.mark.parametrize("prec", [F64, F32])
-def test_film4096_point_source_is_the_newell_tensor(prec):
-    """configs[4] at N = 4096 (fp64 runs the half-tile pass B: a full 8192-row tile does not fit one CTA): the field
-    of ONE magnetised cell is -Ms N(r - r0) m at every cell; sampled cells against the oracle's quad-precision
-    tensor, including the far corners of the film and the source's neighbours."""
+@pytest.mark.parametrize("n", [4096, 2048, 1024])
+def test_film_point_source_is_the_newell_tensor(n, prec):
+    """configs[4] at N = 4096 (fp64 runs the cluster pass B: a full 8192-row tile does not fit one CTA), 2048 (fp32: the
+    generic TMA pass B at 2-column tiles and the padded x tile at 4 lines per CTA) and 1024: the field of ONE
+    magnetised cell is -Ms N(r - r0) m at every cell; sampled cells against the oracle's quad-precision tensor,
+    including the far corners of the film and the source's neighbours."""
     from paper_2406_16064_b200 import Sim
     import torch
-    w = wl.cfg5(4096, with_m=False)
+    w = wl.cfg5(n, with_m=False)
     s = Sim(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, prec=prec)
     wl.apply(s, w)
     s.set_A(0.0); s.set_H_ext(0, 0, 0)
-    i0, j0 = 1234, 3071
+    i0, j0 = (1234 * n) // 4096, (3071 * n) // 4096
     mvec = np.array([0.6, -0.64, 0.48])
-    dm = torch.zeros((3, 1, 4096, 4096), dtype=s.dtype, device=s.device)
+    dm = torch.zeros((3, 1, n, n), dtype=s.dtype, device=s.device)
     dm[:, 0, j0, i0] = torch.tensor(mvec, dtype=s.dtype)
     H = s.effective_field(dm)
     rng = np.random.default_rng(7)
-    cells = [(i0, j0), (i0 + 1, j0), (i0, j0 - 1), (i0 - 1, j0 + 1), (0, 0), (4095, 4095), (0, 4095), (4095, 0), (i0, 0), (2048, 2048)]
-    cells += [(int(a), int(b)) for a, b in rng.integers(0, 4096, (30, 2))]
+    cells = [(i0, j0), (i0 + 1, j0), (i0, j0 - 1), (i0 - 1, j0 + 1), (0, 0), (n - 1, n - 1), (0, n - 1), (n - 1, 0), (i0, 0), (n // 2, n // 2)]
+    cells += [(int(a), int(b)) for a, b in rng.integers(0, n, (30, 2))]
     cells += [(i0 + int(a), j0 + int(b)) for a, b in rng.integers(-12, 13, (30, 2))]
     worst = 0.0
     for (i, j) in cells:
