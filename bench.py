@@ -173,10 +173,13 @@ def algorithmic_bytes(w, esize):
     """per RHS 39 N s (film) / 89 N s (3-D); DOPRI5 step = 7 RHS + 102 N s.
     Per kernel class (units of N s): pass B is SURVEY's "last forward + multiply + first inverse (+K^)" row,
     16 (film) / 30 (3-D); this build does z inside the x passes, so A = 4 + 6 / 4 + 12 and C = 6 + 3 / 12 + 3
-    (DESIGN.md §5); the stage kernel reads H_d, m, Ms and writes k: 13 (+3 per earlier k_j it reads)."""
+    (DESIGN.md §5); the stage kernel reads H_d, m, Ms and writes k: 13, and a DOPRI5 stage s also reads the s earlier
+    k_j (3 each), reads m0 and writes the next stage's input (3 + 3, stages that have one): over the seven launches of a
+    step that is SURVEY's 102 = 3 (0+1+...+6) + 18 + 18 + 3 extra N s, so the AVERAGE stage launch moves (7*13 + 99)/7 =
+    27.1 N s — the figure the per-class time (an average over all stage launches) is divided into."""
     N = w.N
     three_d = w.nz > 1
-    per_class = {"fwd_xz": 16 if three_d else 10, "y_conv": 30 if three_d else 16, "inv_zx": 15 if three_d else 9, "llg_stage": 13}
+    per_class = {"fwd_xz": 16 if three_d else 10, "y_conv": 30 if three_d else 16, "inv_zx": 15 if three_d else 9, "llg_stage": (7 * 13 + 99) / 7.0}
     return {"rhs": (89 if three_d else 39) * N * esize, "step": (7 * (89 if three_d else 39) + 102) * N * esize,
             "class": {k: v * N * esize for k, v in per_class.items()}}
 
@@ -367,6 +370,26 @@ def measure(args, w, prec_name, rank, world, local, barrier, dev, sample_clocks)
     torch.cuda.synchronize()
     e2e_sec = time.perf_counter() - t0
 
+    # sustained: the run length BASELINE.json configs[3] specifies (1000 fixed-dt steps), with the clocks of that window
+    sus = None
+    if args.sustained_steps > 0:
+        sus_sampler = ClockSampler(local) if sample_clocks else None
+        if sus_sampler:
+            sus_sampler.start()
+            time.sleep(0.02)
+        u0, u1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        th0 = time.perf_counter()
+        u0.record()
+        for _ in range(args.sustained_steps):
+            s.step(dm, w.dt, sync=False)
+        u1.record()
+        barrier()
+        th1 = time.perf_counter()
+        sus_sec, sus_units = aggregate_over_ranks(u0.elapsed_time(u1) * 1e-3, w.N * RHS_PER_STEP * args.sustained_steps, dev)
+        sus = {"steps": args.sustained_steps, "seconds": sus_sec, "units": sus_units, "clocks": sus_sampler.stop(th0, th1) if sus_sampler else None}
+        assert bool(torch.isfinite(dm).all()), "non-finite magnetisation after the sustained run"
+
     units = w.N * RHS_PER_STEP * args.steps
     ev_max = aggregate_over_ranks(ev_sec, units, dev)[0] if ev_sec is not None else None
     sec_max, units_all = aggregate_over_ranks(sec, units, dev)
@@ -386,7 +409,14 @@ def measure(args, w, prec_name, rank, world, local, barrier, dev, sample_clocks)
     achieved = dom_bytes / (dom_avg * 1e-3) / 1e9
     step_gbs = ab["step"] * args.steps / sec / 1e9
     tot = sum(prof_ms)
+    if sus is not None:
+        sus_gbs = ab["step"] * sus["steps"] / sus["seconds"] / 1e9
+        sus = {"steps": sus["steps"], "value": sus["units"] / sus["seconds"], "unit": UNIT, "ms_per_step": 1e3 * sus["seconds"] / sus["steps"],
+               "seconds": sus["seconds"], "step_frac": sus_gbs / peak, "step_frac_nominal_8TBs": sus_gbs / 8000.0, "clocks": sus["clocks"],
+               "note": "BASELINE.json configs[3]'s own run length (fixed-dt DOPRI5 steps, one CUDA graph launch each), timed with CUDA events "
+                       "after the short region above; reported beside `value`, not instead of it"}
     return {
+        "sustained": sus,
         "value": units_all / sec_max, "ms_per_step": 1e3 * sec_max / args.steps, "dtype": prec_name,
         "e2e": {"value": e2e_units / e2e_max, "unit": UNIT, "h2d_bytes_per_step": 3 * w.N * esize, "d2h_bytes_per_step": 3 * w.N * esize,
                 "api": "mm_run_host (pinned host m in, one DOPRI5 step, m out)"},
@@ -408,6 +438,52 @@ def measure(args, w, prec_name, rank, world, local, barrier, dev, sample_clocks)
                      "step_algorithmic_gbs": step_gbs, "step_frac": step_gbs / peak, "step_frac_nominal_8TBs": step_gbs / 8000.0,
                      "mm_version": version},
     }
+
+
+def film_point(n, prec_name, local, steps=15, warm=3):
+    """One point of BASELINE.json configs[4] (N x N x 1 film, demag + exchange + Zeeman): `steps` fixed-dt DOPRI5 steps
+    (15 steps = 105 RHS evaluations; configs[4] asks for 100) timed with CUDA events as one graph launch per step, then a
+    profiled pass for the per-kernel averages.  Fractions are against the measured HBM peak with the film byte model
+    of SURVEY 8(d) — for N = 1024 the working set (about 45 MB in fp32) fits the 126 MB L2, so that point is not HBM-bound
+    by construction and its fraction is a comparison figure only."""
+    import torch
+    from paper_2406_16064_b200 import Sim, F32, F64, workloads as wl
+    w = wl.cfg5(n)
+    prec = F64 if prec_name == "f64" else F32
+    esize = 8 if prec == F64 else 4
+    s = Sim(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, prec=prec, device=local)
+    wl.apply(s, w)
+    dm = s.to_device(w.m0)
+    for _ in range(warm + 2):
+        s.step(dm, w.dt, sync=False)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(steps):
+        s.step(dm, w.dt, sync=False)
+    e1.record()
+    torch.cuda.synchronize()
+    sec = e0.elapsed_time(e1) * 1e-3
+    s.set_profiling(True)
+    for _ in range(5):
+        s.step(dm, w.dt, sync=False)
+    torch.cuda.synchronize()
+    ms, cnt = s.get_profile()
+    s.set_profiling(False)
+    assert bool(torch.isfinite(dm).all())
+    del s, dm
+    torch.cuda.empty_cache()
+    peak, _ = measured_peaks()
+    ab = algorithmic_bytes(w, esize)
+    per = {c: ms[i] / cnt[i] for i, c in enumerate(CLASSES) if cnt[i]}
+    frac = {c: ab["class"][c] / (per[c] * 1e-3) / 1e9 / peak for c in per}
+    dom = max(per, key=lambda c: per[c] * cnt[CLASSES.index(c)])
+    weakest = min(frac, key=frac.get)
+    gbs = ab["step"] * steps / sec / 1e9
+    return {"n": n, "dtype": prec_name, "value": w.N * RHS_PER_STEP * steps / sec, "unit": UNIT, "ms_per_step": 1e3 * sec / steps,
+            "us_per_rhs": 1e6 * sec / steps / RHS_PER_STEP, "step_frac": gbs / peak, "step_frac_nominal_8TBs": gbs / 8000.0,
+            "kernel": dom, "frac": frac[dom], "weakest_kernel": weakest, "weakest_frac": frac[weakest],
+            "kernel_us": {c: 1e3 * v for c, v in per.items()}, "kernel_frac": frac}
 
 
 def run_mm(args):
@@ -449,10 +525,14 @@ def run_mm(args):
             "events_region": top["events_region"],
             "cpu_baseline": cpu,
         }
+        line["sustained"] = top["sustained"]
         if len(precs) > 1:
             o = res["f64"]
-            line["fp64"] = {k: o[k] for k in ("value", "ms_per_step", "dtype", "e2e", "gpu_launches", "clocks", "roofline", "events_region")}
+            line["fp64"] = {k: o[k] for k in ("value", "ms_per_step", "dtype", "e2e", "gpu_launches", "clocks", "roofline", "events_region", "sustained")}
             line["fp64"]["unit"] = UNIT
+        if args.films and world == 1 and args.workload == "cfg4":
+            # BASELINE.json configs[4], the paper's own throughput shape: the weakest numbers of this build
+            line["films"] = [film_point(n, p, local) for n in (1024, 4096) for p in precs]
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
@@ -474,6 +554,8 @@ def main():
     ap.add_argument("--workload", default="cfg4")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-kernel-events", action="store_true", help="no CUDA events inside the timed region (whole-step CUDA graphs stay on)")
+    ap.add_argument("--sustained-steps", type=int, default=1000, help="length of the `sustained` leg (configs[3]: 1000 steps); 0 skips it")
+    ap.add_argument("--no-films", dest="films", action="store_false", help="skip the N x N x 1 film points (configs[4]) of the default line")
     args = ap.parse_args()
     world_env = os.environ.get("WORLD_SIZE")
     if world_env is None and args.gpus > 1:
